@@ -1,0 +1,512 @@
+// oracle/kso.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, obviously-correct CPU statement (FP64) of what the hot path computes:
+// the plane-wave Kohn-Sham Hamiltonian apply and the block-Davidson iteration around it
+// (arxiv 2501.08697 = /root/reference/PAPER.md, §III.A, §III.B, §II.A.1).
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+// call it.  It shares no code, header, table or helper with the CUDA path under
+// paper_2501_08697_b200/csrc/.  No BLAS / FFTW / LAPACK: own recursive mixed-radix FFT, explicit
+// H(G,G'), cyclic Hermitian Jacobi, block Davidson.  OpenMP over bands / rows only.
+//
+// Units: Rydberg atomic units (reading C1): kinetic term |k+G|^2, no 1/2.
+//
+// Pins (tests/test_oracle_*.py, -m "not gpu"):
+//   kso_fft3d      direct O(n^2) DFT on tiny grids, delta <-> plane wave, Parseval, numpy.fft
+//   kso_pw_list    counts vs Omega ecut^{3/2}/(6 pi^2), inversion symmetry, numpy enumeration
+//   kso_hpsi       explicit H(G,G') (kso_explicit_h), V=1 identity, shift theorem, Hermiticity,
+//                  single-projector closed form, p-triplet closed form
+//   kso_explicit_h rebuilt entry by entry in numpy from Eq. 32 / Eq. 4 in the test
+//   kso_jacobi     2x2 closed form, A C = C Theta, C^H C = I, numpy.linalg.eigvalsh
+//   kso_davidson   V=0: sorted |k+G|^2 exactly; constant shift; brute-force Jacobi / eigvalsh of
+//                  explicit H on cfg 0 and the shrunk variants; Ritz values monotone
+//   Eigenvalues of cfg 1, 3, 4 at FULL size: parity unpinned by anything external.
+#include <algorithm>
+#include <cmath>
+#include <complex>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef std::complex<double> cplx;
+static const double PI = 3.14159265358979323846264338327950288;
+
+// ------------------------------------------------------------------------------------------------
+// FFT.  sign=+1:  X[k] = sum_j x[j] e^{+2 pi i jk/n}  (G -> r, unnormalised: Eq. 31)
+//       sign=-1:  X[k] = sum_j x[j] e^{-2 pi i jk/n}  (r -> G, the caller divides by N: Eq. 36)
+// Recursive decimation in time on the smallest prime factor; generic O(p^2) butterfly.
+// ------------------------------------------------------------------------------------------------
+static int smallest_factor(int n) {
+  for (int p = 2; p * p <= n; ++p)
+    if (n % p == 0) return p;
+  return n;
+}
+
+// out[k] = sum_j in[j*stride] * w[(j*k mod n) * (N0/n)],  w[t] = e^{sign 2 pi i t/N0}
+static void fft_rec(const cplx* in, long stride, cplx* out, int n, const cplx* w, int N0) {
+  if (n == 1) { out[0] = in[0]; return; }
+  const int p = smallest_factor(n), m = n / p, step = N0 / n;
+  for (int r = 0; r < p; ++r) fft_rec(in + r * stride, stride * p, out + (long)r * m, m, w, N0);
+  std::vector<cplx> t(p);
+  for (int k = 0; k < m; ++k) {
+    for (int r = 0; r < p; ++r) t[r] = out[(long)r * m + k];
+    for (int q = 0; q < p; ++q) {
+      const int kk = k + q * m;
+      cplx s(0.0, 0.0);
+      for (int r = 0; r < p; ++r) s += t[r] * w[(long)(((long)r * kk) % n) * step];
+      out[kk] = s;
+    }
+  }
+}
+
+static std::vector<cplx> twiddles(int n, int sign) {
+  std::vector<cplx> w(n);
+  for (int t = 0; t < n; ++t) {
+    const double a = 2.0 * PI * (double)t / (double)n;
+    w[t] = cplx(std::cos(a), sign * std::sin(a));
+  }
+  return w;
+}
+
+// 3D transform of a[n1][n2][n3] (n3 fastest), axis by axis.
+static void fft3d(int n1, int n2, int n3, cplx* a, int sign) {
+  const int nn[3] = {n1, n2, n3};
+  const long st[3] = {(long)n2 * n3, (long)n3, 1};
+  for (int ax = 0; ax < 3; ++ax) {
+    const int n = nn[ax];
+    const std::vector<cplx> w = twiddles(n, sign);
+    std::vector<cplx> line(n), res(n);
+    const int o1 = (ax + 1) % 3, o2 = (ax + 2) % 3;
+    for (int i = 0; i < nn[o1]; ++i)
+      for (int j = 0; j < nn[o2]; ++j) {
+        cplx* base = a + i * st[o1] + j * st[o2];
+        for (int t = 0; t < n; ++t) line[t] = base[t * st[ax]];
+        fft_rec(line.data(), 1, res.data(), n, w.data(), n);
+        for (int t = 0; t < n; ++t) base[t * st[ax]] = res[t];
+      }
+  }
+}
+
+extern "C" int kso_fft3d(int n1, int n2, int n3, cplx* a, int sign) {
+  if (n1 < 1 || n2 < 1 || n3 < 1 || (sign != 1 && sign != -1)) return -1;
+  fft3d(n1, n2, n3, a, sign);
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Plane-wave list: keep G = m1 b1 + m2 b2 + m3 b3 iff |k+G|^2 <= ecutwfc (inclusive; reading C2),
+// order m1 slowest, m3 fastest, each ascending (reading C3).  Eq. 31, L500-505.
+// ------------------------------------------------------------------------------------------------
+static void recip(const double* cell, double b[9]) {
+  const double* a1 = cell; const double* a2 = cell + 3; const double* a3 = cell + 6;
+  double c23[3] = {a2[1] * a3[2] - a2[2] * a3[1], a2[2] * a3[0] - a2[0] * a3[2], a2[0] * a3[1] - a2[1] * a3[0]};
+  double c31[3] = {a3[1] * a1[2] - a3[2] * a1[1], a3[2] * a1[0] - a3[0] * a1[2], a3[0] * a1[1] - a3[1] * a1[0]};
+  double c12[3] = {a1[1] * a2[2] - a1[2] * a2[1], a1[2] * a2[0] - a1[0] * a2[2], a1[0] * a2[1] - a1[1] * a2[0]};
+  const double vol = a1[0] * c23[0] + a1[1] * c23[1] + a1[2] * c23[2];
+  for (int i = 0; i < 3; ++i) {
+    b[i] = 2 * PI * c23[i] / vol; b[3 + i] = 2 * PI * c31[i] / vol; b[6 + i] = 2 * PI * c12[i] / vol;
+  }
+}
+
+static int pw_enumerate(const double* cell, const double* kf, double ecut, std::vector<int>* mil,
+                        std::vector<double>* g2out) {
+  double b[9]; recip(cell, b);
+  double kc[3];
+  for (int i = 0; i < 3; ++i) kc[i] = kf[0] * b[i] + kf[1] * b[3 + i] + kf[2] * b[6 + i];
+  const double rmax = std::sqrt(ecut) + std::sqrt(kc[0] * kc[0] + kc[1] * kc[1] + kc[2] * kc[2]);
+  int M[3];
+  for (int i = 0; i < 3; ++i) {
+    const double* a = cell + 3 * i;
+    M[i] = (int)std::floor(rmax * std::sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]) / (2 * PI)) + 1;
+  }
+  int count = 0;
+  for (int m1 = -M[0]; m1 <= M[0]; ++m1)
+    for (int m2 = -M[1]; m2 <= M[1]; ++m2)
+      for (int m3 = -M[2]; m3 <= M[2]; ++m3) {
+        const double f[3] = {m1 + kf[0], m2 + kf[1], m3 + kf[2]};
+        double q[3];
+        for (int i = 0; i < 3; ++i) q[i] = f[0] * b[i] + f[1] * b[3 + i] + f[2] * b[6 + i];
+        const double g2 = q[0] * q[0] + q[1] * q[1] + q[2] * q[2];
+        if (g2 <= ecut) {
+          if (mil) { mil->push_back(m1); mil->push_back(m2); mil->push_back(m3); }
+          if (g2out) g2out->push_back(g2);
+          ++count;
+        }
+      }
+  return count;
+}
+
+extern "C" int kso_pw_count(const double* cell, const double* kf, double ecut, int* npw) {
+  *npw = pw_enumerate(cell, kf, ecut, nullptr, nullptr);
+  return 0;
+}
+extern "C" int kso_pw_list(const double* cell, const double* kf, double ecut, int* miller, double* g2) {
+  std::vector<int> m; std::vector<double> g;
+  pw_enumerate(cell, kf, ecut, &m, &g);
+  std::memcpy(miller, m.data(), m.size() * sizeof(int));
+  if (g2) std::memcpy(g2, g.data(), g.size() * sizeof(double));
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Context
+// ------------------------------------------------------------------------------------------------
+struct kso_ctx {
+  int n1, n2, n3, npw, nproj, natom;
+  long N;
+  std::vector<int> miller;      // [npw][3]
+  std::vector<long> idx;        // grid index of G_j : (m mod n), n3 fastest (reading C5)
+  std::vector<double> g2;       // |k+G|^2 (Ry)
+  std::vector<cplx> vhat;       // V_loc(G) as passed, [n1][n2][n3]
+  std::vector<double> vr;       // V(r) = Re sum_m vhat[m] e^{+2 pi i m.j/n}
+  std::vector<cplx> beta;       // [nproj][npw]
+  std::vector<int> off;         // [natom+1]
+  std::vector<double> D;        // concatenated per-atom blocks
+  std::vector<long> doff;       // offset of each atom's block in D
+};
+
+static inline int pmod(int a, int n) { int r = a % n; return r < 0 ? r + n : r; }
+
+extern "C" int kso_create(kso_ctx** out, const double* cell, const double* kf, double ecut, const int* grid,
+                          const cplx* vloc_g, int nproj, const cplx* beta, int natom, const int* proj_offset,
+                          const double* D) {
+  kso_ctx* c = new kso_ctx;
+  c->n1 = grid[0]; c->n2 = grid[1]; c->n3 = grid[2];
+  c->N = (long)c->n1 * c->n2 * c->n3;
+  c->npw = pw_enumerate(cell, kf, ecut, &c->miller, &c->g2);
+  c->idx.resize(c->npw);
+  for (int j = 0; j < c->npw; ++j) {
+    const int* m = &c->miller[3 * j];
+    if (2 * std::abs(m[0]) >= c->n1 || 2 * std::abs(m[1]) >= c->n2 || 2 * std::abs(m[2]) >= c->n3) { delete c; return -2; }
+    c->idx[j] = ((long)pmod(m[0], c->n1) * c->n2 + pmod(m[1], c->n2)) * c->n3 + pmod(m[2], c->n3);
+  }
+  c->vhat.assign(vloc_g, vloc_g + c->N);
+  std::vector<cplx> v(c->vhat);
+  fft3d(c->n1, c->n2, c->n3, v.data(), +1);
+  double vmax = 0, imax = 0;
+  for (long i = 0; i < c->N; ++i) { vmax = std::max(vmax, std::abs(v[i].real())); imax = std::max(imax, std::abs(v[i].imag())); }
+  if (imax > 1e-12 * std::max(vmax, 1e-300) && imax > 0) { delete c; return -5; }
+  c->vr.resize(c->N);
+  for (long i = 0; i < c->N; ++i) c->vr[i] = v[i].real();
+  c->nproj = nproj; c->natom = natom;
+  if (nproj > 0) {
+    c->beta.assign(beta, beta + (long)nproj * c->npw);
+    c->off.assign(proj_offset, proj_offset + natom + 1);
+    long o = 0;
+    for (int a = 0; a < natom; ++a) { c->doff.push_back(o); const int np = c->off[a + 1] - c->off[a]; o += (long)np * np; }
+    c->D.assign(D, D + o);
+    if (c->off[natom] != nproj) { delete c; return -1; }
+  }
+  *out = c;
+  return 0;
+}
+extern "C" void kso_destroy(kso_ctx* c) { delete c; }
+extern "C" int kso_npw(const kso_ctx* c) { return c->npw; }
+extern "C" int kso_get_vr(const kso_ctx* c, double* out) { std::memcpy(out, c->vr.data(), c->N * sizeof(double)); return 0; }
+extern "C" int kso_num_threads() {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+// ------------------------------------------------------------------------------------------------
+// H psi, dual-space form:  Eq. 32 (L507) kinetic + local, Eq. 3-4 (L217-221) nonlocal.
+//   per band: zero grid; scatter; unnormalised inverse DFT (+); times V(r); forward DFT (-);
+//   hpsi(G_j) = g2_j psi(G_j) + grid[idx_j]/N ;  B = beta^H psi ; B <- D B ; hpsi += beta B.
+// ------------------------------------------------------------------------------------------------
+extern "C" int kso_hpsi(const kso_ctx* c, const cplx* psi, cplx* hpsi, int nb) {
+  const int npw = c->npw;
+#pragma omp parallel
+  {
+    std::vector<cplx> g(c->N);
+#pragma omp for schedule(dynamic, 1)
+    for (int b = 0; b < nb; ++b) {
+      const cplx* p = psi + (long)b * npw;
+      cplx* h = hpsi + (long)b * npw;
+      std::fill(g.begin(), g.end(), cplx(0, 0));
+      for (int j = 0; j < npw; ++j) g[c->idx[j]] = p[j];
+      fft3d(c->n1, c->n2, c->n3, g.data(), +1);
+      for (long i = 0; i < c->N; ++i) g[i] *= c->vr[i];
+      fft3d(c->n1, c->n2, c->n3, g.data(), -1);
+      const double inv = 1.0 / (double)c->N;
+      for (int j = 0; j < npw; ++j) h[j] = c->g2[j] * p[j] + g[c->idx[j]] * inv;
+    }
+  }
+  if (c->nproj == 0) return 0;
+  const int P = c->nproj;
+  std::vector<cplx> B((long)P * nb), DB((long)P * nb);
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int p = 0; p < P; ++p)
+    for (int b = 0; b < nb; ++b) {
+      const cplx* be = &c->beta[(long)p * npw];
+      const cplx* ps = psi + (long)b * npw;
+      double sr = 0, si = 0;   // conj(beta) * psi
+      for (int j = 0; j < npw; ++j) {
+        sr += be[j].real() * ps[j].real() + be[j].imag() * ps[j].imag();
+        si += be[j].real() * ps[j].imag() - be[j].imag() * ps[j].real();
+      }
+      B[(long)p * nb + b] = cplx(sr, si);
+    }
+  for (int a = 0; a < c->natom; ++a) {
+    const int p0 = c->off[a], np = c->off[a + 1] - p0;
+    const double* Da = &c->D[c->doff[a]];
+    for (int p = 0; p < np; ++p)
+      for (int b = 0; b < nb; ++b) {
+        cplx s(0, 0);
+        for (int q = 0; q < np; ++q) s += Da[p * np + q] * B[(long)(p0 + q) * nb + b];
+        DB[(long)(p0 + p) * nb + b] = s;
+      }
+  }
+#pragma omp parallel for schedule(static)
+  for (int b = 0; b < nb; ++b) {
+    cplx* h = hpsi + (long)b * npw;
+    for (int p = 0; p < P; ++p) {
+      const cplx* be = &c->beta[(long)p * npw];
+      const double cr = DB[(long)p * nb + b].real(), ci = DB[(long)p * nb + b].imag();
+      for (int j = 0; j < npw; ++j)
+        h[j] += cplx(be[j].real() * cr - be[j].imag() * ci, be[j].real() * ci + be[j].imag() * cr);
+    }
+  }
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Explicit H(G,G') -- the definition, row-major H[j][j']:
+//   H = |k+G_j|^2 delta_jj' + vhat[(m_j - m_j') mod n] + sum_a sum_{p,p' in a} beta_p(j) D^a_pp' conj(beta_p'(j'))
+// ------------------------------------------------------------------------------------------------
+extern "C" int kso_explicit_h(const kso_ctx* c, cplx* H) {
+  const int npw = c->npw;
+#pragma omp parallel for schedule(static)
+  for (int j = 0; j < npw; ++j) {
+    const int* mj = &c->miller[3 * j];
+    for (int l = 0; l < npw; ++l) {
+      const int* ml = &c->miller[3 * l];
+      const long id = ((long)pmod(mj[0] - ml[0], c->n1) * c->n2 + pmod(mj[1] - ml[1], c->n2)) * c->n3 + pmod(mj[2] - ml[2], c->n3);
+      cplx h = c->vhat[id];
+      if (j == l) h += c->g2[j];
+      for (int a = 0; a < c->natom && c->nproj > 0; ++a) {
+        const int p0 = c->off[a], np = c->off[a + 1] - p0;
+        const double* Da = &c->D[c->doff[a]];
+        for (int p = 0; p < np; ++p)
+          for (int q = 0; q < np; ++q)
+            if (Da[p * np + q] != 0.0)
+              h += c->beta[(long)(p0 + p) * npw + j] * Da[p * np + q] * std::conj(c->beta[(long)(p0 + q) * npw + l]);
+      }
+      H[(long)j * npw + l] = h;
+    }
+  }
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Cyclic-by-row two-sided Hermitian Jacobi.  A row-major n x n, destroyed.
+// theta ascending; C row-major, COLUMN i is the unit eigenvector of theta[i].
+// Rotation for pivot (p,q), a_pq = |a_pq| e^{i phi}:  J = diag(1, e^{-i phi}) * [[c, s], [-s, c]],
+// tau = (a_qq - a_pp) / (2|a_pq|), t = sign(tau)/(|tau| + sqrt(1+tau^2)).
+// Stop: off(A)_F <= 1e-15 ||A||_F or 60 sweeps.  Returns the number of sweeps.
+// ------------------------------------------------------------------------------------------------
+extern "C" int kso_jacobi(int n, cplx* A, double* theta, cplx* C) {
+  std::vector<cplx> V((long)n * n, cplx(0, 0));
+  for (int i = 0; i < n; ++i) V[(long)i * n + i] = 1.0;
+  int sweep = 0;
+  for (; sweep < 60; ++sweep) {
+    double off = 0, tot = 0;
+    for (int i = 0; i < n; ++i)
+      for (int j = 0; j < n; ++j) { const double a = std::norm(A[(long)i * n + j]); tot += a; if (i != j) off += a; }
+    if (off <= 1e-30 * tot) break;   // (1e-15)^2
+    for (int p = 0; p < n - 1; ++p)
+      for (int q = p + 1; q < n; ++q) {
+        const cplx apq = A[(long)p * n + q];
+        const double ab = std::abs(apq);
+        if (ab == 0.0) continue;
+        const double app = A[(long)p * n + p].real(), aqq = A[(long)q * n + q].real();
+        const double tau = (aqq - app) / (2.0 * ab);
+        const double t = (tau >= 0 ? 1.0 : -1.0) / (std::fabs(tau) + std::sqrt(1.0 + tau * tau));
+        const double cs = 1.0 / std::sqrt(1.0 + t * t), sn = t * cs;
+        const cplx e = apq / ab;               // e^{i phi}
+        const cplx ec = std::conj(e);
+        // columns: A <- A J
+        for (int i = 0; i < n; ++i) {
+          const cplx x = A[(long)i * n + p], y = A[(long)i * n + q];
+          A[(long)i * n + p] = cs * x - sn * ec * y;
+          A[(long)i * n + q] = sn * x + cs * ec * y;
+        }
+        // rows: A <- J^H A
+        for (int j = 0; j < n; ++j) {
+          const cplx x = A[(long)p * n + j], y = A[(long)q * n + j];
+          A[(long)p * n + j] = cs * x - sn * e * y;
+          A[(long)q * n + j] = sn * x + cs * e * y;
+        }
+        A[(long)p * n + q] = 0.0; A[(long)q * n + p] = 0.0;
+        A[(long)p * n + p] = cplx(A[(long)p * n + p].real(), 0.0);
+        A[(long)q * n + q] = cplx(A[(long)q * n + q].real(), 0.0);
+        for (int i = 0; i < n; ++i) {
+          const cplx x = V[(long)i * n + p], y = V[(long)i * n + q];
+          V[(long)i * n + p] = cs * x - sn * ec * y;
+          V[(long)i * n + q] = sn * x + cs * ec * y;
+        }
+      }
+  }
+  std::vector<int> ord(n);
+  for (int i = 0; i < n; ++i) ord[i] = i;
+  std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) { return A[(long)a * n + a].real() < A[(long)b * n + b].real(); });
+  for (int i = 0; i < n; ++i) {
+    theta[i] = A[(long)ord[i] * n + ord[i]].real();
+    double nr = 0;
+    for (int r = 0; r < n; ++r) nr += std::norm(V[(long)r * n + ord[i]]);
+    nr = 1.0 / std::sqrt(nr);
+    for (int r = 0; r < n; ++r) C[(long)r * n + i] = V[(long)r * n + ord[i]] * nr;
+  }
+  return sweep;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Small dense helpers for Davidson (vectors are rows of length npw).
+// ------------------------------------------------------------------------------------------------
+static inline cplx cdot(const cplx* a, const cplx* b, int n) {  // a^H b
+  double sr = 0, si = 0;
+  for (int j = 0; j < n; ++j) {
+    sr += a[j].real() * b[j].real() + a[j].imag() * b[j].imag();
+    si += a[j].real() * b[j].imag() - a[j].imag() * b[j].real();
+  }
+  return cplx(sr, si);
+}
+static inline void caxpy(cplx al, const cplx* x, cplx* y, int n) {  // y += al x
+  const double ar = al.real(), ai = al.imag();
+  for (int j = 0; j < n; ++j)
+    y[j] = cplx(y[j].real() + ar * x[j].real() - ai * x[j].imag(), y[j].imag() + ar * x[j].imag() + ai * x[j].real());
+}
+static inline double nrm2(const cplx* a, int n) {
+  double s = 0;
+  for (int j = 0; j < n; ++j) s += std::norm(a[j]);
+  return std::sqrt(s);
+}
+
+// Hc = V^H W (m x m), symmetrised, Jacobi; X = V C[:, :nb], HX = W C[:, :nb].
+static void rayleigh_ritz(int npw, int m, int nb, const std::vector<cplx>& V, const std::vector<cplx>& W,
+                          std::vector<cplx>& X, std::vector<cplx>& HX, std::vector<double>& eps) {
+  std::vector<cplx> Hc((long)m * m), C((long)m * m);
+  std::vector<double> th(m);
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int i = 0; i < m; ++i)
+    for (int j = 0; j < m; ++j) Hc[(long)i * m + j] = cdot(&V[(long)i * npw], &W[(long)j * npw], npw);
+  for (int i = 0; i < m; ++i)
+    for (int j = i; j < m; ++j) {
+      const cplx s = 0.5 * (Hc[(long)i * m + j] + std::conj(Hc[(long)j * m + i]));
+      Hc[(long)i * m + j] = s; Hc[(long)j * m + i] = std::conj(s);
+    }
+  kso_jacobi(m, Hc.data(), th.data(), C.data());
+  X.assign((long)nb * npw, cplx(0, 0)); HX.assign((long)nb * npw, cplx(0, 0));
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < nb; ++i)
+    for (int r = 0; r < m; ++r) {
+      caxpy(C[(long)r * m + i], &V[(long)r * npw], &X[(long)i * npw], npw);
+      caxpy(C[(long)r * m + i], &W[(long)r * npw], &HX[(long)i * npw], npw);
+    }
+  eps.assign(th.begin(), th.begin() + nb);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Block Davidson, exactly the listing of SURVEY §8(c.2) / DESIGN.md (the paper names the method at
+// L326, L547, L578 but prints no listing; reading C10).  Teter-Payne-Allan diagonal preconditioner
+// (reading C11; the paper's ref 134, L1558), subspace <= max_sub_factor * nb (north_star: 2),
+// convergence: all residual 2-norms <= tol (reading C12).
+// ritz_hist (nullable): [max_iter+1][nb] Ritz values after the initial RR and after each expansion.
+// returns 0 converged, 1 not converged (best X, eps, residuals still written), <0 error.
+// ------------------------------------------------------------------------------------------------
+extern "C" int kso_davidson(const kso_ctx* c, cplx* psi, double* eig, int nb, double tol, int max_iter,
+                            double* resid, int* iters_out, long long* nhpsi_out, double* ritz_hist,
+                            int max_sub_factor) {
+  const int npw = c->npw;
+  if (nb < 1 || nb > npw || max_sub_factor < 2) return -1;
+  const int mmax = max_sub_factor * nb;
+  std::vector<cplx> X(psi, psi + (long)nb * npw), HX, V, W, R((long)nb * npw), T;
+  std::vector<double> eps(nb), rho(nb);
+  // step 0: modified Gram-Schmidt, two passes
+  for (int i = 0; i < nb; ++i) {
+    cplx* x = &X[(long)i * npw];
+    const double n0 = nrm2(x, npw);
+    for (int pass = 0; pass < 2; ++pass)
+      for (int j = 0; j < i; ++j) caxpy(-cdot(&X[(long)j * npw], x, npw), &X[(long)j * npw], x, npw);
+    const double n1 = nrm2(x, npw);
+    if (!(n1 > 1e-10 * n0) || n0 == 0.0) return -3;
+    for (int j = 0; j < npw; ++j) x[j] /= n1;
+  }
+  // step 1: initial Rayleigh-Ritz
+  W.resize((long)nb * npw);
+  kso_hpsi(c, X.data(), W.data(), nb);
+  long long nh = nb;
+  V = X;
+  { std::vector<cplx> X2, HX2; rayleigh_ritz(npw, nb, nb, V, W, X2, HX2, eps); X.swap(X2); HX.swap(HX2); }
+  V = X; W = HX;
+  int m = nb, it = 0, status = 1;
+  if (ritz_hist) std::copy(eps.begin(), eps.end(), ritz_hist);
+  for (;;) {
+    // step 2: residuals
+    int nu = 0;
+    std::vector<int> U;
+    for (int i = 0; i < nb; ++i) {
+      for (int j = 0; j < npw; ++j) R[(long)i * npw + j] = HX[(long)i * npw + j] - eps[i] * X[(long)i * npw + j];
+      rho[i] = nrm2(&R[(long)i * npw], npw);
+      if (rho[i] > tol) U.push_back(i);
+    }
+    nu = (int)U.size();
+    if (nu == 0) { status = 0; break; }
+    if (it >= max_iter) break;
+    // step 3: T_i = K_i R_i (Teter-Payne-Allan)
+    T.assign((long)nu * npw, cplx(0, 0));
+    std::vector<double> tn0(nu);
+    for (int u = 0; u < nu; ++u) {
+      const int i = U[u];
+      double ekin = 0;
+      for (int j = 0; j < npw; ++j) ekin += c->g2[j] * std::norm(X[(long)i * npw + j]);
+      ekin = std::max(ekin, 1e-3);
+      for (int j = 0; j < npw; ++j) {
+        const double x = c->g2[j] / ekin;
+        const double nx = 27.0 + 18.0 * x + 12.0 * x * x + 8.0 * x * x * x;
+        const double K = nx / (nx + 16.0 * x * x * x * x);
+        T[(long)u * npw + j] = K * R[(long)i * npw + j];
+      }
+      tn0[u] = nrm2(&T[(long)u * npw], npw);
+    }
+    // step 4: restart
+    if (m + nu > mmax) { V = X; W = HX; m = nb; }
+    // step 5: project out V (twice) and the kept T's (MGS, twice); drop rule
+    int kept = 0;
+    for (int u = 0; u < nu; ++u) {
+      cplx* t = &T[(long)u * npw];
+      for (int pass = 0; pass < 2; ++pass) {
+        for (int r = 0; r < m; ++r) caxpy(-cdot(&V[(long)r * npw], t, npw), &V[(long)r * npw], t, npw);
+        for (int r = 0; r < kept; ++r) caxpy(-cdot(&T[(long)r * npw], t, npw), &T[(long)r * npw], t, npw);
+      }
+      const double n1 = nrm2(t, npw);
+      if (!(n1 >= 1e-10 * tn0[u]) || tn0[u] == 0.0) continue;   // dependent: drop
+      cplx* dst = &T[(long)kept * npw];
+      for (int j = 0; j < npw; ++j) dst[j] = t[j] / n1;
+      ++kept;
+    }
+    nu = kept;
+    if (nu == 0) break;   // KS_NOTCONV
+    // step 6: expand
+    std::vector<cplx> HT((long)nu * npw);
+    kso_hpsi(c, T.data(), HT.data(), nu);
+    nh += nu;
+    V.insert(V.end(), T.begin(), T.begin() + (long)nu * npw);
+    W.insert(W.end(), HT.begin(), HT.end());
+    m += nu;
+    // step 7: Rayleigh-Ritz
+    rayleigh_ritz(npw, m, nb, V, W, X, HX, eps);
+    ++it;
+    if (ritz_hist) std::copy(eps.begin(), eps.end(), ritz_hist + (long)it * nb);
+  }
+  std::memcpy(psi, X.data(), (long)nb * npw * sizeof(cplx));
+  std::copy(eps.begin(), eps.end(), eig);
+  if (resid) std::copy(rho.begin(), rho.end(), resid);
+  if (iters_out) *iters_out = it;
+  if (nhpsi_out) *nhpsi_out = nh;
+  return status;
+}

@@ -1,0 +1,319 @@
+"""Pins for the CPU oracle (oracle/kso.cpp) against what the paper's definitions and the
+mathematics fix -- never against itself.  All CPU; see SURVEY.md §8(c.4).
+
+Citations: PAPER.md Eq. 31 L502 (PW expansion, +i sign), Eq. 32 L507 (KS equation in PW basis),
+Eq. 36 L531 (-i sign, 1/N), Eq. 3-4 L217-221 (KB nonlocal), Fig. 10 L549-570 (residual, K)."""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_2501_08697_b200 import inputs as I
+
+GOLD = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "survey_c5.json")))
+
+
+# ----------------------------------------------------------------------------- FFT
+def _direct_dft3(a, sign):
+    """O(n^2) per axis, dense DFT matrices written from the definition."""
+    out = a.astype(np.complex128)
+    for ax, n in enumerate(a.shape):
+        j = np.arange(n)
+        F = np.exp(sign * 2j * np.pi * np.outer(j, j) / n)
+        out = np.moveaxis(np.tensordot(F, np.moveaxis(out, ax, 0), axes=(1, 0)), 0, ax)
+    return out
+
+
+@pytest.mark.parametrize("shape", [(6, 4, 9), (3, 2, 5), (1, 7, 8), (12, 1, 27), (10, 14, 2)])
+@pytest.mark.parametrize("sign", [1, -1])
+def test_fft_vs_direct_dft(oracle_mod, shape, sign):
+    rng = np.random.default_rng(1)
+    a = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+    got = oracle_mod.fft3d(a, sign)
+    assert np.abs(got - _direct_dft3(a, sign)).max() < 1e-12
+    lib = np.fft.ifftn(a) * a.size if sign == 1 else np.fft.fftn(a)
+    assert np.abs(got - lib).max() < 1e-12
+
+
+def test_fft_delta_planewave_parseval_roundtrip(oracle_mod):
+    n = (24, 18, 16)
+    m = (5, -3, 2)
+    a = np.zeros(n, dtype=np.complex128)
+    a[m[0] % n[0], m[1] % n[1], m[2] % n[2]] = 1.0
+    r = oracle_mod.fft3d(a, +1)           # Eq. 31: a single coefficient -> e^{+i G.r}
+    j = np.meshgrid(*[np.arange(k) for k in n], indexing="ij")
+    pw = np.exp(2j * np.pi * sum(m[i] * j[i] / n[i] for i in range(3)))
+    assert np.abs(r - pw).max() < 1e-13
+    back = oracle_mod.fft3d(pw, -1) / a.size   # Eq. 36: plane wave -> a single delta
+    assert np.abs(back - a).max() < 1e-13
+    rng = np.random.default_rng(2)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    X = oracle_mod.fft3d(x, -1)
+    assert abs(np.vdot(X, X).real - x.size * np.vdot(x, x).real) < 1e-9 * x.size
+    assert np.abs(oracle_mod.fft3d(X, +1) - x.size * x).max() < 1e-9
+
+
+# ----------------------------------------------------------------------------- G sphere
+@pytest.mark.parametrize("c,npw", [(0, 515), (1, 37073), (3, 124289), (4, 110907)])
+def test_pw_counts(oracle_mod, c, npw):
+    cfg = I.config(c)
+    mil, g2 = oracle_mod.pw_list(cfg.cell, cfg.kpts[0], cfg.ecutwfc)
+    assert mil.shape[0] == npw == GOLD["npw"][str(c)]
+    omega = abs(np.linalg.det(cfg.cell))
+    est = omega * cfg.ecutwfc ** 1.5 / (6 * math.pi ** 2)     # volume of the sphere / (2pi)^3/Omega
+    assert abs(npw - est) < 6.0 * npw ** (2.0 / 3.0) ** 1.0 * 0.1 + 30
+    s = set(map(tuple, mil.tolist()))
+    assert all((-a, -b, -d) in s for (a, b, d) in s)          # Gamma: inversion symmetric
+    assert (g2 <= cfg.ecutwfc).all() and g2.min() == 0.0
+    assert np.min(np.abs(g2 - cfg.ecutwfc)) > 1e-3            # reading C2: <= vs < cannot matter
+
+
+def test_pw_list_matches_generator_and_order(oracle_mod):
+    cfg = I.config(2)
+    counts = []
+    for ik in (0, 21, 42, 63):
+        mil, g2 = oracle_mod.pw_list(cfg.cell, cfg.kpts[ik], cfg.ecutwfc)
+        m2, g22, _ = I.pw_list(cfg.cell, cfg.kpts[ik], cfg.ecutwfc)
+        assert np.array_equal(mil, m2) and np.abs(g2 - g22).max() < 1e-12
+        key = (mil[:, 0].astype(np.int64) * 1000 + mil[:, 1]) * 1000 + mil[:, 2]
+        assert (np.diff(key) > 0).all()                        # m1 slowest, m3 fastest, ascending
+        counts.append(mil.shape[0])
+    assert counts[0] == 8459 and counts[1] == 8487
+    assert GOLD["npw"]["2_min"] <= min(counts) and max(counts) <= GOLD["npw"]["2_max"]
+    # non-orthogonal cell, k != 0: brute force over a big box
+    cell = np.array([[5.0, 0.3, 0.0], [0.0, 4.0, 0.7], [0.5, 0.0, 6.0]])
+    k = (0.21, -0.4, 0.33)
+    mil, g2 = oracle_mod.pw_list(cell, k, 7.0)
+    b = 2 * np.pi * np.linalg.inv(cell).T
+    rr = np.arange(-12, 13)
+    mm = np.array(np.meshgrid(rr, rr, rr, indexing="ij")).reshape(3, -1).T
+    q = (mm + np.array(k)) @ b
+    keep = (q ** 2).sum(1) <= 7.0
+    assert np.array_equal(mil, mm[keep].astype(np.int32))
+
+
+# ----------------------------------------------------------------------------- potential
+def test_cfg0_inputs_and_vr(oracle_mod):
+    p = I.make_problem(0)
+    g = GOLD["cfg0"]
+    assert np.abs(p.tau - np.array(g["tau"])).max() < 1e-11
+    assert abs(p.vloc_g[0, 0, 0].real - g["vhat0"]) < 1e-11
+    o = oracle_mod.Oracle.from_problem(p)
+    vr = o.vr()
+    assert abs(vr.min() - g["vr_min"]) < 1e-8
+    # V(r) against the real-space sum of Gaussian wells (minimum image +-1 cells), reading C6/C7:
+    n = 24
+    x = np.arange(n) * 10.0 / n
+    R = np.stack(np.meshgrid(x, x, x, indexing="ij"), -1)
+    ref = np.zeros((n, n, n))
+    for t in p.tau:
+        for s in np.array(np.meshgrid(*[[-1, 0, 1]] * 3, indexing="ij")).reshape(3, -1).T:
+            d = R - t - 10.0 * s
+            ref += -I.A_LOC * np.exp(-(d ** 2).sum(-1) / (2 * I.SIGMA_LOC ** 2))
+    assert np.abs(vr - ref).max() < 2e-5 * np.abs(ref).max()
+
+
+def _tiny(with_beta=True, **kw):
+    return I.make_problem(0, ecutwfc=4.0, grid=(16, 16, 16), nbands=4, with_beta=with_beta, **kw)
+
+
+def test_local_identity_and_shift(oracle_mod):
+    p = _tiny(with_beta=False)
+    v = np.zeros(p.vloc_g.shape, dtype=np.complex128)
+    v[0, 0, 0] = 1.0                                            # V(r) == 1
+    o = oracle_mod.Oracle(p.cell, p.k_frac, p.ecutwfc, p.grid, v)
+    hp = o.hpsi(p.psi0)
+    assert np.abs(hp - (p.g2 + 1.0) * p.psi0).max() < 1e-13
+    # V_hat = delta_{m,m0} + delta_{m,-m0}  (real V = 2 cos(G0.r)): local term is psi(G-G0)+psi(G+G0)
+    m0 = np.array([1, -2, 1])
+    v[:] = 0
+    v[tuple(m0 % 16)] = 1.0
+    v[tuple((-m0) % 16)] = 1.0
+    o = oracle_mod.Oracle(p.cell, p.k_frac, p.ecutwfc, p.grid, v)
+    hp = o.hpsi(p.psi0) - p.g2 * p.psi0
+    look = {tuple(m): j for j, m in enumerate(p.miller.tolist())}
+    ref = np.zeros_like(p.psi0)
+    for j, m in enumerate(p.miller):
+        for sgn in (1, -1):
+            src = look.get(tuple((m - sgn * m0).tolist()))
+            if src is not None:
+                ref[:, j] += p.psi0[:, src]
+    assert np.abs(hp - ref).max() < 1e-13
+
+
+def _explicit_h_numpy(p):
+    """Eq. 32 + Eq. 4 entry by entry (vectorised indexing), independent of kso_explicit_h."""
+    n = p.grid
+    d = p.miller[:, None, :] - p.miller[None, :, :]
+    H = p.vloc_g[d[..., 0] % n[0], d[..., 1] % n[1], d[..., 2] % n[2]].copy()
+    H[np.diag_indices(p.npw)] += p.g2
+    for a in range(p.natom):
+        p0, p1 = p.proj_offset[a], p.proj_offset[a + 1]
+        npj = p1 - p0
+        Da = p.D[sum((p.proj_offset[i + 1] - p.proj_offset[i]) ** 2 for i in range(a)):][: npj * npj].reshape(npj, npj)
+        b = p.beta[p0:p1]                                      # [np][npw]
+        H += b.T @ Da @ b.conj()
+    return H
+
+
+@pytest.mark.parametrize("which", ["tiny", "s2", "s4"])
+def test_hpsi_equals_explicit_h(oracle_mod, which):
+    p = _tiny() if which == "tiny" else I.make_shrunk(which, nbands=3)
+    o = oracle_mod.Oracle.from_problem(p)
+    Hn = _explicit_h_numpy(p)
+    assert np.abs(Hn - Hn.conj().T).max() < 1e-14
+    Ho = o.explicit_h()
+    assert np.abs(Ho - Hn).max() < 1e-13
+    hp = o.hpsi(p.psi0)
+    ref = p.psi0 @ Hn.T
+    assert np.linalg.norm(hp - ref) / np.linalg.norm(ref) < 1e-13
+
+
+def test_hermiticity_and_nonlocal_closed_forms(oracle_mod):
+    p = I.make_shrunk("s2", nbands=2)
+    o = oracle_mod.Oracle.from_problem(p)
+    rng = np.random.default_rng(5)
+    phi = rng.standard_normal((2, p.npw)) + 1j * rng.standard_normal((2, p.npw))
+    a = np.vdot(phi[0], o.hpsi(phi[1:2])[0])
+    b = np.vdot(phi[1], o.hpsi(phi[0:1])[0])
+    assert abs(a - np.conj(b)) < 1e-11 * abs(a)
+    # single projector, V=0: H psi - g2 psi = D beta (beta^H psi)
+    v0 = np.zeros(p.vloc_g.shape, dtype=np.complex128)
+    o1 = oracle_mod.Oracle(p.cell, p.k_frac, p.ecutwfc, p.grid, v0, p.beta[2:3], np.array([0, 1], np.int32), np.array([-0.7]))
+    full = o1.hpsi(phi)
+    ref = -0.7 * np.outer(phi @ p.beta[2].conj(), p.beta[2])
+    assert np.abs(ref).max() > 1e-6
+    assert np.abs(full - p.g2 * phi - ref).max() < 1e-14 * np.abs(full).max()
+    # p-triplet closed form (pins the generator's Y_1m): sum_m beta_1m(q) conj(beta_1m(q')) =
+    #   (3/(4 pi Omega)) (q.q') exp(-rc^2 (q^2+q'^2)/2) exp(-i (q-q').tau)
+    _, _, q = I.pw_list(p.cell, p.k_frac, p.ecutwfc)
+    omega = abs(np.linalg.det(p.cell))
+    trip = p.beta[2:5]                                          # atom 0, p(rc=1.0): rows 2,3,4
+    lhs = trip.T @ trip.conj()
+    q2 = (q ** 2).sum(1)
+    rhs = (3 / (4 * np.pi * omega)) * (q @ q.T) * np.exp(-0.5 * (q2[:, None] + q2[None, :])) \
+        * np.exp(-1j * ((q @ p.tau[0])[:, None] - (q @ p.tau[0])[None, :]))
+    assert np.abs(lhs - rhs).max() < 1e-15
+    # rank of the nonlocal part <= P
+    o2 = oracle_mod.Oracle(p.cell, p.k_frac, p.ecutwfc, p.grid, v0, p.beta, p.proj_offset, p.D)
+    Hnl = o2.explicit_h() - np.diag(p.g2)
+    assert np.linalg.matrix_rank(Hnl, tol=1e-10) <= p.nproj
+
+
+def test_translation_and_time_reversal(oracle_mod):
+    # rigid translation of all atoms: H' = U H U^H, spectrum unchanged (exact)
+    cfg = I.config(2)
+    ecut, grid = 6.0, (20, 20, 20)
+    k = np.array(cfg.kpts[5])
+    t = np.array([0.37, -1.1, 2.2])
+    ev = []
+    for shift, kk in ((0 * t, k), (t, k), (0 * t, -k)):
+        tau = I._diamond_sites(1) + shift
+        m, g2, q = I.pw_list(cfg.cell, kk, ecut)
+        v = I.vloc_g(cfg.cell, tau, grid, 4 * ecut)
+        beta, off, D = I.projectors(cfg.cell, tau, cfg.channels, q)
+        o = oracle_mod.Oracle(cfg.cell, kk, ecut, grid, v, beta, off, D)
+        ev.append(np.linalg.eigvalsh(o.explicit_h()))
+    assert np.abs(ev[0] - ev[1]).max() < 1e-11
+    assert np.abs(ev[0] - ev[2]).max() < 1e-11                  # eps(k) = eps(-k)
+
+
+# ----------------------------------------------------------------------------- Jacobi
+def test_jacobi_2x2_closed_form(oracle_mod):
+    a, g, bta = 1.3, -0.4, 0.8 - 0.6j
+    th, Cm, _ = oracle_mod.jacobi(np.array([[a, bta], [np.conj(bta), g]]))
+    mid, rad = 0.5 * (a + g), math.hypot(0.5 * (a - g), abs(bta))
+    assert np.abs(th - np.array([mid - rad, mid + rad])).max() < 1e-15
+
+
+@pytest.mark.parametrize("n", [1, 2, 7, 40])
+def test_jacobi_random_hermitian(oracle_mod, n):
+    rng = np.random.default_rng(n)
+    A = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+    A = A + A.conj().T
+    if n == 7:
+        A[:, 3] = A[:, 2]; A[3, :] = A[2, :]; A[3, 3] = A[2, 2]   # rank deficiency / degenerate pair
+    th, Cm, sweeps = oracle_mod.jacobi(A)
+    assert np.abs(A @ Cm - Cm * th).max() < 1e-13 * max(1.0, np.abs(A).max()) * n
+    assert np.abs(Cm.conj().T @ Cm - np.eye(n)).max() < 1e-13
+    assert np.abs(th - np.linalg.eigvalsh(A)).max() < 1e-13 * n
+    assert (np.diff(th) >= 0).all() and sweeps < 30
+
+
+def test_jacobi_diagonal_returns_itself(oracle_mod):
+    d = np.array([3.0, -1.0, 2.0, 0.0])
+    th, Cm, sweeps = oracle_mod.jacobi(np.diag(d).astype(np.complex128))
+    assert np.array_equal(th, np.sort(d)) and sweeps == 0
+    assert np.abs(np.abs(Cm) - np.eye(4)[:, np.argsort(d)]).max() == 0
+
+
+# ----------------------------------------------------------------------------- Davidson
+def test_davidson_free_electron_exact(oracle_mod):
+    """north_star: V_loc = 0, no projectors => eigenvalues are the sorted |k+G|^2 exactly."""
+    p = I.make_problem(0, with_beta=False, with_vloc=False, nbands=8)
+    o = oracle_mod.Oracle.from_problem(p)
+    r = o.davidson(p.psi0, tol=1e-9)
+    assert r["converged"]
+    assert np.abs(r["eig"] - np.sort(p.g2)[:8]).max() < 1e-12
+    lev = (2 * np.pi / 10.0) ** 2
+    assert abs(lev - GOLD["cfg0"]["free_levels"][1][0]) < 1e-11
+    assert np.abs(r["eig"] - np.array([0] + [lev] * 6 + [2 * lev])).max() < 1e-12
+    # constant potential shifts every eigenvalue by that constant (north_star)
+    v = np.zeros(p.vloc_g.shape, dtype=np.complex128)
+    v[0, 0, 0] = -0.321
+    o2 = oracle_mod.Oracle(p.cell, p.k_frac, p.ecutwfc, p.grid, v)
+    r2 = o2.davidson(p.psi0, tol=1e-9)
+    assert np.abs(r2["eig"] - (r["eig"] - 0.321)).max() < 1e-12
+
+
+def test_davidson_cfg0_vs_bruteforce_and_survey(oracle_mod):
+    p = I.make_problem(0)
+    o = oracle_mod.Oracle.from_problem(p)
+    r = o.davidson(p.psi0, tol=1e-8, history=True)
+    assert r["converged"] and r["resid"].max() <= 1e-8
+    w = np.linalg.eigvalsh(_explicit_h_numpy(p))
+    assert np.abs(r["eig"] - w[:8]).max() < 1e-12
+    assert np.abs(w[:10] - np.array(GOLD["cfg0"]["eig10"])).max() < 2e-12
+    X = r["psi"]
+    assert np.abs(X.conj() @ X.T - np.eye(8)).max() < 1e-12
+    hx = o.hpsi(X)
+    assert np.abs(np.linalg.norm(hx - r["eig"][:, None] * X, axis=1) - r["resid"]).max() < 1e-12
+    # Ritz values decrease monotonically and bound the exact ones from above (Cauchy interlacing)
+    h = r["ritz_hist"]
+    assert (np.diff(h, axis=0) <= 1e-12).all() and (h >= w[:8] - 1e-12).all()
+    assert r["nhpsi"] == 168 and r["iters"] in (31, 32)         # 168 band-applications
+    # subspace never larger than 2 nb is implied by nhpsi bookkeeping; 3 nb converges in fewer steps
+    r3 = o.davidson(p.psi0, tol=1e-8, max_sub_factor=3)
+    assert r3["iters"] < r["iters"] and np.abs(r3["eig"] - w[:8]).max() < 1e-12
+
+
+def test_davidson_small_vs_oracle_jacobi_bruteforce(oracle_mod):
+    """Brute force entirely without numpy.linalg: oracle Jacobi on the oracle's explicit H."""
+    p = I.make_problem(0, ecutwfc=5.0, grid=(18, 18, 18), nbands=6)
+    o = oracle_mod.Oracle.from_problem(p)
+    th, Cm, _ = oracle_mod.jacobi(o.explicit_h())
+    r = o.davidson(p.psi0, tol=1e-9)
+    assert r["converged"] and np.abs(r["eig"] - th[:6]).max() < 1e-12
+    assert np.abs(th - np.linalg.eigvalsh(_explicit_h_numpy(p))).max() < 1e-12
+
+
+@pytest.mark.parametrize("name", ["s1", "s2", "s3", "s4"])
+def test_davidson_shrunk_vs_bruteforce(oracle_mod, name):
+    p = I.make_shrunk(name)
+    o = oracle_mod.Oracle.from_problem(p)
+    w = np.linalg.eigvalsh(o.explicit_h())
+    r = o.davidson(p.psi0, tol=1e-8)
+    nb = p.nbands
+    assert r["converged"] and r["resid"].max() <= 1e-8
+    gap = max(w[nb] - w[nb - 1], 1e-3)
+    assert np.abs(r["eig"] - w[:nb]).max() < max(1e-12, (1e-8) ** 2 / gap * 10)
+    assert np.abs(r["psi"].conj() @ r["psi"].T - np.eye(nb)).max() < 1e-12
+
+
+def test_davidson_max_iter_reports_not_converged(oracle_mod):
+    p = I.make_problem(0)
+    o = oracle_mod.Oracle.from_problem(p)
+    r = o.davidson(p.psi0, tol=1e-8, max_iter=3)
+    assert not r["converged"] and r["iters"] == 3 and r["resid"].max() > 1e-8
