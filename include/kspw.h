@@ -1,0 +1,106 @@
+/* kspw.h -- C ABI of libkspw.so: plane-wave Kohn-Sham H*psi and block-Davidson on one B200 (sm_100a).
+ *
+ * What the calls compute is fixed by arxiv 2501.08697 (ABACUS review; /root/reference/PAPER.md):
+ *   - plane-wave expansion psi_nk(r) = sum_G c_nk(G) e^{i(k+G).r}                  Eq. 31
+ *   - KS equation in the PW basis: kinetic (k+G)^2 delta_GG' + V(G-G')            Eq. 32
+ *     (Rydberg atomic units here: |k+G|^2, no 1/2 -- DESIGN.md reading C1)
+ *   - norm-conserving nonlocal part V_KB = sum D_ll' |beta_lm><beta_l'm'|          Eq. 3-4
+ *   - H*psi = FFTs + BLAS, the expensive step of iterative diagonalization         L572-574
+ *   - Davidson iterative diagonalization (named only; listing = DESIGN.md §3)     L326, L547, L578
+ *   - r->G transform sign and 1/N normalisation                                   Eq. 36
+ *
+ * Conventions:
+ *   ks_c128      interleaved complex128 (re, im).
+ *   PW order     m1 slowest, m3 fastest, each ascending over the sphere |k+G|^2 <= ecutwfc (C2, C3);
+ *                ks_pw_list returns exactly this order; psi / hpsi / beta use it.
+ *   Block layout psi[nbands][npw], band-major (a band is a contiguous vector).
+ *   Grid layout  [n1][n2][n3], n3 fastest, FFT index order (m mod n) -- only vloc_g uses it (C5).
+ *   HOST / DEVICE is stated per pointer.  Every call returns int: 0 ok, >0 soft status, <0 error.
+ *   Nothing here throws or aborts; ks_last_error() gives the text of the last failure.
+ *   All device work is enqueued on the context's stream (default: the legacy default stream).
+ *   There is no CPU fallback: without a CUDA device ks_create returns KS_ECUDA.
+ */
+#ifndef KSPW_H
+#define KSPW_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ks_ctx ks_ctx;              /* opaque, owned by the library */
+typedef struct { double re, im; } ks_c128;
+
+#define KS_OK        0
+#define KS_NOTCONV   1   /* ks_davidson: max_iter reached; best X, eps, residuals still written */
+#define KS_EINVAL   -1   /* bad argument */
+#define KS_EGRID    -2   /* grid violates n_i > 2 m_psi,i + m_V,i, n_i > 2 m_V,i, or size unsupported */
+#define KS_ENOMEM   -3   /* device or host allocation failed / shared memory budget exceeded */
+#define KS_ECUDA    -4   /* CUDA runtime error (no device, launch failure, ...) */
+#define KS_EVLOC    -5   /* V(r) not real within 1e-12 max|V| */
+
+/* ---- pure host helpers (no GPU needed): the G sphere of Eq. 31 ------------------------------- */
+/* cell: HOST [9], rows a1 a2 a3 (bohr).  k_frac: HOST [3], k in units of b1 b2 b3.  ecutwfc in Ry. */
+int ks_pw_count(const double cell[9], const double k_frac[3], double ecutwfc, int* npw /*HOST out*/);
+/* miller: HOST out [npw][3];  g2: HOST out [npw] = |k+G|^2 (Ry), may be NULL. */
+int ks_pw_list(const double cell[9], const double k_frac[3], double ecutwfc, int* miller, double* g2);
+
+/* ---- context: one k-point -------------------------------------------------------------------- */
+/* All inputs are HOST arrays and are copied; the caller may free them on return.
+ *   grid        n1 n2 n3; each must be one of ks_supported_sizes() and satisfy the alias rule.
+ *   vloc_g      [n1][n2][n3] Fourier-series coefficients of V_loc (Eq. 32's V(G-G')), FFT index order.
+ *   beta        [nproj][npw], ks_pw_list order (Eq. 4's |beta_lm>, as beta(k+G)).  nproj may be 0.
+ *   proj_offset [natom+1], projector rows of atom a are proj_offset[a] .. proj_offset[a+1]-1.
+ *   D           concatenated per-atom real symmetric blocks, atom a's block is np_a x np_a row-major. */
+int ks_create(ks_ctx** out, const double cell[9], const double k_frac[3], double ecutwfc,
+              const int grid[3], const ks_c128* vloc_g, int nproj, const ks_c128* beta, int natom,
+              const int* proj_offset, const double* D);
+void ks_destroy(ks_ctx* ctx);
+int ks_npw(const ks_ctx* ctx);
+int ks_set_stream(ks_ctx* ctx, void* cuda_stream /* cudaStream_t; NULL = default stream */);
+/* number of bands per FFT batch (0 = automatic, sized so one batch of planes stays L2-resident) */
+int ks_set_fft_batch(ks_ctx* ctx, int nbatch);
+const char* ks_last_error(const ks_ctx* ctx);   /* ctx may be NULL: last ks_create failure */
+/* writes up to cap supported FFT lengths to sizes (HOST), returns how many exist */
+int ks_supported_sizes(int* sizes, int cap);
+
+/* ---- the hot path ---------------------------------------------------------------------------- */
+/* hpsi = H psi for a block of bands (steps H1-H8 of DESIGN.md §1).
+ * psi, hpsi: DEVICE [nbands][npw], caller-owned, must not alias.  Asynchronous on the stream. */
+int ks_hpsi(ks_ctx* ctx, const ks_c128* psi, ks_c128* hpsi, int nbands);
+/* same through HOST buffers (copies H2D / D2H inside, synchronises before returning) */
+int ks_hpsi_host(ks_ctx* ctx, const ks_c128* psi_host, ks_c128* hpsi_host, int nbands);
+
+/* Lowest nbands eigenpairs by block Davidson (steps D0-D9), subspace <= 2 nbands, S = I.
+ *   psi    DEVICE [nbands][npw]  in: start vectors (any full-rank block), out: orthonormal eigvecs
+ *   eig    DEVICE [nbands] out, ascending (Ry)
+ *   resid  DEVICE [nbands] out, ||H x_i - eps_i x_i||_2, may be NULL
+ *   tol    convergence: every residual norm <= tol;  max_iter: subspace expansions allowed
+ *   iters_out, band_applications_out: HOST out, may be NULL
+ * Synchronises the stream once per iteration (reads nbands residual norms back). */
+int ks_davidson(ks_ctx* ctx, ks_c128* psi, double* eig, int nbands, double tol, int max_iter,
+                double* resid, int* iters_out, long long* band_applications_out);
+int ks_davidson_host(ks_ctx* ctx, ks_c128* psi_host, double* eig_host, int nbands, double tol,
+                     int max_iter, double* resid_host, int* iters_out,
+                     long long* band_applications_out);
+/* per-phase device time of the last ks_davidson, milliseconds, HOST out [8]:
+ * hpsi, projection GEMMs, eigensolves, rotation GEMMs, residual+precondition, orthonormalise GEMMs,
+ * total, reserved.  Only filled when KSPW_PROFILE=1 is set in the environment (adds syncs). */
+int ks_davidson_profile(const ks_ctx* ctx, double* ms);
+
+/* ---- building blocks, exported for unit parity tests and the roofline microbenchmarks -------- */
+/* C[M][N] (column-major, ldc) = A^H B;  A: DEVICE K x M column-major lda, B: K x N column-major ldb. */
+int ks_zgemm_hn(void* stream, int M, int N, int K, const ks_c128* A, long lda, const ks_c128* B,
+                long ldb, ks_c128* C, long ldc);
+/* C[M][N] (column-major) = A B (accumulate=0) or C += A B (accumulate=1); A: M x K, B: K x N. */
+int ks_zgemm_nn(void* stream, int M, int N, int K, const ks_c128* A, long lda, const ks_c128* B,
+                long ldb, ks_c128* C, long ldc, int accumulate);
+/* Hermitian eigenproblem A = C diag(theta) C^H by (block) Jacobi.  A: DEVICE n x n column-major (lda),
+ * destroyed; theta: DEVICE [n] ascending; C: DEVICE n x n column-major (ldc), column i <-> theta[i]. */
+int ks_eigh(void* stream, int n, ks_c128* A, long lda, double* theta, ks_c128* C, long ldc,
+            int* sweeps_out /*HOST, may be NULL*/);
+/* register-resident DMMA m8n8k4 microbenchmark: achieved FP64 tensor TFLOP/s (roofline denominator) */
+int ks_dmma_peak(double* tflops_out /*HOST*/, double* dfma_tflops_out /*HOST, plain DFMA, may be NULL*/);
+#ifdef __cplusplus
+}
+#endif
+#endif /* KSPW_H */

@@ -1,0 +1,347 @@
+// davidson.cu -- block Davidson for the lowest nbands eigenpairs of H psi = eps psi, S = I
+// (DESIGN.md §3 listing, steps D0-D9; the paper names the method at PAPER.md L326, L547, L578 and prints
+// no listing; the residual p - lambda psi and the preconditioner K are Fig. 10, `vecdiv` L578).
+//
+// Everything runs on the device; the host only sequences launches and reads nbands residual norms (and
+// the Gram-matrix eigenvalues of the orthonormalisation) back per iteration.
+//   D0  X = orth(psi0)                        Gram matrix + Jacobi eigh (canonical orthonormalisation) x2
+//   D1  W = H V                               ks_hpsi_impl on the new block only
+//   D2  Hc[:, new] = V^H W_new                DMMA GEMM (K = npw), mirrored to keep Hc Hermitian
+//   D3  Hc = C Theta C^H                      Jacobi (eigh.cu)
+//   D4  X = V C[:, :nb], HX = W C[:, :nb]     DMMA GEMMs (M = npw)
+//   D5  rho_i = ||HX_i - eps_i X_i||, Ekin_i  fused reduction, one CTA per band
+//   D6  T_i = K_i (HX_i - eps_i X_i)          Teter-Payne-Allan diagonal polynomial, fused, unconverged only
+//   D7  T <- (I - V V^H) T (x2, x1) ; T <- T U Lambda^{-1/2}, dropping lambda < 1e-10 lambda_max ; twice
+//   D8  V <- [V, T], restart V <- X when m + nu > 2 nb
+//   D9  psi <- X, eig, residuals
+// Difference from the oracle listing (reading C10): the orthonormalisation is Gram/eigh based instead of
+// modified Gram-Schmidt.  Both span the same space up to the drop rule; the converged pairs agree.
+#include "ctx.h"
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <vector>
+
+#define RED_THREADS 256
+
+__device__ __forceinline__ double block_sum(double v, double* sh) {
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+  __syncthreads();
+  double s = 0;
+  if (threadIdx.x < 32) {
+    s = (threadIdx.x < blockDim.x / 32) ? sh[threadIdx.x] : 0.0;
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  }
+  __syncthreads();
+  return s;   // valid in thread 0
+}
+
+// D5: rho_i = ||HX_i - eps_i X_i||_2 , ekin_i = sum_G g2 |X_i|^2
+__global__ void __launch_bounds__(RED_THREADS) k_resid_norms(int npw, const cplx* __restrict__ X, const cplx* __restrict__ HX,
+                                                             const double* __restrict__ eps, const double* __restrict__ g2,
+                                                             double* __restrict__ rho, double* __restrict__ ekin) {
+  __shared__ double sh[RED_THREADS / 32];
+  const int i = blockIdx.x;
+  const cplx* x = X + (size_t)i * npw;
+  const cplx* h = HX + (size_t)i * npw;
+  const double e = eps[i];
+  double r2 = 0, ek = 0;
+  for (int j = threadIdx.x; j < npw; j += blockDim.x) {
+    const cplx a = x[j], b = h[j];
+    const double rx = b.x - e * a.x, ry = b.y - e * a.y;
+    r2 += rx * rx + ry * ry;
+    ek += g2[j] * (a.x * a.x + a.y * a.y);
+  }
+  r2 = block_sum(r2, sh);
+  ek = block_sum(ek, sh);
+  if (threadIdx.x == 0) { rho[i] = sqrt(r2); ekin[i] = ek; }
+}
+
+// D6: T_u = K_i (HX_i - eps_i X_i), i = idx[u];  K = n(x)/(n(x) + 16 x^4), n = 27 + 18x + 12x^2 + 8x^3,
+// x = g2 / max(ekin_i, 1e-3)   (Teter-Payne-Allan; reading C11)
+__global__ void k_precond(int npw, int nu, const int* __restrict__ idx, const cplx* __restrict__ X, const cplx* __restrict__ HX,
+                          const double* __restrict__ eps, const double* __restrict__ ekin, const double* __restrict__ g2,
+                          cplx* __restrict__ T) {
+  const int u = blockIdx.y, i = idx[u];
+  const double e = eps[i], ek = fmax(ekin[i], 1e-3);
+  for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < npw; j += gridDim.x * blockDim.x) {
+    const cplx a = X[(size_t)i * npw + j], b = HX[(size_t)i * npw + j];
+    const double x = g2[j] / ek;
+    const double nx = 27.0 + 18.0 * x + 12.0 * x * x + 8.0 * x * x * x;
+    const double K = nx / (nx + 16.0 * x * x * x * x);
+    T[(size_t)u * npw + j] = cmake(K * (b.x - e * a.x), K * (b.y - e * a.y));
+  }
+}
+
+// column 2-norms of a block, then scaling to unit norm
+__global__ void __launch_bounds__(RED_THREADS) k_col_norm2(int npw, const cplx* __restrict__ T, double* __restrict__ out) {
+  __shared__ double sh[RED_THREADS / 32];
+  const cplx* t = T + (size_t)blockIdx.x * npw;
+  double s = 0;
+  for (int j = threadIdx.x; j < npw; j += blockDim.x) { const cplx a = t[j]; s += a.x * a.x + a.y * a.y; }
+  s = block_sum(s, sh);
+  if (threadIdx.x == 0) out[blockIdx.x] = s;
+}
+__global__ void k_col_scale(int npw, cplx* __restrict__ T, const double* __restrict__ n2) {
+  const double nn = n2[blockIdx.y];
+  const double s = nn > 0.0 ? rsqrt(nn) : 0.0;
+  const double sc = nn > 0.0 ? s * (1.5 - 0.5 * nn * s * s) : 0.0;   // one Newton step on rsqrt: full FP64 accuracy
+  cplx* t = T + (size_t)blockIdx.y * npw;
+  for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < npw; j += gridDim.x * blockDim.x) t[j] = cscale(sc, t[j]);
+}
+
+// small-matrix helpers (column-major)
+__global__ void k_negate(long n, cplx* __restrict__ a) {
+  const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (i < n) a[i] = cmake(-a[i].x, -a[i].y);
+}
+__global__ void k_set_diag(int m, long ld, cplx* __restrict__ H, const double* __restrict__ d) {
+  const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (e >= (long)m * m) return;
+  const int i = (int)(e % m), j = (int)(e / m);
+  H[(long)j * ld + i] = cmake(i == j ? d[i] : 0.0, 0.0);
+}
+// after the new columns Hc[0:m1, m0:m1] were written: mirror them into the rows and symmetrise the corner
+__global__ void k_mirror(int m0, int m1, long ld, cplx* __restrict__ H) {
+  const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  const int nn = m1 - m0;
+  if (e >= (long)m1 * nn) return;
+  const int i = (int)(e % m1), j = m0 + (int)(e / m1);
+  if (i < m0) {
+    const cplx a = H[(long)j * ld + i];
+    H[(long)i * ld + j] = cconj(a);
+  } else if (i <= j) {
+    const cplx a = H[(long)j * ld + i], b = H[(long)i * ld + j];
+    const cplx s = cmake(0.5 * (a.x + b.x), (i == j) ? 0.0 : 0.5 * (a.y - b.y));
+    H[(long)j * ld + i] = s;
+    H[(long)i * ld + j] = cconj(s);
+  }
+}
+__global__ void k_copy_mat(int m, int n, const cplx* __restrict__ a, long lda, cplx* __restrict__ b, long ldb) {
+  const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (e >= (long)m * n) return;
+  const int i = (int)(e % m), j = (int)(e / m);
+  b[(long)j * ldb + i] = a[(long)j * lda + i];
+}
+// Mout[:, r] = U[:, r0 + r] / sqrt(lam[r0 + r]),  r < nk   (canonical orthonormalisation)
+__global__ void k_canon(int nu, int r0, int nk, const cplx* __restrict__ U, long ldu, const double* __restrict__ lam,
+                        cplx* __restrict__ Mout, long ldm) {
+  const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (e >= (long)nu * nk) return;
+  const int i = (int)(e % nu), r = (int)(e / nu);
+  const double s = 1.0 / sqrt(lam[r0 + r]);
+  Mout[(long)r * ldm + i] = cscale(s, U[(long)(r0 + r) * ldu + i]);
+}
+
+// ------------------------------------------------------------------------------------------------
+void ks_davidson_free(DavidsonWs* w) {
+  cudaFree(w->V); cudaFree(w->W); cudaFree(w->X); cudaFree(w->HX); cudaFree(w->T);
+  cudaFree(w->Hc); cudaFree(w->Cm); cudaFree(w->Hwork); cudaFree(w->S); cudaFree(w->Us);
+  cudaFree(w->theta); cudaFree(w->rho); cudaFree(w->ekin); cudaFree(w->lam); cudaFree(w->idx);
+  *w = DavidsonWs();
+}
+
+static int reserve(ks_ctx* c, int nb) {
+  DavidsonWs& w = c->dws;
+  if (nb <= w.nb_cap) return KS_OK;
+  ks_davidson_free(&w);
+  const size_t npw = c->P.npw, vb = sizeof(cplx) * npw;
+  const size_t m = 2 * (size_t)nb;
+  KS_CUDA_CHECK(cudaMalloc(&w.V, vb * m), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.W, vb * m), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.X, vb * nb), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.HX, vb * nb), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.T, vb * nb), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.Hc, sizeof(cplx) * m * m), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.Cm, sizeof(cplx) * m * m), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.Hwork, sizeof(cplx) * m * m), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.S, sizeof(cplx) * m * nb), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.Us, sizeof(cplx) * (size_t)nb * nb), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.theta, sizeof(double) * m), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.rho, sizeof(double) * nb), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.ekin, sizeof(double) * nb), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.lam, sizeof(double) * nb), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.idx, sizeof(int) * nb), c->err);
+  w.nb_cap = nb;
+  return KS_OK;
+}
+
+struct Phase {   // optional per-phase timing (KSPW_PROFILE=1): adds a stream sync per phase
+  bool on = false;
+  cudaEvent_t a = nullptr, b = nullptr;
+  cudaStream_t st = 0;
+  double* acc = nullptr;
+  void init(cudaStream_t s, double* ms) {
+    const char* e = getenv("KSPW_PROFILE");
+    on = e && atoi(e) > 0;
+    st = s; acc = ms;
+    for (int i = 0; i < 8; ++i) ms[i] = 0;
+    if (on) { cudaEventCreate(&a); cudaEventCreate(&b); }
+  }
+  void begin() { if (on) cudaEventRecord(a, st); }
+  void end(int ph) {
+    if (!on) return;
+    cudaEventRecord(b, st);
+    cudaEventSynchronize(b);
+    float ms = 0;
+    cudaEventElapsedTime(&ms, a, b);
+    acc[ph] += ms;
+  }
+  void done() { if (on) { cudaEventDestroy(a); cudaEventDestroy(b); } }
+};
+enum { PH_HPSI = 0, PH_PROJ = 1, PH_EIGH = 2, PH_ROT = 3, PH_RESID = 4, PH_ORTH = 5, PH_TOTAL = 6 };
+
+#define RC(x) do { int rc__ = (x); if (rc__ < 0) return rc__; } while (0)
+
+// One pass of D7/D0:  src (npw x nu) -> dst (npw x nk): optional projection against V[0:m] (nproj times),
+// unit column norms, Gram matrix, Jacobi eigh, drop lambda < 1e-10 lambda_max, dst = src U Lambda^{-1/2}.
+static int orth_pass(ks_ctx* c, cplx* src, int nu, cplx* dst, int m, int nproj_pass, int* nk_out, Phase& ph) {
+  DavidsonWs& w = c->dws;
+  const int npw = c->P.npw;
+  cudaStream_t st = c->stream;
+  ph.begin();
+  for (int p = 0; p < nproj_pass && m > 0; ++p) {
+    RC(ks_gemm_hn(st, m, nu, npw, w.V, npw, src, npw, w.S, m, &c->gws, c->err));
+    k_negate<<<ceil_div((long)m * nu, 256), 256, 0, st>>>((long)m * nu, w.S);
+    RC(ks_gemm_nn(st, npw, nu, m, w.V, npw, w.S, m, src, npw, 1, c->err));
+  }
+  k_col_norm2<<<nu, RED_THREADS, 0, st>>>(npw, src, w.lam);
+  k_col_scale<<<dim3(std::max(1, std::min(64, ceil_div(npw, 1024))), nu), 256, 0, st>>>(npw, src, w.lam);
+  RC(ks_gemm_hn(st, nu, nu, npw, src, npw, src, npw, w.Us, nu, &c->gws, c->err));
+  ph.end(PH_ORTH);
+  ph.begin();
+  RC(ks_eigh_run(st, nu, w.Us, nu, w.lam, w.S, nu, &c->ews, nullptr, c->err));   // S <- eigenvectors (nu x nu)
+  std::vector<double> lam(nu);
+  KS_CUDA_CHECK(cudaMemcpyAsync(lam.data(), w.lam, sizeof(double) * nu, cudaMemcpyDeviceToHost, st), c->err);
+  KS_CUDA_CHECK(cudaStreamSynchronize(st), c->err);
+  ph.end(PH_EIGH);
+  const double lmax = lam[nu - 1];
+  int r0 = 0;
+  while (r0 < nu && !(lam[r0] > 1e-10 * lmax)) ++r0;
+  const int nk = nu - r0;
+  *nk_out = nk;
+  if (nk == 0) return KS_OK;
+  ph.begin();
+  k_canon<<<ceil_div((long)nu * nk, 256), 256, 0, st>>>(nu, r0, nk, w.S, nu, w.lam, w.Us, nu);
+  RC(ks_gemm_nn(st, npw, nk, nu, src, npw, w.Us, nu, dst, npw, 0, c->err));
+  ph.end(PH_ORTH);
+  return KS_OK;
+}
+
+int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int max_iter, double* resid, int* iters_out,
+                     long long* nhpsi_out) {
+  if (!c) return KS_EINVAL;
+  const int npw = c->P.npw;
+  if (!psi || !eig || nb < 1 || nb > npw || !(tol > 0) || max_iter < 0) { c->err = "ks_davidson: bad argument"; return KS_EINVAL; }
+  RC(reserve(c, nb));
+  DavidsonWs& w = c->dws;
+  cudaStream_t st = c->stream;
+  const size_t vb = sizeof(cplx) * (size_t)npw;
+  const long ldh = 2L * nb;
+  Phase ph, tot;
+  ph.init(st, c->prof_ms);
+  double dummy[8];
+  tot.init(st, dummy);
+  tot.acc = c->prof_ms;
+  tot.begin();
+
+  // D0: orthonormalise the start block (two canonical passes)
+  int nk = 0;
+  KS_CUDA_CHECK(cudaMemcpyAsync(w.T, psi, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
+  RC(orth_pass(c, w.T, nb, w.X, 0, 0, &nk, ph));
+  if (nk < nb) { c->err = "ks_davidson: start block is rank deficient"; return KS_EINVAL; }
+  RC(orth_pass(c, w.X, nb, w.V, 0, 0, &nk, ph));
+  if (nk < nb) { c->err = "ks_davidson: start block is rank deficient"; return KS_EINVAL; }
+  // D1-D4: initial Rayleigh-Ritz
+  ph.begin();
+  RC(ks_hpsi_impl(c, w.V, w.W, nb));
+  ph.end(PH_HPSI);
+  long long nh = nb;
+  ph.begin();
+  RC(ks_gemm_hn(st, nb, nb, npw, w.V, npw, w.W, npw, w.Hwork, nb, &c->gws, c->err));
+  ph.end(PH_PROJ);
+  ph.begin();
+  RC(ks_eigh_run(st, nb, w.Hwork, nb, w.theta, w.Cm, ldh, &c->ews, nullptr, c->err));
+  ph.end(PH_EIGH);
+  ph.begin();
+  RC(ks_gemm_nn(st, npw, nb, nb, w.V, npw, w.Cm, ldh, w.X, npw, 0, c->err));
+  RC(ks_gemm_nn(st, npw, nb, nb, w.W, npw, w.Cm, ldh, w.HX, npw, 0, c->err));
+  KS_CUDA_CHECK(cudaMemcpyAsync(w.V, w.X, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
+  KS_CUDA_CHECK(cudaMemcpyAsync(w.W, w.HX, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
+  k_set_diag<<<ceil_div((long)nb * nb, 256), 256, 0, st>>>(nb, ldh, w.Hc, w.theta);
+  ph.end(PH_ROT);
+  int m = nb, it = 0, status = KS_NOTCONV;
+  std::vector<double> rho(nb);
+  std::vector<int> idx(nb);
+  for (;;) {
+    // D5
+    ph.begin();
+    k_resid_norms<<<nb, RED_THREADS, 0, st>>>(npw, w.X, w.HX, w.theta, c->P.d_g2, w.rho, w.ekin);
+    KS_CUDA_CHECK(cudaMemcpyAsync(rho.data(), w.rho, sizeof(double) * nb, cudaMemcpyDeviceToHost, st), c->err);
+    KS_CUDA_CHECK(cudaStreamSynchronize(st), c->err);
+    ph.end(PH_RESID);
+    int nu = 0;
+    for (int i = 0; i < nb; ++i)
+      if (!(rho[i] <= tol)) idx[nu++] = i;
+    if (nu == 0) { status = KS_OK; break; }
+    if (it >= max_iter) break;
+    // D8 (restart)
+    if (m + nu > 2 * nb) {
+      KS_CUDA_CHECK(cudaMemcpyAsync(w.V, w.X, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
+      KS_CUDA_CHECK(cudaMemcpyAsync(w.W, w.HX, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
+      k_set_diag<<<ceil_div((long)nb * nb, 256), 256, 0, st>>>(nb, ldh, w.Hc, w.theta);
+      m = nb;
+    }
+    // D6
+    ph.begin();
+    KS_CUDA_CHECK(cudaMemcpyAsync(w.idx, idx.data(), sizeof(int) * nu, cudaMemcpyHostToDevice, st), c->err);
+    k_precond<<<dim3(std::max(1, std::min(64, ceil_div(npw, 1024))), nu), 256, 0, st>>>(npw, nu, w.idx, w.X, w.HX, w.theta, w.ekin,
+                                                                                      c->P.d_g2, w.T);
+    ph.end(PH_RESID);
+    // D7: two passes; the result lands in V[m : m+nk]
+    cplx* Vnew = w.V + (size_t)m * npw;
+    RC(orth_pass(c, w.T, nu, Vnew, m, 2, &nk, ph));
+    if (nk == 0) break;
+    int nk2 = 0;
+    RC(orth_pass(c, Vnew, nk, w.T, m, 1, &nk2, ph));
+    if (nk2 == 0) break;
+    nk = nk2;
+    KS_CUDA_CHECK(cudaMemcpyAsync(Vnew, w.T, vb * nk, cudaMemcpyDeviceToDevice, st), c->err);
+    // D1
+    cplx* Wnew = w.W + (size_t)m * npw;
+    ph.begin();
+    RC(ks_hpsi_impl(c, Vnew, Wnew, nk));
+    ph.end(PH_HPSI);
+    nh += nk;
+    // D2
+    ph.begin();
+    const int m1 = m + nk;
+    RC(ks_gemm_hn(st, m1, nk, npw, w.V, npw, Wnew, npw, w.Hc + (size_t)m * ldh, ldh, &c->gws, c->err));
+    k_mirror<<<ceil_div((long)m1 * nk, 256), 256, 0, st>>>(m, m1, ldh, w.Hc);
+    ph.end(PH_PROJ);
+    m = m1;
+    // D3
+    ph.begin();
+    k_copy_mat<<<ceil_div((long)m * m, 256), 256, 0, st>>>(m, m, w.Hc, ldh, w.Hwork, m);
+    RC(ks_eigh_run(st, m, w.Hwork, m, w.theta, w.Cm, ldh, &c->ews, nullptr, c->err));
+    ph.end(PH_EIGH);
+    // D4
+    ph.begin();
+    RC(ks_gemm_nn(st, npw, nb, m, w.V, npw, w.Cm, ldh, w.X, npw, 0, c->err));
+    RC(ks_gemm_nn(st, npw, nb, m, w.W, npw, w.Cm, ldh, w.HX, npw, 0, c->err));
+    ph.end(PH_ROT);
+    ++it;
+  }
+  // D9
+  KS_CUDA_CHECK(cudaMemcpyAsync(psi, w.X, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
+  KS_CUDA_CHECK(cudaMemcpyAsync(eig, w.theta, sizeof(double) * nb, cudaMemcpyDeviceToDevice, st), c->err);
+  if (resid) KS_CUDA_CHECK(cudaMemcpyAsync(resid, w.rho, sizeof(double) * nb, cudaMemcpyDeviceToDevice, st), c->err);
+  KS_CUDA_CHECK(cudaStreamSynchronize(st), c->err);
+  tot.end(PH_TOTAL);
+  ph.done();
+  tot.done();
+  if (iters_out) *iters_out = it;
+  if (nhpsi_out) *nhpsi_out = nh;
+  return status;
+}

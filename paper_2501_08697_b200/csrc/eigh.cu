@@ -1,0 +1,420 @@
+// eigh.cu -- Jacobi Hermitian eigensolver for the subspace matrix (DESIGN.md step D3) and for the
+// Gram matrices of the orthonormalisation (D0, D7).  The paper is silent on the subspace solver
+// (north_star: "a Jacobi-style Hermitian eigensolver kernel"); the oracle uses cyclic-by-row Jacobi,
+// this file uses parallel (round-robin) ordering -- the results agree to round-off.
+//
+//   n <= 64   one CTA: A and the accumulated rotations V live in shared memory; every round applies
+//             n/2 disjoint complex Givens rotations (two-sided), n-1 rounds per sweep.
+//   n  > 64   two-sided BLOCK Jacobi with 32-wide blocks: every round solves nblk/2 independent 64x64
+//             pair problems with the one-CTA kernel (a few inner sweeps), then applies the 64x64
+//             unitary blocks U to the columns of A and V and the rows of A as 64x64x64 complex GEMM
+//             tiles on the FP64 tensor path (DMMA).
+// Rotation for pivot (p,q), a_pq = |a_pq| e^{i phi}:  J = diag(1, e^{-i phi}) [[c, s], [-s, c]],
+// tau = (a_qq - a_pp)/(2|a_pq|), t = sign(tau)/(|tau| + sqrt(1 + tau^2))  (same formula as the oracle).
+#include "mma.cuh"
+#include "plan.h"
+#include <algorithm>
+#include <vector>
+
+#define JB 32            // block size of the block method
+#define JS (2 * JB)      // pair problem size
+#define JTHREADS 512
+#define JPAD 1.0e30      // diagonal of padding rows: decoupled (zero off-diagonals) and sorts last
+
+// round-robin pair k of round r for n (even) players: (n-1, r) for k = 0, else ((r+k) % (n-1), (r-k) % (n-1))
+__host__ __device__ __forceinline__ void rr_pair(int n, int r, int k, int* p, int* q) {
+  int a, b;
+  if (k == 0) { a = n - 1; b = r; }
+  else { a = (r + k) % (n - 1); b = (r - k + (n - 1)) % (n - 1); }
+  *p = a < b ? a : b;
+  *q = a < b ? b : a;
+}
+
+// ------------------------------------------------------------------------------------------------
+// one CTA per pair problem.  ns = 2*nbk (even, <= 64).  Gathers rows/cols {I*nbk.., J*nbk..} of Ap.
+// U (ns x ns, column-major, ld = ns) receives the accumulated rotations; dout (nullable) the diagonal.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(JTHREADS) k_jacobi_cta(const cplx* __restrict__ Ap, long ld, int nbk,
+                                                        const int2* __restrict__ pairs, cplx* __restrict__ U,
+                                                        double* __restrict__ dout, int max_sweeps, double tol2) {
+  extern __shared__ cplx sm[];
+  const int ns = 2 * nbk, LD = ns + 1;
+  cplx* As = sm;                       // As[i*LD + j] = A[i][j]
+  cplx* Vs = As + ns * LD;
+  double* rc = (double*)(Vs + ns * LD);        // c[k]
+  double* rs = rc + JS / 2;                    // s[k]
+  cplx* re = (cplx*)(rs + JS / 2);             // e^{i phi}[k]
+  __shared__ double red[2][JTHREADS / 32];
+  __shared__ int stop;
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const int2 pr = pairs[blockIdx.x];
+  for (int e = tid; e < ns * ns; e += nt) {
+    const int i = e % ns, j = e / ns;    // column-major global read: consecutive threads -> consecutive rows
+    const int gi = (i < nbk ? pr.x * nbk + i : pr.y * nbk + i - nbk);
+    const int gj = (j < nbk ? pr.x * nbk + j : pr.y * nbk + j - nbk);
+    As[i * LD + j] = Ap[(long)gj * ld + gi];
+    Vs[i * LD + j] = cmake(i == j ? 1.0 : 0.0, 0.0);
+  }
+  __syncthreads();
+  for (int sweep = 0; sweep < max_sweeps; ++sweep) {
+    // convergence: off(A)_F^2 <= tol2 * ||A||_F^2 (padding rows excluded through their zero off-diagonals
+    // and by capping the diagonal contribution)
+    double off = 0, tot = 0;
+    for (int e = tid; e < ns * ns; e += nt) {
+      const int i = e / ns, j = e % ns;
+      const cplx a = As[i * LD + j];
+      const double v = a.x * a.x + a.y * a.y;
+      if (i != j) { off += v; tot += v; }
+      else if (fabs(a.x) < 0.5 * JPAD) tot += v;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+      off += __shfl_xor_sync(0xffffffffu, off, o);
+      tot += __shfl_xor_sync(0xffffffffu, tot, o);
+    }
+    if ((tid & 31) == 0) { red[0][tid >> 5] = off; red[1][tid >> 5] = tot; }
+    __syncthreads();
+    if (tid == 0) {
+      double a = 0, b = 0;
+      for (int w = 0; w < nt / 32; ++w) { a += red[0][w]; b += red[1][w]; }
+      stop = (a <= tol2 * b) ? 1 : 0;
+    }
+    __syncthreads();
+    if (stop) break;
+    for (int r = 0; r < ns - 1; ++r) {
+      if (tid < ns / 2) {
+        int p, q;
+        rr_pair(ns, r, tid, &p, &q);
+        const cplx apq = As[p * LD + q];
+        const double ab = sqrt(apq.x * apq.x + apq.y * apq.y);
+        double c = 1.0, s = 0.0;
+        cplx e = cmake(1.0, 0.0);
+        if (ab > 0.0) {
+          const double tau = (As[q * LD + q].x - As[p * LD + p].x) / (2.0 * ab);
+          const double t = (tau >= 0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
+          c = 1.0 / sqrt(1.0 + t * t);
+          s = t * c;
+          e = cmake(apq.x / ab, apq.y / ab);
+        }
+        rc[tid] = c; rs[tid] = s; re[tid] = e;
+      }
+      __syncthreads();
+      // columns of A and V:  x' = c x - s conj(e) y ,  y' = s x + c conj(e) y
+      for (int it = tid; it < (ns / 2) * ns; it += nt) {
+        const int i = it % ns, k = it / ns;
+        int p, q;
+        rr_pair(ns, r, k, &p, &q);
+        const double c = rc[k], s = rs[k];
+        const cplx ec = cconj(re[k]);
+        {
+          const cplx x = As[i * LD + p], y = cmul(ec, As[i * LD + q]);
+          As[i * LD + p] = cmake(c * x.x - s * y.x, c * x.y - s * y.y);
+          As[i * LD + q] = cmake(s * x.x + c * y.x, s * x.y + c * y.y);
+        }
+        {
+          const cplx x = Vs[i * LD + p], y = cmul(ec, Vs[i * LD + q]);
+          Vs[i * LD + p] = cmake(c * x.x - s * y.x, c * x.y - s * y.y);
+          Vs[i * LD + q] = cmake(s * x.x + c * y.x, s * x.y + c * y.y);
+        }
+      }
+      __syncthreads();
+      // rows of A:  x' = c x - s e y ,  y' = s x + c e y
+      for (int it = tid; it < (ns / 2) * ns; it += nt) {
+        const int j = it % ns, k = it / ns;
+        int p, q;
+        rr_pair(ns, r, k, &p, &q);
+        const double c = rc[k], s = rs[k];
+        const cplx x = As[p * LD + j], y = cmul(re[k], As[q * LD + j]);
+        As[p * LD + j] = cmake(c * x.x - s * y.x, c * x.y - s * y.y);
+        As[q * LD + j] = cmake(s * x.x + c * y.x, s * x.y + c * y.y);
+      }
+      __syncthreads();
+      if (tid < ns / 2) {
+        int p, q;
+        rr_pair(ns, r, tid, &p, &q);
+        if (rs[tid] != 0.0) {
+          As[p * LD + q] = cmake(0.0, 0.0);
+          As[q * LD + p] = cmake(0.0, 0.0);
+        }
+        As[p * LD + p].y = 0.0;
+        As[q * LD + q].y = 0.0;
+      }
+      __syncthreads();
+    }
+  }
+  cplx* Uo = U + (size_t)blockIdx.x * ns * ns;
+  for (int e = tid; e < ns * ns; e += nt) {
+    const int i = e % ns, j = e / ns;
+    Uo[(size_t)j * ns + i] = Vs[i * LD + j];
+  }
+  if (dout)
+    for (int i = tid; i < ns; i += nt) dout[(size_t)blockIdx.x * ns + i] = As[i * LD + i].x;
+}
+
+// ------------------------------------------------------------------------------------------------
+// block updates: 64 x 64 x 64 complex GEMM tiles on DMMA, 8 warps as 2 (M) x 4 (N), warp tile 32 x 16
+// ------------------------------------------------------------------------------------------------
+#define JLDM (JS + 2)    // m-contiguous tile, == 2 (mod 8)
+#define JLDK (JS + 4)    // k-contiguous tile, == 4 (mod 8)
+
+__device__ __forceinline__ int blk_index(int2 pr, int i) { return i < JB ? pr.x * JB + i : pr.y * JB + i - JB; }
+
+// columns: X[:, IJ] <- X[:, IJ] U   for X = A (z = 0) and X = V (z = 1); rows m0 .. m0+63
+__global__ void __launch_bounds__(256) k_jac_col(cplx* __restrict__ Ap, cplx* __restrict__ Vp, long ld,
+                                                 const int2* __restrict__ pairs, const cplx* __restrict__ U) {
+  extern __shared__ cplx sm[];
+  cplx* sP = sm;                   // [k][m]
+  cplx* sU = sm + JS * JLDM;       // [n][k]
+  cplx* X = blockIdx.z ? Vp : Ap;
+  const int2 pr = pairs[blockIdx.y];
+  const int m0 = blockIdx.x * JS, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const cplx* Up = U + (size_t)blockIdx.y * JS * JS;
+  for (int e = tid; e < JS * JS; e += 256) {
+    const int a = e % JS, b = e / JS;
+    sP[b * JLDM + a] = X[(long)blk_index(pr, b) * ld + m0 + a];   // k = b (column), m = a
+    sU[b * JLDK + a] = Up[e];                                      // n = b, k = a
+  }
+  __syncthreads();
+  const int wm = warp & 1, wn = warp >> 1, fr = lane >> 2, fk = lane & 3;
+  double cre[4][2][2], cim[4][2][2];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 2; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
+#pragma unroll 4
+  for (int ks = 0; ks < JS; ks += 4) {
+    cplx af[4], bf[2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) af[i] = sP[(ks + fk) * JLDM + wm * 32 + i * 8 + fr];
+#pragma unroll
+    for (int j = 0; j < 2; ++j) bf[j] = sU[(wn * 16 + j * 8 + fr) * JLDK + ks + fk];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const double nai = -af[i].y;
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        dmma(cre[i][j][0], cre[i][j][1], af[i].x, bf[j].x);
+        dmma(cim[i][j][0], cim[i][j][1], af[i].x, bf[j].y);
+        dmma(cre[i][j][0], cre[i][j][1], nai, bf[j].y);
+        dmma(cim[i][j][0], cim[i][j][1], af[i].y, bf[j].x);
+      }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int m = m0 + wm * 32 + i * 8 + fr, n = wn * 16 + j * 8 + 2 * fk + h;
+        X[(long)blk_index(pr, n) * ld + m] = cmake(cre[i][j][h], cim[i][j][h]);
+      }
+}
+
+// rows: A[IJ, :] <- U^H A[IJ, :]   for columns n0 .. n0+63
+__global__ void __launch_bounds__(256) k_jac_row(cplx* __restrict__ Ap, long ld, const int2* __restrict__ pairs,
+                                                 const cplx* __restrict__ U) {
+  extern __shared__ cplx sm[];
+  cplx* sU = sm;                   // [m][k]  (U column m)
+  cplx* sB = sm + JS * JLDK;       // [n][k]  (A[IJ(k)][n0+n])
+  const int2 pr = pairs[blockIdx.y];
+  const int n0 = blockIdx.x * JS, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const cplx* Up = U + (size_t)blockIdx.y * JS * JS;
+  for (int e = tid; e < JS * JS; e += 256) {
+    const int a = e % JS, b = e / JS;
+    sU[b * JLDK + a] = Up[e];
+    sB[b * JLDK + a] = Ap[(long)(n0 + b) * ld + blk_index(pr, a)];
+  }
+  __syncthreads();
+  const int wm = warp & 1, wn = warp >> 1, fr = lane >> 2, fk = lane & 3;
+  double cre[4][2][2], cim[4][2][2];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 2; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
+#pragma unroll 4
+  for (int ks = 0; ks < JS; ks += 4) {
+    cplx af[4], bf[2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) af[i] = sU[(wm * 32 + i * 8 + fr) * JLDK + ks + fk];
+#pragma unroll
+    for (int j = 0; j < 2; ++j) bf[j] = sB[(wn * 16 + j * 8 + fr) * JLDK + ks + fk];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const double nai = -af[i].y;
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {   // conj(u) a
+        dmma(cre[i][j][0], cre[i][j][1], af[i].x, bf[j].x);
+        dmma(cim[i][j][0], cim[i][j][1], af[i].x, bf[j].y);
+        dmma(cre[i][j][0], cre[i][j][1], af[i].y, bf[j].y);
+        dmma(cim[i][j][0], cim[i][j][1], nai, bf[j].x);
+      }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int m = wm * 32 + i * 8 + fr, n = n0 + wn * 16 + j * 8 + 2 * fk + h;
+        Ap[(long)n * ld + blk_index(pr, m)] = cmake(cre[i][j][h], cim[i][j][h]);
+      }
+}
+
+// ------------------------------------------------------------------------------------------------
+// small helpers
+// ------------------------------------------------------------------------------------------------
+__global__ void k_pad_copy(const cplx* __restrict__ A, long lda, int n, cplx* __restrict__ Ap, cplx* __restrict__ Vp, int np) {
+  const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (e >= (long)np * np) return;
+  const int i = (int)(e % np), j = (int)(e / np);
+  cplx v = cmake(0.0, 0.0);
+  if (i < n && j < n) {
+    // Hermitian part of the input: (A + A^H)/2, diagonal real
+    const cplx a = A[(long)j * lda + i], b = A[(long)i * lda + j];
+    v = cmake(0.5 * (a.x + b.x), 0.5 * (a.y - b.y));
+  } else if (i == j) {
+    v = cmake(JPAD, 0.0);
+  }
+  Ap[e] = v;
+  if (Vp) Vp[e] = cmake(i == j ? 1.0 : 0.0, 0.0);
+}
+__global__ void k_offnorm(const cplx* __restrict__ Ap, int np, int n, double* __restrict__ red) {
+  double off = 0, tot = 0;
+  for (long e = blockIdx.x * (long)blockDim.x + threadIdx.x; e < (long)np * np; e += (long)gridDim.x * blockDim.x) {
+    const int i = (int)(e % np), j = (int)(e / np);
+    if (i < n && j < n) {
+      const cplx a = Ap[e];
+      const double v = a.x * a.x + a.y * a.y;
+      tot += v;
+      if (i != j) off += v;
+    }
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    off += __shfl_xor_sync(0xffffffffu, off, o);
+    tot += __shfl_xor_sync(0xffffffffu, tot, o);
+  }
+  if ((threadIdx.x & 31) == 0) { atomicAdd(&red[0], off); atomicAdd(&red[1], tot); }
+}
+__global__ void k_diag(const cplx* __restrict__ Ap, int np, double* __restrict__ d) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < np) d[i] = Ap[(long)i * np + i].x;
+}
+// rank by counting (ties by index): order[rank] = i, theta[rank] = d[i] for rank < n
+__global__ void k_rank(const double* __restrict__ d, int np, int n, int* __restrict__ order, double* __restrict__ theta) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= np) return;
+  const double di = d[i];
+  int r = 0;
+  for (int j = 0; j < np; ++j) {
+    const double dj = d[j];
+    r += (dj < di || (dj == di && j < i)) ? 1 : 0;
+  }
+  order[r] = i;
+  if (r < n) theta[r] = di;
+}
+__global__ void k_gather_cols(const cplx* __restrict__ Vp, int np, const int* __restrict__ order, int n,
+                              cplx* __restrict__ C, long ldc) {
+  const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (e >= (long)n * n) return;
+  const int i = (int)(e % n), r = (int)(e / n);
+  C[(long)r * ldc + i] = Vp[(long)order[r] * np + i];
+}
+
+void ks_eigh_free(EighWs* ws) {
+  cudaFree(ws->U); cudaFree(ws->Ap); cudaFree(ws->Vp); cudaFree(ws->diag); cudaFree(ws->red);
+  cudaFree(ws->order); cudaFree(ws->pairs);
+  *ws = EighWs();
+}
+
+static int eigh_reserve(EighWs* ws, int np, std::string& err) {
+  if (np > ws->cap) {
+    cudaFree(ws->U); cudaFree(ws->Ap); cudaFree(ws->Vp); cudaFree(ws->diag); cudaFree(ws->order);
+    ws->U = ws->Ap = ws->Vp = nullptr; ws->diag = nullptr; ws->order = nullptr; ws->cap = 0;
+    const size_t nu = std::max<size_t>((size_t)(np / JS + 1) * JS * JS, (size_t)JS * JS);
+    KS_CUDA_CHECK(cudaMalloc(&ws->U, sizeof(cplx) * nu), err);
+    KS_CUDA_CHECK(cudaMalloc(&ws->Ap, sizeof(cplx) * (size_t)np * np), err);
+    KS_CUDA_CHECK(cudaMalloc(&ws->Vp, sizeof(cplx) * (size_t)np * np), err);
+    KS_CUDA_CHECK(cudaMalloc(&ws->diag, sizeof(double) * np), err);
+    KS_CUDA_CHECK(cudaMalloc(&ws->order, sizeof(int) * np), err);
+    ws->cap = np;
+  }
+  if (!ws->red) KS_CUDA_CHECK(cudaMalloc(&ws->red, 2 * sizeof(double)), err);
+  return KS_OK;
+}
+
+int ks_eigh_run(cudaStream_t st, int n, cplx* A, long lda, double* theta, cplx* C, long ldc, EighWs* ws,
+                int* sweeps_out, std::string& err) {
+  if (n <= 0) return KS_OK;
+  if (!ws) { err = "ks_eigh: no workspace"; return KS_EINVAL; }
+  static bool opted = false;
+  const size_t smem_cta = sizeof(cplx) * 2 * JS * (JS + 1) + sizeof(double) * JS + sizeof(cplx) * (JS / 2);
+  const size_t smem_col = sizeof(cplx) * JS * (JLDM + JLDK), smem_row = sizeof(cplx) * 2 * JS * JLDK;
+  if (!opted) {
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_jacobi_cta, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cta), err);
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_jac_col, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_col), err);
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_jac_row, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row), err);
+    opted = true;
+  }
+  const double tol2 = 1e-28;   // off_F <= 1e-14 ||A||_F
+  int sweeps = 0;
+  if (n <= JS) {
+    const int ns = n + (n & 1), nbk = ns / 2;
+    int rc = eigh_reserve(ws, JS, err);
+    if (rc) return rc;
+    if (ws->pairs_nblk != 2) {
+      cudaFree(ws->pairs); ws->pairs = nullptr;
+      KS_CUDA_CHECK(cudaMalloc(&ws->pairs, sizeof(int2)), err);
+      const int2 p01 = make_int2(0, 1);
+      KS_CUDA_CHECK(cudaMemcpyAsync(ws->pairs, &p01, sizeof p01, cudaMemcpyHostToDevice, st), err);
+      KS_CUDA_CHECK(cudaStreamSynchronize(st), err);
+      ws->pairs_nblk = 2;
+    }
+    k_pad_copy<<<ceil_div((long)ns * ns, 256), 256, 0, st>>>(A, lda, n, ws->Ap, nullptr, ns);
+    k_jacobi_cta<<<1, JTHREADS, smem_cta, st>>>(ws->Ap, ns, nbk, ws->pairs, ws->Vp, ws->diag, 40, tol2);
+    k_rank<<<ceil_div(ns, 128), 128, 0, st>>>(ws->diag, ns, n, ws->order, theta);
+    k_gather_cols<<<ceil_div((long)n * n, 256), 256, 0, st>>>(ws->Vp, ns, ws->order, n, C, ldc);
+    KS_CUDA_CHECK(cudaGetLastError(), err);
+    if (sweeps_out) *sweeps_out = -1;   // inner sweeps are not reported back
+    return KS_OK;
+  }
+  int nblk = ceil_div(n, JB);
+  nblk += nblk & 1;
+  const int np = nblk * JB, npair = nblk / 2;
+  int rc = eigh_reserve(ws, np, err);
+  if (rc) return rc;
+  if (ws->pairs_nblk != nblk) {
+    cudaFree(ws->pairs); ws->pairs = nullptr;
+    std::vector<int2> h((size_t)(nblk - 1) * npair);
+    for (int r = 0; r < nblk - 1; ++r)
+      for (int k = 0; k < npair; ++k) {
+        int p, q;
+        rr_pair(nblk, r, k, &p, &q);
+        h[(size_t)r * npair + k] = make_int2(p, q);
+      }
+    KS_CUDA_CHECK(cudaMalloc(&ws->pairs, sizeof(int2) * h.size()), err);
+    KS_CUDA_CHECK(cudaMemcpy(ws->pairs, h.data(), sizeof(int2) * h.size(), cudaMemcpyHostToDevice), err);
+    ws->pairs_nblk = nblk;
+  }
+  k_pad_copy<<<ceil_div((long)np * np, 256), 256, 0, st>>>(A, lda, n, ws->Ap, ws->Vp, np);
+  for (; sweeps < 30; ++sweeps) {
+    double h[2];
+    KS_CUDA_CHECK(cudaMemsetAsync(ws->red, 0, 2 * sizeof(double), st), err);
+    k_offnorm<<<148 * 2, 256, 0, st>>>(ws->Ap, np, n, ws->red);
+    KS_CUDA_CHECK(cudaMemcpyAsync(h, ws->red, sizeof h, cudaMemcpyDeviceToHost, st), err);
+    KS_CUDA_CHECK(cudaStreamSynchronize(st), err);
+    if (h[0] <= tol2 * h[1]) break;
+    for (int r = 0; r < nblk - 1; ++r) {
+      const int2* pr = ws->pairs + (size_t)r * npair;
+      k_jacobi_cta<<<npair, JTHREADS, smem_cta, st>>>(ws->Ap, np, JB, pr, ws->U, nullptr, 6, 1e-30);
+      k_jac_col<<<dim3(np / JS, npair, 2), 256, smem_col, st>>>(ws->Ap, ws->Vp, np, pr, ws->U);
+      k_jac_row<<<dim3(np / JS, npair), 256, smem_row, st>>>(ws->Ap, np, pr, ws->U);
+    }
+  }
+  k_diag<<<ceil_div(np, 128), 128, 0, st>>>(ws->Ap, np, ws->diag);
+  k_rank<<<ceil_div(np, 128), 128, 0, st>>>(ws->diag, np, n, ws->order, theta);
+  k_gather_cols<<<ceil_div((long)n * n, 256), 256, 0, st>>>(ws->Vp, np, ws->order, n, C, ldc);
+  KS_CUDA_CHECK(cudaGetLastError(), err);
+  if (sweeps_out) *sweeps_out = sweeps;
+  return KS_OK;
+}

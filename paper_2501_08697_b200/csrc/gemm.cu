@@ -1,0 +1,317 @@
+// gemm.cu -- complex FP64 GEMMs on the FP64 tensor path (mma.sync m8n8k4 f64 -> SASS DMMA.8x8x4,
+// the only FP64 MMA shape sm_100a has; tcgen05 has no f64 kind).
+//
+//   ks_gemm_hn:  C[M x N] = A^H B   A: K x M, B: K x N column-major, K (= npw) long and contiguous.
+//                Used for beta^H psi (H6), V^H W (D2), V^H T and T^H T (D0, D7).  Split-K over CTAs with a
+//                fixed-order second-pass reduction (deterministic, no atomics).
+//   ks_gemm_nn:  C[M x N] (+)= A B  A: M x K, C: M x N column-major, M (= npw) long and contiguous.
+//                Used for hpsi += beta (D B) (H8), X = V C, HX = W C (D4), T -= V (V^H T) (D7).
+//
+// A complex product is four real DMMAs on split re/im fragments:
+//   C_re += A_re B_re - A_im B_im ,  C_im += A_re B_im + A_im B_re     (signs folded into one negated
+// fragment; for A^H the imaginary part of A is negated instead).
+// Fragment layout of mma.m8n8k4.row.col.f64: lane l holds A[l>>2][l&3], B[l&3][l>>2],
+// C[l>>2][2*(l&3)+{0,1}].  Tiles are staged in shared memory by cp.async (16 B = one complex) in a
+// 3-stage ring; leading dimensions are padded so a quarter-warp's 16-byte loads hit distinct banks.
+#include "mma.cuh"
+#include "plan.h"
+#include <algorithm>
+
+#define GEMM_THREADS 256
+#define GEMM_STAGES 3
+#define KT 16          // complex K elements per stage
+#define LDK (KT + 4)   // "k-contiguous" tile leading dimension: == 4 (mod 8) -> conflict-free fragment loads
+
+// ------------------------------------------------------------------------------------------------
+// C = A^H B.  CTA tile 64 x 64, 8 warps as 2 (M) x 4 (N), warp tile 32 x 16 -> 4 x 2 MMA tiles.
+// ------------------------------------------------------------------------------------------------
+#define HN_MT 64
+#define HN_NT 64
+
+__global__ void __launch_bounds__(GEMM_THREADS) k_gemm_hn(int M, int N, int K, const cplx* __restrict__ A, long lda,
+                                                          const cplx* __restrict__ B, long ldb, cplx* __restrict__ part,
+                                                          int kchunk) {
+  extern __shared__ cplx sm[];
+  cplx* sA = sm;                                     // [stage][HN_MT][LDK]
+  cplx* sB = sm + GEMM_STAGES * HN_MT * LDK;         // [stage][HN_NT][LDK]
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = warp & 1, wn = warp >> 1;
+  const int m0 = blockIdx.y * HN_MT, n0 = blockIdx.x * HN_NT;
+  const int kbeg = blockIdx.z * kchunk, kend = min(K, kbeg + kchunk);
+  const int ntile = (kend - kbeg + KT - 1) / KT;
+
+  auto load_stage = [&](int st, int kt) {
+    const int k0 = kbeg + kt * KT;
+    // 64 columns x 16 k per operand = 1024 elements each; 256 threads -> 4 + 4 per thread
+#pragma unroll
+    for (int r = 0; r < (HN_MT * KT) / GEMM_THREADS; ++r) {
+      const int e = tid + r * GEMM_THREADS, col = e / KT, kk = e % KT;
+      const bool ok = (m0 + col < M) && (k0 + kk < kend);
+      cp16(&sA[(st * HN_MT + col) * LDK + kk], ok ? &A[(long)(m0 + col) * lda + k0 + kk] : A, ok);
+    }
+#pragma unroll
+    for (int r = 0; r < (HN_NT * KT) / GEMM_THREADS; ++r) {
+      const int e = tid + r * GEMM_THREADS, col = e / KT, kk = e % KT;
+      const bool ok = (n0 + col < N) && (k0 + kk < kend);
+      cp16(&sB[(st * HN_NT + col) * LDK + kk], ok ? &B[(long)(n0 + col) * ldb + k0 + kk] : B, ok);
+    }
+  };
+
+  double cre[4][2][2], cim[4][2][2];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 2; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
+
+  for (int s = 0; s < GEMM_STAGES - 1; ++s) {
+    if (s < ntile) load_stage(s, s);
+    cp_commit();
+  }
+  const int fr = lane >> 2, fk = lane & 3;
+  for (int kt = 0; kt < ntile; ++kt) {
+    cp_wait<GEMM_STAGES - 2>();
+    __syncthreads();
+    if (kt + GEMM_STAGES - 1 < ntile) load_stage((kt + GEMM_STAGES - 1) % GEMM_STAGES, kt + GEMM_STAGES - 1);
+    cp_commit();
+    const cplx* a = sA + ((kt % GEMM_STAGES) * HN_MT + wm * 32) * LDK;
+    const cplx* b = sB + ((kt % GEMM_STAGES) * HN_NT + wn * 16) * LDK;
+#pragma unroll
+    for (int ks = 0; ks < KT; ks += 4) {
+      cplx af[4], bf[2];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) af[i] = a[(i * 8 + fr) * LDK + ks + fk];
+#pragma unroll
+      for (int j = 0; j < 2; ++j) bf[j] = b[(j * 8 + fr) * LDK + ks + fk];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const double nai = -af[i].y;
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {   // conj(a) b = (ar br + ai bi) + i (ar bi - ai br)
+          dmma(cre[i][j][0], cre[i][j][1], af[i].x, bf[j].x);
+          dmma(cim[i][j][0], cim[i][j][1], af[i].x, bf[j].y);
+          dmma(cre[i][j][0], cre[i][j][1], af[i].y, bf[j].y);
+          dmma(cim[i][j][0], cim[i][j][1], nai, bf[j].x);
+        }
+      }
+    }
+  }
+  cp_wait<0>();
+  // partial tile -> part[z][n][m] (column-major M x N per split)
+  cplx* out = part + (size_t)blockIdx.z * M * N;
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int m = m0 + wm * 32 + i * 8 + fr, n = n0 + wn * 16 + j * 8 + 2 * fk + h;
+        if (m < M && n < N) out[(size_t)n * M + m] = cmake(cre[i][j][h], cim[i][j][h]);
+      }
+}
+
+__global__ void k_splitk_reduce(int M, int N, int nsplit, const cplx* __restrict__ part, cplx* __restrict__ C, long ldc) {
+  const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (i >= (long)M * N) return;
+  double sr = 0, si = 0;
+  for (int z = 0; z < nsplit; ++z) {   // fixed order: deterministic
+    const cplx p = part[(size_t)z * M * N + i];
+    sr += p.x; si += p.y;
+  }
+  C[(i / M) * ldc + (i % M)] = cmake(sr, si);
+}
+
+int ks_gemm_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
+               long ldc, GemmWs* ws, std::string& err) {
+  if (M <= 0 || N <= 0) return KS_OK;
+  if (K < 0 || !ws) { err = "ks_gemm_hn: bad argument"; return KS_EINVAL; }
+  static bool opted = false;
+  const size_t smem = sizeof(cplx) * GEMM_STAGES * (HN_MT + HN_NT) * LDK;
+  if (!opted) {
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_gemm_hn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err);
+    opted = true;
+  }
+  const int tm = ceil_div(M, HN_MT), tn = ceil_div(N, HN_NT);
+  // split K so that ~4 waves of CTAs exist, each with at least 8 k-tiles
+  int nsplit = std::max(1, std::min(ceil_div(4 * 148 * 2, tm * tn), std::max(1, K / (8 * KT))));
+  int kchunk = ceil_div(std::max(K, 1), nsplit);
+  kchunk = ceil_div(kchunk, KT) * KT;
+  nsplit = std::max(1, ceil_div(std::max(K, 1), kchunk));
+  const size_t need = sizeof(cplx) * (size_t)nsplit * M * N;
+  if (ws->bytes < need) {
+    if (ws->part) cudaFree(ws->part);
+    ws->part = nullptr; ws->bytes = 0;
+    KS_CUDA_CHECK(cudaMalloc(&ws->part, need), err);
+    ws->bytes = need;
+  }
+  dim3 grid(tn, tm, nsplit);
+  k_gemm_hn<<<grid, GEMM_THREADS, smem, st>>>(M, N, K, A, lda, B, ldb, ws->part, kchunk);
+  k_splitk_reduce<<<ceil_div((long)M * N, 256), 256, 0, st>>>(M, N, nsplit, ws->part, C, ldc);
+  KS_CUDA_CHECK(cudaGetLastError(), err);
+  return KS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// C (+)= A B.  CTA tile 128 (M) x 64 (N), 8 warps as 4 (M) x 2 (N), warp tile 32 x 32 -> 4 x 4 MMA tiles.
+// ------------------------------------------------------------------------------------------------
+#define NN_MT 128
+#define NN_NT 64
+#define LDM (NN_MT + 2)   // "m-contiguous" tile leading dimension: == 2 (mod 8)
+
+__global__ void __launch_bounds__(GEMM_THREADS) k_gemm_nn(int M, int N, int K, const cplx* __restrict__ A, long lda,
+                                                          const cplx* __restrict__ B, long ldb, cplx* __restrict__ C,
+                                                          long ldc, int accumulate) {
+  extern __shared__ cplx sm[];
+  cplx* sA = sm;                                   // [stage][KT][LDM]
+  cplx* sB = sm + GEMM_STAGES * KT * LDM;          // [stage][NN_NT][LDK]
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = warp & 3, wn = warp >> 2;
+  const int m0 = blockIdx.x * NN_MT, n0 = blockIdx.y * NN_NT;
+  const int ntile = (K + KT - 1) / KT;
+
+  auto load_stage = [&](int st, int kt) {
+    const int k0 = kt * KT;
+#pragma unroll
+    for (int r = 0; r < (NN_MT * KT) / GEMM_THREADS; ++r) {
+      const int e = tid + r * GEMM_THREADS, kk = e / NN_MT, mm = e % NN_MT;
+      const bool ok = (m0 + mm < M) && (k0 + kk < K);
+      cp16(&sA[(st * KT + kk) * LDM + mm], ok ? &A[(long)(k0 + kk) * lda + m0 + mm] : A, ok);
+    }
+#pragma unroll
+    for (int r = 0; r < (NN_NT * KT) / GEMM_THREADS; ++r) {
+      const int e = tid + r * GEMM_THREADS, col = e / KT, kk = e % KT;
+      const bool ok = (n0 + col < N) && (k0 + kk < K);
+      cp16(&sB[(st * NN_NT + col) * LDK + kk], ok ? &B[(long)(n0 + col) * ldb + k0 + kk] : B, ok);
+    }
+  };
+
+  double cre[4][4][2], cim[4][4][2];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
+
+  for (int s = 0; s < GEMM_STAGES - 1; ++s) {
+    if (s < ntile) load_stage(s, s);
+    cp_commit();
+  }
+  const int fr = lane >> 2, fk = lane & 3;
+  for (int kt = 0; kt < ntile; ++kt) {
+    cp_wait<GEMM_STAGES - 2>();
+    __syncthreads();
+    if (kt + GEMM_STAGES - 1 < ntile) load_stage((kt + GEMM_STAGES - 1) % GEMM_STAGES, kt + GEMM_STAGES - 1);
+    cp_commit();
+    const cplx* a = sA + (kt % GEMM_STAGES) * KT * LDM + wm * 32;
+    const cplx* b = sB + ((kt % GEMM_STAGES) * NN_NT + wn * 32) * LDK;
+#pragma unroll
+    for (int ks = 0; ks < KT; ks += 4) {
+      cplx af[4], bf[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) af[i] = a[(ks + fk) * LDM + i * 8 + fr];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) bf[j] = b[(j * 8 + fr) * LDK + ks + fk];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const double nai = -af[i].y;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {   // a b = (ar br - ai bi) + i (ar bi + ai br)
+          dmma(cre[i][j][0], cre[i][j][1], af[i].x, bf[j].x);
+          dmma(cim[i][j][0], cim[i][j][1], af[i].x, bf[j].y);
+          dmma(cre[i][j][0], cre[i][j][1], nai, bf[j].y);
+          dmma(cim[i][j][0], cim[i][j][1], af[i].y, bf[j].x);
+        }
+      }
+    }
+  }
+  cp_wait<0>();
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int m = m0 + wm * 32 + i * 8 + fr, n = n0 + wn * 32 + j * 8 + 2 * fk + h;
+        if (m < M && n < N) {
+          cplx* p = &C[(long)n * ldc + m];
+          cplx v = cmake(cre[i][j][h], cim[i][j][h]);
+          if (accumulate) { const cplx o = *p; v.x += o.x; v.y += o.y; }
+          *p = v;
+        }
+      }
+}
+
+int ks_gemm_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
+               long ldc, int accumulate, std::string& err) {
+  if (M <= 0 || N <= 0) return KS_OK;
+  if (K < 0) { err = "ks_gemm_nn: bad argument"; return KS_EINVAL; }
+  static bool opted = false;
+  const size_t smem = sizeof(cplx) * GEMM_STAGES * (KT * LDM + NN_NT * LDK);
+  if (!opted) {
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_gemm_nn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err);
+    opted = true;
+  }
+  dim3 grid(ceil_div(M, NN_MT), ceil_div(N, NN_NT));
+  k_gemm_nn<<<grid, GEMM_THREADS, smem, st>>>(M, N, K, A, lda, B, ldb, C, ldc, accumulate);
+  KS_CUDA_CHECK(cudaGetLastError(), err);
+  return KS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Roofline denominators: register-resident DMMA and DFMA loops (no memory traffic).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_dmma_peak(double* out, int iters) {
+  double c[16][2];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) c[i][0] = c[i][1] = 0.0;
+  const double a = 1.0 + 1e-9 * threadIdx.x, b = 1.0 - 1e-9 * threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) dmma(c[i][0], c[i][1], a, b);
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += c[i][0] + c[i][1];
+  if (s == 12345.678) out[0] = s;
+}
+__global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters) {
+  double c[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) c[i] = 1e-3 * i;
+  const double a = 1.0 + 1e-9 * threadIdx.x, b = 1e-9 * threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) c[i] = fma(c[i], a, b);
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += c[i];
+  if (s == 12345.678) out[0] = s;
+}
+
+int ks_peak_run(double* dmma_tf, double* dfma_tf, std::string& err) {
+  double* d = nullptr;
+  KS_CUDA_CHECK(cudaMalloc(&d, 8), err);
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int blocks = 148 * 4, iters = 20000;
+  float best_m = 1e30f, best_f = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0);
+    k_dmma_peak<<<blocks, 256>>>(d, iters);
+    cudaEventRecord(e1);
+    KS_CUDA_CHECK(cudaEventSynchronize(e1), err);
+    float ms; cudaEventElapsedTime(&ms, e0, e1);
+    if (rep) best_m = std::min(best_m, ms);
+    cudaEventRecord(e0);
+    k_dfma_peak<<<blocks, 256>>>(d, iters);
+    cudaEventRecord(e1);
+    KS_CUDA_CHECK(cudaEventSynchronize(e1), err);
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (rep) best_f = std::min(best_f, ms);
+  }
+  // per warp and iteration: 16 DMMA x 512 flop ; per thread and iteration: 16 DFMA x 2 flop
+  const double fl_m = (double)blocks * 8 * iters * 16 * 512.0, fl_f = (double)blocks * 256 * iters * 16 * 2.0;
+  if (dmma_tf) *dmma_tf = fl_m / (best_m * 1e-3) / 1e12;
+  if (dfma_tf) *dfma_tf = fl_f / (best_f * 1e-3) / 1e12;
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+  return KS_OK;
+}

@@ -1,0 +1,437 @@
+// hpsi_kernels.cu -- the dual-space local part of H*psi (DESIGN.md steps H1-H5) as three kernels:
+//
+//   k_inv_yz  per (band, live x-plane): scatter the plane's G-sphere coefficients onto its z-sticks in
+//             shared memory (H1), inverse FFT along z on the sticks only, then along y for the plane
+//             (H2, pruned: PAPER.md Eq. 31, e^{+i}); writes the live plane [y'][z'] once.
+//   k_x       per (band, y', z'-chunk): inverse FFT along x from the live planes (zero fill in shared
+//             memory), multiply by V(r) (H3, Eq. 32), forward FFT along x, write the live planes
+//             back in place.  The full n1*n2*n3 cube never exists in HBM.
+//   k_fwd_yz  per (band, live x-plane): forward FFT along y, keep the stick columns, forward FFT along z
+//             (H4, Eq. 36, e^{-i} and 1/N), gather + kinetic term  hpsi = |k+G|^2 psi + (.)/N  (H5).
+//
+// All intermediates are in "position" order (fft.cuh): type-A transforms leave their output
+// transposed, type-B transforms consume exactly that order, and V(r) is stored permuted once at
+// ks_create, so no reordering pass exists.  Thread mapping is lines-first: consecutive threads work
+// on consecutive lines, whose stride in shared memory is odd (or 1), so the 16-byte accesses of a
+// quarter-warp fall in distinct banks.
+#include "fft.cuh"
+#include "plan.h"
+#include <cmath>
+#include <vector>
+
+
+cudaError_t ks_fft_init_constants() {
+  static bool done = false;
+  if (done) return cudaSuccess;
+  std::vector<double2> w(KS_WTAB);
+  const double PI = 3.14159265358979323846264338327950288;
+  for (int t = 0; t < KS_WTAB; ++t) {
+    // exact quarter-turn symmetry: evaluate in the first octant
+    const double a = 2.0 * PI * (double)t / (double)KS_WTAB;
+    w[t] = make_double2(std::cos(a), std::sin(a));
+  }
+  cudaError_t e = cudaMemcpyToSymbol(c_wtab, w.data(), sizeof(double2) * KS_WTAB);
+  if (e == cudaSuccess) done = true;
+  return e;
+}
+
+// ------------------------------------------------------------------------------------------------
+// supported sizes
+// ------------------------------------------------------------------------------------------------
+#define KS_X_SIZES(X) X(16) X(18) X(24) X(32) X(36) X(48) X(54) X(64) X(72) X(96) X(128)
+#define KS_YZ_PAIRS(X) \
+  X(16, 16) X(18, 18) X(24, 24) X(32, 32) X(36, 36) X(48, 48) X(54, 54) X(64, 64) X(72, 72) \
+  X(96, 96) X(128, 128) X(18, 64) X(96, 288)
+
+void ks_fft_factors(int n, int* R1, int* R2) {
+  *R1 = 0; *R2 = 0;
+  switch (n) {
+#define C_(N_) case N_: *R1 = fac<N_>::R1; *R2 = fac<N_>::R2; break;
+    C_(16) C_(18) C_(24) C_(32) C_(36) C_(48) C_(54) C_(64) C_(72) C_(96) C_(128) C_(144) C_(192) C_(256) C_(288)
+#undef C_
+    default: break;
+  }
+}
+bool ks_fft_size_supported(int n) {
+#define C_(N_) if (n == N_) return true;
+  KS_X_SIZES(C_)
+#undef C_
+  return false;
+}
+bool ks_fft_yz_supported(int n2, int n3) {
+#define C_(A_, B_) if (n2 == A_ && n3 == B_) return true;
+  KS_YZ_PAIRS(C_)
+#undef C_
+  return false;
+}
+int ks_fft_sizes(int* out, int cap) {
+  const int all[] = {
+#define C_(N_) N_,
+      KS_X_SIZES(C_)
+#undef C_
+  };
+  const int n = (int)(sizeof(all) / sizeof(int));
+  for (int i = 0; i < n && i < cap; ++i) out[i] = all[i];
+  return n;
+}
+
+// ------------------------------------------------------------------------------------------------
+// create-time kernels: plain DFT along one axis (O(N n)), permute + realness check
+// ------------------------------------------------------------------------------------------------
+__global__ void k_dft_axis(const cplx* __restrict__ in, cplx* __restrict__ out, long N, int n, long stride,
+                           const cplx* __restrict__ tw) {
+  const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const int k = (int)((i / stride) % n);
+  const long base = i - (long)k * stride;
+  double sr = 0, si = 0;
+  for (int j = 0; j < n; ++j) {
+    const cplx a = in[base + (long)j * stride];
+    const cplx w = tw[(int)(((long)j * k) % n)];
+    sr += a.x * w.x - a.y * w.y;
+    si += a.x * w.y + a.y * w.x;
+  }
+  out[i] = cmake(sr, si);
+}
+
+__global__ void k_vperm(const cplx* __restrict__ v, double* __restrict__ vperm, int n1, int n2, int n3,
+                        int a1, int b1, int a2, int b2, int a3, int b3, double* __restrict__ maxes) {
+  const long N = (long)n1 * n2 * n3;
+  const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  double re = 0, im = 0;
+  if (i < N) {
+    const int pz = (int)(i % n3), py = (int)((i / n3) % n2), px = (int)(i / ((long)n3 * n2));
+    const int x = perm_index(px, a1, b1), y = perm_index(py, a2, b2), z = perm_index(pz, a3, b3);
+    const cplx a = v[((long)x * n2 + y) * n3 + z];
+    vperm[i] = a.x;
+    re = fabs(a.x); im = fabs(a.y);
+  }
+  // block max -> atomicMax on the bit pattern (non-negative doubles order like unsigned integers)
+  for (int o = 16; o > 0; o >>= 1) {
+    re = fmax(re, __shfl_xor_sync(0xffffffffu, re, o));
+    im = fmax(im, __shfl_xor_sync(0xffffffffu, im, o));
+  }
+  if ((threadIdx.x & 31) == 0) {
+    atomicMax((unsigned long long*)&maxes[0], (unsigned long long)__double_as_longlong(re));
+    atomicMax((unsigned long long*)&maxes[1], (unsigned long long)__double_as_longlong(im));
+  }
+}
+
+int ks_build_vperm(HpsiPlan& P, const cplx* vhat_host, cudaStream_t st, std::string& err) {
+  const long N = P.N;
+  cplx *a = nullptr, *b = nullptr;
+  double* mx = nullptr;
+  KS_CUDA_CHECK(cudaMalloc(&a, N * sizeof(cplx)), err);
+  KS_CUDA_CHECK(cudaMalloc(&b, N * sizeof(cplx)), err);
+  KS_CUDA_CHECK(cudaMalloc(&mx, 2 * sizeof(double)), err);
+  KS_CUDA_CHECK(cudaMemsetAsync(mx, 0, 2 * sizeof(double), st), err);
+  KS_CUDA_CHECK(cudaMemcpyAsync(a, vhat_host, N * sizeof(cplx), cudaMemcpyHostToDevice, st), err);
+  const int nn[3] = {P.n1, P.n2, P.n3};
+  const long stv[3] = {(long)P.n2 * P.n3, (long)P.n3, 1};
+  const int nblk = ceil_div(N, 256);
+  for (int ax = 0; ax < 3; ++ax) {
+    k_dft_axis<<<nblk, 256, 0, st>>>(a, b, N, nn[ax], stv[ax], P.d_tw[ax]);
+    std::swap(a, b);
+  }
+  int f[6];
+  for (int ax = 0; ax < 3; ++ax) ks_fft_factors(nn[ax], &f[2 * ax], &f[2 * ax + 1]);
+  k_vperm<<<nblk, 256, 0, st>>>(a, P.d_vperm, P.n1, P.n2, P.n3, f[0], f[1], f[2], f[3], f[4], f[5], mx);
+  double h[2];
+  KS_CUDA_CHECK(cudaMemcpyAsync(h, mx, sizeof h, cudaMemcpyDeviceToHost, st), err);
+  KS_CUDA_CHECK(cudaStreamSynchronize(st), err);
+  cudaFree(a); cudaFree(b); cudaFree(mx);
+  if (h[1] > 1e-12 * h[0] && h[1] > 0.0) {
+    char buf[160];
+    snprintf(buf, sizeof buf, "V(r) is not real: max|Im| = %.3e, max|Re| = %.3e", h[1], h[0]);
+    err = buf;
+    return KS_EVLOC;
+  }
+  return KS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// shared-memory carve-up of the yz kernels
+// ------------------------------------------------------------------------------------------------
+struct YzArgs {
+  const cplx* psi;      // [nb][npw]
+  cplx* hpsi;           // [nb][npw] (forward kernel only)
+  cplx* planes;         // [nb][L1][NY][NZ]
+  const int* plane_s0;
+  const int* plane_y0;
+  const int* plane_pw0;
+  const int* pw_pos;
+  const double* g2;
+  const cplx* tw_y;
+  const cplx* tw_z;
+  int npw, L1, smax, zc;
+  double invN;
+};
+
+#define KS_YZ_THREADS 256
+
+template <int NY, int NZ>
+__global__ void __launch_bounds__(KS_YZ_THREADS) k_inv_yz(YzArgs a) {
+  constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = fac<NZ>::R1, R2z = fac<NZ>::R2;
+  constexpr int SZ = NZ | 1;
+  extern __shared__ cplx sm[];
+  cplx* tw_y = sm;
+  cplx* tw_z = tw_y + NY;
+  cplx* stile = tw_z + NZ;
+  cplx* ytile = stile + (size_t)a.smax * SZ;
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const int lx = blockIdx.x, b = blockIdx.y;
+  const int s0 = a.plane_s0[lx], S = a.plane_s0[lx + 1] - s0;
+  const int y0 = a.plane_y0[lx];
+  const int pw0 = a.plane_pw0[lx], pw1 = a.plane_pw0[lx + 1];
+  const int ZC = a.zc;
+  for (int i = tid; i < NY; i += nt) tw_y[i] = a.tw_y[i];
+  for (int i = tid; i < NZ; i += nt) tw_z[i] = a.tw_z[i];
+  for (int i = tid; i < S * SZ; i += nt) stile[i] = cmake(0.0, 0.0);
+  __syncthreads();
+  // H1: scatter this plane's coefficients onto its sticks
+  const cplx* psi = a.psi + (size_t)b * a.npw;
+  for (int j = pw0 + tid; j < pw1; j += nt) stile[a.pw_pos[j]] = psi[j];
+  __syncthreads();
+  // H2 (z): type-A inverse FFT on each stick, lines-first mapping
+  for (int it = tid; it < S * R2z; it += nt) lineA_stage1<NZ, +1>(stile + (it % S) * SZ, 1, it / S, tw_z);
+  __syncthreads();
+  for (int it = tid; it < S * R1z; it += nt) lineA_stage2<NZ, +1>(stile + (it % S) * SZ, 1, it / S);
+  __syncthreads();
+  // H2 (y): for each chunk of z positions, type-A inverse FFT along y; output straight to HBM
+  cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ);
+  for (int c = 0; c < NZ / ZC; ++c) {
+    for (int it = tid; it < ZC * R2y; it += nt) {
+      const int pz = it % ZC, j2 = it / ZC, p = c * ZC + pz;
+      cplx v[R1y];
+#pragma unroll
+      for (int j1 = 0; j1 < R1y; ++j1) {
+        int s = j1 * R2y + j2 - y0;
+        if (s < 0) s += NY;
+        v[j1] = (s < S) ? stile[s * SZ + p] : cmake(0.0, 0.0);
+      }
+      dft<R1y, +1>(v);
+#pragma unroll
+      for (int k1 = 0; k1 < R1y; ++k1)
+        ytile[(k1 * R2y + j2) * ZC + pz] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw_y, j2 * k1);
+    }
+    __syncthreads();
+    for (int it = tid; it < ZC * R1y; it += nt) {
+      const int pz = it % ZC, k1 = it / ZC;
+      cplx v[R2y];
+#pragma unroll
+      for (int j2 = 0; j2 < R2y; ++j2) v[j2] = ytile[(k1 * R2y + j2) * ZC + pz];
+      dft<R2y, +1>(v);
+#pragma unroll
+      for (int k2 = 0; k2 < R2y; ++k2) plane[(size_t)(k1 * R2y + k2) * NZ + c * ZC + pz] = v[k2];
+    }
+    __syncthreads();
+  }
+}
+
+template <int NY, int NZ>
+__global__ void __launch_bounds__(KS_YZ_THREADS) k_fwd_yz(YzArgs a) {
+  constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = fac<NZ>::R1, R2z = fac<NZ>::R2;
+  constexpr int SZ = NZ | 1;
+  extern __shared__ cplx sm[];
+  cplx* tw_y = sm;
+  cplx* tw_z = tw_y + NY;
+  cplx* stile = tw_z + NZ;
+  cplx* ytile = stile + (size_t)a.smax * SZ;
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const int lx = blockIdx.x, b = blockIdx.y;
+  const int s0 = a.plane_s0[lx], S = a.plane_s0[lx + 1] - s0;
+  const int y0 = a.plane_y0[lx];
+  const int pw0 = a.plane_pw0[lx], pw1 = a.plane_pw0[lx + 1];
+  const int ZC = a.zc;
+  for (int i = tid; i < NY; i += nt) tw_y[i] = a.tw_y[i];
+  for (int i = tid; i < NZ; i += nt) tw_z[i] = a.tw_z[i];
+  const cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ);
+  for (int c = 0; c < NZ / ZC; ++c) {
+    for (int i = tid; i < NY * ZC; i += nt) ytile[i] = plane[(size_t)(i / ZC) * NZ + c * ZC + (i % ZC)];
+    __syncthreads();
+    // H4 (y): type-B forward FFT along y
+    for (int it = tid; it < ZC * R1y; it += nt) lineB_stage1<NY, -1>(ytile + (it % ZC), ZC, it / ZC, tw_y);
+    __syncthreads();
+    for (int it = tid; it < ZC * R2y; it += nt) {
+      const int pz = it % ZC, q2 = it / ZC;
+      cplx v[R1y];
+#pragma unroll
+      for (int k1 = 0; k1 < R1y; ++k1) v[k1] = ytile[(k1 * R2y + q2) * ZC + pz];
+      dft<R1y, -1>(v);
+#pragma unroll
+      for (int q1 = 0; q1 < R1y; ++q1) {   // natural y = q1*R2y + q2; keep the stick columns only
+        int s = q1 * R2y + q2 - y0;
+        if (s < 0) s += NY;
+        if (s < S) stile[s * SZ + c * ZC + pz] = v[q1];
+      }
+    }
+    __syncthreads();
+  }
+  // H4 (z): type-B forward FFT on each stick
+  for (int it = tid; it < S * R1z; it += nt) lineB_stage1<NZ, -1>(stile + (it % S) * SZ, 1, it / S, tw_z);
+  __syncthreads();
+  for (int it = tid; it < S * R2z; it += nt) lineB_stage2<NZ, -1>(stile + (it % S) * SZ, 1, it / S);
+  __syncthreads();
+  // H5: gather + kinetic term
+  const cplx* psi = a.psi + (size_t)b * a.npw;
+  cplx* hpsi = a.hpsi + (size_t)b * a.npw;
+  for (int j = pw0 + tid; j < pw1; j += nt) {
+    const cplx g = stile[a.pw_pos[j]], p = psi[j];
+    const double k = a.g2[j];
+    hpsi[j] = cmake(fma(k, p.x, g.x * a.invN), fma(k, p.y, g.y * a.invN));
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// x pass: inverse FFT, V(r) multiply, forward FFT in one kernel
+// ------------------------------------------------------------------------------------------------
+struct XArgs {
+  cplx* planes;         // [nb][L1][NY][NZ], in place
+  const double* vperm;  // [NX][NY][NZ]
+  const cplx* tw_x;
+  int L1, x0, ny, nz, zc;
+};
+#define KS_X_THREADS 256
+
+template <int NX>
+__global__ void __launch_bounds__(KS_X_THREADS) k_x(XArgs a) {
+  constexpr int R1 = fac<NX>::R1, R2 = fac<NX>::R2;
+  extern __shared__ cplx sm[];
+  cplx* tw = sm;
+  cplx* tile = sm + NX;
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const int ZC = a.zc, nchunk = a.nz / ZC;
+  const int c = blockIdx.x % nchunk, yp = blockIdx.x / nchunk, b = blockIdx.y;
+  const size_t pstride = (size_t)a.ny * a.nz;
+  cplx* base = a.planes + (size_t)b * a.L1 * pstride + (size_t)yp * a.nz + c * ZC;
+  const double* vbase = a.vperm + (size_t)yp * a.nz + c * ZC;
+  for (int i = tid; i < NX; i += nt) tw[i] = a.tw_x[i];
+  for (int i = tid; i < NX * ZC; i += nt) {
+    const int x = i / ZC, pz = i % ZC;
+    int lx = x - a.x0;
+    if (lx < 0) lx += NX;
+    tile[i] = (lx < a.L1) ? base[(size_t)lx * pstride + pz] : cmake(0.0, 0.0);
+  }
+  __syncthreads();
+  for (int it = tid; it < ZC * R2; it += nt) lineA_stage1<NX, +1>(tile + (it % ZC), ZC, it / ZC, tw);
+  __syncthreads();
+  // type-A stage 2, V(r), type-B stage 1 on the same R2 elements, in registers
+  for (int it = tid; it < ZC * R1; it += nt) {
+    const int pz = it % ZC, k1 = it / ZC;
+    cplx v[R2];
+#pragma unroll
+    for (int j2 = 0; j2 < R2; ++j2) v[j2] = tile[(k1 * R2 + j2) * ZC + pz];
+    dft<R2, +1>(v);
+#pragma unroll
+    for (int k2 = 0; k2 < R2; ++k2) {
+      const double vr = __ldg(vbase + (size_t)(k1 * R2 + k2) * pstride + pz);
+      v[k2] = cmake(v[k2].x * vr, v[k2].y * vr);
+    }
+    dft<R2, -1>(v);
+#pragma unroll
+    for (int q2 = 0; q2 < R2; ++q2)
+      tile[(k1 * R2 + q2) * ZC + pz] = (q2 == 0) ? v[0] : mul_tw<-1>(v[q2], tw, k1 * q2);
+  }
+  __syncthreads();
+  for (int it = tid; it < ZC * R2; it += nt) {
+    const int pz = it % ZC, q2 = it / ZC;
+    cplx v[R1];
+#pragma unroll
+    for (int k1 = 0; k1 < R1; ++k1) v[k1] = tile[(k1 * R2 + q2) * ZC + pz];
+    dft<R1, -1>(v);
+#pragma unroll
+    for (int q1 = 0; q1 < R1; ++q1) {   // natural x = q1*R2 + q2; only the live planes are kept
+      int lx = q1 * R2 + q2 - a.x0;
+      if (lx < 0) lx += NX;
+      if (lx < a.L1) base[(size_t)lx * pstride + pz] = v[q1];
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// host: configuration and launch
+// ------------------------------------------------------------------------------------------------
+static const size_t KS_SMEM_MAX = 227 * 1024;
+
+static size_t yz_smem(const HpsiPlan& P, int zc) {
+  const size_t SZ = (size_t)(P.n3 | 1);
+  return sizeof(cplx) * ((size_t)P.n2 + P.n3 + (size_t)P.smax * SZ + (size_t)P.n2 * zc);
+}
+static size_t x_smem(const HpsiPlan& P, int zc) { return sizeof(cplx) * ((size_t)P.n1 + (size_t)P.n1 * zc); }
+
+template <typename K>
+static cudaError_t opt_in(K kern, size_t bytes) {
+  return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+int ks_hpsi_configure(HpsiPlan& P, std::string& err) {
+  if (!ks_fft_size_supported(P.n1) || !ks_fft_yz_supported(P.n2, P.n3)) {
+    char b[200];
+    snprintf(b, sizeof b, "FFT grid %dx%dx%d is not in the supported set (see ks_supported_sizes; n2,n3 must be a supported pair)",
+             P.n1, P.n2, P.n3);
+    err = b;
+    return KS_EGRID;
+  }
+  // z-chunk: largest of 32/16/8/... dividing n3 that fits; prefer two CTAs per SM for the yz kernels
+  const int cand[] = {32, 16, 8, 4, 2, 1};
+  P.zc_yz = 0;
+  for (int pass = 0; pass < 2 && !P.zc_yz; ++pass)
+    for (int zc : cand) {
+      if (P.n3 % zc) continue;
+      const size_t need = yz_smem(P, zc);
+      if (need <= (pass == 0 ? KS_SMEM_MAX / 2 - 1024 : KS_SMEM_MAX)) { P.zc_yz = zc; break; }
+      if (pass == 0 && zc <= 8) break;   // do not shrink below 8 just to reach two CTAs/SM
+    }
+  if (!P.zc_yz) { err = "yz kernels: stick tile does not fit in 227 KB of shared memory"; return KS_ENOMEM; }
+  P.smem_yz = yz_smem(P, P.zc_yz);
+  P.zc_x = 0;
+  for (int zc : cand) {
+    if (P.n3 % zc) continue;
+    if (x_smem(P, zc) <= 56 * 1024) { P.zc_x = zc; break; }   // >= 4 CTAs per SM
+  }
+  if (!P.zc_x) { err = "x kernel: tile does not fit"; return KS_ENOMEM; }
+  P.smem_x = x_smem(P, P.zc_x);
+  cudaError_t e = cudaSuccess;
+#define C_(A_, B_)                                                              \
+  if (P.n2 == A_ && P.n3 == B_) {                                               \
+    e = opt_in(k_inv_yz<A_, B_>, P.smem_yz);                                    \
+    if (e == cudaSuccess) e = opt_in(k_fwd_yz<A_, B_>, P.smem_yz);              \
+  }
+  KS_YZ_PAIRS(C_)
+#undef C_
+  KS_CUDA_CHECK(e, err);
+#define C_(N_) if (P.n1 == N_) e = opt_in(k_x<N_>, P.smem_x);
+  KS_X_SIZES(C_)
+#undef C_
+  KS_CUDA_CHECK(e, err);
+  return KS_OK;
+}
+
+int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb, cudaStream_t st,
+                         std::string& err) {
+  if (nb <= 0) return KS_OK;
+  if (nb > P.batch_cap) { err = "internal: FFT batch larger than workspace"; return KS_EINVAL; }
+  YzArgs a;
+  a.psi = psi; a.hpsi = hpsi; a.planes = P.d_planes;
+  a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.plane_pw0 = P.d_plane_pw0;
+  a.pw_pos = P.d_pw_pos; a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
+  a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.zc = P.zc_yz; a.invN = 1.0 / (double)P.N;
+  XArgs x;
+  x.planes = P.d_planes; x.vperm = P.d_vperm; x.tw_x = P.d_tw[0];
+  x.L1 = P.L1; x.x0 = P.x0; x.ny = P.n2; x.nz = P.n3; x.zc = P.zc_x;
+  const dim3 gyz(P.L1, nb), gx((P.n3 / P.zc_x) * P.n2, nb);
+  bool launched = false;
+#define C_(A_, B_) \
+  if (P.n2 == A_ && P.n3 == B_) { k_inv_yz<A_, B_><<<gyz, KS_YZ_THREADS, P.smem_yz, st>>>(a); launched = true; }
+  KS_YZ_PAIRS(C_)
+#undef C_
+  if (!launched) { err = "internal: no yz kernel"; return KS_EGRID; }
+#define C_(N_) if (P.n1 == N_) k_x<N_><<<gx, KS_X_THREADS, P.smem_x, st>>>(x);
+  KS_X_SIZES(C_)
+#undef C_
+#define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_fwd_yz<A_, B_><<<gyz, KS_YZ_THREADS, P.smem_yz, st>>>(a);
+  KS_YZ_PAIRS(C_)
+#undef C_
+  KS_CUDA_CHECK(cudaGetLastError(), err);
+  return KS_OK;
+}

@@ -1,0 +1,71 @@
+// plan.h -- internal (host) description of one k-point's H*psi plan and the launchers the
+// translation units of libkspw.so share.  Not part of the C ABI (include/kspw.h).
+#pragma once
+#include "common.cuh"
+#include <vector>
+
+struct HpsiPlan {
+  int n1 = 0, n2 = 0, n3 = 0, npw = 0;
+  long N = 0;
+  int L1 = 0;          // number of live x-planes (distinct m1 of the sphere)
+  int x0 = 0;          // natural x index (m1min mod n1) of live plane 0; plane lx is x = (x0+lx) mod n1
+  int nsticks = 0;     // z-sticks (distinct (m1,m2)) of the sphere
+  int smax = 0;        // max sticks in one plane
+  int zc_yz = 0, zc_x = 0;        // z-chunk sizes of the yz kernels and of the x kernel
+  size_t smem_yz = 0, smem_x = 0;
+  // device arrays
+  int* d_plane_s0 = nullptr;   // [L1+1] first stick of each plane
+  int* d_plane_y0 = nullptr;   // [L1]   natural y index (m2min mod n2) of the plane's first stick
+  int* d_plane_pw0 = nullptr;  // [L1+1] first plane wave of each plane (PWs of a plane are contiguous)
+  int* d_pw_pos = nullptr;     // [npw]  position of PW j in its plane's stick tile: s_local*SZ + z
+  double* d_g2 = nullptr;      // [npw]  |k+G|^2
+  double* d_vperm = nullptr;   // [n1][n2][n3] V(r) in position (type-A output) order on all three axes
+  cplx* d_tw[3] = {nullptr, nullptr, nullptr};  // e^{+2 pi i t/n_i}
+  cplx* d_planes = nullptr;    // workspace [batch][L1][n2][n3]
+  int batch_cap = 0;           // bands the workspace holds
+};
+
+bool ks_fft_size_supported(int n);
+bool ks_fft_yz_supported(int n2, int n3);
+int ks_fft_sizes(int* out, int cap);
+void ks_fft_factors(int n, int* R1, int* R2);
+cudaError_t ks_fft_init_constants();
+
+// V(r) = Re sum_m vhat[m] e^{+2 pi i m.j/n} on the device by a plain O(N n) DFT per axis (create time
+// only), checked real, stored permuted.  vhat_host: [n1][n2][n3].  Returns KS_* and fills err.
+int ks_build_vperm(HpsiPlan& P, const cplx* vhat_host, cudaStream_t st, std::string& err);
+
+// fill zc_*/smem_* for the plan and opt the kernels into large dynamic shared memory
+int ks_hpsi_configure(HpsiPlan& P, std::string& err);
+
+// local + kinetic part: hpsi[b][j] = g2[j] psi[b][j] + (1/N) FFT^-[ V(r) FFT^+[psi_b] ](G_j) for nb bands
+// (nb <= batch_cap), three launches on `st`.
+int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb, cudaStream_t st,
+                         std::string& err);
+
+// ---- dense kernels (gemm.cu, eigh.cu) ----
+struct GemmWs {          // split-K partial sums
+  cplx* part = nullptr;
+  size_t bytes = 0;
+};
+int ks_gemm_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb,
+               cplx* C, long ldc, GemmWs* ws, std::string& err);
+int ks_gemm_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb,
+               cplx* C, long ldc, int accumulate, std::string& err);
+
+int ks_peak_run(double* dmma_tf, double* dfma_tf, std::string& err);
+
+struct EighWs {
+  cplx* U = nullptr;       // per-pair rotation blocks [nblk/2][64*64]
+  cplx* Ap = nullptr;      // padded working copy of A   [np*np]
+  cplx* Vp = nullptr;      // padded eigenvector accumulator [np*np]
+  double* diag = nullptr;  // [np]
+  double* red = nullptr;   // [2] off^2, tot^2
+  int* order = nullptr;    // [np]
+  int2* pairs = nullptr;   // [(nblk-1)][nblk/2] block pairs of every round
+  int cap = 0;             // padded n the buffers hold
+  int pairs_nblk = 0;      // nblk the pair table was built for
+};
+int ks_eigh_run(cudaStream_t st, int n, cplx* A, long lda, double* theta, cplx* C, long ldc, EighWs* ws,
+                int* sweeps_out, std::string& err);
+void ks_eigh_free(EighWs* ws);
