@@ -1,0 +1,335 @@
+#!/usr/bin/env python
+"""bench.py -- H psi band-applications/s and Davidson time-to-converge on the BASELINE.json workloads.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference] [--no-davidson]
+
+A "step" is one ks_hpsi block apply of the config's nbands bands (steps H1-H8 of DESIGN.md §1: scatter, pruned
+inverse FFT, V(r), forward FFT, gather + kinetic, beta^H psi, D, beta (D B)); `value` = band applications
+per second over the K timed steps.  The second half of BASELINE.json's metric, Davidson time-to-converge
+(steps D0-D9, which call the same ks_hpsi on every new block), is measured in the same run and reported in
+the `davidson` object.  Inputs are seeded synthetic (paper_2501_08697_b200/inputs.py).
+One JSON line on stdout (rank 0).  N > 1 (torchrun): every rank runs the same workload on its own GPU
+(k-points / band blocks are independent: weak scaling, no data-path collective).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+from paper_2501_08697_b200 import inputs as I  # noqa: E402
+
+METRIC = "hpsi_band_applications_per_s"
+UNIT = "band-applications/s"
+NOMINAL_FP64_OVER_BF16 = 45.0 / 2250.0   # guide's nominal B200 FP64-tensor / bf16-tensor ratio
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1: Si64-like)")
+    ap.add_argument("--k-index", type=int, default=0)
+    ap.add_argument("--impl", default="kspw", choices=["kspw", "reference"])
+    ap.add_argument("--no-davidson", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--davidson-max-iter", type=int, default=400)
+    ap.add_argument("--fft-batch", type=int, default=0)
+    return ap.parse_args()
+
+
+def workload_name(p):
+    return "cfg%d %s: cell %s bohr, ecutwfc %g Ry, npw %d, grid %dx%dx%d, nproj %d, nbands %d" % (
+        p.cfg.index, p.cfg.name, "x".join("%g" % np.linalg.norm(a) for a in p.cell), p.ecutwfc, p.npw,
+        p.grid[0], p.grid[1], p.grid[2], p.nproj, p.nbands)
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return dict(hbm_gbs=d["hbm_gbs"], bf16=d["bf16_tflops"], bf16_sus=d.get("bf16_tflops_sustained"), src="measured")
+    return dict(hbm_gbs=6650.0, bf16=1590.0, bf16_sus=1400.0, src="fallback")
+
+
+# ------------------------------------------------------------------------------------------------
+# oracle legs (cpu_baseline, --impl reference): the oracle as it stands, on the host cores
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(p, nsample, reps=1):
+    from oracle import kso
+    o = kso.Oracle.from_problem(p)
+    sel = np.unique(np.linspace(0, p.nbands - 1, nsample).astype(int))
+    psi = np.ascontiguousarray(p.psi0[sel])
+    times = []
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        o.hpsi(psi)
+        times.append(time.perf_counter() - t0)
+    return len(sel), times, kso.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import kso
+    p = I.make_problem(args.config, args.k_index)
+    nthreads = kso.num_threads()
+    nsample = min(p.nbands, max(nthreads, 8))
+    ns, times, _ = oracle_sample(p, nsample, reps=args.warmup + args.steps)
+    timed = times[args.warmup:]
+    tot = sum(timed)
+    value = ns * len(timed) / tot
+    sample = "%d of %d bands per step (kso_hpsi, OpenMP over bands), %d steps" % (ns, p.nbands, len(timed))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(timed), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
+        "config": {"workload": workload_name(p), "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": nthreads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.path = index, None, "/tmp/kspw_clocks_%d.csv" % os.getpid()
+
+    def start(self):
+        try:
+            self.f = open(self.path, "w")
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                         stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.f.close()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in open(self.path):
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        try:
+            os.remove(self.path)
+        except OSError:
+            pass
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+# algorithmic bytes / flops per launch
+# ------------------------------------------------------------------------------------------------
+def plan_counts(p):
+    m = p.miller
+    L1 = int(m[:, 0].max() - m[:, 0].min() + 1)
+    return L1
+
+
+def kernel_models(p, nb_per_launch):
+    """bytes or flops ONE launch of each kernel moves/does when it processes nb_per_launch bands."""
+    n1, n2, n3 = (int(x) for x in p.grid)
+    L1 = plan_counts(p)
+    planes = 16.0 * L1 * n2 * n3
+    npw, P = p.npw, p.nproj
+    return {
+        "k_inv_yz": ("hbm", nb_per_launch * (16.0 * npw + planes)),
+        "k_x": ("hbm", nb_per_launch * 2.0 * planes + 8.0 * n1 * n2 * n3),
+        "k_fwd_yz": ("hbm", nb_per_launch * (planes + 32.0 * npw) + 8.0 * npw),
+        "k_gemm_hn+reduce": ("tensor", 8.0 * P * nb_per_launch * npw),
+        "k_apply_D": ("alu", 0.0),
+        "k_gemm_nn": ("tensor", 8.0 * P * nb_per_launch * npw),
+    }
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl")
+    from paper_2501_08697_b200 import kspw
+
+    p = I.make_problem(args.config, args.k_index)
+    ctx = kspw.Context.from_problem(p)
+    if args.fft_batch:
+        ctx.set_fft_batch(args.fft_batch)
+    stream = torch.cuda.current_stream()
+    ctx.set_stream(stream)
+    nb, npw = p.nbands, p.npw
+    psi = torch.from_numpy(p.psi0).cuda()
+    hpsi = torch.empty_like(psi)
+    resident_bytes = psi.numel() * 16 * 2 + p.beta.size * 16
+    flush = None
+    if resident_bytes < 2 * 126e6:   # inputs not clearly larger than L2: flush between timed iterations
+        flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed_steps(fn, k):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
+        for a, b in ev:
+            if flush is not None:
+                flush.fill_(1.0)
+            a.record(stream)
+            fn()
+            b.record(stream)
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in ev)
+
+    for _ in range(max(args.warmup, 3)):
+        ctx.hpsi(psi, out=hpsi)
+    barrier()
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    ctx.profile_begin()
+    ms = timed_steps(lambda: ctx.hpsi(psi, out=hpsi), args.steps)
+    prof = ctx.profile_end()
+    barrier()
+    # end-to-end through the C ABI with pinned HOST buffers (H2D + D2H inside the timed region)
+    hin = torch.from_numpy(p.psi0).pin_memory()
+    hout = torch.empty_like(hin).pin_memory()
+    hin_np, hout_np = hin.numpy(), hout.numpy()
+    ctx.hpsi_host(hin_np, hout_np)
+    t0 = time.perf_counter()
+    e2e_steps = max(1, min(args.steps, 5))
+    for _ in range(e2e_steps):
+        ctx.hpsi_host(hin_np, hout_np)
+    e2e_s = time.perf_counter() - t0
+    # Davidson time-to-converge (one warm-up solve + one timed solve), same context
+    dav = None
+    if not args.no_davidson:
+        work = psi.clone()
+        ctx.davidson(work, tol=1e-8, max_iter=args.davidson_max_iter)
+        work.copy_(psi)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        r = ctx.davidson(work, tol=1e-8, max_iter=args.davidson_max_iter)
+        b.record(stream)
+        torch.cuda.synchronize()
+        dsec = a.elapsed_time(b) * 1e-3
+        dav = {"time_to_converge_s": dsec, "iterations": r["iters"], "band_applications": r["band_applications"],
+               "converged": bool(r["converged"]), "max_resid": float(r["resid"].max().item()), "tol": 1e-8,
+               "band_applications_per_s": r["band_applications"] / dsec,
+               "eig_min": float(r["eig"][0].item()), "eig_max": float(r["eig"][-1].item())}
+    clk = clocks.stop() if rank == 0 else None
+    tmax = torch.tensor([ms, e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms, e2e_s = float(tmax[0]), float(tmax[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    value = world * nb * args.steps / (ms * 1e-3)
+    pk = peaks()
+    dmma_tf, dfma_tf = kspw.ks_dmma_peak()
+    nbatch_launches = prof["k_x"][1] // max(args.steps, 1)          # FFT launches per step
+    nb_per_fft_launch = nb / max(nbatch_launches, 1)
+    models = kernel_models(p, nb_per_fft_launch)
+    gmodels = kernel_models(p, nb)
+    rows = {}
+    for name, (tms, nl) in prof.items():
+        if nl == 0 or tms <= 0:
+            continue
+        kind, per = (models if name.startswith(("k_inv", "k_x", "k_fwd")) else gmodels)[name]
+        nlaunch = nl if not name.startswith("k_gemm_hn") else nl // 2
+        avg_ms = tms / nlaunch
+        if kind == "hbm":
+            ach, peak, unit = per / (avg_ms * 1e-3) / 1e9, pk["hbm_gbs"], "GB/s"
+        elif kind == "tensor":
+            ach, peak, unit = per / (avg_ms * 1e-3) / 1e12, dmma_tf, "TFLOP/s"
+        else:
+            ach, peak, unit = 0.0, 1.0, ""
+        rows[name] = {"bound": kind, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak if peak else None,
+                      "avg_launch_ms": avg_ms, "launches": nlaunch, "share_of_step": tms / ms}
+    dom = max((k for k in rows if rows[k]["bound"] != "alu"), key=lambda k: rows[k]["share_of_step"])
+    roof = dict(rows[dom])
+    roof.update({"kernel": dom, "traffic": None,
+                 "peak_source": ("MEASURED_PEAKS.json hbm_gbs (%s)" % pk["src"]) if roof["bound"] == "hbm" else
+                 "live register-resident DMMA m8n8k4 microbenchmark (ks_dmma_peak); bf16 measured x nominal ratio = %.1f TFLOP/s"
+                 % (pk["bf16"] * NOMINAL_FP64_OVER_BF16)})
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64 (complex128)", "data": "synthetic",
+        "config": {"workload": workload_name(p), "step": "one ks_hpsi block apply of %d bands (H1-H8)" % nb,
+                   "l2": "flushed between timed iterations" if flush is not None else
+                   "inputs (psi+hpsi+beta = %.0f MB) larger than the 126 MB L2, no flush" % (resident_bytes / 1e6),
+                   "fft_batch_bands": nb_per_fft_launch, "parallelism": "replicas x%d" % world},
+        "clocks": clk,
+        "e2e": {"value": world * nb * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nb * npw * 16,
+                "d2h_bytes_per_step": nb * npw * 16, "api": "ks_hpsi_host (pinned host buffers)"},
+        "gpu_launches": int(sum(v[1] for v in prof.values())),
+        "roofline": roof,
+        "roofline_all": rows,
+        "peaks": {"hbm_gbs": pk["hbm_gbs"], "source": pk["src"], "dmma_tflops_live": dmma_tf, "dfma_tflops_live": dfma_tf},
+        "davidson": dav,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        from oracle import kso
+        nthreads = kso.num_threads()
+        nsample = min(nb, max(nthreads, 8))
+        ns, times, _ = oracle_sample(p, nsample, reps=1)
+        line["cpu_baseline"] = {"value": ns / times[0], "unit": UNIT, "cores": nthreads, "kind": "oracle",
+                                "sample": "%d of %d bands, one kso_hpsi call (OpenMP over bands), %.1f s" % (ns, nb, times[0])}
+    else:
+        line["cpu_baseline"] = None
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

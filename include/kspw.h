@@ -87,6 +87,14 @@ int ks_davidson_host(ks_ctx* ctx, ks_c128* psi_host, double* eig_host, int nband
  * total, reserved.  Only filled when KSPW_PROFILE=1 is set in the environment (adds syncs). */
 int ks_davidson_profile(const ks_ctx* ctx, double* ms);
 
+/* Per-kernel device time of ks_hpsi between ks_profile_begin and ks_profile_end, by CUDA events recorded
+ * on the context's stream around each launch (no host synchronisation while profiling is on).
+ * ms, launches: HOST out [8], indexed 0 k_inv_yz (H1+H2 z,y), 1 k_x (H2 x, H3, H4 x), 2 k_fwd_yz (H4 y,z, H5),
+ * 3 beta^H psi GEMM + split-K reduce (H6), 4 D apply (H7), 5 beta (D B) GEMM (H8); 6-7 reserved.
+ * launches counts the kernels launched per entry since ks_profile_begin.  ks_profile_end synchronises. */
+int ks_profile_begin(ks_ctx* ctx);
+int ks_profile_end(ks_ctx* ctx, double* ms, long long* launches);
+
 /* ---- building blocks, exported for unit parity tests and the roofline microbenchmarks -------- */
 /* C[M][N] (column-major, ldc) = A^H B;  A: DEVICE K x M column-major lda, B: K x N column-major ldb. */
 int ks_zgemm_hn(void* stream, int M, int N, int K, const ks_c128* A, long lda, const ks_c128* B,

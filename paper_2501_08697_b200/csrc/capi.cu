@@ -250,6 +250,8 @@ extern "C" void ks_destroy(ks_ctx* c) {
   cudaFree(c->gws.part);
   ks_eigh_free(&c->ews);
   ks_davidson_free(&c->dws);
+  for (auto& r : c->krecs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+  for (auto e : c->kpool) cudaEventDestroy(e);
   delete c;
 }
 
@@ -288,8 +290,8 @@ __global__ void k_apply_D(int nproj, int nb, const cplx* __restrict__ B, cplx* _
 
 int ks_hpsi_impl(ks_ctx* c, const cplx* psi, cplx* hpsi, int nb) {
   if (!c) return KS_EINVAL;
+  if (nb == 0) return KS_OK;   // empty block: nothing to do (pointers may be NULL)
   if (!psi || !hpsi || nb < 0) { c->err = "ks_hpsi: bad argument"; return KS_EINVAL; }
-  if (nb == 0) return KS_OK;
   const HpsiPlan& P = c->P;
   {
     const char* a = (const char*)psi;
@@ -299,8 +301,12 @@ int ks_hpsi_impl(ks_ctx* c, const cplx* psi, cplx* hpsi, int nb) {
   }
   for (int b0 = 0; b0 < nb; b0 += c->fft_batch) {
     const int n = std::min(c->fft_batch, nb - b0);
-    const int rc = ks_hpsi_local_launch(P, psi + (size_t)b0 * P.npw, hpsi + (size_t)b0 * P.npw, n, c->stream, c->err);
-    if (rc) return rc;
+    for (int stage = 0; stage < 3; ++stage) {
+      ks_kprof_begin(c, KP_INV_YZ + stage, 1);
+      const int rc = ks_hpsi_local_launch(P, psi + (size_t)b0 * P.npw, hpsi + (size_t)b0 * P.npw, n, c->stream, c->err, stage);
+      ks_kprof_end(c);
+      if (rc) return rc;
+    }
   }
   if (c->nproj > 0) {
     if (nb > c->nl_cap) {
@@ -310,14 +316,60 @@ int ks_hpsi_impl(ks_ctx* c, const cplx* psi, cplx* hpsi, int nb) {
       KS_CUDA_CHECK(cudaMalloc(&c->d_DB, sizeof(cplx) * (size_t)c->nproj * nb), c->err);
       c->nl_cap = nb;
     }
+    ks_kprof_begin(c, KP_GEMM_HN, 2);
     int rc = ks_gemm_hn(c->stream, c->nproj, nb, P.npw, c->d_beta, P.npw, psi, P.npw, c->d_B, c->nproj, &c->gws, c->err);
+    ks_kprof_end(c);
     if (rc) return rc;
+    ks_kprof_begin(c, KP_APPLY_D, 1);
     k_apply_D<<<ceil_div((long)c->nproj * nb, 256), 256, 0, c->stream>>>(c->nproj, nb, c->d_B, c->d_DB, c->d_proj_atom,
                                                                          c->d_off, c->d_doff, c->d_D);
+    ks_kprof_end(c);
+    ks_kprof_begin(c, KP_GEMM_NN, 1);
     rc = ks_gemm_nn(c->stream, P.npw, nb, c->nproj, c->d_beta, P.npw, c->d_DB, c->nproj, hpsi, P.npw, 1, c->err);
+    ks_kprof_end(c);
     if (rc) return rc;
   }
   KS_CUDA_CHECK(cudaGetLastError(), c->err);
+  return KS_OK;
+}
+
+// ---- per-kernel event timing (bench.py's roofline object) ----
+void ks_kprof_begin(ks_ctx* c, int phase, int launches) {
+  c->klaunch[phase] += launches;
+  if (!c->kprof_on) return;
+  ks_ctx::KRec r;
+  r.phase = phase;
+  for (cudaEvent_t* e : {&r.a, &r.b}) {
+    if (c->kpool.empty()) cudaEventCreate(e);
+    else { *e = c->kpool.back(); c->kpool.pop_back(); }
+  }
+  cudaEventRecord(r.a, c->stream);
+  c->krecs.push_back(r);
+}
+void ks_kprof_end(ks_ctx* c) {
+  if (!c->kprof_on || c->krecs.empty()) return;
+  cudaEventRecord(c->krecs.back().b, c->stream);
+}
+extern "C" int ks_profile_begin(ks_ctx* c) {
+  if (!c) return KS_EINVAL;
+  for (auto& r : c->krecs) { c->kpool.push_back(r.a); c->kpool.push_back(r.b); }
+  c->krecs.clear();
+  for (int i = 0; i < 8; ++i) c->klaunch[i] = 0;
+  c->kprof_on = true;
+  return KS_OK;
+}
+extern "C" int ks_profile_end(ks_ctx* c, double* ms, long long* launches) {
+  if (!c || !ms || !launches) return KS_EINVAL;
+  KS_CUDA_CHECK(cudaStreamSynchronize(c->stream), c->err);
+  for (int i = 0; i < 8; ++i) { ms[i] = 0; launches[i] = c->klaunch[i]; }
+  for (auto& r : c->krecs) {
+    float t = 0;
+    cudaEventElapsedTime(&t, r.a, r.b);
+    ms[r.phase] += t;
+    c->kpool.push_back(r.a); c->kpool.push_back(r.b);
+  }
+  c->krecs.clear();
+  c->kprof_on = false;
   return KS_OK;
 }
 

@@ -33,8 +33,18 @@ struct ks_ctx {
   cudaStream_t stream = 0;
   int fft_batch = 0;             // bands per FFT batch
   double prof_ms[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  // per-kernel CUDA-event timing of ks_hpsi (ks_profile_begin / ks_profile_end); no host syncs while on
+  bool kprof_on = false;
+  struct KRec { int phase; cudaEvent_t a, b; };
+  std::vector<KRec> krecs;
+  std::vector<cudaEvent_t> kpool;
+  long long klaunch[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   std::string err;
 };
+
+enum { KP_INV_YZ = 0, KP_X = 1, KP_FWD_YZ = 2, KP_GEMM_HN = 3, KP_APPLY_D = 4, KP_GEMM_NN = 5 };
+void ks_kprof_begin(ks_ctx* c, int phase, int launches);
+void ks_kprof_end(ks_ctx* c);
 
 int ks_hpsi_impl(ks_ctx* c, const cplx* psi, cplx* hpsi, int nb);
 int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int max_iter, double* resid,

@@ -408,7 +408,7 @@ int ks_hpsi_configure(HpsiPlan& P, std::string& err) {
 }
 
 int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb, cudaStream_t st,
-                         std::string& err) {
+                         std::string& err, int stage) {
   if (nb <= 0) return KS_OK;
   if (nb > P.batch_cap) { err = "internal: FFT batch larger than workspace"; return KS_EINVAL; }
   YzArgs a;
@@ -420,18 +420,21 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
   x.planes = P.d_planes; x.vperm = P.d_vperm; x.tw_x = P.d_tw[0];
   x.L1 = P.L1; x.x0 = P.x0; x.ny = P.n2; x.nz = P.n3; x.zc = P.zc_x;
   const dim3 gyz(P.L1, nb), gx((P.n3 / P.zc_x) * P.n2, nb);
-  bool launched = false;
-#define C_(A_, B_) \
-  if (P.n2 == A_ && P.n3 == B_) { k_inv_yz<A_, B_><<<gyz, KS_YZ_THREADS, P.smem_yz, st>>>(a); launched = true; }
-  KS_YZ_PAIRS(C_)
+  if (stage < 0 || stage == 0) {
+#define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_inv_yz<A_, B_><<<gyz, KS_YZ_THREADS, P.smem_yz, st>>>(a);
+    KS_YZ_PAIRS(C_)
 #undef C_
-  if (!launched) { err = "internal: no yz kernel"; return KS_EGRID; }
+  }
+  if (stage < 0 || stage == 1) {
 #define C_(N_) if (P.n1 == N_) k_x<N_><<<gx, KS_X_THREADS, P.smem_x, st>>>(x);
-  KS_X_SIZES(C_)
+    KS_X_SIZES(C_)
 #undef C_
+  }
+  if (stage < 0 || stage == 2) {
 #define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_fwd_yz<A_, B_><<<gyz, KS_YZ_THREADS, P.smem_yz, st>>>(a);
-  KS_YZ_PAIRS(C_)
+    KS_YZ_PAIRS(C_)
 #undef C_
+  }
   KS_CUDA_CHECK(cudaGetLastError(), err);
   return KS_OK;
 }

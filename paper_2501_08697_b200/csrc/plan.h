@@ -40,8 +40,9 @@ int ks_hpsi_configure(HpsiPlan& P, std::string& err);
 
 // local + kinetic part: hpsi[b][j] = g2[j] psi[b][j] + (1/N) FFT^-[ V(r) FFT^+[psi_b] ](G_j) for nb bands
 // (nb <= batch_cap), three launches on `st`.
+// stage: 0 = k_inv_yz, 1 = k_x, 2 = k_fwd_yz, -1 = all three in order.
 int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb, cudaStream_t st,
-                         std::string& err);
+                         std::string& err, int stage = -1);
 
 // ---- dense kernels (gemm.cu, eigh.cu) ----
 struct GemmWs {          // split-K partial sums

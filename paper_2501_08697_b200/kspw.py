@@ -35,6 +35,8 @@ _lib.ks_hpsi_host.argtypes = [_vp, _vp, _vp, _i]
 _lib.ks_davidson.argtypes = [_vp, _vp, _vp, _i, _d, _i, _vp, _vp, _vp]
 _lib.ks_davidson_host.argtypes = [_vp, _vp, _vp, _i, _d, _i, _vp, _vp, _vp]
 _lib.ks_davidson_profile.argtypes = [_vp, _vp]
+_lib.ks_profile_begin.argtypes = [_vp]
+_lib.ks_profile_end.argtypes = [_vp, _vp, _vp]
 _lib.ks_zgemm_hn.argtypes = [_vp, _i, _i, _i, _vp, _l, _vp, _l, _vp, _l]
 _lib.ks_zgemm_nn.argtypes = [_vp, _i, _i, _i, _vp, _l, _vp, _l, _vp, _l, _i]
 _lib.ks_eigh.argtypes = [_vp, _i, _vp, _l, _vp, _vp, _l, _vp]
@@ -43,7 +45,7 @@ _lib.ks_dmma_peak.argtypes = [_vp, _vp]
 KS_OK, KS_NOTCONV = 0, 1
 EXPORTS = ("ks_pw_count", "ks_pw_list", "ks_create", "ks_destroy", "ks_npw", "ks_set_stream", "ks_set_fft_batch",
            "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_davidson", "ks_davidson_host",
-           "ks_davidson_profile", "ks_zgemm_hn", "ks_zgemm_nn", "ks_eigh", "ks_dmma_peak")
+           "ks_davidson_profile", "ks_profile_begin", "ks_profile_end", "ks_zgemm_hn", "ks_zgemm_nn", "ks_eigh", "ks_dmma_peak")
 
 
 class KsError(RuntimeError):
@@ -188,6 +190,18 @@ class Context:
         rc = self._check(_lib.ks_davidson_host(self._h, _hp(psi), _hp(eig), nb, float(tol), int(max_iter), _hp(res),
                                                C.byref(it), C.byref(nh)))
         return dict(psi=psi, eig=eig, resid=res, iters=it.value, band_applications=nh.value, converged=(rc == 0))
+
+    KERNELS = ("k_inv_yz", "k_x", "k_fwd_yz", "k_gemm_hn+reduce", "k_apply_D", "k_gemm_nn")
+
+    def profile_begin(self):
+        self._check(_lib.ks_profile_begin(self._h))
+
+    def profile_end(self):
+        """Returns {kernel: (ms, launches)} accumulated since profile_begin (synchronises)."""
+        ms = np.zeros(8)
+        n = np.zeros(8, dtype=np.int64)
+        self._check(_lib.ks_profile_end(self._h, _hp(ms), _hp(n)))
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(self.KERNELS)}
 
     def davidson_profile(self):
         ms = np.zeros(8)
