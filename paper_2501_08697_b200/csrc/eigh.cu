@@ -14,6 +14,7 @@
 #include "mma.cuh"
 #include "plan.h"
 #include <algorithm>
+#include <cstdlib>
 #include <vector>
 
 #define JB 32            // block size of the block method
@@ -357,6 +358,11 @@ int ks_eigh_run(cudaStream_t st, int n, cplx* A, long lda, double* theta, cplx* 
     opted = true;
   }
   const double tol2 = 1e-28;   // off_F <= 1e-14 ||A||_F
+  static int inner = 0;        // inner sweeps of the 64x64 pair problems in the block method
+  if (!inner) {
+    const char* e = getenv("KSPW_JAC_INNER");
+    inner = (e && atoi(e) > 0) ? atoi(e) : 6;
+  }
   int sweeps = 0;
   if (n <= JS) {
     const int ns = n + (n & 1), nbk = ns / 2;
@@ -406,7 +412,7 @@ int ks_eigh_run(cudaStream_t st, int n, cplx* A, long lda, double* theta, cplx* 
     if (h[0] <= tol2 * h[1]) break;
     for (int r = 0; r < nblk - 1; ++r) {
       const int2* pr = ws->pairs + (size_t)r * npair;
-      k_jacobi_cta<<<npair, JTHREADS, smem_cta, st>>>(ws->Ap, np, JB, pr, ws->U, nullptr, 6, 1e-30);
+      k_jacobi_cta<<<npair, JTHREADS, smem_cta, st>>>(ws->Ap, np, JB, pr, ws->U, nullptr, inner, 1e-30);
       k_jac_col<<<dim3(np / JS, npair, 2), 256, smem_col, st>>>(ws->Ap, ws->Vp, np, pr, ws->U);
       k_jac_row<<<dim3(np / JS, npair), 256, smem_row, st>>>(ws->Ap, np, pr, ws->U);
     }
