@@ -4,18 +4,20 @@
 //
 // Everything runs on the device; the host only sequences launches and reads nbands residual norms (and
 // the Gram-matrix eigenvalues of the orthonormalisation) back per iteration.
-//   D0  X = orth(psi0)                        Gram matrix + Jacobi eigh (canonical orthonormalisation) x2
+//   D0  X = orth(psi0)                        Gram matrix + Cholesky (CholQR2)
 //   D1  W = H V                               ks_hpsi_impl on the new block only
 //   D2  Hc[:, new] = V^H W_new                DMMA GEMM (K = npw), mirrored to keep Hc Hermitian
 //   D3  Hc = C Theta C^H                      Jacobi (eigh.cu)
 //   D4  X = V C[:, :nb], HX = W C[:, :nb]     DMMA GEMMs (M = npw)
 //   D5  rho_i = ||HX_i - eps_i X_i||, Ekin_i  fused reduction, one CTA per band
 //   D6  T_i = K_i (HX_i - eps_i X_i)          Teter-Payne-Allan diagonal polynomial, fused, unconverged only
-//   D7  T <- (I - V V^H) T (x2, x1) ; T <- T U Lambda^{-1/2}, dropping lambda < 1e-10 lambda_max ; twice
+//   D7  T <- (I - V V^H) T (x2, x1) ; G = T^H T = R^H R (Cholesky with the Gram-Schmidt drop rule) ;
+//       T <- T R^{-1} ; twice (CholQR2)
 //   D8  V <- [V, T], restart V <- X when m + nu > 2 nb
 //   D9  psi <- X, eig, residuals
-// Difference from the oracle listing (reading C10): the orthonormalisation is Gram/eigh based instead of
-// modified Gram-Schmidt.  Both span the same space up to the drop rule; the converged pairs agree.
+// Difference from the oracle listing (reading C10): the orthonormalisation is Gram/Cholesky based (CholQR2,
+// the BLAS-3 form of Gram-Schmidt, same column order and the same kind of drop rule) instead of modified
+// Gram-Schmidt.  Both span the same space; the converged pairs agree.
 #include "ctx.h"
 #include <algorithm>
 #include <cmath>
@@ -124,14 +126,92 @@ __global__ void k_copy_mat(int m, int n, const cplx* __restrict__ a, long lda, c
   const int i = (int)(e % m), j = (int)(e / m);
   b[(long)j * ldb + i] = a[(long)j * lda + i];
 }
-// Mout[:, r] = U[:, r0 + r] / sqrt(lam[r0 + r]),  r < nk   (canonical orthonormalisation)
-__global__ void k_canon(int nu, int r0, int nk, const cplx* __restrict__ U, long ldu, const double* __restrict__ lam,
-                        cplx* __restrict__ Mout, long ldm) {
-  const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
-  if (e >= (long)nu * nk) return;
-  const int i = (int)(e % nu), r = (int)(e / nu);
-  const double s = 1.0 / sqrt(lam[r0 + r]);
-  Mout[(long)r * ldm + i] = cscale(s, U[(long)(r0 + r) * ldu + i]);
+// ------------------------------------------------------------------------------------------------
+// Orthonormalisation through the Gram matrix G = T^H T (unit diagonal): right-looking Cholesky
+// G = R^H R in one CTA, DROPPING column j when its remaining diagonal d_j = ||t_j - proj||^2 / ||t_j||^2
+// falls below thr (the Gram-Schmidt drop rule of the listing, in the same column order), then
+// M = R_kept^{-1} embedded in nu x nk, so that T M is orthonormal.  G is column-major; its upper
+// triangle is overwritten by R (R[j][k] at G[k*ld + j], k >= j).
+// ------------------------------------------------------------------------------------------------
+#define CHOL_THREADS 1024
+__global__ void __launch_bounds__(CHOL_THREADS) k_chol_drop(int n, cplx* __restrict__ G, long ld, double thr,
+                                                          int* __restrict__ kept, int* __restrict__ nk_out) {
+  extern __shared__ cplx rowj[];          // [n] current row of R
+  __shared__ double s_inv;
+  __shared__ int s_keep;
+  const int tid = threadIdx.x, nt = blockDim.x;
+  for (int j = 0; j < n; ++j) {
+    if (tid == 0) {
+      const double d = G[(long)j * ld + j].x;
+      s_keep = (d > thr) ? 1 : 0;
+      if (s_keep) {
+        const double r = sqrt(d);
+        G[(long)j * ld + j] = cmake(r, 0.0);
+        s_inv = 1.0 / r;
+      } else {
+        G[(long)j * ld + j] = cmake(0.0, 0.0);   // marks the column as dropped
+      }
+    }
+    __syncthreads();
+    if (!s_keep) continue;
+    const double inv = s_inv;
+    for (int k = j + 1 + tid; k < n; k += nt) {
+      const cplx v = cscale(inv, G[(long)k * ld + j]);
+      G[(long)k * ld + j] = v;
+      rowj[k] = v;
+    }
+    __syncthreads();
+    // trailing update of the upper triangle: G[i][k] -= conj(R[j][i]) R[j][k],  j < i <= k
+    const int m = n - j - 1;
+    for (long e = tid; e < (long)m * m; e += nt) {
+      const int i = j + 1 + (int)(e % m), k = j + 1 + (int)(e / m);
+      if (i <= k) {
+        const cplx a = rowj[i], b = rowj[k];
+        cplx g = G[(long)k * ld + i];
+        g.x -= a.x * b.x + a.y * b.y;
+        g.y -= a.x * b.y - a.y * b.x;
+        G[(long)k * ld + i] = g;
+      }
+    }
+    __syncthreads();
+  }
+  if (tid == 0) {
+    int nk = 0;
+    for (int j = 0; j < n; ++j)
+      if (G[(long)j * ld + j].x > 0.0) kept[nk++] = j;
+    *nk_out = nk;
+  }
+}
+
+// one warp per kept column jj: x = R_kept^{-1} e_jj by back substitution; M[:, jj] (nu rows) = scatter(x)
+__global__ void __launch_bounds__(128) k_trinv(int nu, const cplx* __restrict__ R, long ld, const int* __restrict__ kept, int nk,
+                                               cplx* __restrict__ M, long ldm) {
+  extern __shared__ cplx xs[];            // [4][nk]
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int jj = blockIdx.x * 4 + w;
+  if (jj >= nk) return;
+  cplx* x = xs + (size_t)w * nk;
+  for (int i = lane; i < nu; i += 32) M[(long)jj * ldm + i] = cmake(0.0, 0.0);
+  for (int ii = jj; ii >= 0; --ii) {
+    const int i = kept[ii];
+    double sr = 0, si = 0;
+    for (int kk = ii + 1 + lane; kk <= jj; kk += 32) {
+      const cplx r = R[(long)kept[kk] * ld + i], v = x[kk];
+      sr += r.x * v.x - r.y * v.y;
+      si += r.x * v.y + r.y * v.x;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+      sr += __shfl_xor_sync(0xffffffffu, sr, o);
+      si += __shfl_xor_sync(0xffffffffu, si, o);
+    }
+    if (lane == 0) {
+      const double rii = R[(long)i * ld + i].x;
+      x[ii] = cmake(((ii == jj ? 1.0 : 0.0) - sr) / rii, -si / rii);
+    }
+    __syncwarp();
+  }
+  __syncwarp();
+  for (int ii = lane; ii <= jj; ii += 32) M[(long)jj * ldm + kept[ii]] = x[ii];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -162,7 +242,7 @@ static int reserve(ks_ctx* c, int nb) {
   KS_CUDA_CHECK(cudaMalloc(&w.rho, sizeof(double) * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.ekin, sizeof(double) * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.lam, sizeof(double) * nb), c->err);
-  KS_CUDA_CHECK(cudaMalloc(&w.idx, sizeof(int) * nb), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.idx, sizeof(int) * (nb + 1)), c->err);
   w.nb_cap = nb;
   return KS_OK;
 }
@@ -195,7 +275,9 @@ enum { PH_HPSI = 0, PH_PROJ = 1, PH_EIGH = 2, PH_ROT = 3, PH_RESID = 4, PH_ORTH 
 #define RC(x) do { int rc__ = (x); if (rc__ < 0) return rc__; } while (0)
 
 // One pass of D7/D0:  src (npw x nu) -> dst (npw x nk): optional projection against V[0:m] (nproj times),
-// unit column norms, Gram matrix, Jacobi eigh, drop lambda < 1e-10 lambda_max, dst = src U Lambda^{-1/2}.
+// unit column norms, Gram matrix G, Cholesky G = R^H R dropping columns whose remaining squared norm is
+// below 1e-12 of the original (norm ratio 1e-6; the Gram form cannot resolve the listing's 1e-10),
+// dst = src R_kept^{-1}.
 static int orth_pass(ks_ctx* c, cplx* src, int nu, cplx* dst, int m, int nproj_pass, int* nk_out, Phase& ph) {
   DavidsonWs& w = c->dws;
   const int npw = c->P.npw;
@@ -211,20 +293,21 @@ static int orth_pass(ks_ctx* c, cplx* src, int nu, cplx* dst, int m, int nproj_p
   RC(ks_gemm_hn(st, nu, nu, npw, src, npw, src, npw, w.Us, nu, &c->gws, c->err));
   ph.end(PH_ORTH);
   ph.begin();
-  RC(ks_eigh_run(st, nu, w.Us, nu, w.lam, w.S, nu, &c->ews, nullptr, c->err));   // S <- eigenvectors (nu x nu)
-  std::vector<double> lam(nu);
-  KS_CUDA_CHECK(cudaMemcpyAsync(lam.data(), w.lam, sizeof(double) * nu, cudaMemcpyDeviceToHost, st), c->err);
+  static bool opted = false;
+  if (!opted) {
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_trinv, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 16 * 2048), c->err);
+    opted = true;
+  }
+  k_chol_drop<<<1, CHOL_THREADS, sizeof(cplx) * nu, st>>>(nu, w.Us, nu, 1e-12, w.idx, w.idx + nu);
+  int nk = 0;
+  KS_CUDA_CHECK(cudaMemcpyAsync(&nk, w.idx + nu, sizeof(int), cudaMemcpyDeviceToHost, st), c->err);
   KS_CUDA_CHECK(cudaStreamSynchronize(st), c->err);
-  ph.end(PH_EIGH);
-  const double lmax = lam[nu - 1];
-  int r0 = 0;
-  while (r0 < nu && !(lam[r0] > 1e-10 * lmax)) ++r0;
-  const int nk = nu - r0;
   *nk_out = nk;
-  if (nk == 0) return KS_OK;
+  if (nk == 0) { ph.end(PH_EIGH); return KS_OK; }
+  k_trinv<<<ceil_div(nk, 4), 128, sizeof(cplx) * 4 * nk, st>>>(nu, w.Us, nu, w.idx, nk, w.S, nu);
+  ph.end(PH_EIGH);
   ph.begin();
-  k_canon<<<ceil_div((long)nu * nk, 256), 256, 0, st>>>(nu, r0, nk, w.S, nu, w.lam, w.Us, nu);
-  RC(ks_gemm_nn(st, npw, nk, nu, src, npw, w.Us, nu, dst, npw, 0, c->err));
+  RC(ks_gemm_nn(st, npw, nk, nu, src, npw, w.S, nu, dst, npw, 0, c->err));
   ph.end(PH_ORTH);
   return KS_OK;
 }

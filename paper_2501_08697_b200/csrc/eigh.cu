@@ -19,7 +19,7 @@
 
 #define JB 32            // block size of the block method
 #define JS (2 * JB)      // pair problem size
-#define JTHREADS 512
+#define JTHREADS 1024
 #define JPAD 1.0e30      // diagonal of padding rows: decoupled (zero off-diagonals) and sorts last
 
 // round-robin pair k of round r for n (even) players: (n-1, r) for k = 0, else ((r+k) % (n-1), (r-k) % (n-1))
@@ -34,17 +34,24 @@ __host__ __device__ __forceinline__ void rr_pair(int n, int r, int k, int* p, in
 // ------------------------------------------------------------------------------------------------
 // one CTA per pair problem.  ns = 2*nbk (even, <= 64).  Gathers rows/cols {I*nbk.., J*nbk..} of Ap.
 // U (ns x ns, column-major, ld = ns) receives the accumulated rotations; dout (nullable) the diagonal.
+//
+// A round applies ns/2 disjoint rotations J_k = [[c, sg], [-conj(sg), c]] (sg = s e^{i phi}; this is the
+// rotation of the header times diag(1, e^{i phi}), which zeroes the same pivot).  Two barriers per round:
+//   phase 1  ns/2 threads: (c, sg) from a_pp, a_qq, a_pq.  With a = |a_pq|^2, d = (a_qq - a_pp)/2,
+//            r = sqrt(d^2 + a):  z = sign(d) a_pq / (|d| + r),  c = rsqrt(1 + |z|^2),  sg = c z.
+//   phase 2  one thread per 2x2 block (k, l):  A[{p_k,q_k},{p_l,q_l}] <- J_k^H (.) J_l  and
+//            V[{p_k,q_k},{p_l,q_l}] <- (.) J_l, all in registers.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(JTHREADS) k_jacobi_cta(const cplx* __restrict__ Ap, long ld, int nbk,
                                                         const int2* __restrict__ pairs, cplx* __restrict__ U,
                                                         double* __restrict__ dout, int max_sweeps, double tol2) {
   extern __shared__ cplx sm[];
-  const int ns = 2 * nbk, LD = ns + 1;
+  const int ns = 2 * nbk, LD = ns + 1, hp = ns / 2;
   cplx* As = sm;                       // As[i*LD + j] = A[i][j]
   cplx* Vs = As + ns * LD;
-  double* rc = (double*)(Vs + ns * LD);        // c[k]
-  double* rs = rc + JS / 2;                    // s[k]
-  cplx* re = (cplx*)(rs + JS / 2);             // e^{i phi}[k]
+  cplx* rsg = Vs + ns * LD;            // sg[k]
+  double* rc = (double*)(rsg + JS / 2);                 // c[k]
+  uchar2* sched = (uchar2*)(rc + JS / 2);               // [ns-1][hp] pivot pairs of every round
   __shared__ double red[2][JTHREADS / 32];
   __shared__ int stop;
   const int tid = threadIdx.x, nt = blockDim.x;
@@ -56,10 +63,14 @@ __global__ void __launch_bounds__(JTHREADS) k_jacobi_cta(const cplx* __restrict_
     As[i * LD + j] = Ap[(long)gj * ld + gi];
     Vs[i * LD + j] = cmake(i == j ? 1.0 : 0.0, 0.0);
   }
+  for (int e = tid; e < (ns - 1) * hp; e += nt) {
+    int p, q;
+    rr_pair(ns, e / hp, e % hp, &p, &q);
+    sched[e] = make_uchar2((unsigned char)p, (unsigned char)q);
+  }
   __syncthreads();
   for (int sweep = 0; sweep < max_sweeps; ++sweep) {
-    // convergence: off(A)_F^2 <= tol2 * ||A||_F^2 (padding rows excluded through their zero off-diagonals
-    // and by capping the diagonal contribution)
+    // convergence: off(A)_F^2 <= tol2 * ||A||_F^2 (padding rows: zero off-diagonals, diagonal excluded)
     double off = 0, tot = 0;
     for (int e = tid; e < ns * ns; e += nt) {
       const int i = e / ns, j = e % ns;
@@ -82,62 +93,58 @@ __global__ void __launch_bounds__(JTHREADS) k_jacobi_cta(const cplx* __restrict_
     __syncthreads();
     if (stop) break;
     for (int r = 0; r < ns - 1; ++r) {
-      if (tid < ns / 2) {
-        int p, q;
-        rr_pair(ns, r, tid, &p, &q);
+      const uchar2* sr = sched + r * hp;
+      if (tid < hp) {
+        const int p = sr[tid].x, q = sr[tid].y;
         const cplx apq = As[p * LD + q];
-        const double ab = sqrt(apq.x * apq.x + apq.y * apq.y);
-        double c = 1.0, s = 0.0;
-        cplx e = cmake(1.0, 0.0);
-        if (ab > 0.0) {
-          const double tau = (As[q * LD + q].x - As[p * LD + p].x) / (2.0 * ab);
-          const double t = (tau >= 0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
-          c = 1.0 / sqrt(1.0 + t * t);
-          s = t * c;
-          e = cmake(apq.x / ab, apq.y / ab);
+        const double a = apq.x * apq.x + apq.y * apq.y;
+        double c = 1.0;
+        cplx sg = cmake(0.0, 0.0);
+        if (a > 0.0) {
+          const double d = 0.5 * (As[q * LD + q].x - As[p * LD + p].x);
+          const double rr = sqrt(fma(d, d, a));
+          const double inv = (d >= 0.0 ? 1.0 : -1.0) / (fabs(d) + rr);
+          const cplx z = cmake(apq.x * inv, apq.y * inv);
+          c = rsqrt(fma(z.x, z.x, fma(z.y, z.y, 1.0)));
+          sg = cmake(c * z.x, c * z.y);
         }
-        rc[tid] = c; rs[tid] = s; re[tid] = e;
+        rc[tid] = c;
+        rsg[tid] = sg;
       }
       __syncthreads();
-      // columns of A and V:  x' = c x - s conj(e) y ,  y' = s x + c conj(e) y
-      for (int it = tid; it < (ns / 2) * ns; it += nt) {
-        const int i = it % ns, k = it / ns;
-        int p, q;
-        rr_pair(ns, r, k, &p, &q);
-        const double c = rc[k], s = rs[k];
-        const cplx ec = cconj(re[k]);
-        {
-          const cplx x = As[i * LD + p], y = cmul(ec, As[i * LD + q]);
-          As[i * LD + p] = cmake(c * x.x - s * y.x, c * x.y - s * y.y);
-          As[i * LD + q] = cmake(s * x.x + c * y.x, s * x.y + c * y.y);
+      for (int it = tid; it < hp * hp; it += nt) {
+        const int l = it % hp, k = it / hp;
+        const int pk = sr[k].x, qk = sr[k].y, pl = sr[l].x, ql = sr[l].y;
+        const double ck = rc[k], cl = rc[l];
+        const cplx sk = rsg[k], sl = rsg[l];
+        // right multiply by J_l:  x' = c x - conj(sg) y ,  y' = sg x + c y
+        cplx a00 = As[pk * LD + pl], a01 = As[pk * LD + ql], a10 = As[qk * LD + pl], a11 = As[qk * LD + ql];
+        cplx v00 = Vs[pk * LD + pl], v01 = Vs[pk * LD + ql], v10 = Vs[qk * LD + pl], v11 = Vs[qk * LD + ql];
+        const cplx slc = cconj(sl);
+#define ROTR(x, y)                                                              \
+        {                                                                       \
+          const cplx tx = csub(cscale(cl, x), cmul(slc, y));                    \
+          const cplx ty = cadd(cmul(sl, x), cscale(cl, y));                     \
+          x = tx; y = ty;                                                       \
         }
-        {
-          const cplx x = Vs[i * LD + p], y = cmul(ec, Vs[i * LD + q]);
-          Vs[i * LD + p] = cmake(c * x.x - s * y.x, c * x.y - s * y.y);
-          Vs[i * LD + q] = cmake(s * x.x + c * y.x, s * x.y + c * y.y);
+        ROTR(a00, a01) ROTR(a10, a11) ROTR(v00, v01) ROTR(v10, v11)
+#undef ROTR
+        // left multiply by J_k^H:  rp' = c rp - sg rq ,  rq' = conj(sg) rp + c rq
+        const cplx skc = cconj(sk);
+#define ROTL(x, y)                                                              \
+        {                                                                       \
+          const cplx tx = csub(cscale(ck, x), cmul(sk, y));                     \
+          const cplx ty = cadd(cmul(skc, x), cscale(ck, y));                    \
+          x = tx; y = ty;                                                       \
         }
-      }
-      __syncthreads();
-      // rows of A:  x' = c x - s e y ,  y' = s x + c e y
-      for (int it = tid; it < (ns / 2) * ns; it += nt) {
-        const int j = it % ns, k = it / ns;
-        int p, q;
-        rr_pair(ns, r, k, &p, &q);
-        const double c = rc[k], s = rs[k];
-        const cplx x = As[p * LD + j], y = cmul(re[k], As[q * LD + j]);
-        As[p * LD + j] = cmake(c * x.x - s * y.x, c * x.y - s * y.y);
-        As[q * LD + j] = cmake(s * x.x + c * y.x, s * x.y + c * y.y);
-      }
-      __syncthreads();
-      if (tid < ns / 2) {
-        int p, q;
-        rr_pair(ns, r, tid, &p, &q);
-        if (rs[tid] != 0.0) {
-          As[p * LD + q] = cmake(0.0, 0.0);
-          As[q * LD + p] = cmake(0.0, 0.0);
+        ROTL(a00, a10) ROTL(a01, a11)
+#undef ROTL
+        if (k == l) {
+          if (sk.x != 0.0 || sk.y != 0.0) { a01 = cmake(0.0, 0.0); a10 = cmake(0.0, 0.0); }
+          a00.y = 0.0; a11.y = 0.0;
         }
-        As[p * LD + p].y = 0.0;
-        As[q * LD + q].y = 0.0;
+        As[pk * LD + pl] = a00; As[pk * LD + ql] = a01; As[qk * LD + pl] = a10; As[qk * LD + ql] = a11;
+        Vs[pk * LD + pl] = v00; Vs[pk * LD + ql] = v01; Vs[qk * LD + pl] = v10; Vs[qk * LD + ql] = v11;
       }
       __syncthreads();
     }
@@ -152,42 +159,45 @@ __global__ void __launch_bounds__(JTHREADS) k_jacobi_cta(const cplx* __restrict_
 }
 
 // ------------------------------------------------------------------------------------------------
-// block updates: 64 x 64 x 64 complex GEMM tiles on DMMA, 8 warps as 2 (M) x 4 (N), warp tile 32 x 16
+// block updates: (rows x JSZ x JSZ) complex GEMM tiles on DMMA.  JSZ = pair size (2 blocks of JSZ/2).
+// 8 warps, warp tile 32 x 16 MMA layout (4 x 2 m8n8k4 tiles, four real DMMAs per complex product).
 // ------------------------------------------------------------------------------------------------
-#define JLDM (JS + 2)    // m-contiguous tile, == 2 (mod 8)
-#define JLDK (JS + 4)    // k-contiguous tile, == 4 (mod 8)
+template <int JSZ>
+__device__ __forceinline__ int blk_index(int2 pr, int i) {
+  return i < JSZ / 2 ? pr.x * (JSZ / 2) + i : pr.y * (JSZ / 2) + i - JSZ / 2;
+}
 
-__device__ __forceinline__ int blk_index(int2 pr, int i) { return i < JB ? pr.x * JB + i : pr.y * JB + i - JB; }
-
-// columns: X[:, IJ] <- X[:, IJ] U   for X = A (z = 0) and X = V (z = 1); rows m0 .. m0+63
-__global__ void __launch_bounds__(256) k_jac_col(cplx* __restrict__ Ap, cplx* __restrict__ Vp, long ld,
+// columns: X[:, IJ] <- X[:, IJ] U   for X = A (z = 0) and X = V (z = 1); rows m0 .. m0+MT-1
+template <int JSZ>
+__global__ void __launch_bounds__(256) k_jac_col(cplx* __restrict__ Ap, cplx* __restrict__ Vp, long ld, int np,
                                                  const int2* __restrict__ pairs, const cplx* __restrict__ U) {
+  constexpr int WN = JSZ / 16, WM = 8 / WN, MT = WM * 32, LDMJ = MT + 2, LDKJ = JSZ + 4;
   extern __shared__ cplx sm[];
   cplx* sP = sm;                   // [k][m]
-  cplx* sU = sm + JS * JLDM;       // [n][k]
+  cplx* sU = sm + JSZ * LDMJ;      // [n][k]
   cplx* X = blockIdx.z ? Vp : Ap;
   const int2 pr = pairs[blockIdx.y];
-  const int m0 = blockIdx.x * JS, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const cplx* Up = U + (size_t)blockIdx.y * JS * JS;
-  for (int e = tid; e < JS * JS; e += 256) {
-    const int a = e % JS, b = e / JS;
-    sP[b * JLDM + a] = X[(long)blk_index(pr, b) * ld + m0 + a];   // k = b (column), m = a
-    sU[b * JLDK + a] = Up[e];                                      // n = b, k = a
+  const int m0 = blockIdx.x * MT, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const cplx* Up = U + (size_t)blockIdx.y * JSZ * JSZ;
+  for (int e = tid; e < JSZ * MT; e += 256) {
+    const int a = e % MT, b = e / MT;                            // m = a, k = b
+    sP[b * LDMJ + a] = (m0 + a < np) ? X[(long)blk_index<JSZ>(pr, b) * ld + m0 + a] : cmake(0.0, 0.0);
   }
+  for (int e = tid; e < JSZ * JSZ; e += 256) sU[(e / JSZ) * LDKJ + (e % JSZ)] = Up[e];   // n = e / JSZ, k = e % JSZ
   __syncthreads();
-  const int wm = warp & 1, wn = warp >> 1, fr = lane >> 2, fk = lane & 3;
+  const int wm = warp % WM, wn = warp / WM, fr = lane >> 2, fk = lane & 3;
   double cre[4][2][2], cim[4][2][2];
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
     for (int j = 0; j < 2; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
 #pragma unroll 4
-  for (int ks = 0; ks < JS; ks += 4) {
+  for (int ks = 0; ks < JSZ; ks += 4) {
     cplx af[4], bf[2];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) af[i] = sP[(ks + fk) * JLDM + wm * 32 + i * 8 + fr];
+    for (int i = 0; i < 4; ++i) af[i] = sP[(ks + fk) * LDMJ + wm * 32 + i * 8 + fr];
 #pragma unroll
-    for (int j = 0; j < 2; ++j) bf[j] = sU[(wn * 16 + j * 8 + fr) * JLDK + ks + fk];
+    for (int j = 0; j < 2; ++j) bf[j] = sU[(wn * 16 + j * 8 + fr) * LDKJ + ks + fk];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       const double nai = -af[i].y;
@@ -207,38 +217,40 @@ __global__ void __launch_bounds__(256) k_jac_col(cplx* __restrict__ Ap, cplx* __
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         const int m = m0 + wm * 32 + i * 8 + fr, n = wn * 16 + j * 8 + 2 * fk + h;
-        X[(long)blk_index(pr, n) * ld + m] = cmake(cre[i][j][h], cim[i][j][h]);
+        if (m < np) X[(long)blk_index<JSZ>(pr, n) * ld + m] = cmake(cre[i][j][h], cim[i][j][h]);
       }
 }
 
-// rows: A[IJ, :] <- U^H A[IJ, :]   for columns n0 .. n0+63
-__global__ void __launch_bounds__(256) k_jac_row(cplx* __restrict__ Ap, long ld, const int2* __restrict__ pairs,
+// rows: A[IJ, :] <- U^H A[IJ, :]   for columns n0 .. n0+NT-1
+template <int JSZ>
+__global__ void __launch_bounds__(256) k_jac_row(cplx* __restrict__ Ap, long ld, int np, const int2* __restrict__ pairs,
                                                  const cplx* __restrict__ U) {
+  constexpr int WM = JSZ / 32, WN = 8 / WM, NT = WN * 16, LDKJ = JSZ + 4;
   extern __shared__ cplx sm[];
   cplx* sU = sm;                   // [m][k]  (U column m)
-  cplx* sB = sm + JS * JLDK;       // [n][k]  (A[IJ(k)][n0+n])
+  cplx* sB = sm + JSZ * LDKJ;      // [n][k]  (A[IJ(k)][n0+n])
   const int2 pr = pairs[blockIdx.y];
-  const int n0 = blockIdx.x * JS, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const cplx* Up = U + (size_t)blockIdx.y * JS * JS;
-  for (int e = tid; e < JS * JS; e += 256) {
-    const int a = e % JS, b = e / JS;
-    sU[b * JLDK + a] = Up[e];
-    sB[b * JLDK + a] = Ap[(long)(n0 + b) * ld + blk_index(pr, a)];
+  const int n0 = blockIdx.x * NT, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const cplx* Up = U + (size_t)blockIdx.y * JSZ * JSZ;
+  for (int e = tid; e < JSZ * JSZ; e += 256) sU[(e / JSZ) * LDKJ + (e % JSZ)] = Up[e];
+  for (int e = tid; e < JSZ * NT; e += 256) {
+    const int a = e % JSZ, b = e / JSZ;                          // k = a, n = b
+    sB[b * LDKJ + a] = (n0 + b < np) ? Ap[(long)(n0 + b) * ld + blk_index<JSZ>(pr, a)] : cmake(0.0, 0.0);
   }
   __syncthreads();
-  const int wm = warp & 1, wn = warp >> 1, fr = lane >> 2, fk = lane & 3;
+  const int wm = warp % WM, wn = warp / WM, fr = lane >> 2, fk = lane & 3;
   double cre[4][2][2], cim[4][2][2];
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
     for (int j = 0; j < 2; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
 #pragma unroll 4
-  for (int ks = 0; ks < JS; ks += 4) {
+  for (int ks = 0; ks < JSZ; ks += 4) {
     cplx af[4], bf[2];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) af[i] = sU[(wm * 32 + i * 8 + fr) * JLDK + ks + fk];
+    for (int i = 0; i < 4; ++i) af[i] = sU[(wm * 32 + i * 8 + fr) * LDKJ + ks + fk];
 #pragma unroll
-    for (int j = 0; j < 2; ++j) bf[j] = sB[(wn * 16 + j * 8 + fr) * JLDK + ks + fk];
+    for (int j = 0; j < 2; ++j) bf[j] = sB[(wn * 16 + j * 8 + fr) * LDKJ + ks + fk];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       const double nai = -af[i].y;
@@ -258,7 +270,7 @@ __global__ void __launch_bounds__(256) k_jac_row(cplx* __restrict__ Ap, long ld,
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         const int m = wm * 32 + i * 8 + fr, n = n0 + wn * 16 + j * 8 + 2 * fk + h;
-        Ap[(long)n * ld + blk_index(pr, m)] = cmake(cre[i][j][h], cim[i][j][h]);
+        if (n < np) Ap[(long)n * ld + blk_index<JSZ>(pr, m)] = cmake(cre[i][j][h], cim[i][j][h]);
       }
 }
 
@@ -344,24 +356,76 @@ static int eigh_reserve(EighWs* ws, int np, std::string& err) {
   return KS_OK;
 }
 
+template <int JSZ>
+static int block_sweeps(cudaStream_t st, int n, const cplx* A, long lda, EighWs* ws, double tol2, int inner, int* sweeps_out,
+                        std::string& err) {
+  constexpr int JBK = JSZ / 2;
+  constexpr int WNc = JSZ / 16, MT = (8 / WNc) * 32;          // k_jac_col tile rows
+  constexpr int WMr = JSZ / 32, NT = (8 / WMr) * 16;          // k_jac_row tile columns
+  const size_t smem_cta = sizeof(cplx) * 2 * JS * (JS + 1) + sizeof(cplx) * (JS / 2) + sizeof(double) * (JS / 2) + 2 * (JS - 1) * (JS / 2) + 64;
+  const size_t smem_col = sizeof(cplx) * (JSZ * (MT + 2) + JSZ * (JSZ + 4));
+  const size_t smem_row = sizeof(cplx) * (JSZ * (JSZ + 4) + NT * (JSZ + 4));
+  static bool opted = false;
+  if (!opted) {
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_jac_col<JSZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_col), err);
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_jac_row<JSZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row), err);
+    opted = true;
+  }
+  int nblk = ceil_div(n, JBK);
+  nblk += nblk & 1;
+  const int np = nblk * JBK, npair = nblk / 2;
+  int rc = eigh_reserve(ws, np, err);
+  if (rc) return rc;
+  ws->np = np;
+  if (ws->pairs_nblk != nblk) {
+    cudaFree(ws->pairs); ws->pairs = nullptr;
+    std::vector<int2> h((size_t)(nblk - 1) * npair);
+    for (int r = 0; r < nblk - 1; ++r)
+      for (int k = 0; k < npair; ++k) {
+        int p, q;
+        rr_pair(nblk, r, k, &p, &q);
+        h[(size_t)r * npair + k] = make_int2(p, q);
+      }
+    KS_CUDA_CHECK(cudaMalloc(&ws->pairs, sizeof(int2) * h.size()), err);
+    KS_CUDA_CHECK(cudaMemcpy(ws->pairs, h.data(), sizeof(int2) * h.size(), cudaMemcpyHostToDevice), err);
+    ws->pairs_nblk = nblk;
+  }
+  k_pad_copy<<<ceil_div((long)np * np, 256), 256, 0, st>>>(A, lda, n, ws->Ap, ws->Vp, np);
+  int sweeps = 0;
+  for (; sweeps < 40; ++sweeps) {
+    double h[2];
+    KS_CUDA_CHECK(cudaMemsetAsync(ws->red, 0, 2 * sizeof(double), st), err);
+    k_offnorm<<<148 * 2, 256, 0, st>>>(ws->Ap, np, n, ws->red);
+    KS_CUDA_CHECK(cudaMemcpyAsync(h, ws->red, sizeof h, cudaMemcpyDeviceToHost, st), err);
+    KS_CUDA_CHECK(cudaStreamSynchronize(st), err);
+    if (h[0] <= tol2 * h[1]) break;
+    for (int r = 0; r < nblk - 1; ++r) {
+      const int2* pr = ws->pairs + (size_t)r * npair;
+      k_jacobi_cta<<<npair, JSZ * JSZ / 4, smem_cta, st>>>(ws->Ap, np, JBK, pr, ws->U, nullptr, inner, 1e-30);
+      k_jac_col<JSZ><<<dim3(ceil_div(np, MT), npair, 2), 256, smem_col, st>>>(ws->Ap, ws->Vp, np, np, pr, ws->U);
+      k_jac_row<JSZ><<<dim3(ceil_div(np, NT), npair), 256, smem_row, st>>>(ws->Ap, np, np, pr, ws->U);
+    }
+  }
+  KS_CUDA_CHECK(cudaGetLastError(), err);
+  *sweeps_out = sweeps;
+  return KS_OK;
+}
+
 int ks_eigh_run(cudaStream_t st, int n, cplx* A, long lda, double* theta, cplx* C, long ldc, EighWs* ws,
                 int* sweeps_out, std::string& err) {
   if (n <= 0) return KS_OK;
   if (!ws) { err = "ks_eigh: no workspace"; return KS_EINVAL; }
   static bool opted = false;
-  const size_t smem_cta = sizeof(cplx) * 2 * JS * (JS + 1) + sizeof(double) * JS + sizeof(cplx) * (JS / 2);
-  const size_t smem_col = sizeof(cplx) * JS * (JLDM + JLDK), smem_row = sizeof(cplx) * 2 * JS * JLDK;
+  const size_t smem_cta = sizeof(cplx) * 2 * JS * (JS + 1) + sizeof(cplx) * (JS / 2) + sizeof(double) * (JS / 2) + 2 * (JS - 1) * (JS / 2) + 64;
   if (!opted) {
     KS_CUDA_CHECK(cudaFuncSetAttribute(k_jacobi_cta, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cta), err);
-    KS_CUDA_CHECK(cudaFuncSetAttribute(k_jac_col, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_col), err);
-    KS_CUDA_CHECK(cudaFuncSetAttribute(k_jac_row, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row), err);
     opted = true;
   }
   const double tol2 = 1e-28;   // off_F <= 1e-14 ||A||_F
   static int inner = 0;        // inner sweeps of the 64x64 pair problems in the block method
   if (!inner) {
     const char* e = getenv("KSPW_JAC_INNER");
-    inner = (e && atoi(e) > 0) ? atoi(e) : 6;
+    inner = (e && atoi(e) > 0) ? atoi(e) : 1;
   }
   int sweeps = 0;
   if (n <= JS) {
@@ -384,39 +448,17 @@ int ks_eigh_run(cudaStream_t st, int n, cplx* A, long lda, double* theta, cplx* 
     if (sweeps_out) *sweeps_out = -1;   // inner sweeps are not reported back
     return KS_OK;
   }
-  int nblk = ceil_div(n, JB);
-  nblk += nblk & 1;
-  const int np = nblk * JB, npair = nblk / 2;
-  int rc = eigh_reserve(ws, np, err);
+  int rc = 0;
+  static int force_blk = -1;
+  if (force_blk < 0) {
+    const char* e = getenv("KSPW_JAC_PAIR");
+    force_blk = e ? atoi(e) : 0;
+  }
+  const bool use32 = force_blk == 32 || (force_blk != 64 && n <= 640);
+  if (use32) rc = block_sweeps<32>(st, n, A, lda, ws, tol2, inner, &sweeps, err);
+  else rc = block_sweeps<64>(st, n, A, lda, ws, tol2, inner, &sweeps, err);
   if (rc) return rc;
-  if (ws->pairs_nblk != nblk) {
-    cudaFree(ws->pairs); ws->pairs = nullptr;
-    std::vector<int2> h((size_t)(nblk - 1) * npair);
-    for (int r = 0; r < nblk - 1; ++r)
-      for (int k = 0; k < npair; ++k) {
-        int p, q;
-        rr_pair(nblk, r, k, &p, &q);
-        h[(size_t)r * npair + k] = make_int2(p, q);
-      }
-    KS_CUDA_CHECK(cudaMalloc(&ws->pairs, sizeof(int2) * h.size()), err);
-    KS_CUDA_CHECK(cudaMemcpy(ws->pairs, h.data(), sizeof(int2) * h.size(), cudaMemcpyHostToDevice), err);
-    ws->pairs_nblk = nblk;
-  }
-  k_pad_copy<<<ceil_div((long)np * np, 256), 256, 0, st>>>(A, lda, n, ws->Ap, ws->Vp, np);
-  for (; sweeps < 30; ++sweeps) {
-    double h[2];
-    KS_CUDA_CHECK(cudaMemsetAsync(ws->red, 0, 2 * sizeof(double), st), err);
-    k_offnorm<<<148 * 2, 256, 0, st>>>(ws->Ap, np, n, ws->red);
-    KS_CUDA_CHECK(cudaMemcpyAsync(h, ws->red, sizeof h, cudaMemcpyDeviceToHost, st), err);
-    KS_CUDA_CHECK(cudaStreamSynchronize(st), err);
-    if (h[0] <= tol2 * h[1]) break;
-    for (int r = 0; r < nblk - 1; ++r) {
-      const int2* pr = ws->pairs + (size_t)r * npair;
-      k_jacobi_cta<<<npair, JTHREADS, smem_cta, st>>>(ws->Ap, np, JB, pr, ws->U, nullptr, inner, 1e-30);
-      k_jac_col<<<dim3(np / JS, npair, 2), 256, smem_col, st>>>(ws->Ap, ws->Vp, np, pr, ws->U);
-      k_jac_row<<<dim3(np / JS, npair), 256, smem_row, st>>>(ws->Ap, np, pr, ws->U);
-    }
-  }
+  const int np = ws->np;
   k_diag<<<ceil_div(np, 128), 128, 0, st>>>(ws->Ap, np, ws->diag);
   k_rank<<<ceil_div(np, 128), 128, 0, st>>>(ws->diag, np, n, ws->order, theta);
   k_gather_cols<<<ceil_div((long)n * n, 256), 256, 0, st>>>(ws->Vp, np, ws->order, n, C, ldc);

@@ -65,6 +65,7 @@ struct EighWs {
   int* order = nullptr;    // [np]
   int2* pairs = nullptr;   // [(nblk-1)][nblk/2] block pairs of every round
   int cap = 0;             // padded n the buffers hold
+  int np = 0;              // padded n of the current run
   int pairs_nblk = 0;      // nblk the pair table was built for
 };
 int ks_eigh_run(cudaStream_t st, int n, cplx* A, long lda, double* theta, cplx* C, long ldc, EighWs* ws,
