@@ -285,65 +285,97 @@ __global__ void __launch_bounds__(KS_YZ_THREADS) k_fwd_yz(YzArgs a) {
 // ------------------------------------------------------------------------------------------------
 // x pass: inverse FFT, V(r) multiply, forward FFT in one kernel
 // ------------------------------------------------------------------------------------------------
+// A CTA owns ZC consecutive (y',z') columns of one band and all NX x-positions.  The first codelet
+// pass reads the live planes straight from global memory into registers (rows that are not live are
+// zeros and never touched), the last one writes the live planes back from registers, so the tile
+// crosses shared memory only between the passes (two barriers per tile).  Thread t works on column
+// t % ZC and on the codelet lines t / ZC, t / ZC + G, ... (G = NT / ZC); every shared-memory offset is
+// a compile-time multiple of ZC plus one per-thread base.
 struct XArgs {
-  cplx* planes;         // [nb][L1][NY][NZ], in place
-  const double* vperm;  // [NX][NY][NZ]
+  cplx* planes;         // [nb][L1][NY*NZ], in place
+  const double* vperm;  // [NX][NY*NZ]
   const cplx* tw_x;
-  int L1, x0, ny, nz, zc;
+  int L1, x0;
+  long ncol;            // NY*NZ
 };
-#define KS_X_THREADS 256
+
+template <int NX> struct xcfg { static constexpr int ZC = 32, NT = 128, MINB = 4; };
+template <> struct xcfg<18> { static constexpr int ZC = 32, NT = 96, MINB = 4; };
+template <> struct xcfg<36> { static constexpr int ZC = 32, NT = 96, MINB = 4; };
+template <> struct xcfg<54> { static constexpr int ZC = 32, NT = 96, MINB = 4; };
+template <> struct xcfg<128> { static constexpr int ZC = 32, NT = 256, MINB = 2; };
 
 template <int NX>
-__global__ void __launch_bounds__(KS_X_THREADS) k_x(XArgs a) {
+__global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB) k_x(XArgs a) {
   constexpr int R1 = fac<NX>::R1, R2 = fac<NX>::R2;
+  constexpr int ZC = xcfg<NX>::ZC, NT = xcfg<NX>::NT, G = NT / ZC;
+  static_assert(NT % ZC == 0, "thread count must be a multiple of the column chunk");
   extern __shared__ cplx sm[];
   cplx* tw = sm;
   cplx* tile = sm + NX;
-  const int tid = threadIdx.x, nt = blockDim.x;
-  const int ZC = a.zc, nchunk = a.nz / ZC;
-  const int c = blockIdx.x % nchunk, yp = blockIdx.x / nchunk, b = blockIdx.y;
-  const size_t pstride = (size_t)a.ny * a.nz;
-  cplx* base = a.planes + (size_t)b * a.L1 * pstride + (size_t)yp * a.nz + c * ZC;
-  const double* vbase = a.vperm + (size_t)yp * a.nz + c * ZC;
-  for (int i = tid; i < NX; i += nt) tw[i] = a.tw_x[i];
-  for (int i = tid; i < NX * ZC; i += nt) {
-    const int x = i / ZC, pz = i % ZC;
-    int lx = x - a.x0;
-    if (lx < 0) lx += NX;
-    tile[i] = (lx < a.L1) ? base[(size_t)lx * pstride + pz] : cmake(0.0, 0.0);
+  const int tid = threadIdx.x, pz = tid % ZC, g = tid / ZC;
+  const unsigned ncol = (unsigned)a.ncol;      // one band's live planes (L1*ncol elements) fit 32-bit offsets
+  const unsigned col = blockIdx.x * ZC + pz;
+  const bool colok = col < ncol;              // ragged last chunk
+  cplx* base = a.planes + (size_t)blockIdx.y * a.L1 * a.ncol + (colok ? col : 0);
+  const double* vbase = a.vperm + (colok ? col : 0);
+  cplx* tcol = tile + pz;
+
+  auto load_in = [&](cplx (&v)[R1], int j2) {
+#pragma unroll
+    for (int j1 = 0; j1 < R1; ++j1) {
+      int lx = j1 * R2 + j2 - a.x0;
+      if (lx < 0) lx += NX;
+      v[j1] = (lx < a.L1 && colok) ? base[(unsigned)lx * ncol] : cmake(0.0, 0.0);
+    }
+  };
+  // pass 1 (type-A stage 1): global -> registers -> DFT-R1 -> twiddle -> tile
+  {
+    cplx v[R1];
+    int j2 = g;
+    if (j2 < R2) load_in(v, j2);
+    for (int i = tid; i < NX; i += NT) tw[i] = a.tw_x[i];
+    __syncthreads();
+    while (j2 < R2) {
+      dft<R1, +1>(v);
+      cplx* o = tcol + j2 * ZC;
+#pragma unroll
+      for (int k1 = 0; k1 < R1; ++k1) o[k1 * R2 * ZC] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw, j2 * k1);
+      j2 += G;
+      if (j2 < R2) load_in(v, j2);
+    }
   }
   __syncthreads();
-  for (int it = tid; it < ZC * R2; it += nt) lineA_stage1<NX, +1>(tile + (it % ZC), ZC, it / ZC, tw);
-  __syncthreads();
-  // type-A stage 2, V(r), type-B stage 1 on the same R2 elements, in registers
-  for (int it = tid; it < ZC * R1; it += nt) {
-    const int pz = it % ZC, k1 = it / ZC;
-    cplx v[R2];
+  // pass 2: type-A stage 2, V(r), type-B stage 1 on the same R2 elements, in registers
+  for (int k1 = g; k1 < R1; k1 += G) {
+    double vr[R2];
+    const double* vp = vbase + (size_t)k1 * R2 * a.ncol;
 #pragma unroll
-    for (int j2 = 0; j2 < R2; ++j2) v[j2] = tile[(k1 * R2 + j2) * ZC + pz];
+    for (int k2 = 0; k2 < R2; ++k2) vr[k2] = __ldg(vp + (unsigned)k2 * ncol);
+    cplx v[R2];
+    cplx* t = tcol + k1 * R2 * ZC;
+#pragma unroll
+    for (int j2 = 0; j2 < R2; ++j2) v[j2] = t[j2 * ZC];
     dft<R2, +1>(v);
 #pragma unroll
-    for (int k2 = 0; k2 < R2; ++k2) {
-      const double vr = __ldg(vbase + (size_t)(k1 * R2 + k2) * pstride + pz);
-      v[k2] = cmake(v[k2].x * vr, v[k2].y * vr);
-    }
+    for (int k2 = 0; k2 < R2; ++k2) v[k2] = cmake(v[k2].x * vr[k2], v[k2].y * vr[k2]);
     dft<R2, -1>(v);
 #pragma unroll
-    for (int q2 = 0; q2 < R2; ++q2)
-      tile[(k1 * R2 + q2) * ZC + pz] = (q2 == 0) ? v[0] : mul_tw<-1>(v[q2], tw, k1 * q2);
+    for (int q2 = 0; q2 < R2; ++q2) t[q2 * ZC] = (q2 == 0) ? v[0] : mul_tw<-1>(v[q2], tw, k1 * q2);
   }
   __syncthreads();
-  for (int it = tid; it < ZC * R2; it += nt) {
-    const int pz = it % ZC, q2 = it / ZC;
+  // pass 3 (type-B stage 2): tile -> DFT-R1 -> live planes (natural x = q1*R2 + q2)
+  for (int q2 = g; q2 < R2; q2 += G) {
     cplx v[R1];
+    const cplx* t = tcol + q2 * ZC;
 #pragma unroll
-    for (int k1 = 0; k1 < R1; ++k1) v[k1] = tile[(k1 * R2 + q2) * ZC + pz];
+    for (int k1 = 0; k1 < R1; ++k1) v[k1] = t[k1 * R2 * ZC];
     dft<R1, -1>(v);
 #pragma unroll
-    for (int q1 = 0; q1 < R1; ++q1) {   // natural x = q1*R2 + q2; only the live planes are kept
+    for (int q1 = 0; q1 < R1; ++q1) {
       int lx = q1 * R2 + q2 - a.x0;
       if (lx < 0) lx += NX;
-      if (lx < a.L1) base[(size_t)lx * pstride + pz] = v[q1];
+      if (lx < a.L1 && colok) base[(unsigned)lx * ncol] = v[q1];
     }
   }
 }
@@ -357,7 +389,7 @@ static size_t yz_smem(const HpsiPlan& P, int zc) {
   const size_t SZ = (size_t)(P.n3 | 1);
   return sizeof(cplx) * ((size_t)P.n2 + P.n3 + (size_t)P.smax * SZ + (size_t)P.n2 * zc);
 }
-static size_t x_smem(const HpsiPlan& P, int zc) { return sizeof(cplx) * ((size_t)P.n1 + (size_t)P.n1 * zc); }
+template <int NX> static constexpr size_t x_smem() { return sizeof(cplx) * ((size_t)NX + (size_t)NX * xcfg<NX>::ZC); }
 
 template <typename K>
 static cudaError_t opt_in(K kern, size_t bytes) {
@@ -384,13 +416,6 @@ int ks_hpsi_configure(HpsiPlan& P, std::string& err) {
     }
   if (!P.zc_yz) { err = "yz kernels: stick tile does not fit in 227 KB of shared memory"; return KS_ENOMEM; }
   P.smem_yz = yz_smem(P, P.zc_yz);
-  P.zc_x = 0;
-  for (int zc : cand) {
-    if (P.n3 % zc) continue;
-    if (x_smem(P, zc) <= 56 * 1024) { P.zc_x = zc; break; }   // >= 4 CTAs per SM
-  }
-  if (!P.zc_x) { err = "x kernel: tile does not fit"; return KS_ENOMEM; }
-  P.smem_x = x_smem(P, P.zc_x);
   cudaError_t e = cudaSuccess;
 #define C_(A_, B_)                                                              \
   if (P.n2 == A_ && P.n3 == B_) {                                               \
@@ -400,7 +425,7 @@ int ks_hpsi_configure(HpsiPlan& P, std::string& err) {
   KS_YZ_PAIRS(C_)
 #undef C_
   KS_CUDA_CHECK(e, err);
-#define C_(N_) if (P.n1 == N_) e = opt_in(k_x<N_>, P.smem_x);
+#define C_(N_) if (P.n1 == N_) { P.zc_x = xcfg<N_>::ZC; P.smem_x = x_smem<N_>(); e = opt_in(k_x<N_>, P.smem_x); }
   KS_X_SIZES(C_)
 #undef C_
   KS_CUDA_CHECK(e, err);
@@ -418,15 +443,15 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
   a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.zc = P.zc_yz; a.invN = 1.0 / (double)P.N;
   XArgs x;
   x.planes = P.d_planes; x.vperm = P.d_vperm; x.tw_x = P.d_tw[0];
-  x.L1 = P.L1; x.x0 = P.x0; x.ny = P.n2; x.nz = P.n3; x.zc = P.zc_x;
-  const dim3 gyz(P.L1, nb), gx((P.n3 / P.zc_x) * P.n2, nb);
+  x.L1 = P.L1; x.x0 = P.x0; x.ncol = (long)P.n2 * P.n3;
+  const dim3 gyz(P.L1, nb), gx(ceil_div(x.ncol, P.zc_x), nb);
   if (stage < 0 || stage == 0) {
 #define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_inv_yz<A_, B_><<<gyz, KS_YZ_THREADS, P.smem_yz, st>>>(a);
     KS_YZ_PAIRS(C_)
 #undef C_
   }
   if (stage < 0 || stage == 1) {
-#define C_(N_) if (P.n1 == N_) k_x<N_><<<gx, KS_X_THREADS, P.smem_x, st>>>(x);
+#define C_(N_) if (P.n1 == N_) k_x<N_><<<gx, xcfg<N_>::NT, P.smem_x, st>>>(x);
     KS_X_SIZES(C_)
 #undef C_
   }
