@@ -110,7 +110,7 @@ static int auto_batch(const HpsiPlan& P) {
   const char* env = getenv("KSPW_FFT_BATCH");
   if (env && atoi(env) > 0) return atoi(env);
   const double per = 16.0 * P.L1 * P.n2 * P.n3;
-  int b = (int)(80.0e6 / per);     // keep one batch of live planes inside the 126 MB L2
+  int b = (int)(512.0e6 / per);    // several waves of CTAs per launch; the planes stream through HBM (L2 cannot hold a useful batch)
   return std::max(2, std::min(b, 1024));
 }
 
@@ -144,8 +144,8 @@ static int create_impl(ks_ctx* c, const double* cell, const double* kf, double e
     }
   }
   // live planes, sticks, position maps (PW order is m1 slowest, so planes and sticks are contiguous runs)
-  const int SZ = P.n3 | 1;
-  std::vector<int> plane_s0, plane_y0, plane_pw0, pw_pos(P.npw);
+  std::vector<int> plane_s0, plane_y0;
+  std::vector<int4> stick;
   int nst = 0, smax = 0, cur_m1 = 0, cur_m2 = 0, cur_m3 = 0, s_in_plane = 0;
   for (int j = 0; j < P.npw; ++j) {
     const int m1 = mil[3 * j], m2 = mil[3 * j + 1], m3 = mil[3 * j + 2];
@@ -154,7 +154,6 @@ static int create_impl(ks_ctx* c, const double* cell, const double* kf, double e
     if (new_plane) {
       if (j && m1 != cur_m1 + 1) { err = "G sphere: live x-planes are not contiguous"; return KS_EINVAL; }
       plane_s0.push_back(nst);
-      plane_pw0.push_back(j);
       plane_y0.push_back(pmod(m2, P.n2));
       smax = std::max(smax, s_in_plane);
       s_in_plane = 0;
@@ -162,13 +161,13 @@ static int create_impl(ks_ctx* c, const double* cell, const double* kf, double e
     if (new_stick) {
       if (!new_plane && m2 != cur_m2 + 1) { err = "G sphere: sticks of a plane are not contiguous in m2"; return KS_EINVAL; }
       ++nst; ++s_in_plane;
+      stick.push_back(make_int4(j, pmod(m3, P.n3), 0, 0));
     } else if (m3 != cur_m3 + 1) { err = "G sphere: a stick is not contiguous in m3"; return KS_EINVAL; }
-    pw_pos[j] = (s_in_plane - 1) * SZ + pmod(m3, P.n3);
+    ++stick.back().z;
     cur_m1 = m1; cur_m2 = m2; cur_m3 = m3;
   }
   smax = std::max(smax, s_in_plane);
   plane_s0.push_back(nst);
-  plane_pw0.push_back(P.npw);
   P.L1 = (int)plane_y0.size();
   P.x0 = pmod(mil[0], P.n1);
   P.nsticks = nst;
@@ -177,8 +176,7 @@ static int create_impl(ks_ctx* c, const double* cell, const double* kf, double e
   int rc;
   if ((rc = upload(&P.d_plane_s0, plane_s0, err))) return rc;
   if ((rc = upload(&P.d_plane_y0, plane_y0, err))) return rc;
-  if ((rc = upload(&P.d_plane_pw0, plane_pw0, err))) return rc;
-  if ((rc = upload(&P.d_pw_pos, pw_pos, err))) return rc;
+  if ((rc = upload(&P.d_stick, stick, err))) return rc;
   if ((rc = upload(&P.d_g2, g2, err))) return rc;
   for (int ax = 0; ax < 3; ++ax) {
     const int n = grid[ax];
@@ -242,7 +240,7 @@ extern "C" int ks_create(ks_ctx** out, const double cell[9], const double k_frac
 extern "C" void ks_destroy(ks_ctx* c) {
   if (!c) return;
   HpsiPlan& P = c->P;
-  cudaFree(P.d_plane_s0); cudaFree(P.d_plane_y0); cudaFree(P.d_plane_pw0); cudaFree(P.d_pw_pos);
+  cudaFree(P.d_plane_s0); cudaFree(P.d_plane_y0); cudaFree(P.d_stick);
   cudaFree(P.d_g2); cudaFree(P.d_vperm); cudaFree(P.d_planes);
   for (int i = 0; i < 3; ++i) cudaFree(P.d_tw[i]);
   cudaFree(c->d_beta); cudaFree(c->d_D); cudaFree(c->d_proj_atom); cudaFree(c->d_off); cudaFree(c->d_doff);

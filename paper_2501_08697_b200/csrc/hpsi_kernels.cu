@@ -150,135 +150,212 @@ int ks_build_vperm(HpsiPlan& P, const cplx* vhat_host, cudaStream_t st, std::str
 }
 
 // ------------------------------------------------------------------------------------------------
-// shared-memory carve-up of the yz kernels
+// yz kernels: one CTA per (band, live x-plane)
 // ------------------------------------------------------------------------------------------------
+// Shared memory: tw_y[NY], tw_z[NZ], stile[smax][NZ|1] (the plane's z-sticks), ytile[NY][ZC] (one chunk of
+// z' positions during the y transform).  The first codelet pass of the inverse kernel reads psi straight
+// from global memory (a stick's coefficients are a contiguous run of psi: no zero fill, no scatter pass,
+// no index array), the last pass of the forward kernel writes hpsi straight from registers (gather,
+// 1/N and the kinetic term fused).  Stick passes map threads lines-first over (stick, codelet line) with an
+// odd stick stride; y passes map thread t to column t % ZC and lines t / ZC, t / ZC + G, ...
 struct YzArgs {
   const cplx* psi;      // [nb][npw]
   cplx* hpsi;           // [nb][npw] (forward kernel only)
   cplx* planes;         // [nb][L1][NY][NZ]
-  const int* plane_s0;
-  const int* plane_y0;
-  const int* plane_pw0;
-  const int* pw_pos;
+  const int* plane_s0;  // [L1+1] first stick of each plane
+  const int* plane_y0;  // [L1]   natural y index of the plane's first stick
+  const int4* stick;    // [nsticks] {first PW, natural z index of the first PW, number of PWs, 0}
   const double* g2;
   const cplx* tw_y;
   const cplx* tw_z;
-  int npw, L1, smax, zc;
+  int npw, L1, smax;
   double invN;
 };
 
-#define KS_YZ_THREADS 256
+constexpr int yz_pick_zc(int nz) {
+  for (int zc = 32; zc >= 1; --zc)
+    if (nz % zc == 0) return zc;
+  return 1;
+}
+template <int NY, int NZ> struct yzcfg { static constexpr int ZC = yz_pick_zc(NZ), NT = 256; };
+template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 512; };
+template <> struct yzcfg<96, 288> { static constexpr int ZC = 16, NT = 256; };
+
+// lines-first walk over (stick s, line j) pairs: item it = j*S + s, it = tid, tid + NT, ...
+struct StickWalk {
+  int s, j, ds, dj, S;
+  __device__ __forceinline__ StickWalk(int tid, int nt, int S_) : S(S_) {
+    s = tid % S; j = tid / S; ds = nt % S; dj = nt / S;
+  }
+  __device__ __forceinline__ void next() {
+    s += ds; j += dj;
+    if (s >= S) { s -= S; ++j; }
+  }
+};
 
 template <int NY, int NZ>
-__global__ void __launch_bounds__(KS_YZ_THREADS) k_inv_yz(YzArgs a) {
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_inv_yz(YzArgs a) {
   constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = fac<NZ>::R1, R2z = fac<NZ>::R2;
-  constexpr int SZ = NZ | 1;
+  constexpr int SZ = NZ | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
   extern __shared__ cplx sm[];
   cplx* tw_y = sm;
   cplx* tw_z = tw_y + NY;
   cplx* stile = tw_z + NZ;
   cplx* ytile = stile + (size_t)a.smax * SZ;
-  const int tid = threadIdx.x, nt = blockDim.x;
+  const int tid = threadIdx.x;
   const int lx = blockIdx.x, b = blockIdx.y;
   const int s0 = a.plane_s0[lx], S = a.plane_s0[lx + 1] - s0;
   const int y0 = a.plane_y0[lx];
-  const int pw0 = a.plane_pw0[lx], pw1 = a.plane_pw0[lx + 1];
-  const int ZC = a.zc;
-  for (int i = tid; i < NY; i += nt) tw_y[i] = a.tw_y[i];
-  for (int i = tid; i < NZ; i += nt) tw_z[i] = a.tw_z[i];
-  for (int i = tid; i < S * SZ; i += nt) stile[i] = cmake(0.0, 0.0);
-  __syncthreads();
-  // H1: scatter this plane's coefficients onto its sticks
   const cplx* psi = a.psi + (size_t)b * a.npw;
-  for (int j = pw0 + tid; j < pw1; j += nt) stile[a.pw_pos[j]] = psi[j];
-  __syncthreads();
-  // H2 (z): type-A inverse FFT on each stick, lines-first mapping
-  for (int it = tid; it < S * R2z; it += nt) lineA_stage1<NZ, +1>(stile + (it % S) * SZ, 1, it / S, tw_z);
-  __syncthreads();
-  for (int it = tid; it < S * R1z; it += nt) lineA_stage2<NZ, +1>(stile + (it % S) * SZ, 1, it / S);
-  __syncthreads();
-  // H2 (y): for each chunk of z positions, type-A inverse FFT along y; output straight to HBM
-  cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ);
-  for (int c = 0; c < NZ / ZC; ++c) {
-    for (int it = tid; it < ZC * R2y; it += nt) {
-      const int pz = it % ZC, j2 = it / ZC, p = c * ZC + pz;
-      cplx v[R1y];
+  // H1 + H2 (z) pass 1: psi -> registers -> DFT-R1z -> twiddle -> stick tile (type A, inverse)
+  {
+    StickWalk w(tid, NT, S);
+    cplx v[R1z];
+    auto load_in = [&]() {
+      const int4 si = __ldg(a.stick + s0 + w.s);
+      const cplx* src = psi + si.x;
 #pragma unroll
-      for (int j1 = 0; j1 < R1y; ++j1) {
-        int s = j1 * R2y + j2 - y0;
-        if (s < 0) s += NY;
-        v[j1] = (s < S) ? stile[s * SZ + p] : cmake(0.0, 0.0);
+      for (int j1 = 0; j1 < R1z; ++j1) {
+        int idx = j1 * R2z + w.j - si.y;
+        if (idx < 0) idx += NZ;
+        v[j1] = (idx < si.z) ? src[idx] : cmake(0.0, 0.0);
       }
-      dft<R1y, +1>(v);
+    };
+    if (w.j < R2z) load_in();
+    for (int i = tid; i < NY; i += NT) tw_y[i] = a.tw_y[i];
+    for (int i = tid; i < NZ; i += NT) tw_z[i] = a.tw_z[i];
+    __syncthreads();
+    while (w.j < R2z) {
+      dft<R1z, +1>(v);
+      cplx* o = stile + w.s * SZ + w.j;
+      const int j2 = w.j;
 #pragma unroll
-      for (int k1 = 0; k1 < R1y; ++k1)
-        ytile[(k1 * R2y + j2) * ZC + pz] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw_y, j2 * k1);
+      for (int k1 = 0; k1 < R1z; ++k1) o[k1 * R2z] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw_z, j2 * k1);
+      w.next();
+      if (w.j < R2z) load_in();
+    }
+  }
+  __syncthreads();
+  for (StickWalk w(tid, NT, S); w.j < R1z; w.next()) lineA_stage2<NZ, +1>(stile + w.s * SZ, 1, w.j);
+  __syncthreads();
+  // H2 (y): for each chunk of z' positions, type-A inverse FFT along y; output straight to HBM
+  cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ);
+  const int pz = tid % ZC, g = tid / ZC;
+  for (int c = 0; c < NZ / ZC; ++c) {
+    if (g < G) {
+      for (int j2 = g; j2 < R2y; j2 += G) {
+        cplx v[R1y];
+        const cplx* src = stile + c * ZC + pz;
+#pragma unroll
+        for (int j1 = 0; j1 < R1y; ++j1) {
+          int s = j1 * R2y + j2 - y0;
+          if (s < 0) s += NY;
+          v[j1] = (s < S) ? src[s * SZ] : cmake(0.0, 0.0);
+        }
+        dft<R1y, +1>(v);
+        cplx* o = ytile + j2 * ZC + pz;
+#pragma unroll
+        for (int k1 = 0; k1 < R1y; ++k1) o[k1 * R2y * ZC] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw_y, j2 * k1);
+      }
     }
     __syncthreads();
-    for (int it = tid; it < ZC * R1y; it += nt) {
-      const int pz = it % ZC, k1 = it / ZC;
-      cplx v[R2y];
+    if (g < G) {
+      for (int k1 = g; k1 < R1y; k1 += G) {
+        cplx v[R2y];
+        const cplx* t = ytile + k1 * R2y * ZC + pz;
 #pragma unroll
-      for (int j2 = 0; j2 < R2y; ++j2) v[j2] = ytile[(k1 * R2y + j2) * ZC + pz];
-      dft<R2y, +1>(v);
+        for (int j2 = 0; j2 < R2y; ++j2) v[j2] = t[j2 * ZC];
+        dft<R2y, +1>(v);
+        cplx* o = plane + (size_t)(k1 * R2y) * NZ + c * ZC + pz;
 #pragma unroll
-      for (int k2 = 0; k2 < R2y; ++k2) plane[(size_t)(k1 * R2y + k2) * NZ + c * ZC + pz] = v[k2];
+        for (int k2 = 0; k2 < R2y; ++k2) o[k2 * NZ] = v[k2];
+      }
     }
     __syncthreads();
   }
 }
 
 template <int NY, int NZ>
-__global__ void __launch_bounds__(KS_YZ_THREADS) k_fwd_yz(YzArgs a) {
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_fwd_yz(YzArgs a) {
   constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = fac<NZ>::R1, R2z = fac<NZ>::R2;
-  constexpr int SZ = NZ | 1;
+  constexpr int SZ = NZ | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
   extern __shared__ cplx sm[];
   cplx* tw_y = sm;
   cplx* tw_z = tw_y + NY;
   cplx* stile = tw_z + NZ;
   cplx* ytile = stile + (size_t)a.smax * SZ;
-  const int tid = threadIdx.x, nt = blockDim.x;
+  const int tid = threadIdx.x;
   const int lx = blockIdx.x, b = blockIdx.y;
   const int s0 = a.plane_s0[lx], S = a.plane_s0[lx + 1] - s0;
   const int y0 = a.plane_y0[lx];
-  const int pw0 = a.plane_pw0[lx], pw1 = a.plane_pw0[lx + 1];
-  const int ZC = a.zc;
-  for (int i = tid; i < NY; i += nt) tw_y[i] = a.tw_y[i];
-  for (int i = tid; i < NZ; i += nt) tw_z[i] = a.tw_z[i];
   const cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ);
-  for (int c = 0; c < NZ / ZC; ++c) {
-    for (int i = tid; i < NY * ZC; i += nt) ytile[i] = plane[(size_t)(i / ZC) * NZ + c * ZC + (i % ZC)];
-    __syncthreads();
-    // H4 (y): type-B forward FFT along y
-    for (int it = tid; it < ZC * R1y; it += nt) lineB_stage1<NY, -1>(ytile + (it % ZC), ZC, it / ZC, tw_y);
-    __syncthreads();
-    for (int it = tid; it < ZC * R2y; it += nt) {
-      const int pz = it % ZC, q2 = it / ZC;
-      cplx v[R1y];
+  const int pz = tid % ZC, g = tid / ZC;
+  // H4 (y) pass 1 of a chunk: plane -> registers -> DFT-R2y -> twiddle -> ytile (type B, forward)
+  auto load_in = [&](cplx (&v)[R2y], int c, int k1) {
+    const cplx* src = plane + (size_t)(k1 * R2y) * NZ + c * ZC + pz;
 #pragma unroll
-      for (int k1 = 0; k1 < R1y; ++k1) v[k1] = ytile[(k1 * R2y + q2) * ZC + pz];
-      dft<R1y, -1>(v);
+    for (int k2 = 0; k2 < R2y; ++k2) v[k2] = src[k2 * NZ];
+  };
+  {
+    cplx v[R2y];
+    if (g < G && g < R1y) load_in(v, 0, g);
+    for (int i = tid; i < NY; i += NT) tw_y[i] = a.tw_y[i];
+    for (int i = tid; i < NZ; i += NT) tw_z[i] = a.tw_z[i];
+    __syncthreads();
+    for (int c = 0; c < NZ / ZC; ++c) {
+      if (g < G) {
+        for (int k1 = g; k1 < R1y; k1 += G) {
+          if (k1 != g || c != 0) load_in(v, c, k1);
+          dft<R2y, -1>(v);
+          cplx* o = ytile + k1 * R2y * ZC + pz;
 #pragma unroll
-      for (int q1 = 0; q1 < R1y; ++q1) {   // natural y = q1*R2y + q2; keep the stick columns only
-        int s = q1 * R2y + q2 - y0;
-        if (s < 0) s += NY;
-        if (s < S) stile[s * SZ + c * ZC + pz] = v[q1];
+          for (int q2 = 0; q2 < R2y; ++q2) o[q2 * ZC] = (q2 == 0) ? v[0] : mul_tw<-1>(v[q2], tw_y, k1 * q2);
+        }
       }
+      __syncthreads();
+      if (g < G) {
+        for (int q2 = g; q2 < R2y; q2 += G) {
+          cplx u[R1y];
+          const cplx* t = ytile + q2 * ZC + pz;
+#pragma unroll
+          for (int k1 = 0; k1 < R1y; ++k1) u[k1] = t[k1 * R2y * ZC];
+          dft<R1y, -1>(u);
+          cplx* o = stile + c * ZC + pz;
+#pragma unroll
+          for (int q1 = 0; q1 < R1y; ++q1) {   // natural y = q1*R2y + q2; keep the stick columns only
+            int s = q1 * R2y + q2 - y0;
+            if (s < 0) s += NY;
+            if (s < S) o[s * SZ] = u[q1];
+          }
+        }
+      }
+      __syncthreads();
     }
-    __syncthreads();
   }
   // H4 (z): type-B forward FFT on each stick
-  for (int it = tid; it < S * R1z; it += nt) lineB_stage1<NZ, -1>(stile + (it % S) * SZ, 1, it / S, tw_z);
+  for (StickWalk w(tid, NT, S); w.j < R1z; w.next()) lineB_stage1<NZ, -1>(stile + w.s * SZ, 1, w.j, tw_z);
   __syncthreads();
-  for (int it = tid; it < S * R2z; it += nt) lineB_stage2<NZ, -1>(stile + (it % S) * SZ, 1, it / S);
-  __syncthreads();
-  // H5: gather + kinetic term
+  // last pass + H5: DFT-R1z, then hpsi = |k+G|^2 psi + (.)/N written straight to the stick's run of hpsi
   const cplx* psi = a.psi + (size_t)b * a.npw;
   cplx* hpsi = a.hpsi + (size_t)b * a.npw;
-  for (int j = pw0 + tid; j < pw1; j += nt) {
-    const cplx g = stile[a.pw_pos[j]], p = psi[j];
-    const double k = a.g2[j];
-    hpsi[j] = cmake(fma(k, p.x, g.x * a.invN), fma(k, p.y, g.y * a.invN));
+  for (StickWalk w(tid, NT, S); w.j < R2z; w.next()) {
+    const int4 si = __ldg(a.stick + s0 + w.s);
+    cplx v[R1z];
+    const cplx* t = stile + w.s * SZ + w.j;
+#pragma unroll
+    for (int k1 = 0; k1 < R1z; ++k1) v[k1] = t[k1 * R2z];
+    dft<R1z, -1>(v);
+#pragma unroll
+    for (int q1 = 0; q1 < R1z; ++q1) {       // natural z = q1*R2z + q2
+      int idx = q1 * R2z + w.j - si.y;
+      if (idx < 0) idx += NZ;
+      if (idx < si.z) {
+        const int j = si.x + idx;
+        const cplx p = psi[j];
+        const double k = __ldg(a.g2 + j);
+        hpsi[j] = cmake(fma(k, p.x, v[q1].x * a.invN), fma(k, p.y, v[q1].y * a.invN));
+      }
+    }
   }
 }
 
@@ -404,21 +481,13 @@ int ks_hpsi_configure(HpsiPlan& P, std::string& err) {
     err = b;
     return KS_EGRID;
   }
-  // z-chunk: largest of 32/16/8/... dividing n3 that fits; prefer two CTAs per SM for the yz kernels
-  const int cand[] = {32, 16, 8, 4, 2, 1};
-  P.zc_yz = 0;
-  for (int pass = 0; pass < 2 && !P.zc_yz; ++pass)
-    for (int zc : cand) {
-      if (P.n3 % zc) continue;
-      const size_t need = yz_smem(P, zc);
-      if (need <= (pass == 0 ? KS_SMEM_MAX / 2 - 1024 : KS_SMEM_MAX)) { P.zc_yz = zc; break; }
-      if (pass == 0 && zc <= 8) break;   // do not shrink below 8 just to reach two CTAs/SM
-    }
-  if (!P.zc_yz) { err = "yz kernels: stick tile does not fit in 227 KB of shared memory"; return KS_ENOMEM; }
-  P.smem_yz = yz_smem(P, P.zc_yz);
   cudaError_t e = cudaSuccess;
+  P.zc_yz = 0;
 #define C_(A_, B_)                                                              \
   if (P.n2 == A_ && P.n3 == B_) {                                               \
+    P.zc_yz = yzcfg<A_, B_>::ZC;                                                \
+    P.smem_yz = yz_smem(P, P.zc_yz);                                            \
+    if (P.smem_yz > KS_SMEM_MAX) { err = "yz kernels: stick tile does not fit in 227 KB of shared memory"; return KS_ENOMEM; } \
     e = opt_in(k_inv_yz<A_, B_>, P.smem_yz);                                    \
     if (e == cudaSuccess) e = opt_in(k_fwd_yz<A_, B_>, P.smem_yz);              \
   }
@@ -438,15 +507,15 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
   if (nb > P.batch_cap) { err = "internal: FFT batch larger than workspace"; return KS_EINVAL; }
   YzArgs a;
   a.psi = psi; a.hpsi = hpsi; a.planes = P.d_planes;
-  a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.plane_pw0 = P.d_plane_pw0;
-  a.pw_pos = P.d_pw_pos; a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
-  a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.zc = P.zc_yz; a.invN = 1.0 / (double)P.N;
+  a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.stick = P.d_stick;
+  a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
+  a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.invN = 1.0 / (double)P.N;
   XArgs x;
   x.planes = P.d_planes; x.vperm = P.d_vperm; x.tw_x = P.d_tw[0];
   x.L1 = P.L1; x.x0 = P.x0; x.ncol = (long)P.n2 * P.n3;
   const dim3 gyz(P.L1, nb), gx(ceil_div(x.ncol, P.zc_x), nb);
   if (stage < 0 || stage == 0) {
-#define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_inv_yz<A_, B_><<<gyz, KS_YZ_THREADS, P.smem_yz, st>>>(a);
+#define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_inv_yz<A_, B_><<<gyz, yzcfg<A_, B_>::NT, P.smem_yz, st>>>(a);
     KS_YZ_PAIRS(C_)
 #undef C_
   }
@@ -456,7 +525,7 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
 #undef C_
   }
   if (stage < 0 || stage == 2) {
-#define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_fwd_yz<A_, B_><<<gyz, KS_YZ_THREADS, P.smem_yz, st>>>(a);
+#define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_fwd_yz<A_, B_><<<gyz, yzcfg<A_, B_>::NT, P.smem_yz, st>>>(a);
     KS_YZ_PAIRS(C_)
 #undef C_
   }

@@ -16,8 +16,8 @@ struct HpsiPlan {
   // device arrays
   int* d_plane_s0 = nullptr;   // [L1+1] first stick of each plane
   int* d_plane_y0 = nullptr;   // [L1]   natural y index (m2min mod n2) of the plane's first stick
-  int* d_plane_pw0 = nullptr;  // [L1+1] first plane wave of each plane (PWs of a plane are contiguous)
-  int* d_pw_pos = nullptr;     // [npw]  position of PW j in its plane's stick tile: s_local*SZ + z
+  int4* d_stick = nullptr;     // [nsticks] {first PW, natural z index (m3min mod n3) of it, number of PWs, 0}:
+                               //           a stick's coefficients are a contiguous run of psi, ascending in m3
   double* d_g2 = nullptr;      // [npw]  |k+G|^2
   double* d_vperm = nullptr;   // [n1][n2][n3] V(r) in position (type-A output) order on all three axes
   cplx* d_tw[3] = {nullptr, nullptr, nullptr};  // e^{+2 pi i t/n_i}
