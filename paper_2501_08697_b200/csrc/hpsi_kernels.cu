@@ -199,7 +199,7 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_inv_yz(YzArgs a) {
   constexpr int SZ = NZ | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
   extern __shared__ cplx sm[];
   cplx* tw_y = sm;
-  cplx* tw_z = tw_y + NY;
+  cplx* tw_z = (NY == NZ) ? tw_y : tw_y + NY;     // equal lengths share one twiddle table
   cplx* stile = tw_z + NZ;
   cplx* ytile = stile + (size_t)a.smax * SZ;
   const int tid = threadIdx.x;
@@ -223,7 +223,8 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_inv_yz(YzArgs a) {
     };
     if (w.j < R2z) load_in();
     for (int i = tid; i < NY; i += NT) tw_y[i] = a.tw_y[i];
-    for (int i = tid; i < NZ; i += NT) tw_z[i] = a.tw_z[i];
+    if (NY != NZ)
+      for (int i = tid; i < NZ; i += NT) tw_z[i] = a.tw_z[i];
     __syncthreads();
     while (w.j < R2z) {
       dft<R1z, +1>(v);
@@ -281,7 +282,7 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_fwd_yz(YzArgs a) {
   constexpr int SZ = NZ | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
   extern __shared__ cplx sm[];
   cplx* tw_y = sm;
-  cplx* tw_z = tw_y + NY;
+  cplx* tw_z = (NY == NZ) ? tw_y : tw_y + NY;     // equal lengths share one twiddle table
   cplx* stile = tw_z + NZ;
   cplx* ytile = stile + (size_t)a.smax * SZ;
   const int tid = threadIdx.x;
@@ -300,7 +301,8 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_fwd_yz(YzArgs a) {
     cplx v[R2y];
     if (g < G && g < R1y) load_in(v, 0, g);
     for (int i = tid; i < NY; i += NT) tw_y[i] = a.tw_y[i];
-    for (int i = tid; i < NZ; i += NT) tw_z[i] = a.tw_z[i];
+    if (NY != NZ)
+      for (int i = tid; i < NZ; i += NT) tw_z[i] = a.tw_z[i];
     __syncthreads();
     for (int c = 0; c < NZ / ZC; ++c) {
       if (g < G) {
@@ -464,7 +466,7 @@ static const size_t KS_SMEM_MAX = 227 * 1024;
 
 static size_t yz_smem(const HpsiPlan& P, int zc) {
   const size_t SZ = (size_t)(P.n3 | 1);
-  return sizeof(cplx) * ((size_t)P.n2 + P.n3 + (size_t)P.smax * SZ + (size_t)P.n2 * zc);
+  return sizeof(cplx) * ((size_t)P.n2 + (P.n2 == P.n3 ? 0 : P.n3) + (size_t)P.smax * SZ + (size_t)P.n2 * zc);
 }
 template <int NX> static constexpr size_t x_smem() { return sizeof(cplx) * ((size_t)NX + (size_t)NX * xcfg<NX>::ZC); }
 
