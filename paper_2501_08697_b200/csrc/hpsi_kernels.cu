@@ -16,7 +16,9 @@
 // quarter-warp fall in distinct banks.
 #include "fft.cuh"
 #include "plan.h"
+#include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <vector>
 
 
@@ -374,7 +376,7 @@ struct XArgs {
   cplx* planes;         // [nb][L1][NY*NZ], in place
   const double* vperm;  // [NX][NY*NZ]
   const cplx* tw_x;
-  int L1, x0;
+  int L1, x0, nb, bg;   // nb bands in the batch, bg bands per CTA (gridDim.y = ceil(nb / bg))
   long ncol;            // NY*NZ
 };
 
@@ -384,11 +386,33 @@ template <> struct xcfg<36> { static constexpr int ZC = 32, NT = 96, MINB = 4; }
 template <> struct xcfg<54> { static constexpr int ZC = 32, NT = 96, MINB = 4; };
 template <> struct xcfg<128> { static constexpr int ZC = 32, NT = 256, MINB = 2; };
 
+// 16-byte global -> shared async copy (LDGSTS), ordered against the surrounding shared-memory accesses
+__device__ __forceinline__ void cp16m(cplx* smem, const cplx* gmem) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_commit_m() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_wait_n(int n) {   // n = groups allowed to stay in flight (uniform per thread)
+  switch (n) {
+    case 0: asm volatile("cp.async.wait_group 0;\n" ::: "memory"); break;
+    case 1: asm volatile("cp.async.wait_group 1;\n" ::: "memory"); break;
+    case 2: asm volatile("cp.async.wait_group 2;\n" ::: "memory"); break;
+    default: asm volatile("cp.async.wait_group 3;\n" ::: "memory"); break;
+  }
+}
+
+// The CTA walks over bg bands with the same columns.  Thread (pz, g) owns the codelet lines j2 = g, g+G, ...
+// in the first AND the last pass, i.e. the tile rows {j1*R2 + j2}: once the last pass of band b has read a
+// line into registers, the same thread refills the live rows of that line with band b+1 by cp.async, and the
+// first pass of band b+1 picks them up with no barrier in between (only its own cp.async group to wait for).
+// The global-load latency of a band is hidden behind the last pass of the band before it.
 template <int NX>
 __global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB) k_x(XArgs a) {
   constexpr int R1 = fac<NX>::R1, R2 = fac<NX>::R2;
   constexpr int ZC = xcfg<NX>::ZC, NT = xcfg<NX>::NT, G = NT / ZC;
+  constexpr int ITEMS = (R2 + G - 1) / G;     // first/last-pass lines per thread
   static_assert(NT % ZC == 0, "thread count must be a multiple of the column chunk");
+  static_assert(ITEMS <= 4, "cp_wait_n covers up to 4 groups in flight");
   extern __shared__ cplx sm[];
   cplx* tw = sm;
   cplx* tile = sm + NX;
@@ -396,65 +420,89 @@ __global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB) k_x(XArgs a) {
   const unsigned ncol = (unsigned)a.ncol;      // one band's live planes (L1*ncol elements) fit 32-bit offsets
   const unsigned col = blockIdx.x * ZC + pz;
   const bool colok = col < ncol;              // ragged last chunk
-  cplx* base = a.planes + (size_t)blockIdx.y * a.L1 * a.ncol + (colok ? col : 0);
+  const int b0 = blockIdx.y * a.bg, b1 = min(b0 + a.bg, a.nb);
+  const size_t bstride = (size_t)a.L1 * a.ncol;
+  cplx* base = a.planes + (size_t)b0 * bstride + (colok ? col : 0);
   const double* vbase = a.vperm + (colok ? col : 0);
   cplx* tcol = tile + pz;
 
-  auto load_in = [&](cplx (&v)[R1], int j2) {
+  // refill the live rows of line j2 from band `src` (one cp.async group per line, committed by every thread)
+  auto prefetch_line = [&](const cplx* src, int j2) {
+    if (j2 < R2 && colok) {
 #pragma unroll
-    for (int j1 = 0; j1 < R1; ++j1) {
-      int lx = j1 * R2 + j2 - a.x0;
-      if (lx < 0) lx += NX;
-      v[j1] = (lx < a.L1 && colok) ? base[(unsigned)lx * ncol] : cmake(0.0, 0.0);
+      for (int j1 = 0; j1 < R1; ++j1) {
+        int lx = j1 * R2 + j2 - a.x0;
+        if (lx < 0) lx += NX;
+        if (lx < a.L1) cp16m(tcol + (j1 * R2 + j2) * ZC, src + (unsigned)lx * ncol);
+      }
     }
+    cp_commit_m();
   };
-  // pass 1 (type-A stage 1): global -> registers -> DFT-R1 -> twiddle -> tile
-  {
-    cplx v[R1];
-    int j2 = g;
-    if (j2 < R2) load_in(v, j2);
-    for (int i = tid; i < NX; i += NT) tw[i] = a.tw_x[i];
-    __syncthreads();
-    while (j2 < R2) {
-      dft<R1, +1>(v);
-      cplx* o = tcol + j2 * ZC;
 #pragma unroll
-      for (int k1 = 0; k1 < R1; ++k1) o[k1 * R2 * ZC] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw, j2 * k1);
-      j2 += G;
-      if (j2 < R2) load_in(v, j2);
+  for (int i = 0; i < ITEMS; ++i) prefetch_line(base, g + i * G);
+  for (int i = tid; i < NX; i += NT) tw[i] = a.tw_x[i];
+  __syncthreads();
+
+  for (int b = b0; b < b1; ++b, base += bstride) {
+    // pass 1 (type-A stage 1): own prefetched rows -> registers -> DFT-R1 -> twiddle -> tile
+#pragma unroll
+    for (int i = 0; i < ITEMS; ++i) {
+      const int j2 = g + i * G;
+      cp_wait_n(ITEMS - 1 - i);
+      if (j2 < R2) {
+        cplx v[R1];
+#pragma unroll
+        for (int j1 = 0; j1 < R1; ++j1) {
+          int lx = j1 * R2 + j2 - a.x0;
+          if (lx < 0) lx += NX;
+          v[j1] = (lx < a.L1 && colok) ? tcol[(j1 * R2 + j2) * ZC] : cmake(0.0, 0.0);
+        }
+        dft<R1, +1>(v);
+        cplx* o = tcol + j2 * ZC;
+#pragma unroll
+        for (int k1 = 0; k1 < R1; ++k1) o[k1 * R2 * ZC] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw, j2 * k1);
+      }
     }
-  }
-  __syncthreads();
-  // pass 2: type-A stage 2, V(r), type-B stage 1 on the same R2 elements, in registers
-  for (int k1 = g; k1 < R1; k1 += G) {
-    double vr[R2];
-    const double* vp = vbase + (size_t)k1 * R2 * a.ncol;
+    __syncthreads();
+    // pass 2: type-A stage 2, V(r), type-B stage 1 on the same R2 elements, in registers
+    for (int k1 = g; k1 < R1; k1 += G) {
+      double vr[R2];
+      const double* vp = vbase + (size_t)k1 * R2 * a.ncol;
 #pragma unroll
-    for (int k2 = 0; k2 < R2; ++k2) vr[k2] = __ldg(vp + (unsigned)k2 * ncol);
-    cplx v[R2];
-    cplx* t = tcol + k1 * R2 * ZC;
+      for (int k2 = 0; k2 < R2; ++k2) vr[k2] = __ldg(vp + (unsigned)k2 * ncol);
+      cplx v[R2];
+      cplx* t = tcol + k1 * R2 * ZC;
 #pragma unroll
-    for (int j2 = 0; j2 < R2; ++j2) v[j2] = t[j2 * ZC];
-    dft<R2, +1>(v);
+      for (int j2 = 0; j2 < R2; ++j2) v[j2] = t[j2 * ZC];
+      dft<R2, +1>(v);
 #pragma unroll
-    for (int k2 = 0; k2 < R2; ++k2) v[k2] = cmake(v[k2].x * vr[k2], v[k2].y * vr[k2]);
-    dft<R2, -1>(v);
+      for (int k2 = 0; k2 < R2; ++k2) v[k2] = cmake(v[k2].x * vr[k2], v[k2].y * vr[k2]);
+      dft<R2, -1>(v);
 #pragma unroll
-    for (int q2 = 0; q2 < R2; ++q2) t[q2 * ZC] = (q2 == 0) ? v[0] : mul_tw<-1>(v[q2], tw, k1 * q2);
-  }
-  __syncthreads();
-  // pass 3 (type-B stage 2): tile -> DFT-R1 -> live planes (natural x = q1*R2 + q2)
-  for (int q2 = g; q2 < R2; q2 += G) {
-    cplx v[R1];
-    const cplx* t = tcol + q2 * ZC;
+      for (int q2 = 0; q2 < R2; ++q2) t[q2 * ZC] = (q2 == 0) ? v[0] : mul_tw<-1>(v[q2], tw, k1 * q2);
+    }
+    __syncthreads();
+    // pass 3 (type-B stage 2): tile -> DFT-R1 -> live planes (natural x = q1*R2 + q2); refill the line
+    const bool more = b + 1 < b1;
 #pragma unroll
-    for (int k1 = 0; k1 < R1; ++k1) v[k1] = t[k1 * R2 * ZC];
-    dft<R1, -1>(v);
+    for (int i = 0; i < ITEMS; ++i) {
+      const int q2 = g + i * G;
+      cplx v[R1];
+      if (q2 < R2) {
+        const cplx* t = tcol + q2 * ZC;
 #pragma unroll
-    for (int q1 = 0; q1 < R1; ++q1) {
-      int lx = q1 * R2 + q2 - a.x0;
-      if (lx < 0) lx += NX;
-      if (lx < a.L1 && colok) base[(unsigned)lx * ncol] = v[q1];
+        for (int k1 = 0; k1 < R1; ++k1) v[k1] = t[k1 * R2 * ZC];
+        dft<R1, -1>(v);
+      }
+      if (more) prefetch_line(base + bstride, q2);   // v is consumed: the line's rows are free
+      if (q2 < R2) {
+#pragma unroll
+        for (int q1 = 0; q1 < R1; ++q1) {
+          int lx = q1 * R2 + q2 - a.x0;
+          if (lx < 0) lx += NX;
+          if (lx < a.L1 && colok) base[(unsigned)lx * ncol] = v[q1];
+        }
+      }
     }
   }
 }
@@ -503,6 +551,16 @@ int ks_hpsi_configure(HpsiPlan& P, std::string& err) {
   return KS_OK;
 }
 
+// bands per k_x CTA: long enough to amortise the prologue and hide the loads, short enough that the grid
+// still has several CTAs per resident slot (148 SMs x 4 CTAs)
+static int ks_x_band_group(int nchunk, int nb) {
+  static const int env = getenv("KSPW_X_BG") ? atoi(getenv("KSPW_X_BG")) : 0;
+  if (env > 0) return std::min(env, nb);
+  int bg = 8;
+  while (bg > 1 && (long)nchunk * ceil_div(nb, bg) < 4L * 148 * 4) bg /= 2;
+  return std::min(bg, nb);
+}
+
 int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb, cudaStream_t st,
                          std::string& err, int stage) {
   if (nb <= 0) return KS_OK;
@@ -515,7 +573,8 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
   XArgs x;
   x.planes = P.d_planes; x.vperm = P.d_vperm; x.tw_x = P.d_tw[0];
   x.L1 = P.L1; x.x0 = P.x0; x.ncol = (long)P.n2 * P.n3;
-  const dim3 gyz(P.L1, nb), gx(ceil_div(x.ncol, P.zc_x), nb);
+  x.nb = nb; x.bg = ks_x_band_group(ceil_div(x.ncol, P.zc_x), nb);
+  const dim3 gyz(P.L1, nb), gx(ceil_div(x.ncol, P.zc_x), ceil_div(nb, x.bg));
   if (stage < 0 || stage == 0) {
 #define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_inv_yz<A_, B_><<<gyz, yzcfg<A_, B_>::NT, P.smem_yz, st>>>(a);
     KS_YZ_PAIRS(C_)
