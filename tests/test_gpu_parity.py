@@ -162,7 +162,7 @@ def test_hpsi_edge_cases(ks, oracle_mod):
     assert _rel(out.cpu().numpy(), ref) <= HPSI_TOL
 
 
-@pytest.mark.parametrize("c,k_index,nsample", [(2, 0, 32), (2, 21, 32), (2, 63, 32), (1, 0, 6)])
+@pytest.mark.parametrize("c,k_index,nsample", [(2, 0, 32), (2, 21, 32), (2, 63, 32), (1, 0, 6), (3, 0, 3), (4, 0, 3)])
 def test_hpsi_full_size(ks, oracle_mod, c, k_index, nsample):
     """Full-size configs in the launch configuration bench.py times (whole block in one call);
     the oracle recomputes a sample of the bands one by one (bands are independent in H psi)."""
@@ -176,6 +176,22 @@ def test_hpsi_full_size(ks, oracle_mod, c, k_index, nsample):
     # property at any size: Hermiticity <phi|H psi> = conj <psi|H phi> over the whole block
     G = p.psi0.conj() @ got.T
     assert np.abs(G - G.conj().T).max() <= 1e-11 * np.abs(G).max()
+
+
+def test_hpsi_ragged_band_group(ks, oracle_mod):
+    """cfg 1 geometry with 31 bands: the x kernel walks over band groups of 2, so the last group is ragged;
+    a 7-band FFT batch adds a ragged last batch on top."""
+    p = I.make_problem(1)
+    ctx = ks.Context.from_problem(p)
+    o = oracle_mod.Oracle.from_problem(p)
+    psi = np.ascontiguousarray(p.psi0[:31])
+    sel = np.array([0, 1, 14, 29, 30])
+    ref = o.hpsi(psi[sel])
+    got = ctx.hpsi(_t(psi)).cpu().numpy()
+    assert _rel(got[sel], ref) <= HPSI_TOL
+    ctx.set_fft_batch(7)
+    got2 = ctx.hpsi(_t(psi)).cpu().numpy()
+    assert np.array_equal(got, got2)          # batching never changes a bit: bands are independent
 
 
 # ------------------------------------------------------------------ Davidson (T3)
