@@ -411,37 +411,57 @@ __global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB) k_x(XArgs a) {
   constexpr int R1 = fac<NX>::R1, R2 = fac<NX>::R2;
   constexpr int ZC = xcfg<NX>::ZC, NT = xcfg<NX>::NT, G = NT / ZC;
   constexpr int ITEMS = (R2 + G - 1) / G;     // first/last-pass lines per thread
+  constexpr int R1P = (R1 + 3) & ~3;          // row-offset table: R2+1 lines of R1P entries (line R2 is all dead)
+  constexpr unsigned DEAD = 0xffffffffu;
   static_assert(NT % ZC == 0, "thread count must be a multiple of the column chunk");
   static_assert(ITEMS <= 4, "cp_wait_n covers up to 4 groups in flight");
   extern __shared__ cplx sm[];
   cplx* tw = sm;
   cplx* tile = sm + NX;
+  unsigned* rofs = reinterpret_cast<unsigned*>(tile + NX * ZC);   // [R2+1][R1P]: element offset of row j1*R2+j2, or DEAD
   const int tid = threadIdx.x, pz = tid % ZC, g = tid / ZC;
   const unsigned ncol = (unsigned)a.ncol;      // one band's live planes (L1*ncol elements) fit 32-bit offsets
   const unsigned col = blockIdx.x * ZC + pz;
-  const bool colok = col < ncol;              // ragged last chunk
+  const bool colok = col < ncol;              // ragged last chunk: such threads use the all-dead table line
   const int b0 = blockIdx.y * a.bg, b1 = min(b0 + a.bg, a.nb);
   const size_t bstride = (size_t)a.L1 * a.ncol;
   cplx* base = a.planes + (size_t)b0 * bstride + (colok ? col : 0);
   const double* vbase = a.vperm + (colok ? col : 0);
   cplx* tcol = tile + pz;
 
+  for (int i = tid; i < (R2 + 1) * R1P; i += NT) {
+    const int j2 = i / R1P, j1 = i % R1P;
+    unsigned o = DEAD;
+    if (j2 < R2 && j1 < R1) {
+      int lx = j1 * R2 + j2 - a.x0;
+      if (lx < 0) lx += NX;
+      if (lx < a.L1) o = (unsigned)lx * ncol;
+    }
+    rofs[i] = o;
+  }
+  for (int i = tid; i < NX; i += NT) tw[i] = a.tw_x[i];
+  __syncthreads();
+
+  // row offsets of line j2 (warp-uniform address: broadcast loads)
+  auto line_offsets = [&](unsigned (&o)[R1P], int j2) {
+    const uint4* t = reinterpret_cast<const uint4*>(rofs + ((colok && j2 < R2) ? j2 : R2) * R1P);
+#pragma unroll
+    for (int q = 0; q < R1P / 4; ++q) {
+      const uint4 u = t[q];
+      o[4 * q] = u.x; o[4 * q + 1] = u.y; o[4 * q + 2] = u.z; o[4 * q + 3] = u.w;
+    }
+  };
   // refill the live rows of line j2 from band `src` (one cp.async group per line, committed by every thread)
   auto prefetch_line = [&](const cplx* src, int j2) {
-    if (j2 < R2 && colok) {
+    unsigned o[R1P];
+    line_offsets(o, j2);
 #pragma unroll
-      for (int j1 = 0; j1 < R1; ++j1) {
-        int lx = j1 * R2 + j2 - a.x0;
-        if (lx < 0) lx += NX;
-        if (lx < a.L1) cp16m(tcol + (j1 * R2 + j2) * ZC, src + (unsigned)lx * ncol);
-      }
-    }
+    for (int j1 = 0; j1 < R1; ++j1)
+      if (o[j1] != DEAD) cp16m(tcol + (j1 * R2 + j2) * ZC, src + o[j1]);
     cp_commit_m();
   };
 #pragma unroll
   for (int i = 0; i < ITEMS; ++i) prefetch_line(base, g + i * G);
-  for (int i = tid; i < NX; i += NT) tw[i] = a.tw_x[i];
-  __syncthreads();
 
   for (int b = b0; b < b1; ++b, base += bstride) {
     // pass 1 (type-A stage 1): own prefetched rows -> registers -> DFT-R1 -> twiddle -> tile
@@ -449,18 +469,16 @@ __global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB) k_x(XArgs a) {
     for (int i = 0; i < ITEMS; ++i) {
       const int j2 = g + i * G;
       cp_wait_n(ITEMS - 1 - i);
-      if (j2 < R2) {
+      if (R2 % G == 0 || j2 < R2) {
+        unsigned o[R1P];
+        line_offsets(o, j2);
         cplx v[R1];
 #pragma unroll
-        for (int j1 = 0; j1 < R1; ++j1) {
-          int lx = j1 * R2 + j2 - a.x0;
-          if (lx < 0) lx += NX;
-          v[j1] = (lx < a.L1 && colok) ? tcol[(j1 * R2 + j2) * ZC] : cmake(0.0, 0.0);
-        }
+        for (int j1 = 0; j1 < R1; ++j1) v[j1] = (o[j1] != DEAD) ? tcol[(j1 * R2 + j2) * ZC] : cmake(0.0, 0.0);
         dft<R1, +1>(v);
-        cplx* o = tcol + j2 * ZC;
+        cplx* out = tcol + j2 * ZC;
 #pragma unroll
-        for (int k1 = 0; k1 < R1; ++k1) o[k1 * R2 * ZC] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw, j2 * k1);
+        for (int k1 = 0; k1 < R1; ++k1) out[k1 * R2 * ZC] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw, j2 * k1);
       }
     }
     __syncthreads();
@@ -487,22 +505,24 @@ __global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB) k_x(XArgs a) {
 #pragma unroll
     for (int i = 0; i < ITEMS; ++i) {
       const int q2 = g + i * G;
+      unsigned o[R1P];
+      line_offsets(o, q2);
       cplx v[R1];
-      if (q2 < R2) {
+      if (R2 % G == 0 || q2 < R2) {
         const cplx* t = tcol + q2 * ZC;
 #pragma unroll
         for (int k1 = 0; k1 < R1; ++k1) v[k1] = t[k1 * R2 * ZC];
         dft<R1, -1>(v);
       }
-      if (more) prefetch_line(base + bstride, q2);   // v is consumed: the line's rows are free
-      if (q2 < R2) {
+      if (more) {                                    // v is consumed: the line's rows are free
 #pragma unroll
-        for (int q1 = 0; q1 < R1; ++q1) {
-          int lx = q1 * R2 + q2 - a.x0;
-          if (lx < 0) lx += NX;
-          if (lx < a.L1 && colok) base[(unsigned)lx * ncol] = v[q1];
-        }
+        for (int j1 = 0; j1 < R1; ++j1)
+          if (o[j1] != DEAD) cp16m(tcol + (j1 * R2 + q2) * ZC, base + bstride + o[j1]);
+        cp_commit_m();
       }
+#pragma unroll
+      for (int q1 = 0; q1 < R1; ++q1)
+        if (o[q1] != DEAD) base[o[q1]] = v[q1];
     }
   }
 }
@@ -516,7 +536,9 @@ static size_t yz_smem(const HpsiPlan& P, int zc) {
   const size_t SZ = (size_t)(P.n3 | 1);
   return sizeof(cplx) * ((size_t)P.n2 + (P.n2 == P.n3 ? 0 : P.n3) + (size_t)P.smax * SZ + (size_t)P.n2 * zc);
 }
-template <int NX> static constexpr size_t x_smem() { return sizeof(cplx) * ((size_t)NX + (size_t)NX * xcfg<NX>::ZC); }
+template <int NX> static constexpr size_t x_smem() {
+  return sizeof(cplx) * ((size_t)NX + (size_t)NX * xcfg<NX>::ZC) + sizeof(unsigned) * (fac<NX>::R2 + 1) * ((fac<NX>::R1 + 3) & ~3);
+}
 
 template <typename K>
 static cudaError_t opt_in(K kern, size_t bytes) {
