@@ -9,6 +9,8 @@ struct DavidsonWs {
   cplx *T = nullptr;                     // [nb][npw]
   cplx *Hc = nullptr, *Cm = nullptr;     // [2nb x 2nb] subspace matrix / eigenvectors (column-major)
   cplx *Hwork = nullptr;                 // [2nb x 2nb] copy destroyed by the eigensolver
+  cplx *Cp = nullptr, *Cq = nullptr;     // [2nb x 2nb] eigenvectors of the previous iteration / of the rotated matrix
+  double *thp = nullptr;                 // [2nb] Ritz values of the previous iteration
   cplx *S = nullptr, *Us = nullptr;      // [2nb x nb] projections / [nb x nb] Gram matrices
   double *theta = nullptr;               // [2nb]
   double *rho = nullptr, *ekin = nullptr, *lam = nullptr;   // [nb]

@@ -120,6 +120,28 @@ __global__ void k_mirror(int m0, int m1, long ld, cplx* __restrict__ H) {
     H[(long)i * ld + j] = cconj(s);
   }
 }
+// D3 warm start: the subspace matrix in the basis Q = diag(C_prev, I).  Fills the leading mp x mp block with
+// diag(theta_prev) and copies the trailing (m-mp) x (m-mp) corner of Hc; the mp x (m-mp) border comes from a GEMM.
+__global__ void k_build_hrot(int mp, int m, const cplx* __restrict__ Hc, long ldh, const double* __restrict__ thp,
+                             cplx* __restrict__ Hr) {
+  const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (e >= (long)m * m) return;
+  const int i = (int)(e % m), j = (int)(e / m);
+  if (i < mp && j < mp) Hr[e] = cmake(i == j ? thp[i] : 0.0, 0.0);
+  else if (i >= mp && j >= mp) Hr[e] = Hc[(long)j * ldh + i];
+}
+__global__ void k_mirror_border(int mp, int m, cplx* __restrict__ Hr) {   // Hr[j][i] = conj(Hr[i][j]), i < mp <= j
+  const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (e >= (long)mp * (m - mp)) return;
+  const int i = (int)(e % mp), j = mp + (int)(e / mp);
+  Hr[(long)i * m + j] = cconj(Hr[(long)j * m + i]);
+}
+__global__ void k_set_identity(int m, long ld, cplx* __restrict__ C) {
+  const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (e >= (long)m * m) return;
+  const int i = (int)(e % m), j = (int)(e / m);
+  C[(long)j * ld + i] = cmake(i == j ? 1.0 : 0.0, 0.0);
+}
 __global__ void k_copy_mat(int m, int n, const cplx* __restrict__ a, long lda, cplx* __restrict__ b, long ldb) {
   const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
   if (e >= (long)m * n) return;
@@ -218,6 +240,7 @@ __global__ void __launch_bounds__(128) k_trinv(int nu, const cplx* __restrict__ 
 void ks_davidson_free(DavidsonWs* w) {
   cudaFree(w->V); cudaFree(w->W); cudaFree(w->X); cudaFree(w->HX); cudaFree(w->T);
   cudaFree(w->Hc); cudaFree(w->Cm); cudaFree(w->Hwork); cudaFree(w->S); cudaFree(w->Us);
+  cudaFree(w->Cp); cudaFree(w->Cq); cudaFree(w->thp);
   cudaFree(w->theta); cudaFree(w->rho); cudaFree(w->ekin); cudaFree(w->lam); cudaFree(w->idx);
   *w = DavidsonWs();
 }
@@ -236,6 +259,9 @@ static int reserve(ks_ctx* c, int nb) {
   KS_CUDA_CHECK(cudaMalloc(&w.Hc, sizeof(cplx) * m * m), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.Cm, sizeof(cplx) * m * m), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.Hwork, sizeof(cplx) * m * m), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.Cp, sizeof(cplx) * m * m), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.Cq, sizeof(cplx) * m * m), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.thp, sizeof(double) * m), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.S, sizeof(cplx) * m * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.Us, sizeof(cplx) * (size_t)nb * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.theta, sizeof(double) * m), c->err);
@@ -354,6 +380,13 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
   KS_CUDA_CHECK(cudaMemcpyAsync(w.W, w.HX, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
   k_set_diag<<<ceil_div((long)nb * nb, 256), 256, 0, st>>>(nb, ldh, w.Hc, w.theta);
   ph.end(PH_ROT);
+  // warm start of the subspace eigensolver (KSPW_WARM=0 switches it off): V = X, so C_prev = I, theta_prev = eps
+  static const bool warm = !(getenv("KSPW_WARM") && atoi(getenv("KSPW_WARM")) == 0);
+  int mp = nb;
+  if (warm) {
+    k_set_identity<<<ceil_div((long)nb * nb, 256), 256, 0, st>>>(nb, ldh, w.Cp);
+    KS_CUDA_CHECK(cudaMemcpyAsync(w.thp, w.theta, sizeof(double) * nb, cudaMemcpyDeviceToDevice, st), c->err);
+  }
   int m = nb, it = 0, status = KS_NOTCONV;
   std::vector<double> rho(nb);
   std::vector<int> idx(nb);
@@ -375,6 +408,10 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
       KS_CUDA_CHECK(cudaMemcpyAsync(w.W, w.HX, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
       k_set_diag<<<ceil_div((long)nb * nb, 256), 256, 0, st>>>(nb, ldh, w.Hc, w.theta);
       m = nb;
+      if (warm) {   // V = X again: C_prev = I; theta_prev[0:nb] already holds eps
+        k_set_identity<<<ceil_div((long)nb * nb, 256), 256, 0, st>>>(nb, ldh, w.Cp);
+        mp = nb;
+      }
     }
     // D6
     ph.begin();
@@ -406,14 +443,30 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
     m = m1;
     // D3
     ph.begin();
-    k_copy_mat<<<ceil_div((long)m * m, 256), 256, 0, st>>>(m, m, w.Hc, ldh, w.Hwork, m);
-    RC(ks_eigh_run(st, m, w.Hwork, m, w.theta, w.Cm, ldh, &c->ews, nullptr, c->err));
+    if (!warm) {
+      k_copy_mat<<<ceil_div((long)m * m, 256), 256, 0, st>>>(m, m, w.Hc, ldh, w.Hwork, m);
+      RC(ks_eigh_run(st, m, w.Hwork, m, w.theta, w.Cm, ldh, &c->ews, nullptr, c->err));
+    } else {
+      // Q = diag(C_prev, I):  Q^H Hc Q = [diag(theta_prev), C_prev^H B; (.)^H, D] -- already diagonal except for the
+      // border that couples the new directions, so the Jacobi sweeps start close to convergence.
+      k_build_hrot<<<ceil_div((long)m * m, 256), 256, 0, st>>>(mp, m, w.Hc, ldh, w.thp, w.Hwork);
+      RC(ks_gemm_hn(st, mp, m - mp, mp, w.Cp, ldh, w.Hc + (size_t)mp * ldh, ldh, w.Hwork + (size_t)mp * m, m, &c->gws, c->err));
+      k_mirror_border<<<ceil_div((long)mp * (m - mp), 256), 256, 0, st>>>(mp, m, w.Hwork);
+      int sw = 0;
+      RC(ks_eigh_run(st, m, w.Hwork, m, w.theta, w.Cq, ldh, &c->ews, &sw, c->err));
+      if (getenv("KSPW_DEBUG_SWEEPS")) fprintf(stderr, "it %d m %d nk %d sweeps %d\n", it, m, nk, sw);
+      // C = Q C'
+      RC(ks_gemm_nn(st, mp, m, mp, w.Cp, ldh, w.Cq, ldh, w.Cm, ldh, 0, c->err));
+      k_copy_mat<<<ceil_div((long)(m - mp) * m, 256), 256, 0, st>>>(m - mp, m, w.Cq + mp, ldh, w.Cm + mp, ldh);
+      KS_CUDA_CHECK(cudaMemcpyAsync(w.thp, w.theta, sizeof(double) * m, cudaMemcpyDeviceToDevice, st), c->err);
+    }
     ph.end(PH_EIGH);
     // D4
     ph.begin();
     RC(ks_gemm_nn(st, npw, nb, m, w.V, npw, w.Cm, ldh, w.X, npw, 0, c->err));
     RC(ks_gemm_nn(st, npw, nb, m, w.W, npw, w.Cm, ldh, w.HX, npw, 0, c->err));
     ph.end(PH_ROT);
+    if (warm) { std::swap(w.Cm, w.Cp); mp = m; }   // C of this iteration is C_prev of the next
     ++it;
   }
   // D9
