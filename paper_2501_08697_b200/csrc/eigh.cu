@@ -44,7 +44,7 @@ __host__ __device__ __forceinline__ void rr_pair(int n, int r, int k, int* p, in
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(JTHREADS) k_jacobi_cta(const cplx* __restrict__ Ap, long ld, int nbk,
                                                         const int2* __restrict__ pairs, cplx* __restrict__ U,
-                                                        double* __restrict__ dout, int max_sweeps, double tol2) {
+                                                        double* __restrict__ dout, int max_sweeps, double tol2, int cross) {
   extern __shared__ cplx sm[];
   const int ns = 2 * nbk, LD = ns + 1, hp = ns / 2;
   cplx* As = sm;                       // As[i*LD + j] = A[i][j]
@@ -63,9 +63,13 @@ __global__ void __launch_bounds__(JTHREADS) k_jacobi_cta(const cplx* __restrict_
     As[i * LD + j] = Ap[(long)gj * ld + gi];
     Vs[i * LD + j] = cmake(i == j ? 1.0 : 0.0, 0.0);
   }
-  for (int e = tid; e < (ns - 1) * hp; e += nt) {
+  // cross != 0: only the pivots that couple the two blocks (p in the first, q in the second): nbk rounds of nbk
+  // disjoint rotations.  The pivots inside a block are swept once per outer sweep, by the round-0 launches.
+  const int nrounds = cross ? nbk : ns - 1;
+  for (int e = tid; e < nrounds * hp; e += nt) {
     int p, q;
-    rr_pair(ns, e / hp, e % hp, &p, &q);
+    if (cross) { p = e % hp; q = nbk + (e % hp + e / hp) % nbk; }
+    else rr_pair(ns, e / hp, e % hp, &p, &q);
     sched[e] = make_uchar2((unsigned char)p, (unsigned char)q);
   }
   __syncthreads();
@@ -92,7 +96,7 @@ __global__ void __launch_bounds__(JTHREADS) k_jacobi_cta(const cplx* __restrict_
     }
     __syncthreads();
     if (stop) break;
-    for (int r = 0; r < ns - 1; ++r) {
+    for (int r = 0; r < nrounds; ++r) {
       const uchar2* sr = sched + r * hp;
       if (tid < hp) {
         const int p = sr[tid].x, q = sr[tid].y;
@@ -101,12 +105,15 @@ __global__ void __launch_bounds__(JTHREADS) k_jacobi_cta(const cplx* __restrict_
         double c = 1.0;
         cplx sg = cmake(0.0, 0.0);
         if (a > 0.0) {
+          // c = sqrt((1 + |d|/r)/2), sg = sign(d) a_pq / (2 r c), r = sqrt(d^2 + |a_pq|^2): the same rotation as
+          // z = sign(d) a_pq / (|d| + r), c = 1/sqrt(1+|z|^2), sg = c z, with two rsqrt and no division
           const double d = 0.5 * (As[q * LD + q].x - As[p * LD + p].x);
-          const double rr = sqrt(fma(d, d, a));
-          const double inv = (d >= 0.0 ? 1.0 : -1.0) / (fabs(d) + rr);
-          const cplx z = cmake(apq.x * inv, apq.y * inv);
-          c = rsqrt(fma(z.x, z.x, fma(z.y, z.y, 1.0)));
-          sg = cmake(c * z.x, c * z.y);
+          const double ir = rsqrt(fma(d, d, a));
+          const double x = fma(0.5 * fabs(d), ir, 0.5);
+          const double ix = rsqrt(x);
+          c = x * ix;
+          const double f = (d >= 0.0 ? 0.5 : -0.5) * ir * ix;
+          sg = cmake(apq.x * f, apq.y * f);
         }
         rc[tid] = c;
         rsg[tid] = sg;
@@ -391,6 +398,7 @@ static int block_sweeps(cudaStream_t st, int n, const cplx* A, long lda, EighWs*
     ws->pairs_nblk = nblk;
   }
   k_pad_copy<<<ceil_div((long)np * np, 256), 256, 0, st>>>(A, lda, n, ws->Ap, ws->Vp, np);
+  static const bool cross_rounds = !(getenv("KSPW_JAC_CROSS") && atoi(getenv("KSPW_JAC_CROSS")) == 0);
   int sweeps = 0;
   for (; sweeps < 40; ++sweeps) {
     double h[2];
@@ -401,7 +409,7 @@ static int block_sweeps(cudaStream_t st, int n, const cplx* A, long lda, EighWs*
     if (h[0] <= tol2 * h[1]) break;
     for (int r = 0; r < nblk - 1; ++r) {
       const int2* pr = ws->pairs + (size_t)r * npair;
-      k_jacobi_cta<<<npair, JSZ * JSZ / 4, smem_cta, st>>>(ws->Ap, np, JBK, pr, ws->U, nullptr, inner, 1e-30);
+      k_jacobi_cta<<<npair, JSZ * JSZ / 4, smem_cta, st>>>(ws->Ap, np, JBK, pr, ws->U, nullptr, inner, 1e-30, (r > 0 && cross_rounds) ? 1 : 0);
       k_jac_col<JSZ><<<dim3(ceil_div(np, MT), npair, 2), 256, smem_col, st>>>(ws->Ap, ws->Vp, np, np, pr, ws->U);
       k_jac_row<JSZ><<<dim3(ceil_div(np, NT), npair), 256, smem_row, st>>>(ws->Ap, np, np, pr, ws->U);
     }
@@ -441,7 +449,7 @@ int ks_eigh_run(cudaStream_t st, int n, cplx* A, long lda, double* theta, cplx* 
       ws->pairs_nblk = 2;
     }
     k_pad_copy<<<ceil_div((long)ns * ns, 256), 256, 0, st>>>(A, lda, n, ws->Ap, nullptr, ns);
-    k_jacobi_cta<<<1, JTHREADS, smem_cta, st>>>(ws->Ap, ns, nbk, ws->pairs, ws->Vp, ws->diag, 40, tol2);
+    k_jacobi_cta<<<1, JTHREADS, smem_cta, st>>>(ws->Ap, ns, nbk, ws->pairs, ws->Vp, ws->diag, 40, tol2, 0);
     k_rank<<<ceil_div(ns, 128), 128, 0, st>>>(ws->diag, ns, n, ws->order, theta);
     k_gather_cols<<<ceil_div((long)n * n, 256), 256, 0, st>>>(ws->Vp, ns, ws->order, n, C, ldc);
     KS_CUDA_CHECK(cudaGetLastError(), err);
@@ -454,7 +462,7 @@ int ks_eigh_run(cudaStream_t st, int n, cplx* A, long lda, double* theta, cplx* 
     const char* e = getenv("KSPW_JAC_PAIR");
     force_blk = e ? atoi(e) : 0;
   }
-  const bool use32 = force_blk == 32 || (force_blk != 64 && n <= 640);
+  const bool use32 = force_blk != 64;   // 32-wide pairs win at every size measured (n = 320 .. 1040)
   if (use32) rc = block_sweeps<32>(st, n, A, lda, ws, tol2, inner, &sweeps, err);
   else rc = block_sweeps<64>(st, n, A, lda, ws, tol2, inner, &sweeps, err);
   if (rc) return rc;
