@@ -15,6 +15,7 @@ struct DavidsonWs {
   double *theta = nullptr;               // [2nb]
   double *rho = nullptr, *ekin = nullptr, *lam = nullptr;   // [nb]
   int *idx = nullptr;                    // [nb] unconverged band list / kept column list
+  int *act = nullptr;                    // [nb] bands whose Ritz vectors are rotated this iteration
 };
 
 struct ks_ctx {

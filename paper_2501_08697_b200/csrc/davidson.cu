@@ -142,6 +142,20 @@ __global__ void k_set_identity(int m, long ld, cplx* __restrict__ C) {
   const int i = (int)(e % m), j = (int)(e / m);
   C[(long)j * ld + i] = cmake(i == j ? 1.0 : 0.0, 0.0);
 }
+// D4 on the unconverged bands only: Cg[:, j] = C[:, idx[j]]  and  X[idx[j]][:] = T[j][:]
+__global__ void k_gather_cols_idx(int m, int nu, const cplx* __restrict__ C, long ldc, const int* __restrict__ idx,
+                                  cplx* __restrict__ Cg) {
+  const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (e >= (long)m * nu) return;
+  const int i = (int)(e % m), j = (int)(e / m);
+  Cg[e] = C[(long)idx[j] * ldc + i];
+}
+__global__ void k_scatter_bands(int npw, int nu, const int* __restrict__ idx, const cplx* __restrict__ T, cplx* __restrict__ X) {
+  const int j = blockIdx.y;
+  cplx* dst = X + (size_t)idx[j] * npw;
+  const cplx* src = T + (size_t)j * npw;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < npw; i += gridDim.x * blockDim.x) dst[i] = src[i];
+}
 __global__ void k_copy_mat(int m, int n, const cplx* __restrict__ a, long lda, cplx* __restrict__ b, long ldb) {
   const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
   if (e >= (long)m * n) return;
@@ -240,7 +254,7 @@ __global__ void __launch_bounds__(128) k_trinv(int nu, const cplx* __restrict__ 
 void ks_davidson_free(DavidsonWs* w) {
   cudaFree(w->V); cudaFree(w->W); cudaFree(w->X); cudaFree(w->HX); cudaFree(w->T);
   cudaFree(w->Hc); cudaFree(w->Cm); cudaFree(w->Hwork); cudaFree(w->S); cudaFree(w->Us);
-  cudaFree(w->Cp); cudaFree(w->Cq); cudaFree(w->thp);
+  cudaFree(w->Cp); cudaFree(w->Cq); cudaFree(w->thp); cudaFree(w->act);
   cudaFree(w->theta); cudaFree(w->rho); cudaFree(w->ekin); cudaFree(w->lam); cudaFree(w->idx);
   *w = DavidsonWs();
 }
@@ -269,6 +283,7 @@ static int reserve(ks_ctx* c, int nb) {
   KS_CUDA_CHECK(cudaMalloc(&w.ekin, sizeof(double) * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.lam, sizeof(double) * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.idx, sizeof(int) * (nb + 1)), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.act, sizeof(int) * nb), c->err);
   w.nb_cap = nb;
   return KS_OK;
 }
@@ -390,6 +405,17 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
   int m = nb, it = 0, status = KS_NOTCONV;
   std::vector<double> rho(nb);
   std::vector<int> idx(nb);
+  // D4 rotates only the bands that are still unconverged (KSPW_ACTIVE_ROT=0: all bands every iteration, as the
+  // listing says); `stale` = some converged band's X, HX are older than the last eigensolve.
+  static const bool active_rot = !(getenv("KSPW_ACTIVE_ROT") && atoi(getenv("KSPW_ACTIVE_ROT")) == 0);
+  bool stale = false;
+  auto rotate_all = [&]() -> int {
+    const cplx* Cl = warm ? w.Cp : w.Cm;      // eigenvectors of the last eigensolve (after the end-of-iteration swap)
+    RC(ks_gemm_nn(st, npw, nb, m, w.V, npw, Cl, ldh, w.X, npw, 0, c->err));
+    RC(ks_gemm_nn(st, npw, nb, m, w.W, npw, Cl, ldh, w.HX, npw, 0, c->err));
+    stale = false;
+    return KS_OK;
+  };
   for (;;) {
     // D5
     ph.begin();
@@ -400,10 +426,19 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
     int nu = 0;
     for (int i = 0; i < nb; ++i)
       if (!(rho[i] <= tol)) idx[nu++] = i;
+    if ((nu == 0 || it >= max_iter) && stale) {
+      // the Ritz vectors of the bands that were already converged have not been rotated since they converged:
+      // bring every band up to date and look at all the residuals again before stopping
+      ph.begin();
+      RC(rotate_all());
+      ph.end(PH_ROT);
+      continue;
+    }
     if (nu == 0) { status = KS_OK; break; }
     if (it >= max_iter) break;
     // D8 (restart)
     if (m + nu > 2 * nb) {
+      if (stale) { ph.begin(); RC(rotate_all()); ph.end(PH_ROT); }
       KS_CUDA_CHECK(cudaMemcpyAsync(w.V, w.X, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
       KS_CUDA_CHECK(cudaMemcpyAsync(w.W, w.HX, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
       k_set_diag<<<ceil_div((long)nb * nb, 256), 256, 0, st>>>(nb, ldh, w.Hc, w.theta);
@@ -463,8 +498,21 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
     ph.end(PH_EIGH);
     // D4
     ph.begin();
-    RC(ks_gemm_nn(st, npw, nb, m, w.V, npw, w.Cm, ldh, w.X, npw, 0, c->err));
-    RC(ks_gemm_nn(st, npw, nb, m, w.W, npw, w.Cm, ldh, w.HX, npw, 0, c->err));
+    if (!active_rot || 2 * nu > nb) {
+      RC(ks_gemm_nn(st, npw, nb, m, w.V, npw, w.Cm, ldh, w.X, npw, 0, c->err));
+      RC(ks_gemm_nn(st, npw, nb, m, w.W, npw, w.Cm, ldh, w.HX, npw, 0, c->err));
+      stale = false;
+    } else {
+      // idx[0:nu] = the bands that were unconverged at this iteration's D5
+      KS_CUDA_CHECK(cudaMemcpyAsync(w.act, idx.data(), sizeof(int) * nu, cudaMemcpyHostToDevice, st), c->err);
+      k_gather_cols_idx<<<ceil_div((long)m * nu, 256), 256, 0, st>>>(m, nu, w.Cm, ldh, w.act, w.S);
+      const dim3 gs(std::max(1, std::min(32, ceil_div(npw, 2048))), nu);
+      RC(ks_gemm_nn(st, npw, nu, m, w.V, npw, w.S, m, w.T, npw, 0, c->err));
+      k_scatter_bands<<<gs, 256, 0, st>>>(npw, nu, w.act, w.T, w.X);
+      RC(ks_gemm_nn(st, npw, nu, m, w.W, npw, w.S, m, w.T, npw, 0, c->err));
+      k_scatter_bands<<<gs, 256, 0, st>>>(npw, nu, w.act, w.T, w.HX);
+      stale = true;
+    }
     ph.end(PH_ROT);
     if (warm) { std::swap(w.Cm, w.Cp); mp = m; }   // C of this iteration is C_prev of the next
     ++it;
