@@ -363,6 +363,73 @@ static int eigh_reserve(EighWs* ws, int np, std::string& err) {
   return KS_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// fused two-sided update for 32-wide pairs: one CTA per 32 x 32 tile.
+//   blockIdx.y <  npair :  A[IJ_a, IJ_b] <- U_a^H A[IJ_a, IJ_b] U_b     (a = blockIdx.y, b = blockIdx.x)
+//   blockIdx.y >= npair :  V[rows, IJ_b] <- V[rows, IJ_b] U_b           (rows = 32 (blockIdx.y - npair) ...)
+// The pairs of a round partition the blocks, so the tiles partition A (and V): every tile is read and written
+// by exactly one CTA and the update is in place with no intermediate pass through global memory.
+// 256 threads as 16 x 16, each owning a 2 x 2 block {ti, ti+16} x {tj, tj+16}; operands row-major with an odd
+// leading dimension (33) in shared memory: a half-warp reads one row segment, conflict-free.
+// ------------------------------------------------------------------------------------------------
+#define JU_LD 33
+__global__ void __launch_bounds__(256) k_jac_upd32(cplx* __restrict__ Ap, cplx* __restrict__ Vp, long ld, int npair,
+                                                   const int2* __restrict__ pairs, const cplx* __restrict__ U) {
+  extern __shared__ cplx sm[];
+  cplx *sT = sm, *sUa = sm + 32 * JU_LD, *sUb = sm + 64 * JU_LD;
+  const int tid = threadIdx.x, b = blockIdx.x;
+  const bool isA = blockIdx.y < npair;
+  const int2 pb = pairs[b];
+  const int2 pa = isA ? pairs[blockIdx.y] : make_int2(0, 0);
+  const int r0 = isA ? 0 : (blockIdx.y - npair) * 32;
+  cplx* X = isA ? Ap : Vp;
+  // loads: e -> (i = e % 32 fastest: consecutive rows of a column-major matrix)
+  for (int e = tid; e < 32 * 32; e += 256) {
+    const int i = e & 31, j = e >> 5;
+    const int gi = isA ? blk_index<32>(pa, i) : r0 + i;
+    const int gj = blk_index<32>(pb, j);
+    sT[i * JU_LD + j] = X[(long)gj * ld + gi];
+    sUb[i * JU_LD + j] = U[(size_t)b * 1024 + e];                 // U_b[k = i][j]
+    if (isA) sUa[i * JU_LD + j] = U[(size_t)blockIdx.y * 1024 + e];   // U_a[k = i][col = j]
+  }
+  __syncthreads();
+  const int ti = tid >> 4, tj = tid & 15;
+  // P = T U_b
+  cplx p00 = cmake(0, 0), p01 = p00, p10 = p00, p11 = p00;
+#pragma unroll 8
+  for (int k = 0; k < 32; ++k) {
+    const cplx a0 = sT[ti * JU_LD + k], a1 = sT[(ti + 16) * JU_LD + k];
+    const cplx b0 = sUb[k * JU_LD + tj], b1 = sUb[k * JU_LD + tj + 16];
+    p00 = cfma(a0, b0, p00); p01 = cfma(a0, b1, p01);
+    p10 = cfma(a1, b0, p10); p11 = cfma(a1, b1, p11);
+  }
+  __syncthreads();
+  sT[ti * JU_LD + tj] = p00; sT[ti * JU_LD + tj + 16] = p01;
+  sT[(ti + 16) * JU_LD + tj] = p10; sT[(ti + 16) * JU_LD + tj + 16] = p11;
+  __syncthreads();
+  if (isA) {
+    // T' = U_a^H P :  T'[i][j] = sum_k conj(U_a[k][i]) P[k][j]
+    cplx q00 = cmake(0, 0), q01 = q00, q10 = q00, q11 = q00;
+#pragma unroll 8
+    for (int k = 0; k < 32; ++k) {
+      const cplx a0 = cconj(sUa[k * JU_LD + ti]), a1 = cconj(sUa[k * JU_LD + ti + 16]);
+      const cplx b0 = sT[k * JU_LD + tj], b1 = sT[k * JU_LD + tj + 16];
+      q00 = cfma(a0, b0, q00); q01 = cfma(a0, b1, q01);
+      q10 = cfma(a1, b0, q10); q11 = cfma(a1, b1, q11);
+    }
+    __syncthreads();
+    sT[ti * JU_LD + tj] = q00; sT[ti * JU_LD + tj + 16] = q01;
+    sT[(ti + 16) * JU_LD + tj] = q10; sT[(ti + 16) * JU_LD + tj + 16] = q11;
+    __syncthreads();
+  }
+  for (int e = tid; e < 32 * 32; e += 256) {
+    const int i = e & 31, j = e >> 5;
+    const int gi = isA ? blk_index<32>(pa, i) : r0 + i;
+    const int gj = blk_index<32>(pb, j);
+    X[(long)gj * ld + gi] = sT[i * JU_LD + j];
+  }
+}
+
 template <int JSZ>
 static int block_sweeps(cudaStream_t st, int n, const cplx* A, long lda, EighWs* ws, double tol2, int inner, int* sweeps_out,
                         std::string& err) {
@@ -376,6 +443,7 @@ static int block_sweeps(cudaStream_t st, int n, const cplx* A, long lda, EighWs*
   if (!opted) {
     KS_CUDA_CHECK(cudaFuncSetAttribute(k_jac_col<JSZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_col), err);
     KS_CUDA_CHECK(cudaFuncSetAttribute(k_jac_row<JSZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row), err);
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_jac_upd32, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(cplx) * 96 * JU_LD)), err);
     opted = true;
   }
   int nblk = ceil_div(n, JBK);
@@ -398,6 +466,7 @@ static int block_sweeps(cudaStream_t st, int n, const cplx* A, long lda, EighWs*
     ws->pairs_nblk = nblk;
   }
   k_pad_copy<<<ceil_div((long)np * np, 256), 256, 0, st>>>(A, lda, n, ws->Ap, ws->Vp, np);
+  static const bool fused_upd = !(getenv("KSPW_JAC_FUSED") && atoi(getenv("KSPW_JAC_FUSED")) == 0);
   static const bool cross_rounds = !(getenv("KSPW_JAC_CROSS") && atoi(getenv("KSPW_JAC_CROSS")) == 0);
   int sweeps = 0;
   for (; sweeps < 40; ++sweeps) {
@@ -410,8 +479,12 @@ static int block_sweeps(cudaStream_t st, int n, const cplx* A, long lda, EighWs*
     for (int r = 0; r < nblk - 1; ++r) {
       const int2* pr = ws->pairs + (size_t)r * npair;
       k_jacobi_cta<<<npair, JSZ * JSZ / 4, smem_cta, st>>>(ws->Ap, np, JBK, pr, ws->U, nullptr, inner, 1e-30, (r > 0 && cross_rounds) ? 1 : 0);
-      k_jac_col<JSZ><<<dim3(ceil_div(np, MT), npair, 2), 256, smem_col, st>>>(ws->Ap, ws->Vp, np, np, pr, ws->U);
-      k_jac_row<JSZ><<<dim3(ceil_div(np, NT), npair), 256, smem_row, st>>>(ws->Ap, np, np, pr, ws->U);
+      if (JSZ == 32 && fused_upd) {
+        k_jac_upd32<<<dim3(npair, npair + np / 32), 256, sizeof(cplx) * 96 * JU_LD, st>>>(ws->Ap, ws->Vp, np, npair, pr, ws->U);
+      } else {
+        k_jac_col<JSZ><<<dim3(ceil_div(np, MT), npair, 2), 256, smem_col, st>>>(ws->Ap, ws->Vp, np, np, pr, ws->U);
+        k_jac_row<JSZ><<<dim3(ceil_div(np, NT), npair), 256, smem_row, st>>>(ws->Ap, np, np, pr, ws->U);
+      }
     }
   }
   KS_CUDA_CHECK(cudaGetLastError(), err);
