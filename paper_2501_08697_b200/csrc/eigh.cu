@@ -42,25 +42,19 @@ __host__ __device__ __forceinline__ void rr_pair(int n, int r, int k, int* p, in
 //   phase 2  one thread per 2x2 block (k, l):  A[{p_k,q_k},{p_l,q_l}] <- J_k^H (.) J_l  and
 //            V[{p_k,q_k},{p_l,q_l}] <- (.) J_l, all in registers.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(JTHREADS) k_jacobi_cta(const cplx* __restrict__ Ap, long ld, int nbk,
-                                                        const int2* __restrict__ pairs, cplx* __restrict__ U,
-                                                        double* __restrict__ dout, int max_sweeps, double tol2, int cross) {
-  extern __shared__ cplx sm[];
+// The solver proper.  Shared memory (caller provides; ns = 2*nbk, LD = ns+1): As[ns*LD] filled with the pair
+// problem (As[i*LD + j] = A[i][j]), Vs[ns*LD] (set to the identity here), then `scr`: >= 16*(JS/2) + 8*(JS/2) +
+// 2*(ns-1)*(ns/2) bytes.  On return As holds the rotated matrix and Vs the accumulated rotations.
+__device__ __forceinline__ void jac_solve_smem(cplx* As, cplx* Vs, void* scr, int nbk, int max_sweeps, double tol2, int cross) {
   const int ns = 2 * nbk, LD = ns + 1, hp = ns / 2;
-  cplx* As = sm;                       // As[i*LD + j] = A[i][j]
-  cplx* Vs = As + ns * LD;
-  cplx* rsg = Vs + ns * LD;            // sg[k]
+  cplx* rsg = (cplx*)scr;              // sg[k]
   double* rc = (double*)(rsg + JS / 2);                 // c[k]
-  uchar2* sched = (uchar2*)(rc + JS / 2);               // [ns-1][hp] pivot pairs of every round
+  uchar2* sched = (uchar2*)(rc + JS / 2);               // [rounds][hp] pivot pairs of every round
   __shared__ double red[2][JTHREADS / 32];
   __shared__ int stop;
   const int tid = threadIdx.x, nt = blockDim.x;
-  const int2 pr = pairs[blockIdx.x];
   for (int e = tid; e < ns * ns; e += nt) {
-    const int i = e % ns, j = e / ns;    // column-major global read: consecutive threads -> consecutive rows
-    const int gi = (i < nbk ? pr.x * nbk + i : pr.y * nbk + i - nbk);
-    const int gj = (j < nbk ? pr.x * nbk + j : pr.y * nbk + j - nbk);
-    As[i * LD + j] = Ap[(long)gj * ld + gi];
+    const int i = e % ns, j = e / ns;
     Vs[i * LD + j] = cmake(i == j ? 1.0 : 0.0, 0.0);
   }
   // cross != 0: only the pivots that couple the two blocks (p in the first, q in the second): nbk rounds of nbk
@@ -156,6 +150,24 @@ __global__ void __launch_bounds__(JTHREADS) k_jacobi_cta(const cplx* __restrict_
       __syncthreads();
     }
   }
+}
+
+__global__ void __launch_bounds__(JTHREADS) k_jacobi_cta(const cplx* __restrict__ Ap, long ld, int nbk,
+                                                        const int2* __restrict__ pairs, cplx* __restrict__ U,
+                                                        double* __restrict__ dout, int max_sweeps, double tol2, int cross) {
+  extern __shared__ cplx sm[];
+  const int ns = 2 * nbk, LD = ns + 1;
+  cplx* As = sm;                       // As[i*LD + j] = A[i][j]
+  cplx* Vs = As + ns * LD;
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const int2 pr = pairs[blockIdx.x];
+  for (int e = tid; e < ns * ns; e += nt) {
+    const int i = e % ns, j = e / ns;    // column-major global read: consecutive threads -> consecutive rows
+    const int gi = (i < nbk ? pr.x * nbk + i : pr.y * nbk + i - nbk);
+    const int gj = (j < nbk ? pr.x * nbk + j : pr.y * nbk + j - nbk);
+    As[i * LD + j] = Ap[(long)gj * ld + gi];
+  }
+  jac_solve_smem(As, Vs, Vs + ns * LD, nbk, max_sweeps, tol2, cross);
   cplx* Uo = U + (size_t)blockIdx.x * ns * ns;
   for (int e = tid; e < ns * ns; e += nt) {
     const int i = e % ns, j = e / ns;
@@ -343,18 +355,19 @@ __global__ void k_gather_cols(const cplx* __restrict__ Vp, int np, const int* __
 
 void ks_eigh_free(EighWs* ws) {
   cudaFree(ws->U); cudaFree(ws->Ap); cudaFree(ws->Vp); cudaFree(ws->diag); cudaFree(ws->red);
-  cudaFree(ws->order); cudaFree(ws->pairs);
+  cudaFree(ws->order); cudaFree(ws->pairs); cudaFree(ws->where); cudaFree(ws->Ap2);
   *ws = EighWs();
 }
 
 static int eigh_reserve(EighWs* ws, int np, std::string& err) {
   if (np > ws->cap) {
-    cudaFree(ws->U); cudaFree(ws->Ap); cudaFree(ws->Vp); cudaFree(ws->diag); cudaFree(ws->order);
-    ws->U = ws->Ap = ws->Vp = nullptr; ws->diag = nullptr; ws->order = nullptr; ws->cap = 0;
+    cudaFree(ws->U); cudaFree(ws->Ap); cudaFree(ws->Vp); cudaFree(ws->diag); cudaFree(ws->order); cudaFree(ws->Ap2);
+    ws->U = ws->Ap = ws->Vp = ws->Ap2 = nullptr; ws->diag = nullptr; ws->order = nullptr; ws->cap = 0;
     const size_t nu = std::max<size_t>((size_t)(np / JS + 1) * JS * JS, (size_t)JS * JS);
     KS_CUDA_CHECK(cudaMalloc(&ws->U, sizeof(cplx) * nu), err);
     KS_CUDA_CHECK(cudaMalloc(&ws->Ap, sizeof(cplx) * (size_t)np * np), err);
     KS_CUDA_CHECK(cudaMalloc(&ws->Vp, sizeof(cplx) * (size_t)np * np), err);
+    KS_CUDA_CHECK(cudaMalloc(&ws->Ap2, sizeof(cplx) * (size_t)np * np), err);
     KS_CUDA_CHECK(cudaMalloc(&ws->diag, sizeof(double) * np), err);
     KS_CUDA_CHECK(cudaMalloc(&ws->order, sizeof(int) * np), err);
     ws->cap = np;
@@ -373,15 +386,14 @@ static int eigh_reserve(EighWs* ws, int np, std::string& err) {
 // leading dimension (33) in shared memory: a half-warp reads one row segment, conflict-free.
 // ------------------------------------------------------------------------------------------------
 #define JU_LD 33
-__global__ void __launch_bounds__(256) k_jac_upd32(cplx* __restrict__ Ap, cplx* __restrict__ Vp, long ld, int npair,
-                                                   const int2* __restrict__ pairs, const cplx* __restrict__ U) {
-  extern __shared__ cplx sm[];
+__device__ __forceinline__ void jac_upd_tile(cplx* sm, cplx* __restrict__ Ap, cplx* __restrict__ Vp, long ld, int npair,
+                                             const int2* __restrict__ pairs, const cplx* __restrict__ U, int b, int ay) {
   cplx *sT = sm, *sUa = sm + 32 * JU_LD, *sUb = sm + 64 * JU_LD;
-  const int tid = threadIdx.x, b = blockIdx.x;
-  const bool isA = blockIdx.y < npair;
+  const int tid = threadIdx.x;
+  const bool isA = ay < npair;
   const int2 pb = pairs[b];
-  const int2 pa = isA ? pairs[blockIdx.y] : make_int2(0, 0);
-  const int r0 = isA ? 0 : (blockIdx.y - npair) * 32;
+  const int2 pa = isA ? pairs[ay] : make_int2(0, 0);
+  const int r0 = isA ? 0 : (ay - npair) * 32;
   cplx* X = isA ? Ap : Vp;
   // loads: e -> (i = e % 32 fastest: consecutive rows of a column-major matrix)
   for (int e = tid; e < 32 * 32; e += 256) {
@@ -390,7 +402,7 @@ __global__ void __launch_bounds__(256) k_jac_upd32(cplx* __restrict__ Ap, cplx* 
     const int gj = blk_index<32>(pb, j);
     sT[i * JU_LD + j] = X[(long)gj * ld + gi];
     sUb[i * JU_LD + j] = U[(size_t)b * 1024 + e];                 // U_b[k = i][j]
-    if (isA) sUa[i * JU_LD + j] = U[(size_t)blockIdx.y * 1024 + e];   // U_a[k = i][col = j]
+    if (isA) sUa[i * JU_LD + j] = U[(size_t)ay * 1024 + e];           // U_a[k = i][col = j]
   }
   __syncthreads();
   const int ti = tid >> 4, tj = tid & 15;
@@ -430,6 +442,147 @@ __global__ void __launch_bounds__(256) k_jac_upd32(cplx* __restrict__ Ap, cplx* 
   }
 }
 
+__global__ void __launch_bounds__(256) k_jac_upd32(cplx* __restrict__ Ap, cplx* __restrict__ Vp, long ld, int npair,
+                                                   const int2* __restrict__ pairs, const cplx* __restrict__ U) {
+  extern __shared__ cplx sm[];
+  jac_upd_tile(sm, Ap, Vp, ld, npair, pairs, U, blockIdx.x, blockIdx.y);
+}
+
+// ------------------------------------------------------------------------------------------------
+// One launch per round (32-wide pairs).  CTAs 0 .. npair-1 solve the pair problems of the NEXT round while
+// the other CTAs apply THIS round's rotations U_cur to A and V (jac_upd_tile).  A next-round pair (I', J')
+// needs only A'[{I',J'},{I',J'}] = four 16 x 16 blocks of U_a^H A[IJ_a, IJ_b] U_b, where a, b are the pairs of
+// this round that hold I', J' (table `where`: block -> (pair index, half)); the solver CTA recomputes those
+// blocks itself from the not yet updated A (reads only; the tile CTAs write A in place, so the reads below go
+// through a snapshot: see the host loop -- A is double buffered).  The pair solves (tens of microseconds on
+// npair SMs) therefore overlap the bulk update instead of serialising with it.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_jac_round32(const cplx* __restrict__ Aold, cplx* __restrict__ Anew, cplx* __restrict__ Vp,
+                                                     long ld, int npair, int nvt, const int2* __restrict__ pairs_cur,
+                                                     const int2* __restrict__ where_cur, const cplx* __restrict__ Ucur,
+                                                     const int2* __restrict__ pairs_next, cplx* __restrict__ Unext,
+                                                     int inner, int cross_next) {
+  extern __shared__ cplx sm[];
+  const int tid = threadIdx.x;
+  if ((int)blockIdx.x >= npair) {
+    // tile CTA: t -> (b, ay); A tiles read Aold and write Anew, V tiles update Vp in place
+    const int t = blockIdx.x - npair, b = t % npair, ay = t / npair;
+    cplx *sT = sm, *sUa = sm + 32 * JU_LD, *sUb = sm + 64 * JU_LD;
+    const bool isA = ay < npair;
+    const int2 pb = pairs_cur[b];
+    const int2 pa = isA ? pairs_cur[ay] : make_int2(0, 0);
+    const int r0 = isA ? 0 : (ay - npair) * 32;
+    const cplx* Xin = isA ? Aold : Vp;
+    cplx* Xout = isA ? Anew : Vp;
+    for (int e = tid; e < 32 * 32; e += 256) {
+      const int i = e & 31, j = e >> 5;
+      const int gi = isA ? blk_index<32>(pa, i) : r0 + i;
+      const int gj = blk_index<32>(pb, j);
+      sT[i * JU_LD + j] = Xin[(long)gj * ld + gi];
+      sUb[i * JU_LD + j] = Ucur[(size_t)b * 1024 + e];
+      if (isA) sUa[i * JU_LD + j] = Ucur[(size_t)ay * 1024 + e];
+    }
+    __syncthreads();
+    const int ti = tid >> 4, tj = tid & 15;
+    cplx p00 = cmake(0, 0), p01 = p00, p10 = p00, p11 = p00;
+#pragma unroll 8
+    for (int k = 0; k < 32; ++k) {
+      const cplx a0 = sT[ti * JU_LD + k], a1 = sT[(ti + 16) * JU_LD + k];
+      const cplx b0 = sUb[k * JU_LD + tj], b1 = sUb[k * JU_LD + tj + 16];
+      p00 = cfma(a0, b0, p00); p01 = cfma(a0, b1, p01);
+      p10 = cfma(a1, b0, p10); p11 = cfma(a1, b1, p11);
+    }
+    __syncthreads();
+    sT[ti * JU_LD + tj] = p00; sT[ti * JU_LD + tj + 16] = p01;
+    sT[(ti + 16) * JU_LD + tj] = p10; sT[(ti + 16) * JU_LD + tj + 16] = p11;
+    __syncthreads();
+    if (isA) {
+      cplx q00 = cmake(0, 0), q01 = q00, q10 = q00, q11 = q00;
+#pragma unroll 8
+      for (int k = 0; k < 32; ++k) {
+        const cplx a0 = cconj(sUa[k * JU_LD + ti]), a1 = cconj(sUa[k * JU_LD + ti + 16]);
+        const cplx b0 = sT[k * JU_LD + tj], b1 = sT[k * JU_LD + tj + 16];
+        q00 = cfma(a0, b0, q00); q01 = cfma(a0, b1, q01);
+        q10 = cfma(a1, b0, q10); q11 = cfma(a1, b1, q11);
+      }
+      __syncthreads();
+      sT[ti * JU_LD + tj] = q00; sT[ti * JU_LD + tj + 16] = q01;
+      sT[(ti + 16) * JU_LD + tj] = q10; sT[(ti + 16) * JU_LD + tj + 16] = q11;
+      __syncthreads();
+    }
+    for (int e = tid; e < 32 * 32; e += 256) {
+      const int i = e & 31, j = e >> 5;
+      const int gi = isA ? blk_index<32>(pa, i) : r0 + i;
+      const int gj = blk_index<32>(pb, j);
+      Xout[(long)gj * ld + gi] = sT[i * JU_LD + j];
+    }
+    return;
+  }
+  // solver CTA for next-round pair p
+  const int p = blockIdx.x;
+  cplx* As = sm;                       // [32][33]
+  cplx* sT = sm + 32 * JU_LD;          // doubles as Vs once As is built
+  cplx* sUa = sm + 64 * JU_LD;
+  cplx* sUb = sm + 96 * JU_LD;
+  const int2 pn = pairs_next[p];
+  const int ti = tid >> 4, tj = tid & 15;
+  for (int bx = 0; bx < 2; ++bx)
+    for (int by = 0; by < 2; ++by) {
+      const int2 wa = where_cur[bx ? pn.y : pn.x], wb = where_cur[by ? pn.y : pn.x];
+      const int2 pa = pairs_cur[wa.x], pb = pairs_cur[wb.x];
+      __syncthreads();
+      for (int e = tid; e < 32 * 32; e += 256) {
+        const int i = e & 31, j = e >> 5;
+        sT[i * JU_LD + j] = Aold[(long)blk_index<32>(pb, j) * ld + blk_index<32>(pa, i)];
+        sUa[i * JU_LD + j] = Ucur[(size_t)wa.x * 1024 + e];
+        sUb[i * JU_LD + j] = Ucur[(size_t)wb.x * 1024 + e];
+      }
+      __syncthreads();
+      // P (32 x 16) = T U_b[:, half_b] : thread (ti, tj) -> rows ti, ti+16, column tj
+      cplx p0 = cmake(0, 0), p1 = p0;
+      const int cb = wb.y * 16 + tj;
+#pragma unroll 8
+      for (int k = 0; k < 32; ++k) {
+        const cplx bb = sUb[k * JU_LD + cb];
+        p0 = cfma(sT[ti * JU_LD + k], bb, p0);
+        p1 = cfma(sT[(ti + 16) * JU_LD + k], bb, p1);
+      }
+      __syncthreads();
+      sT[ti * JU_LD + tj] = p0;
+      sT[(ti + 16) * JU_LD + tj] = p1;
+      __syncthreads();
+      // M (16 x 16) = U_a[:, half_a]^H P : thread (ti, tj) -> element (ti, tj)
+      cplx q = cmake(0, 0);
+      const int ca = wa.y * 16 + ti;
+#pragma unroll 8
+      for (int k = 0; k < 32; ++k) q = cfma(cconj(sUa[k * JU_LD + ca]), sT[k * JU_LD + tj], q);
+      As[(bx * 16 + ti) * JU_LD + by * 16 + tj] = q;
+    }
+  __syncthreads();
+  // exact Hermitian input for the rotations: real diagonal, upper triangle mirrored
+  for (int e = tid; e < 32 * 32; e += 256) {
+    const int i = e >> 5, j = e & 31;
+    if (i == j) As[i * JU_LD + i].y = 0.0;
+  }
+  __syncthreads();
+  for (int e = tid; e < 32 * 32; e += 256) {
+    const int i = e >> 5, j = e & 31;
+    if (i < j) {
+      const cplx u = As[i * JU_LD + j], l = As[j * JU_LD + i];
+      const cplx m = cmake(0.5 * (u.x + l.x), 0.5 * (u.y - l.y));
+      As[i * JU_LD + j] = m;
+      As[j * JU_LD + i] = cconj(m);
+    }
+  }
+  __syncthreads();
+  jac_solve_smem(As, sT, sm + 128 * JU_LD, 16, inner, 1e-30, cross_next);
+  cplx* Uo = Unext + (size_t)p * 1024;
+  for (int e = tid; e < 1024; e += 256) {
+    const int i = e & 31, j = e >> 5;
+    Uo[(size_t)j * 32 + i] = sT[i * JU_LD + j];
+  }
+}
+
 template <int JSZ>
 static int block_sweeps(cudaStream_t st, int n, const cplx* A, long lda, EighWs* ws, double tol2, int inner, int* sweeps_out,
                         std::string& err) {
@@ -463,12 +616,57 @@ static int block_sweeps(cudaStream_t st, int n, const cplx* A, long lda, EighWs*
       }
     KS_CUDA_CHECK(cudaMalloc(&ws->pairs, sizeof(int2) * h.size()), err);
     KS_CUDA_CHECK(cudaMemcpy(ws->pairs, h.data(), sizeof(int2) * h.size(), cudaMemcpyHostToDevice), err);
+    cudaFree(ws->where); ws->where = nullptr;
+    std::vector<int2> wh((size_t)(nblk - 1) * nblk);
+    for (int r = 0; r < nblk - 1; ++r)
+      for (int k = 0; k < npair; ++k) {
+        const int2 pq = h[(size_t)r * npair + k];
+        wh[(size_t)r * nblk + pq.x] = make_int2(k, 0);
+        wh[(size_t)r * nblk + pq.y] = make_int2(k, 1);
+      }
+    KS_CUDA_CHECK(cudaMalloc(&ws->where, sizeof(int2) * wh.size()), err);
+    KS_CUDA_CHECK(cudaMemcpy(ws->where, wh.data(), sizeof(int2) * wh.size(), cudaMemcpyHostToDevice), err);
     ws->pairs_nblk = nblk;
   }
   k_pad_copy<<<ceil_div((long)np * np, 256), 256, 0, st>>>(A, lda, n, ws->Ap, ws->Vp, np);
   static const bool fused_upd = !(getenv("KSPW_JAC_FUSED") && atoi(getenv("KSPW_JAC_FUSED")) == 0);
   static const bool cross_rounds = !(getenv("KSPW_JAC_CROSS") && atoi(getenv("KSPW_JAC_CROSS")) == 0);
+  static const bool one_launch = !(getenv("KSPW_JAC_ROUND") && atoi(getenv("KSPW_JAC_ROUND")) == 0);
   int sweeps = 0;
+  if (JSZ == 32 && fused_upd && one_launch && np >= 512) {   // below ~500 the solver CTAs' own tile products outweigh the overlap
+    // one launch per round: the launch that applies round r also solves the pair problems of round r+1
+    const size_t smem_round = sizeof(cplx) * 128 * JU_LD + 2048;
+    static bool opted2 = false;
+    if (!opted2) {
+      KS_CUDA_CHECK(cudaFuncSetAttribute(k_jac_round32, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_round), err);
+      opted2 = true;
+    }
+    const int nr = nblk - 1, nvt = np / 32;
+    cplx* Ucur = ws->U;
+    cplx* Unext = ws->U + (size_t)npair * 1024;
+    cplx *Acur = ws->Ap, *Aalt = ws->Ap2;
+    k_jacobi_cta<<<npair, 256, smem_cta, st>>>(Acur, np, JBK, ws->pairs, Ucur, nullptr, inner, 1e-30, 0);
+    for (; sweeps < 40; ++sweeps) {
+      double h[2];
+      KS_CUDA_CHECK(cudaMemsetAsync(ws->red, 0, 2 * sizeof(double), st), err);
+      k_offnorm<<<148 * 2, 256, 0, st>>>(Acur, np, n, ws->red);
+      KS_CUDA_CHECK(cudaMemcpyAsync(h, ws->red, sizeof h, cudaMemcpyDeviceToHost, st), err);
+      KS_CUDA_CHECK(cudaStreamSynchronize(st), err);
+      if (h[0] <= tol2 * h[1]) break;
+      for (int r = 0; r < nr; ++r) {
+        const int rn = (r + 1) % nr;
+        k_jac_round32<<<npair + npair * (npair + nvt), 256, smem_round, st>>>(
+            Acur, Aalt, ws->Vp, np, npair, nvt, ws->pairs + (size_t)r * npair, ws->where + (size_t)r * nblk, Ucur,
+            ws->pairs + (size_t)rn * npair, Unext, inner, (rn > 0 && cross_rounds) ? 1 : 0);
+        std::swap(Acur, Aalt);
+        std::swap(Ucur, Unext);
+      }
+    }
+    if (Acur != ws->Ap) std::swap(ws->Ap, ws->Ap2);   // the caller reads the diagonal from ws->Ap
+    KS_CUDA_CHECK(cudaGetLastError(), err);
+    *sweeps_out = sweeps;
+    return KS_OK;
+  }
   for (; sweeps < 40; ++sweeps) {
     double h[2];
     KS_CUDA_CHECK(cudaMemsetAsync(ws->red, 0, 2 * sizeof(double), st), err);

@@ -64,6 +64,8 @@ struct EighWs {
   double* red = nullptr;   // [2] off^2, tot^2
   int* order = nullptr;    // [np]
   int2* pairs = nullptr;   // [(nblk-1)][nblk/2] block pairs of every round
+  int2* where = nullptr;   // [(nblk-1)][nblk] block -> (index of its pair in the round, 0/1 = first/second of the pair)
+  cplx* Ap2 = nullptr;     // second copy of A: the one-launch-per-round path reads one and writes the other
   int cap = 0;             // padded n the buffers hold
   int np = 0;              // padded n of the current run
   int pairs_nblk = 0;      // nblk the pair table was built for
