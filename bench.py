@@ -177,6 +177,23 @@ def kernel_models(p, nb_per_launch):
     }
 
 
+def ncu_traffic(kernel, cfg, bands_per_launch):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed `ncu --set full` capture
+    (profiles/r1_traffic.csv: kernel,cfg,bands_per_launch,dram_read_bytes,dram_write_bytes), scaled to this run's
+    bands per launch; None when no capture of that kernel and config is committed."""
+    path = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    for ln in open(path):
+        f = ln.strip().split(",")
+        if len(f) >= 5 and f[0] == kernel.split("+")[0] and f[1] == str(cfg):
+            try:
+                return (float(f[3]) + float(f[4])) * bands_per_launch / float(f[2])
+            except ValueError:
+                return None
+    return None
+
+
 def main():
     args = parse()
     if args.impl == "reference":
@@ -295,7 +312,9 @@ def main():
                       "avg_launch_ms": avg_ms, "launches": nlaunch, "share_of_step": tms / ms}
     dom = max((k for k in rows if rows[k]["bound"] != "alu"), key=lambda k: rows[k]["share_of_step"])
     roof = dict(rows[dom])
-    roof.update({"kernel": dom, "traffic": None,
+    for name, r in rows.items():
+        r["traffic"] = ncu_traffic(name, p.cfg.index, nb_per_fft_launch if name.startswith(("k_inv", "k_x", "k_fwd")) else nb)
+    roof.update({"kernel": dom, "traffic": rows[dom]["traffic"],
                  "peak_source": ("MEASURED_PEAKS.json hbm_gbs (%s)" % pk["src"]) if roof["bound"] == "hbm" else
                  "live register-resident DMMA m8n8k4 microbenchmark (ks_dmma_peak); bf16 measured x nominal ratio = %.1f TFLOP/s"
                  % (pk["bf16"] * NOMINAL_FP64_OVER_BF16)})
