@@ -179,9 +179,26 @@ constexpr int yz_pick_zc(int nz) {
     if (nz % zc == 0) return zc;
   return 1;
 }
-template <int NY, int NZ> struct yzcfg { static constexpr int ZC = yz_pick_zc(NZ), NT = 256; };
-template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 512; };
-template <> struct yzcfg<96, 288> { static constexpr int ZC = 16, NT = 256; };
+// DBF: the forward kernel splits the y tile into two half-width buffers filled by cp.async one chunk ahead (pays
+// when two CTAs fit per SM; measured: 96x96 213 -> 201 us; 128x128 224 -> 254 us and 96x288 337 -> 376 us, where one CTA fills the SM: off there)
+template <int NY, int NZ> struct yzcfg { static constexpr int ZC = yz_pick_zc(NZ), NT = 256; static constexpr bool DBF = (ZC % 2 == 0); };
+template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 512; static constexpr bool DBF = false; };
+template <> struct yzcfg<96, 288> { static constexpr int ZC = 16, NT = 256; static constexpr bool DBF = false; };
+
+// 16-byte global -> shared async copy (LDGSTS), ordered against the surrounding shared-memory accesses
+__device__ __forceinline__ void cp16m(cplx* smem, const cplx* gmem) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_commit_m() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_wait_n(int n) {   // n = groups allowed to stay in flight (uniform per thread)
+  switch (n) {
+    case 0: asm volatile("cp.async.wait_group 0;\n" ::: "memory"); break;
+    case 1: asm volatile("cp.async.wait_group 1;\n" ::: "memory"); break;
+    case 2: asm volatile("cp.async.wait_group 2;\n" ::: "memory"); break;
+    default: asm volatile("cp.async.wait_group 3;\n" ::: "memory"); break;
+  }
+}
 
 // lines-first walk over (stick s, line j) pairs: item it = j*S + s, it = tid, tid + NT, ...
 struct StickWalk {
@@ -293,6 +310,58 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_fwd_yz(YzArgs a) {
   const int y0 = a.plane_y0[lx];
   const cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ);
   const int pz = tid % ZC, g = tid / ZC;
+  // H4 (y), type B, forward.  The y tile is split into two half-width buffers: while chunk c (ZF = ZC/2 columns) is
+  // transformed in place in one of them, chunk c+1 streams into the other by cp.async, so the plane loads are
+  // in flight during both codelet passes.  (Odd ZC: single buffer, loads straight into registers.)
+  if constexpr (yzcfg<NY, NZ>::DBF) {
+    constexpr int ZF = ZC / 2, GF = NT / ZF, NCF = NZ / ZF;
+    const int fz = tid % ZF, fg = tid / ZF;
+    auto issue = [&](int c) {
+      cplx* dst = ytile + (c & 1) * (NY * ZF);
+      const cplx* src = plane + c * ZF;
+      for (int e = tid; e < NY * ZF; e += NT) cp16m(dst + e, src + (size_t)(e / ZF) * NZ + (e % ZF));
+      cp_commit_m();
+    };
+    issue(0);
+    for (int i = tid; i < NY; i += NT) tw_y[i] = a.tw_y[i];
+    if (NY != NZ)
+      for (int i = tid; i < NZ; i += NT) tw_z[i] = a.tw_z[i];
+    for (int c = 0; c < NCF; ++c) {
+      cp_wait_n(0);
+      __syncthreads();              // chunk c has landed; pass 2 of chunk c-1 is over, its buffer is free
+      if (c + 1 < NCF) issue(c + 1);
+      cplx* yb = ytile + (c & 1) * (NY * ZF) + fz;
+      if (fg < GF) {
+        for (int k1 = fg; k1 < R1y; k1 += GF) {
+          cplx v[R2y];
+          cplx* o = yb + k1 * R2y * ZF;
+#pragma unroll
+          for (int k2 = 0; k2 < R2y; ++k2) v[k2] = o[k2 * ZF];
+          dft<R2y, -1>(v);
+#pragma unroll
+          for (int q2 = 0; q2 < R2y; ++q2) o[q2 * ZF] = (q2 == 0) ? v[0] : mul_tw<-1>(v[q2], tw_y, k1 * q2);
+        }
+      }
+      __syncthreads();
+      if (fg < GF) {
+        for (int q2 = fg; q2 < R2y; q2 += GF) {
+          cplx u[R1y];
+          const cplx* t = yb + q2 * ZF;
+#pragma unroll
+          for (int k1 = 0; k1 < R1y; ++k1) u[k1] = t[k1 * R2y * ZF];
+          dft<R1y, -1>(u);
+          cplx* o = stile + c * ZF + fz;
+#pragma unroll
+          for (int q1 = 0; q1 < R1y; ++q1) {   // natural y = q1*R2y + q2; keep the stick columns only
+            int s = q1 * R2y + q2 - y0;
+            if (s < 0) s += NY;
+            if (s < S) o[s * SZ] = u[q1];
+          }
+        }
+      }
+    }
+    __syncthreads();
+  } else {
   // H4 (y) pass 1 of a chunk: plane -> registers -> DFT-R2y -> twiddle -> ytile (type B, forward)
   auto load_in = [&](cplx (&v)[R2y], int c, int k1) {
     const cplx* src = plane + (size_t)(k1 * R2y) * NZ + c * ZC + pz;
@@ -335,6 +404,7 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_fwd_yz(YzArgs a) {
       }
       __syncthreads();
     }
+  }
   }
   // H4 (z): type-B forward FFT on each stick
   for (StickWalk w(tid, NT, S); w.j < R1z; w.next()) lineB_stage1<NZ, -1>(stile + w.s * SZ, 1, w.j, tw_z);
@@ -385,21 +455,6 @@ template <> struct xcfg<18> { static constexpr int ZC = 32, NT = 96, MINB = 4; }
 template <> struct xcfg<36> { static constexpr int ZC = 32, NT = 96, MINB = 4; };
 template <> struct xcfg<54> { static constexpr int ZC = 32, NT = 96, MINB = 4; };
 template <> struct xcfg<128> { static constexpr int ZC = 32, NT = 256, MINB = 2; };
-
-// 16-byte global -> shared async copy (LDGSTS), ordered against the surrounding shared-memory accesses
-__device__ __forceinline__ void cp16m(cplx* smem, const cplx* gmem) {
-  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_commit_m() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-__device__ __forceinline__ void cp_wait_n(int n) {   // n = groups allowed to stay in flight (uniform per thread)
-  switch (n) {
-    case 0: asm volatile("cp.async.wait_group 0;\n" ::: "memory"); break;
-    case 1: asm volatile("cp.async.wait_group 1;\n" ::: "memory"); break;
-    case 2: asm volatile("cp.async.wait_group 2;\n" ::: "memory"); break;
-    default: asm volatile("cp.async.wait_group 3;\n" ::: "memory"); break;
-  }
-}
 
 // The CTA walks over bg bands with the same columns.  Thread (pz, g) owns the codelet lines j2 = g, g+G, ...
 // in the first AND the last pass, i.e. the tile rows {j1*R2 + j2}: once the last pass of band b has read a
