@@ -23,14 +23,17 @@
 #define LDK (KT + 4)   // "k-contiguous" tile leading dimension: == 4 (mod 8) -> conflict-free fragment loads
 
 // ------------------------------------------------------------------------------------------------
-// C = A^H B.  CTA tile 64 x 64, 8 warps as 2 (M) x 4 (N), warp tile 32 x 16 -> 4 x 2 MMA tiles.
+// C = A^H B.  CTA tile 64 x 32*NJ, 8 warps as 2 (M) x 4 (N), warp tile 32 x 8*NJ -> 4 x NJ MMA tiles.
+// NJ in 1..5 is picked per call so that N is covered with the least padding (N = 160 -> one 160-wide tile,
+// N = 5 unconverged bands -> a 32-wide tile instead of 64).
 // ------------------------------------------------------------------------------------------------
 #define HN_MT 64
-#define HN_NT 64
 
+template <int NJ>
 __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_hn(int M, int N, int K, const cplx* __restrict__ A, long lda,
                                                           const cplx* __restrict__ B, long ldb, cplx* __restrict__ part,
                                                           int kchunk) {
+  constexpr int HN_NT = 32 * NJ;
   extern __shared__ cplx sm[];
   cplx* sA = sm;                                     // [stage][HN_MT][LDK]
   cplx* sB = sm + GEMM_STAGES * HN_MT * LDK;         // [stage][HN_NT][LDK]
@@ -57,11 +60,11 @@ __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_hn(int M, int N, int K, c
     }
   };
 
-  double cre[4][2][2], cim[4][2][2];
+  double cre[4][NJ][2], cim[4][NJ][2];
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
-    for (int j = 0; j < 2; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
+    for (int j = 0; j < NJ; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
 
   for (int s = 0; s < GEMM_STAGES - 1; ++s) {
     if (s < ntile) load_stage(s, s);
@@ -74,19 +77,19 @@ __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_hn(int M, int N, int K, c
     if (kt + GEMM_STAGES - 1 < ntile) load_stage((kt + GEMM_STAGES - 1) % GEMM_STAGES, kt + GEMM_STAGES - 1);
     cp_commit();
     const cplx* a = sA + ((kt % GEMM_STAGES) * HN_MT + wm * 32) * LDK;
-    const cplx* b = sB + ((kt % GEMM_STAGES) * HN_NT + wn * 16) * LDK;
+    const cplx* b = sB + ((kt % GEMM_STAGES) * HN_NT + wn * 8 * NJ) * LDK;
 #pragma unroll
     for (int ks = 0; ks < KT; ks += 4) {
-      cplx af[4], bf[2];
+      cplx af[4], bf[NJ];
 #pragma unroll
       for (int i = 0; i < 4; ++i) af[i] = a[(i * 8 + fr) * LDK + ks + fk];
 #pragma unroll
-      for (int j = 0; j < 2; ++j) bf[j] = b[(j * 8 + fr) * LDK + ks + fk];
+      for (int j = 0; j < NJ; ++j) bf[j] = b[(j * 8 + fr) * LDK + ks + fk];
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
         const double nai = -af[i].y;
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {   // conj(a) b = (ar br + ai bi) + i (ar bi - ai br)
+        for (int j = 0; j < NJ; ++j) {   // conj(a) b = (ar br + ai bi) + i (ar bi - ai br)
           dmma(cre[i][j][0], cre[i][j][1], af[i].x, bf[j].x);
           dmma(cim[i][j][0], cim[i][j][1], af[i].x, bf[j].y);
           dmma(cre[i][j][0], cre[i][j][1], af[i].y, bf[j].y);
@@ -101,10 +104,10 @@ __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_hn(int M, int N, int K, c
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
-    for (int j = 0; j < 2; ++j)
+    for (int j = 0; j < NJ; ++j)
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        const int m = m0 + wm * 32 + i * 8 + fr, n = n0 + wn * 16 + j * 8 + 2 * fk + h;
+        const int m = m0 + wm * 32 + i * 8 + fr, n = n0 + wn * 8 * NJ + j * 8 + 2 * fk + h;
         if (m < M && n < N) out[(size_t)n * M + m] = cmake(cre[i][j][h], cim[i][j][h]);
       }
 }
@@ -120,14 +123,25 @@ __global__ void k_splitk_reduce(int M, int N, int nsplit, const cplx* __restrict
   C[(i / M) * ldc + (i % M)] = cmake(sr, si);
 }
 
-int ks_gemm_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
-               long ldc, GemmWs* ws, std::string& err) {
-  if (M <= 0 || N <= 0) return KS_OK;
-  if (K < 0 || !ws) { err = "ks_gemm_hn: bad argument"; return KS_EINVAL; }
+// N-tile multiplier with the least padded width (ties: the wider tile)
+static int pick_nj(int N, int unit) {
+  int best = 1;
+  long bestpad = -1;
+  for (int nj = 1; nj <= 5; ++nj) {
+    const long w = (long)unit * nj, pad = (N + w - 1) / w * w;
+    if (bestpad < 0 || pad <= bestpad) { best = nj; bestpad = pad; }
+  }
+  return best;
+}
+
+template <int NJ>
+static int launch_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
+                     long ldc, GemmWs* ws, std::string& err) {
+  constexpr int HN_NT = 32 * NJ;
   static bool opted = false;
   const size_t smem = sizeof(cplx) * GEMM_STAGES * (HN_MT + HN_NT) * LDK;
   if (!opted) {
-    KS_CUDA_CHECK(cudaFuncSetAttribute(k_gemm_hn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err);
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_gemm_hn<NJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err);
     opted = true;
   }
   const int tm = ceil_div(M, HN_MT), tn = ceil_div(N, HN_NT);
@@ -144,22 +158,37 @@ int ks_gemm_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, co
     ws->bytes = need;
   }
   dim3 grid(tn, tm, nsplit);
-  k_gemm_hn<<<grid, GEMM_THREADS, smem, st>>>(M, N, K, A, lda, B, ldb, ws->part, kchunk);
+  k_gemm_hn<NJ><<<grid, GEMM_THREADS, smem, st>>>(M, N, K, A, lda, B, ldb, ws->part, kchunk);
   k_splitk_reduce<<<ceil_div((long)M * N, 256), 256, 0, st>>>(M, N, nsplit, ws->part, C, ldc);
   KS_CUDA_CHECK(cudaGetLastError(), err);
   return KS_OK;
 }
 
+int ks_gemm_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
+               long ldc, GemmWs* ws, std::string& err) {
+  if (M <= 0 || N <= 0) return KS_OK;
+  if (K < 0 || !ws) { err = "ks_gemm_hn: bad argument"; return KS_EINVAL; }
+  switch (pick_nj(N, 32)) {
+    case 1: return launch_hn<1>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);
+    case 2: return launch_hn<2>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);
+    case 3: return launch_hn<3>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);
+    case 4: return launch_hn<4>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);
+    default: return launch_hn<5>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
-// C (+)= A B.  CTA tile 128 (M) x 64 (N), 8 warps as 4 (M) x 2 (N), warp tile 32 x 32 -> 4 x 4 MMA tiles.
+// C (+)= A B.  CTA tile 128 (M) x 16*NJ (N), 8 warps as 4 (M) x 2 (N), warp tile 32 x 8*NJ -> 4 x NJ MMA tiles,
+// NJ in 1..5 picked per call for the least padding of N (N = 160 -> two 80-wide tiles, not three 64-wide ones).
 // ------------------------------------------------------------------------------------------------
 #define NN_MT 128
-#define NN_NT 64
 #define LDM (NN_MT + 2)   // "m-contiguous" tile leading dimension: == 2 (mod 8)
 
+template <int NJ>
 __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_nn(int M, int N, int K, const cplx* __restrict__ A, long lda,
                                                           const cplx* __restrict__ B, long ldb, cplx* __restrict__ C,
                                                           long ldc, int accumulate) {
+  constexpr int NN_NT = 16 * NJ;
   extern __shared__ cplx sm[];
   cplx* sA = sm;                                   // [stage][KT][LDM]
   cplx* sB = sm + GEMM_STAGES * KT * LDM;          // [stage][NN_NT][LDK]
@@ -184,11 +213,11 @@ __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_nn(int M, int N, int K, c
     }
   };
 
-  double cre[4][4][2], cim[4][4][2];
+  double cre[4][NJ][2], cim[4][NJ][2];
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
-    for (int j = 0; j < 4; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
+    for (int j = 0; j < NJ; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
 
   for (int s = 0; s < GEMM_STAGES - 1; ++s) {
     if (s < ntile) load_stage(s, s);
@@ -201,19 +230,19 @@ __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_nn(int M, int N, int K, c
     if (kt + GEMM_STAGES - 1 < ntile) load_stage((kt + GEMM_STAGES - 1) % GEMM_STAGES, kt + GEMM_STAGES - 1);
     cp_commit();
     const cplx* a = sA + (kt % GEMM_STAGES) * KT * LDM + wm * 32;
-    const cplx* b = sB + ((kt % GEMM_STAGES) * NN_NT + wn * 32) * LDK;
+    const cplx* b = sB + ((kt % GEMM_STAGES) * NN_NT + wn * 8 * NJ) * LDK;
 #pragma unroll
     for (int ks = 0; ks < KT; ks += 4) {
-      cplx af[4], bf[4];
+      cplx af[4], bf[NJ];
 #pragma unroll
       for (int i = 0; i < 4; ++i) af[i] = a[(ks + fk) * LDM + i * 8 + fr];
 #pragma unroll
-      for (int j = 0; j < 4; ++j) bf[j] = b[(j * 8 + fr) * LDK + ks + fk];
+      for (int j = 0; j < NJ; ++j) bf[j] = b[(j * 8 + fr) * LDK + ks + fk];
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
         const double nai = -af[i].y;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {   // a b = (ar br - ai bi) + i (ar bi + ai br)
+        for (int j = 0; j < NJ; ++j) {   // a b = (ar br - ai bi) + i (ar bi + ai br)
           dmma(cre[i][j][0], cre[i][j][1], af[i].x, bf[j].x);
           dmma(cim[i][j][0], cim[i][j][1], af[i].x, bf[j].y);
           dmma(cre[i][j][0], cre[i][j][1], nai, bf[j].y);
@@ -226,10 +255,10 @@ __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_nn(int M, int N, int K, c
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
-    for (int j = 0; j < 4; ++j)
+    for (int j = 0; j < NJ; ++j)
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        const int m = m0 + wm * 32 + i * 8 + fr, n = n0 + wn * 32 + j * 8 + 2 * fk + h;
+        const int m = m0 + wm * 32 + i * 8 + fr, n = n0 + wn * 8 * NJ + j * 8 + 2 * fk + h;
         if (m < M && n < N) {
           cplx* p = &C[(long)n * ldc + m];
           cplx v = cmake(cre[i][j][h], cim[i][j][h]);
@@ -239,20 +268,33 @@ __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_nn(int M, int N, int K, c
       }
 }
 
+template <int NJ>
+static int launch_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
+                     long ldc, int accumulate, std::string& err) {
+  constexpr int NN_NT = 16 * NJ;
+  static bool opted = false;
+  const size_t smem = sizeof(cplx) * GEMM_STAGES * (KT * LDM + NN_NT * LDK);
+  if (!opted) {
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_gemm_nn<NJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err);
+    opted = true;
+  }
+  dim3 grid(ceil_div(M, NN_MT), ceil_div(N, NN_NT));
+  k_gemm_nn<NJ><<<grid, GEMM_THREADS, smem, st>>>(M, N, K, A, lda, B, ldb, C, ldc, accumulate);
+  KS_CUDA_CHECK(cudaGetLastError(), err);
+  return KS_OK;
+}
+
 int ks_gemm_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
                long ldc, int accumulate, std::string& err) {
   if (M <= 0 || N <= 0) return KS_OK;
   if (K < 0) { err = "ks_gemm_nn: bad argument"; return KS_EINVAL; }
-  static bool opted = false;
-  const size_t smem = sizeof(cplx) * GEMM_STAGES * (KT * LDM + NN_NT * LDK);
-  if (!opted) {
-    KS_CUDA_CHECK(cudaFuncSetAttribute(k_gemm_nn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err);
-    opted = true;
+  switch (pick_nj(N, 16)) {
+    case 1: return launch_nn<1>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
+    case 2: return launch_nn<2>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
+    case 3: return launch_nn<3>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
+    case 4: return launch_nn<4>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
+    default: return launch_nn<5>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
   }
-  dim3 grid(ceil_div(M, NN_MT), ceil_div(N, NN_NT));
-  k_gemm_nn<<<grid, GEMM_THREADS, smem, st>>>(M, N, K, A, lda, B, ldb, C, ldc, accumulate);
-  KS_CUDA_CHECK(cudaGetLastError(), err);
-  return KS_OK;
 }
 
 // ------------------------------------------------------------------------------------------------
