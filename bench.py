@@ -199,16 +199,12 @@ def main():
     if args.impl == "reference":
         return run_reference(args)
     import torch
-    import torch.distributed as dist
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2501_08697_b200 import parallel as PL
+    rank, world, local = PL.env_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     torch.cuda.set_device(local)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl")
+    PL.init("nccl")
     from paper_2501_08697_b200 import kspw
 
     p = I.make_problem(args.config, args.k_index)
@@ -225,10 +221,7 @@ def main():
     if resident_bytes < 2 * 126e6:   # inputs not clearly larger than L2: flush between timed iterations
         flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+    barrier = PL.barrier
 
     def timed_steps(fn, k):
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
@@ -279,16 +272,12 @@ def main():
                "band_applications_per_s": r["band_applications"] / dsec,
                "eig_min": float(r["eig"][0].item()), "eig_max": float(r["eig"][-1].item())}
     clk = clocks.stop() if rank == 0 else None
-    tmax = torch.tensor([ms, e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms, e2e_s = float(tmax[0]), float(tmax[1])
+    ms, e2e_s = PL.max_over_ranks([ms, e2e_s])
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        PL.finalize()
         return 0
 
-    value = world * nb * args.steps / (ms * 1e-3)
+    value = PL.aggregate_throughput(nb * args.steps, world, ms)
     pk = peaks()
     dmma_tf, dfma_tf = kspw.ks_dmma_peak()
     nbatch_launches = prof["k_x"][1] // max(args.steps, 1)          # FFT launches per step
@@ -345,8 +334,7 @@ def main():
     else:
         line["cpu_baseline"] = None
     print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    PL.finalize()
     return 0
 
 
