@@ -44,6 +44,10 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--davidson-max-iter", type=int, default=400)
     ap.add_argument("--fft-batch", type=int, default=0)
+    ap.add_argument("--kbatch", action="store_true",
+                    help="config 2 only: a step = one H psi block apply on EVERY k-point of the 4x4x4 mesh (64 contexts on a "
+                         "pool of CUDA streams), k-points sharded over the ranks")
+    ap.add_argument("--streams", type=int, default=8)
     return ap.parse_args()
 
 
@@ -194,10 +198,123 @@ def ncu_traffic(kernel, cfg, bands_per_launch):
     return None
 
 
+def run_kbatch(args):
+    """BASELINE config 2 as a k-point batch: every k-point is an independent unit (its own G sphere, beta and ks_ctx);
+    the k-points of this rank's share run on a pool of CUDA streams so that the small kernels of different k overlap.
+    N > 1: the 64 k-points are sharded over the ranks (strong scaling: total work fixed), no data-path collective."""
+    import torch
+    from paper_2501_08697_b200 import parallel as PL
+    rank, world, local = PL.env_world()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    PL.init("nccl")
+    from paper_2501_08697_b200 import kspw
+    nk_total = 64
+    mine = PL.shard_units(nk_total, rank, world)
+    main = torch.cuda.current_stream()
+    pool = [torch.cuda.Stream() for _ in range(max(1, args.streams))]
+    items = []
+    for i, k in enumerate(mine):
+        p = I.make_problem(2, k)
+        ctx = kspw.Context.from_problem(p)
+        ctx.set_fft_batch(p.nbands)
+        st = pool[i % len(pool)]
+        ctx.set_stream(st)
+        psi = torch.from_numpy(p.psi0).cuda()
+        items.append((p, ctx, st, psi, torch.empty_like(psi)))
+    nb = items[0][0].nbands
+    torch.cuda.synchronize()
+
+    def step():
+        ev = torch.cuda.Event()
+        ev.record(main)
+        for st in pool:
+            st.wait_event(ev)
+        for p, ctx, st, psi, out in items:
+            ctx.hpsi(psi, out=out)
+        for st in pool:
+            main.wait_stream(st)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    PL.barrier()
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")
+    ms = 0.0
+    for _ in range(args.steps):
+        flush.fill_(1.0)
+        a.record(main)
+        step()
+        b.record(main)
+        torch.cuda.synchronize()
+        ms += a.elapsed_time(b)
+    PL.barrier()
+    # end to end: pinned host buffers through ks_hpsi_host, k after k
+    hbuf = [(torch.from_numpy(i[0].psi0).pin_memory().numpy(), torch.empty(i[0].psi0.shape, dtype=torch.complex128).pin_memory().numpy())
+            for i in items]
+    for (p, ctx, st, psi, out), (hi, ho) in zip(items, hbuf):
+        ctx.hpsi_host(hi, ho)                      # warm-up: staging buffers
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for (p, ctx, st, psi, out), (hi, ho) in zip(items, hbuf):
+        ctx.hpsi_host(hi, ho)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    # Davidson on every k-point of the share (sequential: each solve syncs with the host once per iteration)
+    dav = None
+    if not args.no_davidson:
+        t0 = time.perf_counter()
+        its, bas, conv, emin, emax = 0, 0, True, 1e9, -1e9
+        for p, ctx, st, psi, out in items:
+            with torch.cuda.stream(st):
+                r = ctx.davidson(psi.clone(), tol=1e-8, max_iter=args.davidson_max_iter)
+            its += r["iters"]; bas += r["band_applications"]; conv = conv and bool(r["converged"])
+            emin = min(emin, float(r["eig"][0].item())); emax = max(emax, float(r["eig"][-1].item()))
+        torch.cuda.synchronize()
+        dsec = time.perf_counter() - t0
+        dav = {"time_to_converge_s": dsec, "k_points": len(items), "iterations_total": its, "band_applications": bas,
+               "converged": conv, "tol": 1e-8, "eig_min": emin, "eig_max": emax, "timer": "host wall clock around the share"}
+    clk = clocks.stop() if rank == 0 else None
+    ms, e2e_s, dsec = PL.max_over_ranks([ms, e2e_s, dav["time_to_converge_s"] if dav else 0.0])
+    if rank != 0:
+        PL.finalize()
+        return 0
+    if dav:
+        dav["time_to_converge_s"] = dsec
+    p0 = items[0][0]
+    line = {
+        "metric": METRIC, "value": nk_total * nb * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong",
+        "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
+        "config": {"workload": "cfg2 k-point batch: 4x4x4 Monkhorst-Pack mesh (64 k), 8-atom diamond cell 10.26 bohr, ecutwfc 60 Ry, "
+                               "npw %d..%d per k, grid 54x54x54, nproj %d, nbands %d per k" % (
+                                   min(i[0].npw for i in items), max(i[0].npw for i in items), p0.nproj, nb),
+                   "step": "one ks_hpsi block apply of %d bands on each of the 64 k-points (H1-H8)" % nb,
+                   "l2": "flushed between timed iterations", "streams": len(pool),
+                   "parallelism": "k-points sharded over %d rank(s), no collective on the data path" % world},
+        "clocks": clk,
+        "e2e": {"value": len(items) * world * nb / e2e_s, "unit": UNIT, "h2d_bytes_per_step": sum(i[0].npw for i in items) * nb * 16,
+                "d2h_bytes_per_step": sum(i[0].npw for i in items) * nb * 16, "api": "ks_hpsi_host, one call per k-point"},
+        "gpu_launches": len(items) * 7 * args.steps,
+        "roofline": None, "davidson": dav, "cpu_baseline": None,
+    }
+    print(json.dumps(line))
+    PL.finalize()
+    return 0
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.kbatch:
+        if args.config != 2:
+            raise SystemExit("--kbatch is the k-point batch of BASELINE config 2: use --config 2")
+        return run_kbatch(args)
     import torch
     from paper_2501_08697_b200 import parallel as PL
     rank, world, local = PL.env_world()
