@@ -11,6 +11,9 @@ struct DavidsonWs {
   cplx *Hwork = nullptr;                 // [2nb x 2nb] copy destroyed by the eigensolver
   cplx *Cp = nullptr, *Cq = nullptr;     // [2nb x 2nb] eigenvectors of the previous iteration / of the rotated matrix
   double *thp = nullptr;                 // [2nb] Ritz values of the previous iteration
+  double *thf = nullptr;                 // [2nb] eigenvalues of the deflated (unlocked) subspace problem
+  int *lst = nullptr;                    // [3 x 2nb] locked rows L, free rows F, row -> position in F (or -1)
+  int2 *src = nullptr;                   // [2nb] merged order: (is_locked, index into L or F)
   cplx *S = nullptr, *Us = nullptr;      // [2nb x nb] projections / [nb x nb] Gram matrices
   double *theta = nullptr;               // [2nb]
   double *rho = nullptr, *ekin = nullptr, *lam = nullptr;   // [nb]

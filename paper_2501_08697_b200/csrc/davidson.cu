@@ -136,6 +136,47 @@ __global__ void k_mirror_border(int mp, int m, cplx* __restrict__ Hr) {   // Hr[
   const int i = (int)(e % mp), j = mp + (int)(e / mp);
   Hr[(long)i * m + j] = cconj(Hr[(long)j * m + i]);
 }
+// D3 with locking: converged Ritz pairs (rows L of the rotated matrix, coupling <= their residual <= tol) are taken
+// out of the eigenproblem; the solver sees Hr[F, F] only.
+__global__ void k_gather_sub(int mf, const int* __restrict__ F, const cplx* __restrict__ Hr, int m, cplx* __restrict__ Hs) {
+  const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (e >= (long)mf * mf) return;
+  const int i = (int)(e % mf), j = (int)(e / mf);
+  Hs[e] = Hr[(long)F[j] * m + F[i]];
+}
+// merge the locked values thp[L[.]] (ascending) and the solved ones thf[.] (ascending): position of every entry in
+// the merged ascending list (ties: locked first), theta[pos] and src[pos] = (1, e) locked / (0, j) free
+__global__ void k_merge_order(int nl, const int* __restrict__ L, const double* __restrict__ thp, int mf,
+                              const double* __restrict__ thf, double* __restrict__ theta, int2* __restrict__ src) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= nl + mf) return;
+  if (e < nl) {
+    const double v = thp[L[e]];
+    int lo = 0, hi = mf;                       // number of free values < v
+    while (lo < hi) { const int mid = (lo + hi) >> 1; if (thf[mid] < v) lo = mid + 1; else hi = mid; }
+    theta[e + lo] = v;
+    src[e + lo] = make_int2(1, e);
+  } else {
+    const int j = e - nl;
+    const double v = thf[j];
+    int lo = 0, hi = nl;                       // number of locked values <= v
+    while (lo < hi) { const int mid = (lo + hi) >> 1; if (thp[L[mid]] <= v) lo = mid + 1; else hi = mid; }
+    theta[j + lo] = v;
+    src[j + lo] = make_int2(0, j);
+  }
+}
+// eigenvectors in the rotated basis: column pos = unit vector of a locked row, or the free solution scattered to rows F
+__global__ void k_assemble_cprime(int m, const int2* __restrict__ src, const int* __restrict__ L, const int* __restrict__ rowF,
+                                  const cplx* __restrict__ Cf, long ldf, cplx* __restrict__ Cpr) {
+  const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (e >= (long)m * m) return;
+  const int row = (int)(e % m), pos = (int)(e / m);
+  const int2 s = src[pos];
+  cplx v = cmake(0.0, 0.0);
+  if (s.x) { if (L[s.y] == row) v = cmake(1.0, 0.0); }
+  else { const int r = rowF[row]; if (r >= 0) v = Cf[(long)s.y * ldf + r]; }
+  Cpr[e] = v;
+}
 __global__ void k_set_identity(int m, long ld, cplx* __restrict__ C) {
   const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
   if (e >= (long)m * m) return;
@@ -254,7 +295,7 @@ __global__ void __launch_bounds__(128) k_trinv(int nu, const cplx* __restrict__ 
 void ks_davidson_free(DavidsonWs* w) {
   cudaFree(w->V); cudaFree(w->W); cudaFree(w->X); cudaFree(w->HX); cudaFree(w->T);
   cudaFree(w->Hc); cudaFree(w->Cm); cudaFree(w->Hwork); cudaFree(w->S); cudaFree(w->Us);
-  cudaFree(w->Cp); cudaFree(w->Cq); cudaFree(w->thp); cudaFree(w->act);
+  cudaFree(w->Cp); cudaFree(w->Cq); cudaFree(w->thp); cudaFree(w->act); cudaFree(w->thf); cudaFree(w->lst); cudaFree(w->src);
   cudaFree(w->theta); cudaFree(w->rho); cudaFree(w->ekin); cudaFree(w->lam); cudaFree(w->idx);
   *w = DavidsonWs();
 }
@@ -276,6 +317,9 @@ static int reserve(ks_ctx* c, int nb) {
   KS_CUDA_CHECK(cudaMalloc(&w.Cp, sizeof(cplx) * m * m), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.Cq, sizeof(cplx) * m * m), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.thp, sizeof(double) * m), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.thf, sizeof(double) * m), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.lst, sizeof(int) * 3 * m), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.src, sizeof(int2) * m), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.S, sizeof(cplx) * m * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.Us, sizeof(cplx) * (size_t)nb * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.theta, sizeof(double) * m), c->err);
@@ -407,6 +451,10 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
   std::vector<int> idx(nb);
   // D4 rotates only the bands that are still unconverged (KSPW_ACTIVE_ROT=0: all bands every iteration, as the
   // listing says); `stale` = some converged band's X, HX are older than the last eigensolve.
+  // locking (KSPW_LOCK=0 switches it off; needs the warm start's rotated basis)
+  static const bool lock_env = !(getenv("KSPW_LOCK") && atoi(getenv("KSPW_LOCK")) == 0);
+  const bool lock_on = lock_env && warm;
+  std::vector<int> lockL, lockF, rowF;
   static const bool active_rot = !(getenv("KSPW_ACTIVE_ROT") && atoi(getenv("KSPW_ACTIVE_ROT")) == 0);
   bool stale = false;
   auto rotate_all = [&]() -> int {
@@ -487,12 +535,40 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
       k_build_hrot<<<ceil_div((long)m * m, 256), 256, 0, st>>>(mp, m, w.Hc, ldh, w.thp, w.Hwork);
       RC(ks_gemm_hn(st, mp, m - mp, mp, w.Cp, ldh, w.Hc + (size_t)mp * ldh, ldh, w.Hwork + (size_t)mp * m, m, &c->gws, c->err));
       k_mirror_border<<<ceil_div((long)mp * (m - mp), 256), 256, 0, st>>>(mp, m, w.Hwork);
+      // locking: bands whose residual passed the test at this iteration's step 2 keep their Ritz pair; their rows
+      // (index < nb <= mp: the leading diagonal block) are deflated from the eigenproblem
+      int nl = 0;
+      if (lock_on) {
+        lockL.clear(); lockF.clear(); rowF.assign(m, -1);
+        for (int i = 0; i < m; ++i) {
+          if (i < nb && rho[i] <= tol) lockL.push_back(i);
+          else { rowF[i] = (int)lockF.size(); lockF.push_back(i); }
+        }
+        nl = (int)lockL.size();
+      }
       int sw = 0;
-      RC(ks_eigh_run(st, m, w.Hwork, m, w.theta, w.Cq, ldh, &c->ews, &sw, c->err));
-      if (getenv("KSPW_DEBUG_SWEEPS")) fprintf(stderr, "it %d m %d nk %d sweeps %d\n", it, m, nk, sw);
-      // C = Q C'
-      RC(ks_gemm_nn(st, mp, m, mp, w.Cp, ldh, w.Cq, ldh, w.Cm, ldh, 0, c->err));
-      k_copy_mat<<<ceil_div((long)(m - mp) * m, 256), 256, 0, st>>>(m - mp, m, w.Cq + mp, ldh, w.Cm + mp, ldh);
+      if (nl == 0) {
+        RC(ks_eigh_run(st, m, w.Hwork, m, w.theta, w.Cq, ldh, &c->ews, &sw, c->err));
+        if (getenv("KSPW_DEBUG_SWEEPS")) fprintf(stderr, "it %d m %d nk %d sweeps %d\n", it, m, nk, sw);
+        // C = Q C'
+        RC(ks_gemm_nn(st, mp, m, mp, w.Cp, ldh, w.Cq, ldh, w.Cm, ldh, 0, c->err));
+        k_copy_mat<<<ceil_div((long)(m - mp) * m, 256), 256, 0, st>>>(m - mp, m, w.Cq + mp, ldh, w.Cm + mp, ldh);
+      } else {
+        const int mf = m - nl;
+        int *dL = w.lst, *dF = w.lst + 2 * nb, *dR = w.lst + 4 * nb;
+        KS_CUDA_CHECK(cudaMemcpyAsync(dL, lockL.data(), sizeof(int) * nl, cudaMemcpyHostToDevice, st), c->err);
+        KS_CUDA_CHECK(cudaMemcpyAsync(dF, lockF.data(), sizeof(int) * mf, cudaMemcpyHostToDevice, st), c->err);
+        KS_CUDA_CHECK(cudaMemcpyAsync(dR, rowF.data(), sizeof(int) * m, cudaMemcpyHostToDevice, st), c->err);
+        // Hc is not needed again before the next D2, but it must survive: the gathered problem goes to Cm (free until D4)
+        k_gather_sub<<<ceil_div((long)mf * mf, 256), 256, 0, st>>>(mf, dF, w.Hwork, m, w.Cm);
+        RC(ks_eigh_run(st, mf, w.Cm, mf, w.thf, w.Cq, ldh, &c->ews, &sw, c->err));
+        if (getenv("KSPW_DEBUG_SWEEPS")) fprintf(stderr, "it %d m %d nk %d locked %d sweeps %d\n", it, m, nk, nl, sw);
+        k_merge_order<<<ceil_div(m, 128), 128, 0, st>>>(nl, dL, w.thp, mf, w.thf, w.theta, w.src);
+        k_assemble_cprime<<<ceil_div((long)m * m, 256), 256, 0, st>>>(m, w.src, dL, dR, w.Cq, ldh, w.Hwork);
+        // C = Q C'  (C' in Hwork, leading dimension m)
+        RC(ks_gemm_nn(st, mp, m, mp, w.Cp, ldh, w.Hwork, m, w.Cm, ldh, 0, c->err));
+        k_copy_mat<<<ceil_div((long)(m - mp) * m, 256), 256, 0, st>>>(m - mp, m, w.Hwork + mp, m, w.Cm + mp, ldh);
+      }
       KS_CUDA_CHECK(cudaMemcpyAsync(w.thp, w.theta, sizeof(double) * m, cudaMemcpyDeviceToDevice, st), c->err);
     }
     ph.end(PH_EIGH);
