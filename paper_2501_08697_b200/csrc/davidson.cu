@@ -504,7 +504,8 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
     ph.end(PH_RESID);
     // D7: two passes; the result lands in V[m : m+nk]
     cplx* Vnew = w.V + (size_t)m * npw;
-    RC(orth_pass(c, w.T, nu, Vnew, m, 2, &nk, ph));
+    static const int nproj_first = (getenv("KSPW_ORTH_PROJ") && atoi(getenv("KSPW_ORTH_PROJ")) > 0) ? atoi(getenv("KSPW_ORTH_PROJ")) : 1;   // + one projection in the second pass = the listing's "twice"
+    RC(orth_pass(c, w.T, nu, Vnew, m, nproj_first, &nk, ph));
     if (nk == 0) break;
     int nk2 = 0;
     RC(orth_pass(c, Vnew, nk, w.T, m, 1, &nk2, ph));
