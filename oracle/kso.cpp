@@ -17,6 +17,8 @@
 //                  single-projector closed form, p-triplet closed form
 //   kso_explicit_h rebuilt entry by entry in numpy from Eq. 32 / Eq. 4 in the test
 //   kso_jacobi     2x2 closed form, A C = C Theta, C^H C = I, numpy.linalg.eigvalsh
+//   kso_density    numpy.fft.ifftn on the scattered grid, Parseval sum, one plane wave -> constant, two plane
+//                  waves -> 2 + 2 cos((G1-G2).r) closed form, non-negativity
 //   kso_davidson   V=0: sorted |k+G|^2 exactly; constant shift; brute-force Jacobi / eigvalsh of
 //                  explicit H on cfg 0 and the shrunk variants; Ritz values monotone
 //   Eigenvalues of cfg 1, 3, 4 at FULL size: parity unpinned by anything external.
@@ -270,6 +272,25 @@ extern "C" int kso_hpsi(const kso_ctx* c, const cplx* psi, cplx* hpsi, int nb) {
       for (int j = 0; j < npw; ++j)
         h[j] += cplx(be[j].real() * cr - be[j].imag() * ci, be[j].real() * ci + be[j].imag() * cr);
     }
+  }
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Density build (the step after diagonalisation in the SCF loop, Fig. 3):
+//   rho(r) = sum_b occ_b |psi_b(r)|^2,   psi_b(r) = sum_G c_b(G) e^{+i G.r}   (Eq. 31, unnormalised; the
+// Bloch phase e^{ik.r} has modulus one and drops out; the same form as Eq. 55).  The caller owns the
+// 1/Omega and k-weight factors.  rho: [n1][n2][n3], n3 fastest, natural grid order.  Band by band, in order.
+// ------------------------------------------------------------------------------------------------
+extern "C" int kso_density(const kso_ctx* c, const cplx* psi, const double* occ, int nb, double* rho) {
+  std::vector<cplx> g(c->N);
+  for (long i = 0; i < c->N; ++i) rho[i] = 0.0;
+  for (int b = 0; b < nb; ++b) {
+    const cplx* p = psi + (long)b * c->npw;
+    std::fill(g.begin(), g.end(), cplx(0, 0));
+    for (int j = 0; j < c->npw; ++j) g[c->idx[j]] = p[j];
+    fft3d(c->n1, c->n2, c->n3, g.data(), +1);
+    for (long i = 0; i < c->N; ++i) rho[i] += occ[b] * (g[i].real() * g[i].real() + g[i].imag() * g[i].imag());
   }
   return 0;
 }

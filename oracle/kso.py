@@ -40,6 +40,7 @@ def lib():
         _lib.kso_get_vr.argtypes = [_vp, _vp]
         _lib.kso_hpsi.argtypes = [_vp, _vp, _vp, C.c_int]
         _lib.kso_explicit_h.argtypes = [_vp, _vp]
+        _lib.kso_density.argtypes = [_vp, _vp, _vp, C.c_int, _vp]
         _lib.kso_jacobi.argtypes = [C.c_int, _vp, _vp, _vp]
         _lib.kso_fft3d.argtypes = [C.c_int, C.c_int, C.c_int, _vp, C.c_int]
         _lib.kso_pw_count.argtypes = [_vp, _vp, C.c_double, _vp]
@@ -138,6 +139,16 @@ class Oracle:
         assert psi.ndim == 2 and psi.shape[1] == self.npw
         out = np.empty_like(psi)
         rc = lib().kso_hpsi(self._h, _p(psi), _p(out), psi.shape[0])
+        assert rc == 0
+        return out
+
+    def density(self, psi: np.ndarray, occ: np.ndarray) -> np.ndarray:
+        """rho[n1][n2][n3] = sum_b occ_b |psi_b(r)|^2 (unnormalised inverse transform, Eq. 31)."""
+        psi = np.ascontiguousarray(psi, dtype=np.complex128)
+        occ = np.ascontiguousarray(occ, dtype=np.float64)
+        assert psi.ndim == 2 and psi.shape[1] == self.npw and occ.shape == (psi.shape[0],)
+        out = np.empty(self.grid, dtype=np.float64)
+        rc = lib().kso_density(self._h, _p(psi), _p(occ), psi.shape[0], _p(out))
         assert rc == 0
         return out
 

@@ -317,3 +317,59 @@ def test_davidson_max_iter_reports_not_converged(oracle_mod):
     o = oracle_mod.Oracle.from_problem(p)
     r = o.davidson(p.psi0, tol=1e-8, max_iter=3)
     assert not r["converged"] and r["iters"] == 3 and r["resid"].max() > 1e-8
+
+
+# ----------------------------------------------------------------------------- density
+def test_density_closed_forms_and_library_routine(oracle_mod):
+    """rho(r) = sum_b occ_b |psi_b(r)|^2 with psi(r) = sum_G c(G) e^{+iG.r} (Eq. 31):
+    one plane wave -> constant, two plane waves -> 2 + 2 cos((G1 - G2).r) written from the definition,
+    a random block -> numpy.fft.ifftn on the scattered grid (library routine, not the oracle's own FFT),
+    Parseval sum, non-negativity."""
+    p = I.make_problem(0)
+    o = oracle_mod.Oracle.from_problem(p)
+    n1, n2, n3 = (int(x) for x in p.grid)
+    N = n1 * n2 * n3
+    mil = p.miller
+    # one plane wave
+    c = np.zeros((1, p.npw), complex); c[0, 137] = 0.3 - 0.4j
+    rho = o.density(c, np.array([2.0]))
+    assert np.abs(rho - 2.0 * 0.25).max() < 1e-14
+    # two plane waves with different occupations of two bands
+    ja, jb = 17, 401
+    c = np.zeros((2, p.npw), complex); c[0, ja] = 1.0; c[0, jb] = 1.0; c[1, ja] = 1.0
+    rho = o.density(c, np.array([1.0, 0.5]))
+    dm = mil[ja] - mil[jb]
+    x, y, z = np.meshgrid(np.arange(n1) / n1, np.arange(n2) / n2, np.arange(n3) / n3, indexing="ij")
+    want = 2.0 + 2.0 * np.cos(2 * np.pi * (dm[0] * x + dm[1] * y + dm[2] * z)) + 0.5
+    assert np.abs(rho - want).max() < 1e-13
+    # random block vs numpy.fft (ifftn carries 1/N: the oracle's transform is unnormalised)
+    rng = np.random.default_rng(5)
+    nb = 3
+    psi = rng.standard_normal((nb, p.npw)) + 1j * rng.standard_normal((nb, p.npw))
+    occ = np.array([2.0, 1.0, 0.25])
+    rho = o.density(psi, occ)
+    want = np.zeros((n1, n2, n3))
+    for b in range(nb):
+        g = np.zeros((n1, n2, n3), complex)
+        g[mil[:, 0] % n1, mil[:, 1] % n2, mil[:, 2] % n3] = psi[b]
+        want += occ[b] * np.abs(np.fft.ifftn(g) * N) ** 2
+    assert np.abs(rho - want).max() < 1e-11 * np.abs(want).max()
+    assert rho.min() >= 0.0
+    # Parseval: sum_r rho(r) = N sum_b occ_b ||c_b||^2
+    assert abs(rho.sum() - N * (occ * (np.abs(psi) ** 2).sum(axis=1)).sum()) < 1e-10 * rho.sum()
+
+
+def test_density_k_point_and_noncubic(oracle_mod):
+    """A k != 0 sphere on a non-cubic grid (shrunk slab variant): same pins through numpy.fft."""
+    for name in ("s2", "s4"):
+        p = I.make_shrunk(name)
+        o = oracle_mod.Oracle.from_problem(p)
+        n = [int(x) for x in p.grid]
+        occ = np.linspace(2.0, 0.1, p.nbands)
+        rho = o.density(p.psi0, occ)
+        want = np.zeros(n)
+        for b in range(p.nbands):
+            g = np.zeros(n, complex)
+            g[p.miller[:, 0] % n[0], p.miller[:, 1] % n[1], p.miller[:, 2] % n[2]] = p.psi0[b]
+            want += occ[b] * np.abs(np.fft.ifftn(g) * g.size) ** 2
+        assert np.abs(rho - want).max() < 1e-11 * np.abs(want).max()
