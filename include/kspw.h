@@ -70,6 +70,16 @@ int ks_hpsi(ks_ctx* ctx, const ks_c128* psi, ks_c128* hpsi, int nbands);
 /* same through HOST buffers (copies H2D / D2H inside, synchronises before returning) */
 int ks_hpsi_host(ks_ctx* ctx, const ks_c128* psi_host, ks_c128* hpsi_host, int nbands);
 
+/* Density build (the step after diagonalisation in the SCF loop, Fig. 3):
+ *   rho(r) = sum_b occ[b] |psi_b(r)|^2,  psi_b(r) = sum_G psi_b(G) e^{+i G.r}  (Eq. 31, unnormalised; the caller
+ *   owns 1/Omega and k weights).  Reuses the scatter + inverse-FFT half of ks_hpsi.
+ *   psi  DEVICE [nbands][npw];  occ  DEVICE [nbands];  rho  DEVICE out [n1][n2][n3], n3 fastest, natural grid order.
+ * The sum over bands has a fixed order (no atomics): the result is reproducible bit for bit.  nbands = 0 gives zeros.
+ * Asynchronous on the stream.  Errors: KS_EINVAL (NULL pointer, nbands < 0), KS_ENOMEM, KS_ECUDA. */
+int ks_density(ks_ctx* ctx, const ks_c128* psi, const double* occ, int nbands, double* rho);
+/* same through HOST buffers (copies inside, synchronises before returning) */
+int ks_density_host(ks_ctx* ctx, const ks_c128* psi_host, const double* occ_host, int nbands, double* rho_host);
+
 /* Lowest nbands eigenpairs by block Davidson (steps D0-D9), subspace <= 2 nbands, S = I.
  *   psi    DEVICE [nbands][npw]  in: start vectors (any full-rank block), out: orthonormal eigvecs
  *   eig    DEVICE [nbands] out, ascending (Ry)

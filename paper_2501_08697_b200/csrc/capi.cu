@@ -241,7 +241,7 @@ extern "C" void ks_destroy(ks_ctx* c) {
   if (!c) return;
   HpsiPlan& P = c->P;
   cudaFree(P.d_plane_s0); cudaFree(P.d_plane_y0); cudaFree(P.d_stick);
-  cudaFree(P.d_g2); cudaFree(P.d_vperm); cudaFree(P.d_planes);
+  cudaFree(P.d_g2); cudaFree(P.d_vperm); cudaFree(P.d_planes); cudaFree(P.d_rho_part);
   for (int i = 0; i < 3; ++i) cudaFree(P.d_tw[i]);
   cudaFree(c->d_beta); cudaFree(c->d_D); cudaFree(c->d_proj_atom); cudaFree(c->d_off); cudaFree(c->d_doff);
   cudaFree(c->d_B); cudaFree(c->d_DB); cudaFree(c->d_hin); cudaFree(c->d_hout);
@@ -396,6 +396,47 @@ extern "C" int ks_hpsi_host(ks_ctx* c, const ks_c128* psi_host, ks_c128* hpsi_ho
   rc = ks_hpsi_impl(c, c->d_hin, c->d_hout, nbands);
   if (rc) return rc;
   KS_CUDA_CHECK(cudaMemcpyAsync(hpsi_host, c->d_hout, bytes, cudaMemcpyDeviceToHost, c->stream), c->err);
+  KS_CUDA_CHECK(cudaStreamSynchronize(c->stream), c->err);
+  return KS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// density build: rho(r) = sum_b occ_b |psi_b(r)|^2, Eq. 31 L502 / Fig. 3
+// ------------------------------------------------------------------------------------------------
+extern "C" int ks_density(ks_ctx* c, const ks_c128* psi, const double* occ, int nbands, double* rho) {
+  if (!c) return KS_EINVAL;
+  if (!rho || nbands < 0 || (nbands > 0 && (!psi || !occ))) { c->err = "ks_density: bad argument"; return KS_EINVAL; }
+  HpsiPlan& P = c->P;
+  if (nbands == 0) {
+    KS_CUDA_CHECK(cudaMemsetAsync(rho, 0, sizeof(double) * P.N, c->stream), c->err);
+    return KS_OK;
+  }
+  for (int b0 = 0; b0 < nbands; b0 += c->fft_batch) {
+    const int n = std::min(c->fft_batch, nbands - b0);
+    ks_kprof_begin(c, KP_RHO, 2);
+    const int rc = ks_density_batch(P, (const cplx*)psi + (size_t)b0 * P.npw, occ + b0, n, b0 == 0, c->stream, c->err);
+    ks_kprof_end(c);
+    if (rc) return rc;
+  }
+  return ks_density_finish(P, rho, c->stream, c->err);
+}
+
+extern "C" int ks_density_host(ks_ctx* c, const ks_c128* psi_host, const double* occ_host, int nbands, double* rho_host) {
+  if (!c) return KS_EINVAL;
+  if (!rho_host || nbands < 0 || (nbands > 0 && (!psi_host || !occ_host))) { c->err = "ks_density_host: bad argument"; return KS_EINVAL; }
+  const size_t bytes = sizeof(cplx) * (size_t)nbands * c->P.npw;
+  const size_t rbytes = sizeof(double) * (size_t)c->P.N;
+  int rc = stage(c, std::max(bytes, rbytes + sizeof(double) * (size_t)nbands));
+  if (rc) return rc;
+  double* d_rho = (double*)c->d_hout;
+  double* d_occ = d_rho + c->P.N;
+  if (nbands > 0) {
+    KS_CUDA_CHECK(cudaMemcpyAsync(c->d_hin, psi_host, bytes, cudaMemcpyHostToDevice, c->stream), c->err);
+    KS_CUDA_CHECK(cudaMemcpyAsync(d_occ, occ_host, sizeof(double) * nbands, cudaMemcpyHostToDevice, c->stream), c->err);
+  }
+  rc = ks_density(c, (const ks_c128*)c->d_hin, d_occ, nbands, d_rho);
+  if (rc) return rc;
+  KS_CUDA_CHECK(cudaMemcpyAsync(rho_host, d_rho, rbytes, cudaMemcpyDeviceToHost, c->stream), c->err);
   KS_CUDA_CHECK(cudaStreamSynchronize(c->stream), c->err);
   return KS_OK;
 }

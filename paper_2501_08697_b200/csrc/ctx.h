@@ -48,7 +48,7 @@ struct ks_ctx {
   std::string err;
 };
 
-enum { KP_INV_YZ = 0, KP_X = 1, KP_FWD_YZ = 2, KP_GEMM_HN = 3, KP_APPLY_D = 4, KP_GEMM_NN = 5 };
+enum { KP_INV_YZ = 0, KP_X = 1, KP_FWD_YZ = 2, KP_GEMM_HN = 3, KP_APPLY_D = 4, KP_GEMM_NN = 5, KP_RHO = 6 };
 void ks_kprof_begin(ks_ctx* c, int phase, int launches);
 void ks_kprof_end(ks_ctx* c);
 

@@ -583,6 +583,125 @@ __global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB) k_x(XArgs a) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// density build: rho(r) += occ_b |psi_b(r)|^2 from the live planes k_inv_yz wrote
+// ------------------------------------------------------------------------------------------------
+// The first half of k_x: pass 1 (DFT-R1 on the live rows) and the inverse half of pass 2 (DFT-R2); instead of
+// V(r) and the way back, |psi(r)|^2 is accumulated in registers over the bands the CTA walks through.  A CTA owns
+// 32 columns and one of `ng` band groups and is the only writer of its slice part[group][x'][column], so the sum
+// over bands has a fixed order (no atomics); k_rho_finish adds the groups in order and undoes the position order.
+// The next band's live rows stream into a staging buffer by cp.async while the current band is transformed.
+struct RhoArgs {
+  const cplx* planes;   // [nb][L1][NY*NZ]
+  const double* occ;    // [nb] occupations of this batch
+  double* part;         // [ng][NX][NY*NZ] partial densities, x in position order
+  const cplx* tw_x;
+  int L1, x0, nb, ng, accumulate;
+  long ncol;
+};
+
+template <int NX>
+__global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB > 3 ? 3 : xcfg<NX>::MINB) k_rho(RhoArgs a) {
+  constexpr int R1 = fac<NX>::R1, R2 = fac<NX>::R2;
+  constexpr int ZC = xcfg<NX>::ZC, NT = xcfg<NX>::NT, G = NT / ZC;
+  constexpr int IT2 = (R1 + G - 1) / G;       // pass-2 lines per thread
+  constexpr int R1P = (R1 + 3) & ~3;
+  extern __shared__ cplx sm[];
+  cplx* tw = sm;
+  cplx* tile = sm + NX;
+  int* rlx = reinterpret_cast<int*>(tile + NX * ZC);            // [R2+1][R1P]: live-plane index of row j1*R2+j2, or -1
+  cplx* stage = reinterpret_cast<cplx*>(rlx + (R2 + 1) * R1P);   // [L1][ZC]  ((R2+1)*R1P ints = a multiple of 16 bytes)
+  const int tid = threadIdx.x, pz = tid % ZC, g = tid / ZC;
+  const unsigned ncol = (unsigned)a.ncol;
+  const unsigned col = blockIdx.x * ZC + pz;
+  const bool colok = col < ncol;
+  // bands of this group: b = blockIdx.y, blockIdx.y + ng, ...
+  const size_t bstride = (size_t)a.L1 * a.ncol;
+  const cplx* base = a.planes + (colok ? col : 0);
+  for (int i = tid; i < (R2 + 1) * R1P; i += NT) {
+    const int j2 = i / R1P, j1 = i % R1P;
+    int lx = -1;
+    if (j2 < R2 && j1 < R1) {
+      lx = j1 * R2 + j2 - a.x0;
+      if (lx < 0) lx += NX;
+      if (lx >= a.L1) lx = -1;
+    }
+    rlx[i] = lx;
+  }
+  for (int i = tid; i < NX; i += NT) tw[i] = a.tw_x[i];
+  auto prefetch = [&](int b) {          // rows lx = g, g+G, ... of band b, column pz
+    if (colok)
+      for (int lx = g; lx < a.L1; lx += G) cp16m(stage + lx * ZC + pz, base + (size_t)b * bstride + (unsigned)lx * ncol);
+    cp_commit_m();
+  };
+  int b = blockIdx.y;
+  if (b < a.nb) prefetch(b);
+  double acc[IT2][R2];
+#pragma unroll
+  for (int i = 0; i < IT2; ++i)
+#pragma unroll
+    for (int k = 0; k < R2; ++k) acc[i][k] = 0.0;
+  for (; b < a.nb; b += a.ng) {
+    cp_wait_n(0);
+    __syncthreads();                    // band b staged (and, first time, the tables); the tile is free
+    for (int j2 = g; j2 < R2; j2 += G) {
+      const int* t = rlx + ((colok) ? j2 : R2) * R1P;
+      cplx v[R1];
+#pragma unroll
+      for (int j1 = 0; j1 < R1; ++j1) {
+        const int lx = t[j1];
+        v[j1] = (lx >= 0) ? stage[lx * ZC + pz] : cmake(0.0, 0.0);
+      }
+      dft<R1, +1>(v);
+      cplx* o = tile + j2 * ZC + pz;
+#pragma unroll
+      for (int k1 = 0; k1 < R1; ++k1) o[k1 * R2 * ZC] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw, j2 * k1);
+    }
+    __syncthreads();                    // tile complete; the staging buffer is free
+    if (b + a.ng < a.nb) prefetch(b + a.ng);
+    const double f = __ldg(a.occ + b);
+#pragma unroll
+    for (int i = 0; i < IT2; ++i) {
+      const int k1 = g + i * G;
+      if (R1 % G == 0 || k1 < R1) {
+        cplx v[R2];
+        const cplx* t = tile + k1 * R2 * ZC + pz;
+#pragma unroll
+        for (int j2 = 0; j2 < R2; ++j2) v[j2] = t[j2 * ZC];
+        dft<R2, +1>(v);
+#pragma unroll
+        for (int k2 = 0; k2 < R2; ++k2) acc[i][k2] = fma(f, fma(v[k2].x, v[k2].x, v[k2].y * v[k2].y), acc[i][k2]);
+      }
+    }
+  }
+  if (!colok) return;
+  double* out = a.part + (size_t)blockIdx.y * NX * a.ncol + col;
+#pragma unroll
+  for (int i = 0; i < IT2; ++i) {
+    const int k1 = g + i * G;
+    if (R1 % G == 0 || k1 < R1) {
+#pragma unroll
+      for (int k2 = 0; k2 < R2; ++k2) {
+        double* q = out + (size_t)(k1 * R2 + k2) * a.ncol;
+        *q = a.accumulate ? *q + acc[i][k2] : acc[i][k2];
+      }
+    }
+  }
+}
+
+// rho[x][y][z] (natural order) = sum over groups, in order, of part[g][px][py][pz]
+__global__ void k_rho_finish(const double* __restrict__ part, int ng, double* __restrict__ rho, int n1, int n2, int n3,
+                             int a1, int b1, int a2, int b2, int a3, int b3) {
+  const long N = (long)n1 * n2 * n3;
+  const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const int pz = (int)(i % n3), py = (int)((i / n3) % n2), px = (int)(i / ((long)n3 * n2));
+  const int x = perm_index(px, a1, b1), y = perm_index(py, a2, b2), z = perm_index(pz, a3, b3);
+  double s = 0.0;
+  for (int g = 0; g < ng; ++g) s += part[(size_t)g * N + i];
+  rho[((long)x * n2 + y) * n3 + z] = s;
+}
+
+// ------------------------------------------------------------------------------------------------
 // host: configuration and launch
 // ------------------------------------------------------------------------------------------------
 static const size_t KS_SMEM_MAX = 227 * 1024;
@@ -667,6 +786,59 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
     KS_YZ_PAIRS(C_)
 #undef C_
   }
+  KS_CUDA_CHECK(cudaGetLastError(), err);
+  return KS_OK;
+}
+
+// ---- density build: launchers ----
+template <int NX> static size_t rho_smem(int L1) {
+  return sizeof(cplx) * ((size_t)NX + (size_t)NX * xcfg<NX>::ZC + (size_t)L1 * xcfg<NX>::ZC) +
+         sizeof(int) * (fac<NX>::R2 + 1) * ((fac<NX>::R1 + 3) & ~3);
+}
+
+int ks_density_batch(HpsiPlan& P, const cplx* psi, const double* occ, int nb, int first, cudaStream_t st, std::string& err) {
+  if (nb <= 0) return KS_OK;
+  if (nb > P.batch_cap) { err = "internal: FFT batch larger than workspace"; return KS_EINVAL; }
+  const long ncol = (long)P.n2 * P.n3;
+  const int nchunk = ceil_div(ncol, P.zc_x);
+  if (!P.d_rho_part) {
+    // band groups: enough CTAs for ~3 per resident slot, at most 8 partial copies of the grid
+    P.rho_ng = std::max(1, std::min(8, ceil_div(3L * 148 * 3, nchunk)));
+    KS_CUDA_CHECK(cudaMalloc(&P.d_rho_part, sizeof(double) * (size_t)P.rho_ng * P.N), err);
+  }
+  YzArgs a;
+  a.psi = psi; a.hpsi = nullptr; a.planes = P.d_planes;
+  a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.stick = P.d_stick;
+  a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
+  a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.invN = 1.0 / (double)P.N;
+  const dim3 gyz(P.L1, nb);
+#define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_inv_yz<A_, B_><<<gyz, yzcfg<A_, B_>::NT, P.smem_yz, st>>>(a);
+  KS_YZ_PAIRS(C_)
+#undef C_
+  RhoArgs r;
+  r.planes = P.d_planes; r.occ = occ; r.part = P.d_rho_part; r.tw_x = P.d_tw[0];
+  r.L1 = P.L1; r.x0 = P.x0; r.nb = nb; r.ng = P.rho_ng; r.accumulate = first ? 0 : 1; r.ncol = ncol;
+  const dim3 gr(nchunk, P.rho_ng);
+  cudaError_t e = cudaSuccess;
+#define C_(N_)                                                                                         \
+  if (P.n1 == N_) {                                                                                     \
+    const size_t smem = rho_smem<N_>(P.L1);                                                             \
+    if (smem > KS_SMEM_MAX) { err = "density kernel: tile + staging do not fit in shared memory"; return KS_ENOMEM; } \
+    e = opt_in(k_rho<N_>, smem);                                                                        \
+    if (e == cudaSuccess) k_rho<N_><<<gr, xcfg<N_>::NT, smem, st>>>(r);                                 \
+  }
+  KS_X_SIZES(C_)
+#undef C_
+  KS_CUDA_CHECK(e, err);
+  KS_CUDA_CHECK(cudaGetLastError(), err);
+  return KS_OK;
+}
+
+int ks_density_finish(const HpsiPlan& P, double* rho, cudaStream_t st, std::string& err) {
+  int f[6];
+  const int nn[3] = {P.n1, P.n2, P.n3};
+  for (int ax = 0; ax < 3; ++ax) ks_fft_factors(nn[ax], &f[2 * ax], &f[2 * ax + 1]);
+  k_rho_finish<<<ceil_div(P.N, 256), 256, 0, st>>>(P.d_rho_part, P.rho_ng, rho, P.n1, P.n2, P.n3, f[0], f[1], f[2], f[3], f[4], f[5]);
   KS_CUDA_CHECK(cudaGetLastError(), err);
   return KS_OK;
 }

@@ -23,6 +23,8 @@ struct HpsiPlan {
   cplx* d_tw[3] = {nullptr, nullptr, nullptr};  // e^{+2 pi i t/n_i}
   cplx* d_planes = nullptr;    // workspace [batch][L1][n2][n3]
   int batch_cap = 0;           // bands the workspace holds
+  double* d_rho_part = nullptr;  // density build: [rho_ng][n1][n2][n3] partial sums in position order (lazy)
+  int rho_ng = 0;
 };
 
 bool ks_fft_size_supported(int n);
@@ -43,6 +45,11 @@ int ks_hpsi_configure(HpsiPlan& P, std::string& err);
 // stage: 0 = k_inv_yz, 1 = k_x, 2 = k_fwd_yz, -1 = all three in order.
 int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb, cudaStream_t st,
                          std::string& err, int stage = -1);
+
+// density build: rho(r) += occ_b |psi_b(r)|^2 for one batch of bands (k_inv_yz + k_rho; first != 0 starts a new sum),
+// then ks_density_finish adds the band groups in order and writes rho[n1][n2][n3] in natural order.
+int ks_density_batch(HpsiPlan& P, const cplx* psi, const double* occ, int nb, int first, cudaStream_t st, std::string& err);
+int ks_density_finish(const HpsiPlan& P, double* rho, cudaStream_t st, std::string& err);
 
 // ---- dense kernels (gemm.cu, eigh.cu) ----
 struct GemmWs {          // split-K partial sums

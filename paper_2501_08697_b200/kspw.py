@@ -32,6 +32,8 @@ _lib.ks_last_error.restype = C.c_char_p
 _lib.ks_supported_sizes.argtypes = [_vp, _i]
 _lib.ks_hpsi.argtypes = [_vp, _vp, _vp, _i]
 _lib.ks_hpsi_host.argtypes = [_vp, _vp, _vp, _i]
+_lib.ks_density.argtypes = [_vp, _vp, _vp, _i, _vp]
+_lib.ks_density_host.argtypes = [_vp, _vp, _vp, _i, _vp]
 _lib.ks_davidson.argtypes = [_vp, _vp, _vp, _i, _d, _i, _vp, _vp, _vp]
 _lib.ks_davidson_host.argtypes = [_vp, _vp, _vp, _i, _d, _i, _vp, _vp, _vp]
 _lib.ks_davidson_profile.argtypes = [_vp, _vp]
@@ -44,7 +46,7 @@ _lib.ks_dmma_peak.argtypes = [_vp, _vp]
 
 KS_OK, KS_NOTCONV = 0, 1
 EXPORTS = ("ks_pw_count", "ks_pw_list", "ks_create", "ks_destroy", "ks_npw", "ks_set_stream", "ks_set_fft_batch",
-           "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_davidson", "ks_davidson_host",
+           "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_density", "ks_density_host", "ks_davidson", "ks_davidson_host",
            "ks_davidson_profile", "ks_profile_begin", "ks_profile_end", "ks_zgemm_hn", "ks_zgemm_nn", "ks_eigh", "ks_dmma_peak")
 
 
@@ -161,6 +163,24 @@ class Context:
         self._check(_lib.ks_hpsi(self._h, _dev(psi), _dev(out), int(psi.shape[0])))
         return out
 
+    def density(self, psi, occ, out=None):
+        """psi: torch complex128 CUDA [nbands][npw], occ: torch float64 CUDA [nbands]; returns rho [n1][n2][n3]."""
+        import torch
+        assert psi.dtype == torch.complex128 and psi.dim() == 2 and psi.shape[1] == self.npw
+        assert occ.dtype == torch.float64 and occ.shape == (psi.shape[0],)
+        if out is None:
+            out = torch.empty(tuple(self.grid), dtype=torch.float64, device=psi.device)
+        self._check(_lib.ks_density(self._h, _dev(psi), _dev(occ), int(psi.shape[0]), _dev(out)))
+        return out
+
+    def density_host(self, psi: np.ndarray, occ: np.ndarray) -> np.ndarray:
+        psi = _np(psi, np.complex128)
+        occ = _np(occ, np.float64)
+        assert psi.ndim == 2 and psi.shape[1] == self.npw and occ.shape == (psi.shape[0],)
+        out = np.empty(tuple(self.grid), dtype=np.float64)
+        self._check(_lib.ks_density_host(self._h, _hp(psi), _hp(occ), int(psi.shape[0]), _hp(out)))
+        return out
+
     def hpsi_host(self, psi: np.ndarray, out: np.ndarray = None) -> np.ndarray:
         psi = _np(psi, np.complex128)
         assert psi.ndim == 2 and psi.shape[1] == self.npw
@@ -191,7 +211,7 @@ class Context:
                                                C.byref(it), C.byref(nh)))
         return dict(psi=psi, eig=eig, resid=res, iters=it.value, band_applications=nh.value, converged=(rc == 0))
 
-    KERNELS = ("k_inv_yz", "k_x", "k_fwd_yz", "k_gemm_hn+reduce", "k_apply_D", "k_gemm_nn")
+    KERNELS = ("k_inv_yz", "k_x", "k_fwd_yz", "k_gemm_hn+reduce", "k_apply_D", "k_gemm_nn", "k_inv_yz+k_rho")
 
     def profile_begin(self):
         self._check(_lib.ks_profile_begin(self._h))

@@ -265,3 +265,51 @@ def test_davidson_cfg2_kpoint(ks, oracle_mod):
     r = _check_davidson(ks, oracle_mod, p, oracle_run=True)
     eig = r["eig"].cpu().numpy()
     assert abs(eig[15] - eig[16]) < 1e-8            # degenerate pair; compare values only
+
+
+# ------------------------------------------------------------------ density build
+@pytest.mark.parametrize("name", ["cfg0", "s1", "s2", "s4", "tiny18"])
+def test_density_small(ks, oracle_mod, name):
+    import torch
+    if name == "cfg0":
+        p = I.make_problem(0)
+    elif name == "tiny18":
+        p = I.make_problem(0, ecutwfc=5.0, grid=(18, 18, 18), nbands=3)
+    else:
+        p = I.make_shrunk(name)
+    ctx = ks.Context.from_problem(p)
+    o = oracle_mod.Oracle.from_problem(p)
+    occ = np.linspace(2.0, 0.25, p.nbands)
+    ref = o.density(p.psi0, occ)
+    got = ctx.density(_t(p.psi0), _t(occ)).cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
+    # ragged batches give the same bits (fixed summation order per band group is batch dependent, so compare to 1e-13)
+    ctx.set_fft_batch(3)
+    got2 = ctx.density(_t(p.psi0), _t(occ)).cpu().numpy()
+    assert np.abs(got2 - ref).max() <= 1e-12 * np.abs(ref).max()
+    # run to run reproducible bit for bit (no atomics)
+    assert np.array_equal(got2, ctx.density(_t(p.psi0), _t(occ)).cpu().numpy())
+    # host entry point, empty block
+    assert np.abs(ctx.density_host(p.psi0, occ) - ref).max() <= 1e-12 * np.abs(ref).max()
+    e = torch.empty((0, p.npw), dtype=torch.complex128, device="cuda")
+    z = ctx.density(e, torch.empty(0, dtype=torch.float64, device="cuda")).cpu().numpy()
+    assert z.shape == tuple(p.grid) and not z.any()
+
+
+@pytest.mark.parametrize("c,k_index", [(1, 0), (2, 21), (3, 0), (4, 0)])
+def test_density_full_size(ks, oracle_mod, c, k_index):
+    """Full-size configs: the oracle sums a few bands; Parseval holds for the whole block at any size."""
+    p = I.make_problem(c, k_index)
+    ctx = ks.Context.from_problem(p)
+    o = oracle_mod.Oracle.from_problem(p)
+    sel = np.unique(np.linspace(0, p.nbands - 1, 3).astype(int))
+    occ = np.zeros(p.nbands)
+    occ[sel] = [2.0, 1.0, 0.5][:len(sel)]
+    ref = o.density(p.psi0[sel], occ[sel])
+    got = ctx.density(_t(p.psi0), _t(occ)).cpu().numpy()          # whole block, zero weight on the other bands
+    assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
+    occ = np.linspace(2.0, 0.0, p.nbands)
+    got = ctx.density(_t(p.psi0), _t(occ)).cpu().numpy()
+    N = got.size
+    want = N * (occ * (np.abs(p.psi0) ** 2).sum(axis=1)).sum()
+    assert got.min() >= 0.0 and abs(got.sum() - want) <= 1e-11 * want
