@@ -42,6 +42,7 @@ def parse():
     ap.add_argument("--impl", default="kspw", choices=["kspw", "reference"])
     ap.add_argument("--no-davidson", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-density", action="store_true")
     ap.add_argument("--davidson-max-iter", type=int, default=400)
     ap.add_argument("--fft-batch", type=int, default=0)
     ap.add_argument("--kbatch", action="store_true",
@@ -388,6 +389,22 @@ def main():
                "converged": bool(r["converged"]), "max_resid": float(r["resid"].max().item()), "tol": 1e-8,
                "band_applications_per_s": r["band_applications"] / dsec,
                "eig_min": float(r["eig"][0].item()), "eig_max": float(r["eig"][-1].item())}
+    # density build: rho = sum_b occ_b |psi_b(r)|^2 on the same block, same batching
+    dens = None
+    if not args.no_density:
+        occ = torch.linspace(2.0, 0.0, nb, dtype=torch.float64, device="cuda")
+        rho = torch.empty(tuple(int(x) for x in p.grid), dtype=torch.float64, device="cuda")
+        for _ in range(3):
+            ctx.density(psi, occ, out=rho)
+        torch.cuda.synchronize()
+        dsteps = max(1, args.steps)
+        dms = timed_steps(lambda: ctx.density(psi, occ, out=rho), dsteps) / dsteps
+        n1, n2, n3 = (int(x) for x in p.grid)
+        planes = 16.0 * plan_counts(p) * n2 * n3
+        dbytes = nb * (16.0 * npw + planes) + nb * planes + 2 * 8.0 * n1 * n2 * n3   # k_inv_yz + k_rho reads + partial/rho writes
+        dens = {"bands_per_s": nb / (dms * 1e-3), "ms": dms, "algorithmic_bytes": dbytes,
+                "achieved_gbs": dbytes / (dms * 1e-3) / 1e9, "frac_of_hbm": dbytes / (dms * 1e-3) / 1e9 / peaks()["hbm_gbs"],
+                "sum_check": float(rho.sum().item() / (n1 * n2 * n3 * float((occ * (psi.abs() ** 2).sum(dim=1)).sum().item())))}
     clk = clocks.stop() if rank == 0 else None
     ms, e2e_s = PL.max_over_ranks([ms, e2e_s])
     if rank != 0:
@@ -440,6 +457,7 @@ def main():
         "roofline_all": rows,
         "peaks": {"hbm_gbs": pk["hbm_gbs"], "source": pk["src"], "dmma_tflops_live": dmma_tf, "dfma_tflops_live": dfma_tf},
         "davidson": dav,
+        "density": dens,
     }
     if not args.no_cpu_baseline and world == 1:
         from oracle import kso
