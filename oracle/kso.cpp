@@ -19,6 +19,8 @@
 //   kso_jacobi     2x2 closed form, A C = C Theta, C^H C = I, numpy.linalg.eigvalsh
 //   kso_density    numpy.fft.ifftn on the scattered grid, Parseval sum, one plane wave -> constant, two plane
 //                  waves -> 2 + 2 cos((G1-G2).r) closed form, non-negativity
+//   kso_chebyshev  U p(Lambda) U^H chi from numpy.linalg.eigh of the explicit H with p evaluated by
+//                  numpy.polynomial.chebyshev.chebval; T_n = cos(n arccos x) on an eigenvector; sqrt(Fermi-Dirac)
 //   kso_davidson   V=0: sorted |k+G|^2 exactly; constant shift; brute-force Jacobi / eigvalsh of
 //                  explicit H on cfg 0 and the shrunk variants; Ritz values monotone
 //   Eigenvalues of cfg 1, 3, 4 at FULL size: parity unpinned by anything external.
@@ -291,6 +293,32 @@ extern "C" int kso_density(const kso_ctx* c, const cplx* psi, const double* occ,
     for (int j = 0; j < c->npw; ++j) g[c->idx[j]] = p[j];
     fft3d(c->n1, c->n2, c->n3, g.data(), +1);
     for (long i = 0; i < c->N; ++i) rho[i] += occ[b] * (g[i].real() * g[i].real() + g[i].imag() * g[i].imag());
+  }
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Chebyshev expansion of an operator function applied to a block (the inner loop of sDFT,
+// PAPER.md L588 "Chebyshev expansion scheme", Eq. 54 L680 gamma = f_H^{1/2} chi, orders 25..1200 at L714):
+//   out = sum_{n=0}^{ncoef-1} c_n T_n(Ht) chi,   Ht = (H - ebar)/de  (spectrum of Ht inside [-1, 1]),
+//   T_0 = chi,  T_1 = Ht chi,  T_{n+1} = 2 Ht T_n - T_{n-1}   (the textbook three-term recurrence; the paper
+//   does not print it).  Term by term, in order.
+// ------------------------------------------------------------------------------------------------
+extern "C" int kso_chebyshev(const kso_ctx* c, const cplx* chi, int nb, int ncoef, const double* coef, double ebar,
+                             double de, cplx* out) {
+  const long n = (long)nb * c->npw;
+  std::vector<cplx> tp(chi, chi + n), tc(n), tn(n), h(n);
+  for (long i = 0; i < n; ++i) out[i] = (ncoef > 0 ? coef[0] : 0.0) * chi[i];
+  if (ncoef < 2) return 0;
+  kso_hpsi(c, tp.data(), h.data(), nb);
+  for (long i = 0; i < n; ++i) tc[i] = (h[i] - ebar * tp[i]) / de;
+  for (long i = 0; i < n; ++i) out[i] += coef[1] * tc[i];
+  for (int k = 2; k < ncoef; ++k) {
+    kso_hpsi(c, tc.data(), h.data(), nb);
+    for (long i = 0; i < n; ++i) tn[i] = 2.0 * (h[i] - ebar * tc[i]) / de - tp[i];
+    for (long i = 0; i < n; ++i) out[i] += coef[k] * tn[i];
+    tp.swap(tc);
+    tc.swap(tn);
   }
   return 0;
 }

@@ -41,6 +41,7 @@ def lib():
         _lib.kso_hpsi.argtypes = [_vp, _vp, _vp, C.c_int]
         _lib.kso_explicit_h.argtypes = [_vp, _vp]
         _lib.kso_density.argtypes = [_vp, _vp, _vp, C.c_int, _vp]
+        _lib.kso_chebyshev.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, C.c_double, C.c_double, _vp]
         _lib.kso_jacobi.argtypes = [C.c_int, _vp, _vp, _vp]
         _lib.kso_fft3d.argtypes = [C.c_int, C.c_int, C.c_int, _vp, C.c_int]
         _lib.kso_pw_count.argtypes = [_vp, _vp, C.c_double, _vp]
@@ -149,6 +150,16 @@ class Oracle:
         assert psi.ndim == 2 and psi.shape[1] == self.npw and occ.shape == (psi.shape[0],)
         out = np.empty(self.grid, dtype=np.float64)
         rc = lib().kso_density(self._h, _p(psi), _p(occ), psi.shape[0], _p(out))
+        assert rc == 0
+        return out
+
+    def chebyshev(self, chi: np.ndarray, coef: np.ndarray, ebar: float, de: float) -> np.ndarray:
+        """sum_n coef[n] T_n((H - ebar)/de) chi for a block chi[nb][npw] (three-term recurrence)."""
+        chi = np.ascontiguousarray(chi, dtype=np.complex128)
+        coef = np.ascontiguousarray(coef, dtype=np.float64)
+        assert chi.ndim == 2 and chi.shape[1] == self.npw and de > 0
+        out = np.empty_like(chi)
+        rc = lib().kso_chebyshev(self._h, _p(chi), chi.shape[0], coef.size, _p(coef), float(ebar), float(de), _p(out))
         assert rc == 0
         return out
 

@@ -373,3 +373,56 @@ def test_density_k_point_and_noncubic(oracle_mod):
             g[p.miller[:, 0] % n[0], p.miller[:, 1] % n[1], p.miller[:, 2] % n[2]] = p.psi0[b]
             want += occ[b] * np.abs(np.fft.ifftn(g) * g.size) ** 2
         assert np.abs(rho - want).max() < 1e-11 * np.abs(want).max()
+
+
+# ----------------------------------------------------------------------------- Chebyshev expansion
+def _cheb_setup(oracle_mod):
+    p = I.make_problem(0)
+    o = oracle_mod.Oracle.from_problem(p)
+    H = o.explicit_h()
+    w, U = np.linalg.eigh(H)
+    ebar, de = 0.5 * (w[-1] + w[0]), 0.5 * (w[-1] - w[0]) * 1.02      # spectrum of (H - ebar)/de inside [-1, 1]
+    return p, o, w, U, ebar, de
+
+
+def test_chebyshev_vs_spectral_decomposition(oracle_mod):
+    """out = sum_n c_n T_n(Ht) chi must equal U p(lambda_t) U^H chi with p evaluated by numpy's chebval on the
+    eigenvalues of the explicit H (library eigh + library polynomial evaluation, no recurrence shared)."""
+    p, o, w, U, ebar, de = _cheb_setup(oracle_mod)
+    rng = np.random.default_rng(11)
+    theta = rng.uniform(0.0, 1.0, size=(3, p.npw))
+    chi = np.exp(2j * np.pi * theta) / np.sqrt(3)                    # stochastic orbitals, PAPER.md Eq. 52 L670
+    coef = rng.standard_normal(24) / (1.0 + np.arange(24))
+    got = o.chebyshev(chi, coef, ebar, de)
+    pv = np.polynomial.chebyshev.chebval((w - ebar) / de, coef)
+    want = (U @ (pv[:, None] * (U.conj().T @ chi.T))).T
+    assert np.abs(got - want).max() < 1e-11 * np.abs(want).max()
+    # degenerate orders
+    assert np.abs(o.chebyshev(chi, coef[:1], ebar, de) - coef[0] * chi).max() < 1e-15
+    one = o.chebyshev(chi, np.array([0.0, 1.0]), ebar, de)
+    assert np.abs(one - (o.hpsi(chi) - ebar * chi) / de).max() < 1e-13
+
+
+def test_chebyshev_single_term_is_cos_n_arccos(oracle_mod):
+    """On an eigenvector of H, T_n(Ht) v = cos(n arccos(lambda_t)) v (closed form of the Chebyshev polynomial)."""
+    p, o, w, U, ebar, de = _cheb_setup(oracle_mod)
+    for j, n in ((0, 7), (100, 12), (514, 5)):
+        v = U[:, j][None, :].copy()
+        coef = np.zeros(n + 1); coef[n] = 1.0
+        got = o.chebyshev(v, coef, ebar, de)
+        lam = (w[j] - ebar) / de
+        assert np.abs(got - math.cos(n * math.acos(lam)) * v).max() < 1e-10
+
+
+def test_chebyshev_sqrt_fermi_dirac(oracle_mod):
+    """gamma = f_H^{1/2} chi (Eq. 39, Eq. 54): Chebyshev-Gauss coefficients of sqrt(Fermi-Dirac) at a high
+    temperature reproduce U sqrt(f(lambda)) U^H chi to the interpolation error."""
+    p, o, w, U, ebar, de = _cheb_setup(oracle_mod)
+    mu, kT = 0.2, 0.8
+    f = lambda x: 1.0 / np.sqrt(1.0 + np.exp((x * de + ebar - mu) / kT))
+    coef = np.polynomial.chebyshev.chebinterpolate(f, 48)
+    rng = np.random.default_rng(12)
+    chi = np.exp(2j * np.pi * rng.uniform(size=(2, p.npw))) / np.sqrt(2)
+    got = o.chebyshev(chi, coef, ebar, de)
+    want = (U @ (np.sqrt(1.0 / (1.0 + np.exp((w - mu) / kT)))[:, None] * (U.conj().T @ chi.T))).T
+    assert np.abs(got - want).max() < 1e-9 * np.abs(want).max()
