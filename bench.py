@@ -43,6 +43,7 @@ def parse():
     ap.add_argument("--no-davidson", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-density", action="store_true")
+    ap.add_argument("--no-chebyshev", action="store_true")
     ap.add_argument("--davidson-max-iter", type=int, default=400)
     ap.add_argument("--fft-batch", type=int, default=0)
     ap.add_argument("--kbatch", action="store_true",
@@ -405,6 +406,18 @@ def main():
         dens = {"bands_per_s": nb / (dms * 1e-3), "ms": dms, "algorithmic_bytes": dbytes,
                 "achieved_gbs": dbytes / (dms * 1e-3) / 1e9, "frac_of_hbm": dbytes / (dms * 1e-3) / 1e9 / peaks()["hbm_gbs"],
                 "sum_check": float(rho.sum().item() / (n1 * n2 * n3 * float((occ * (psi.abs() ** 2).sum(dim=1)).sum().item())))}
+    # Chebyshev expansion: order-64 expansion on the block = 63 ks_hpsi block applies + fused axpys
+    cheb = None
+    if not args.no_chebyshev:
+        ncoef = 64
+        coef = 1.0 / (1.0 + np.arange(float(ncoef))) ** 2
+        ebar, de = 0.5 * (p.ecutwfc + 1.0), 0.5 * (p.ecutwfc + 7.0)     # [-3, ecut + 4] Ry contains the spectrum
+        cout = torch.empty_like(psi)
+        ctx.chebyshev(psi, coef[:4], ebar, de, out=cout)
+        torch.cuda.synchronize()
+        cms = timed_steps(lambda: ctx.chebyshev(psi, coef, ebar, de, out=cout), 1)
+        cheb = {"order": ncoef - 1, "ms": cms, "band_applications_per_s": nb * (ncoef - 1) / (cms * 1e-3),
+                "vs_plain_hpsi": (nb * (ncoef - 1) / (cms * 1e-3)) / (nb * args.steps / (ms * 1e-3))}
     clk = clocks.stop() if rank == 0 else None
     ms, e2e_s = PL.max_over_ranks([ms, e2e_s])
     if rank != 0:
@@ -458,6 +471,7 @@ def main():
         "peaks": {"hbm_gbs": pk["hbm_gbs"], "source": pk["src"], "dmma_tflops_live": dmma_tf, "dfma_tflops_live": dfma_tf},
         "davidson": dav,
         "density": dens,
+        "chebyshev": cheb,
     }
     if not args.no_cpu_baseline and world == 1:
         from oracle import kso

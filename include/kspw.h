@@ -80,6 +80,15 @@ int ks_density(ks_ctx* ctx, const ks_c128* psi, const double* occ, int nbands, d
 /* same through HOST buffers (copies inside, synchronises before returning) */
 int ks_density_host(ks_ctx* ctx, const ks_c128* psi_host, const double* occ_host, int nbands, double* rho_host);
 
+/* Chebyshev expansion of an operator function on a block (the inner loop of sDFT: PAPER.md L588,
+ * stochastic orbitals Eq. 52, gamma = f_H^{1/2} chi Eq. 54, orders 25..1200 L714):
+ *   out = sum_{n=0}^{ncoef-1} coef[n] T_n(Ht) chi,  Ht = (H - ebar)/de,  T_0 = chi, T_1 = Ht chi, T_{n+1} = 2 Ht T_n - T_{n-1}.
+ * The caller supplies the coefficients and a scaling with the spectrum of Ht inside [-1, 1] (otherwise T_n grows).
+ *   chi, out  DEVICE [nbands][npw], must not alias;  coef  HOST [ncoef];  ncoef - 1 ks_hpsi block applies.
+ * Asynchronous on the stream.  Errors: KS_EINVAL (NULL, aliasing, de <= 0, ncoef < 0), KS_ENOMEM, KS_ECUDA. */
+int ks_chebyshev(ks_ctx* ctx, const ks_c128* chi, ks_c128* out, int nbands, int ncoef, const double* coef,
+                 double ebar, double de);
+
 /* Lowest nbands eigenpairs by block Davidson (steps D0-D9), subspace <= 2 nbands, S = I.
  *   psi    DEVICE [nbands][npw]  in: start vectors (any full-rank block), out: orthonormal eigvecs
  *   eig    DEVICE [nbands] out, ascending (Ry)

@@ -245,6 +245,7 @@ extern "C" void ks_destroy(ks_ctx* c) {
   for (int i = 0; i < 3; ++i) cudaFree(P.d_tw[i]);
   cudaFree(c->d_beta); cudaFree(c->d_D); cudaFree(c->d_proj_atom); cudaFree(c->d_off); cudaFree(c->d_doff);
   cudaFree(c->d_B); cudaFree(c->d_DB); cudaFree(c->d_hin); cudaFree(c->d_hout);
+  for (int i = 0; i < 3; ++i) cudaFree(c->d_cheb[i]);
   cudaFree(c->gws.part);
   ks_eigh_free(&c->ews);
   ks_davidson_free(&c->dws);
@@ -438,6 +439,75 @@ extern "C" int ks_density_host(ks_ctx* c, const ks_c128* psi_host, const double*
   if (rc) return rc;
   KS_CUDA_CHECK(cudaMemcpyAsync(rho_host, d_rho, rbytes, cudaMemcpyDeviceToHost, c->stream), c->err);
   KS_CUDA_CHECK(cudaStreamSynchronize(c->stream), c->err);
+  return KS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Chebyshev expansion: out = sum_n coef[n] T_n((H - ebar)/de) chi, three-term recurrence on
+// ks_hpsi; the recurrence step and the accumulation are one fused elementwise kernel (96 B per plane wave and band).
+// ------------------------------------------------------------------------------------------------
+// first != 0:  t1 = (h - ebar t0)/de ;            out = c0 t0 + c1 t1     (tp holds t0, result t1 goes to tc)
+// first == 0:  tn = 2 (h - ebar tc)/de - tp ;     out += cn tn            (tn overwrites tp)
+__global__ void k_cheb_step(long n, const cplx* __restrict__ h, cplx* __restrict__ tp, cplx* __restrict__ tc,
+                            cplx* __restrict__ out, double ebar, double inv_de, double c0, double cn, int first) {
+  const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const cplx hv = h[i];
+  if (first) {
+    const cplx t0 = tp[i];
+    const cplx t1 = cmake((hv.x - ebar * t0.x) * inv_de, (hv.y - ebar * t0.y) * inv_de);
+    tc[i] = t1;
+    out[i] = cmake(fma(cn, t1.x, c0 * t0.x), fma(cn, t1.y, c0 * t0.y));
+  } else {
+    const cplx t = tc[i], q = tp[i], o = out[i];
+    const cplx tn = cmake(2.0 * (hv.x - ebar * t.x) * inv_de - q.x, 2.0 * (hv.y - ebar * t.y) * inv_de - q.y);
+    tp[i] = tn;
+    out[i] = cmake(fma(cn, tn.x, o.x), fma(cn, tn.y, o.y));
+  }
+}
+__global__ void k_scale_copy(long n, const cplx* __restrict__ a, double s, cplx* __restrict__ b) {
+  const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+  if (i < n) b[i] = cmake(s * a[i].x, s * a[i].y);
+}
+
+extern "C" int ks_chebyshev(ks_ctx* c, const ks_c128* chi_, ks_c128* out_, int nbands, int ncoef, const double* coef,
+                            double ebar, double de) {
+  if (!c) return KS_EINVAL;
+  if (nbands == 0) return KS_OK;
+  if (!chi_ || !out_ || nbands < 0 || ncoef < 0 || (ncoef > 0 && !coef) || !(de > 0)) { c->err = "ks_chebyshev: bad argument"; return KS_EINVAL; }
+  const cplx* chi = (const cplx*)chi_;
+  cplx* out = (cplx*)out_;
+  const long n = (long)nbands * c->P.npw;
+  const size_t bytes = sizeof(cplx) * (size_t)n;
+  {
+    const char* a = (const char*)chi;
+    const char* b = (const char*)out;
+    if (a < b + bytes && b < a + bytes) { c->err = "ks_chebyshev: chi and out must not alias"; return KS_EINVAL; }
+  }
+  const int nblk = ceil_div(n, 256);
+  if (ncoef < 2) {
+    k_scale_copy<<<nblk, 256, 0, c->stream>>>(n, chi, ncoef == 1 ? coef[0] : 0.0, out);
+    KS_CUDA_CHECK(cudaGetLastError(), c->err);
+    return KS_OK;
+  }
+  if (c->cheb_bytes < bytes) {
+    for (int i = 0; i < 3; ++i) { cudaFree(c->d_cheb[i]); c->d_cheb[i] = nullptr; }
+    c->cheb_bytes = 0;
+    for (int i = 0; i < 3; ++i) KS_CUDA_CHECK(cudaMalloc(&c->d_cheb[i], bytes), c->err);
+    c->cheb_bytes = bytes;
+  }
+  cplx *tp = c->d_cheb[0], *tc = c->d_cheb[1], *h = c->d_cheb[2];
+  KS_CUDA_CHECK(cudaMemcpyAsync(tp, chi, bytes, cudaMemcpyDeviceToDevice, c->stream), c->err);
+  int rc = ks_hpsi_impl(c, tp, h, nbands);
+  if (rc) return rc;
+  k_cheb_step<<<nblk, 256, 0, c->stream>>>(n, h, tp, tc, out, ebar, 1.0 / de, coef[0], coef[1], 1);
+  for (int k = 2; k < ncoef; ++k) {
+    rc = ks_hpsi_impl(c, tc, h, nbands);
+    if (rc) return rc;
+    k_cheb_step<<<nblk, 256, 0, c->stream>>>(n, h, tp, tc, out, ebar, 1.0 / de, 0.0, coef[k], 0);
+    std::swap(tp, tc);      // the new term went into tp: it is the current one now
+  }
+  KS_CUDA_CHECK(cudaGetLastError(), c->err);
   return KS_OK;
 }
 

@@ -32,6 +32,8 @@ struct ks_ctx {
   cplx *d_B = nullptr, *d_DB = nullptr;   // [nproj x nb_cap] column-major
   int nl_cap = 0;
   cplx *d_hin = nullptr, *d_hout = nullptr;   // staging for the *_host entry points
+  cplx *d_cheb[3] = {nullptr, nullptr, nullptr};   // ks_chebyshev: T_{n-1}, T_n, H T_n  [nb_cap][npw] each
+  size_t cheb_bytes = 0;
   size_t host_stage_bytes = 0;
   GemmWs gws;
   EighWs ews;

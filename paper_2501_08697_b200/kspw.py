@@ -34,6 +34,7 @@ _lib.ks_hpsi.argtypes = [_vp, _vp, _vp, _i]
 _lib.ks_hpsi_host.argtypes = [_vp, _vp, _vp, _i]
 _lib.ks_density.argtypes = [_vp, _vp, _vp, _i, _vp]
 _lib.ks_density_host.argtypes = [_vp, _vp, _vp, _i, _vp]
+_lib.ks_chebyshev.argtypes = [_vp, _vp, _vp, _i, _i, _vp, _d, _d]
 _lib.ks_davidson.argtypes = [_vp, _vp, _vp, _i, _d, _i, _vp, _vp, _vp]
 _lib.ks_davidson_host.argtypes = [_vp, _vp, _vp, _i, _d, _i, _vp, _vp, _vp]
 _lib.ks_davidson_profile.argtypes = [_vp, _vp]
@@ -46,7 +47,7 @@ _lib.ks_dmma_peak.argtypes = [_vp, _vp]
 
 KS_OK, KS_NOTCONV = 0, 1
 EXPORTS = ("ks_pw_count", "ks_pw_list", "ks_create", "ks_destroy", "ks_npw", "ks_set_stream", "ks_set_fft_batch",
-           "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_density", "ks_density_host", "ks_davidson", "ks_davidson_host",
+           "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_density", "ks_density_host", "ks_chebyshev", "ks_davidson", "ks_davidson_host",
            "ks_davidson_profile", "ks_profile_begin", "ks_profile_end", "ks_zgemm_hn", "ks_zgemm_nn", "ks_eigh", "ks_dmma_peak")
 
 
@@ -171,6 +172,17 @@ class Context:
         if out is None:
             out = torch.empty(tuple(self.grid), dtype=torch.float64, device=psi.device)
         self._check(_lib.ks_density(self._h, _dev(psi), _dev(occ), int(psi.shape[0]), _dev(out)))
+        return out
+
+    def chebyshev(self, chi, coef, ebar: float, de: float, out=None):
+        """sum_n coef[n] T_n((H - ebar)/de) chi; chi: torch complex128 CUDA [nbands][npw], coef: host floats."""
+        import torch
+        assert chi.dtype == torch.complex128 and chi.dim() == 2 and chi.shape[1] == self.npw
+        coef = _np(coef, np.float64)
+        if out is None:
+            out = torch.empty_like(chi)
+        self._check(_lib.ks_chebyshev(self._h, _dev(chi), _dev(out), int(chi.shape[0]), int(coef.size), _hp(coef),
+                                      float(ebar), float(de)))
         return out
 
     def density_host(self, psi: np.ndarray, occ: np.ndarray) -> np.ndarray:

@@ -313,3 +313,52 @@ def test_density_full_size(ks, oracle_mod, c, k_index):
     N = got.size
     want = N * (occ * (np.abs(p.psi0) ** 2).sum(axis=1)).sum()
     assert got.min() >= 0.0 and abs(got.sum() - want) <= 1e-11 * want
+
+
+# ------------------------------------------------------------------ Chebyshev expansion
+def _stochastic(p, nchi, seed):
+    rng = np.random.default_rng(seed)
+    return np.exp(2j * np.pi * rng.uniform(size=(nchi, p.npw))) / np.sqrt(nchi)      # PAPER.md Eq. 52
+
+
+@pytest.mark.parametrize("name", ["cfg0", "s2", "s4"])
+def test_chebyshev_small(ks, oracle_mod, name):
+    import torch
+    p = I.make_problem(0) if name == "cfg0" else I.make_shrunk(name)
+    ctx = ks.Context.from_problem(p)
+    o = oracle_mod.Oracle.from_problem(p)
+    w = np.linalg.eigvalsh(o.explicit_h())
+    ebar, de = 0.5 * (w[-1] + w[0]), 0.51 * (w[-1] - w[0])
+    chi = _stochastic(p, 5, 3)
+    mu, kT = 0.3, 1.0
+    coef = np.polynomial.chebyshev.chebinterpolate(lambda x: 1.0 / np.sqrt(1.0 + np.exp((x * de + ebar - mu) / kT)), 40)
+    ref = o.chebyshev(chi, coef, ebar, de)
+    got = ctx.chebyshev(_t(chi), coef, ebar, de).cpu().numpy()
+    assert _rel(got, ref) <= 1e-11
+    # degenerate orders and argument checks
+    for nco in (0, 1, 2):
+        assert np.abs(ctx.chebyshev(_t(chi), coef[:nco], ebar, de).cpu().numpy() - o.chebyshev(chi, coef[:nco], ebar, de)).max() <= 1e-13
+    t = _t(chi)
+    with pytest.raises(ks.KsError):
+        ctx.chebyshev(t, coef, ebar, de, out=t)
+    with pytest.raises(ks.KsError):
+        ctx.chebyshev(t, coef, ebar, 0.0)
+    e = torch.empty((0, p.npw), dtype=torch.complex128, device="cuda")
+    assert ctx.chebyshev(e, coef, ebar, de).shape == (0, p.npw)
+
+
+def test_chebyshev_full_size_cfg1(ks, oracle_mod):
+    """cfg 1 geometry, 96 stochastic orbitals, order 12: the oracle follows 2 of them; a zero-order
+    identity and linearity hold for the whole block."""
+    p = I.make_problem(1)
+    ctx = ks.Context.from_problem(p)
+    o = oracle_mod.Oracle.from_problem(p)
+    chi = _stochastic(p, 96, 7)
+    ebar, de = 0.5 * (p.ecutwfc + 4.0 - 3.0), 0.5 * (p.ecutwfc + 4.0 + 3.0)      # generous bounds: [-3, ecut + 4] Ry
+    coef = 1.0 / (1.0 + np.arange(12.0)) ** 2
+    got = ctx.chebyshev(_t(chi), coef, ebar, de).cpu().numpy()
+    sel = np.array([0, 95])
+    ref = o.chebyshev(chi[sel], coef, ebar, de)
+    assert _rel(got[sel], ref) <= 1e-11
+    half = ctx.chebyshev(_t(0.5 * chi), coef, ebar, de).cpu().numpy()
+    assert _rel(2.0 * half, got) <= 1e-14
