@@ -476,8 +476,11 @@ def main():
     if not args.no_cpu_baseline and world == 1:
         from oracle import kso
         nthreads = kso.num_threads()
-        nsample = min(nb, max(nthreads, 8))
-        ns, times, _ = oracle_sample(p, nsample, reps=1)
+        # bounded sample of the same workload: a first call on one band per thread sizes a second call of ~15 s
+        ns0, t0s, _ = oracle_sample(p, min(nb, max(nthreads, 8)), reps=1)
+        rate0 = ns0 / t0s[0]
+        ns1 = int(min(nb, max(ns0, nthreads * round(15.0 * rate0 / nthreads))))
+        ns, times, _ = oracle_sample(p, ns1, reps=1)
         line["cpu_baseline"] = {"value": ns / times[0], "unit": UNIT, "cores": nthreads, "kind": "oracle",
                                 "sample": "%d of %d bands, one kso_hpsi call (OpenMP over bands), %.1f s" % (ns, nb, times[0])}
     else:
