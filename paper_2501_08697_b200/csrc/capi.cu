@@ -246,6 +246,10 @@ extern "C" void ks_destroy(ks_ctx* c) {
   cudaFree(c->d_beta); cudaFree(c->d_D); cudaFree(c->d_proj_atom); cudaFree(c->d_off); cudaFree(c->d_doff);
   cudaFree(c->d_B); cudaFree(c->d_DB); cudaFree(c->d_hin); cudaFree(c->d_hout);
   for (int i = 0; i < 3; ++i) cudaFree(c->d_cheb[i]);
+  if (c->s_in) {
+    cudaStreamDestroy(c->s_in); cudaStreamDestroy(c->s_out); cudaEventDestroy(c->ev_start);
+    for (int i = 0; i < 8; ++i) { cudaEventDestroy(c->ev_in[i]); cudaEventDestroy(c->ev_done[i]); }
+  }
   cudaFree(c->gws.part);
   ks_eigh_free(&c->ews);
   ks_davidson_free(&c->dws);
@@ -386,17 +390,43 @@ static int stage(ks_ctx* c, size_t bytes) {
   return KS_OK;
 }
 
+// Host-buffer entry point, pipelined: the block is cut into up to 8 chunks of bands; chunk i+1 is copied in and chunk
+// i-1 copied out (two copy streams) while chunk i is applied on the context's stream, so with pinned host buffers the
+// PCIe transfers in both directions overlap the kernels.  Bands are independent in H psi: chunking changes no bit.
 extern "C" int ks_hpsi_host(ks_ctx* c, const ks_c128* psi_host, ks_c128* hpsi_host, int nbands) {
   if (!c) return KS_EINVAL;
   if (!psi_host || !hpsi_host || nbands < 0) { c->err = "ks_hpsi_host: bad argument"; return KS_EINVAL; }
   if (nbands == 0) return KS_OK;
-  const size_t bytes = sizeof(cplx) * (size_t)nbands * c->P.npw;
+  const size_t npw = c->P.npw, bytes = sizeof(cplx) * (size_t)nbands * npw;
   int rc = stage(c, bytes);
   if (rc) return rc;
-  KS_CUDA_CHECK(cudaMemcpyAsync(c->d_hin, psi_host, bytes, cudaMemcpyHostToDevice, c->stream), c->err);
-  rc = ks_hpsi_impl(c, c->d_hin, c->d_hout, nbands);
-  if (rc) return rc;
-  KS_CUDA_CHECK(cudaMemcpyAsync(hpsi_host, c->d_hout, bytes, cudaMemcpyDeviceToHost, c->stream), c->err);
+  if (!c->s_in) {
+    KS_CUDA_CHECK(cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking), c->err);
+    KS_CUDA_CHECK(cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking), c->err);
+    KS_CUDA_CHECK(cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming), c->err);
+    for (int i = 0; i < 8; ++i) {
+      KS_CUDA_CHECK(cudaEventCreateWithFlags(&c->ev_in[i], cudaEventDisableTiming), c->err);
+      KS_CUDA_CHECK(cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming), c->err);
+    }
+  }
+  // chunks of >= 32 bands (the GEMM tiles want some width), at most 8 of them
+  const int nchunk = std::max(1, std::min(8, nbands / 32));
+  const int per = ceil_div(nbands, nchunk);
+  KS_CUDA_CHECK(cudaEventRecord(c->ev_start, c->stream), c->err);          // order after earlier work on the stream
+  KS_CUDA_CHECK(cudaStreamWaitEvent(c->s_in, c->ev_start, 0), c->err);
+  for (int i = 0, b0 = 0; b0 < nbands; ++i, b0 += per) {
+    const int n = std::min(per, nbands - b0);
+    const size_t off = (size_t)b0 * npw, cb = sizeof(cplx) * (size_t)n * npw;
+    KS_CUDA_CHECK(cudaMemcpyAsync(c->d_hin + off, (const cplx*)psi_host + off, cb, cudaMemcpyHostToDevice, c->s_in), c->err);
+    KS_CUDA_CHECK(cudaEventRecord(c->ev_in[i], c->s_in), c->err);
+    KS_CUDA_CHECK(cudaStreamWaitEvent(c->stream, c->ev_in[i], 0), c->err);
+    rc = ks_hpsi_impl(c, c->d_hin + off, c->d_hout + off, n);
+    if (rc) return rc;
+    KS_CUDA_CHECK(cudaEventRecord(c->ev_done[i], c->stream), c->err);
+    KS_CUDA_CHECK(cudaStreamWaitEvent(c->s_out, c->ev_done[i], 0), c->err);
+    KS_CUDA_CHECK(cudaMemcpyAsync((cplx*)hpsi_host + off, c->d_hout + off, cb, cudaMemcpyDeviceToHost, c->s_out), c->err);
+  }
+  KS_CUDA_CHECK(cudaStreamSynchronize(c->s_out), c->err);
   KS_CUDA_CHECK(cudaStreamSynchronize(c->stream), c->err);
   return KS_OK;
 }

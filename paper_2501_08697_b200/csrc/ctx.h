@@ -39,6 +39,9 @@ struct ks_ctx {
   EighWs ews;
   DavidsonWs dws;
   cudaStream_t stream = 0;
+  // ks_hpsi_host pipeline: copy-in / copy-out streams and per-chunk events (created at first use)
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  cudaEvent_t ev_in[8] = {}, ev_done[8] = {}, ev_start = nullptr;
   int fft_batch = 0;             // bands per FFT batch
   double prof_ms[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   // per-kernel CUDA-event timing of ks_hpsi (ks_profile_begin / ks_profile_end); no host syncs while on
