@@ -21,6 +21,8 @@
 //                  waves -> 2 + 2 cos((G1-G2).r) closed form, non-negativity
 //   kso_chebyshev  U p(Lambda) U^H chi from numpy.linalg.eigh of the explicit H with p evaluated by
 //                  numpy.polynomial.chebyshev.chebval; T_n = cos(n arccos x) on an eigenvector; sqrt(Fermi-Dirac)
+//   kso_cg         V=0: sorted |k+G|^2 exactly; numpy.linalg.eigvalsh of the explicit H; kso_davidson's eigenvalues;
+//                  residuals, orthonormality, Ritz values above the exact ones
 //   kso_davidson   V=0: sorted |k+G|^2 exactly; constant shift; brute-force Jacobi / eigvalsh of
 //                  explicit H on cfg 0 and the shrunk variants; Ritz values monotone
 //   Eigenvalues of cfg 1, 3, 4 at FULL size: parity unpinned by anything external.
@@ -556,6 +558,106 @@ extern "C" int kso_davidson(const kso_ctx* c, cplx* psi, double* eig, int nb, do
   std::copy(eps.begin(), eps.end(), eig);
   if (resid) std::copy(rho.begin(), rho.end(), resid);
   if (iters_out) *iters_out = it;
+  if (nhpsi_out) *nhpsi_out = nh;
+  return status;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Band-by-band preconditioned conjugate gradient, the only eigensolver the paper prints:
+// PAPER.md Fig. 10 L549-570.  The listing is followed line by line; what it does not print is reading C19 of
+// DESIGN.md (the caption's prose, L570, and its ref 134 Teter-Payne-Allan):
+//   K      the Teter-Payne-Allan diagonal polynomial of the Davidson path (reading C11), x = |k+G|^2 / max(Ekin(psi_i), 1e-3)
+//   gamma  Polak-Ribiere ("by Polak-Ribiere method"):  gamma = Re<g_k - g_{k-1} | r_k> / Re<g_{k-1} | r_{k-1}>,
+//          r = (I - P)(p - lambda psi) the projected gradient, g = (I - P) K r the projected preconditioned one
+//   d      before the rotation d is made orthogonal to psi_i and normalised (the cos/sin update keeps ||psi|| = 1
+//          only then); the un-normalised d_k = g_k + gamma d_{k-1} is what the next step conjugates against
+//   theta  "optimal step size, ensuring maximal energy reduction": the minimiser of
+//          E(theta) = <psi cos + d sin | H | psi cos + d sin>,  tan 2 theta = a / (lambda - b),
+//          a = 2 Re<psi|H d>, b = Re<d|H d>, on the branch of the minimum: theta = atan2(-a, b - lambda) / 2
+//   stop   "convergence not reached": ||r||_2 <= tol/2 (projected gradient), or k_maxiter steps
+//   after the band loop one Rayleigh-Ritz step over the nb vectors orders the pairs and removes the O(tol) couplings
+//   between bands that converged one after the other (the listing returns the psi_i as they are)
+// ------------------------------------------------------------------------------------------------
+extern "C" int kso_cg(const kso_ctx* c, cplx* psi, double* eig, int nb, double tol, int kmaxiter, double* resid,
+                      int* steps_out, long long* nhpsi_out) {
+  const int npw = c->npw;
+  if (nb < 1 || nb > npw || kmaxiter < 1) return -1;
+  std::vector<cplx> X(psi, psi + (long)nb * npw), HX((long)nb * npw);
+  std::vector<cplx> p(npw), r(npw), g(npw), gp(npw), d(npw), dn(npw), h(npw);
+  long long nh = 0;
+  int steps = 0, status = 0;
+  for (int i = 0; i < nb; ++i) {
+    cplx* x = &X[(long)i * npw];
+    // psi_i = (I - sum_{j<i} |psi_j><psi_j|) psi_i, normalised
+    const double n0 = nrm2(x, npw);
+    for (int pass = 0; pass < 2; ++pass)
+      for (int j = 0; j < i; ++j) caxpy(-cdot(&X[(long)j * npw], x, npw), &X[(long)j * npw], x, npw);
+    const double n1 = nrm2(x, npw);
+    if (!(n1 > 1e-10 * n0) || n0 == 0.0) return -3;
+    for (int j = 0; j < npw; ++j) x[j] /= n1;
+    kso_hpsi(c, x, p.data(), 1);
+    ++nh;
+    double lambda = cdot(x, p.data(), npw).real();
+    double zeta_prev = 0.0;
+    bool conv = false;
+    for (int k = 1; k <= kmaxiter; ++k) {
+      // r = (I - P_{<=i}) (p - lambda psi)
+      for (int j = 0; j < npw; ++j) r[j] = p[j] - lambda * x[j];
+      for (int jj = 0; jj <= i; ++jj) caxpy(-cdot(&X[(long)jj * npw], r.data(), npw), &X[(long)jj * npw], r.data(), npw);
+      if (nrm2(r.data(), npw) <= 0.5 * tol) { conv = true; break; }
+      // g = (I - P_{<=i}) K r
+      double ekin = 0;
+      for (int j = 0; j < npw; ++j) ekin += c->g2[j] * std::norm(x[j]);
+      ekin = std::max(ekin, 1e-3);
+      for (int j = 0; j < npw; ++j) {
+        const double xx = c->g2[j] / ekin;
+        const double nx = 27.0 + 18.0 * xx + 12.0 * xx * xx + 8.0 * xx * xx * xx;
+        g[j] = (nx / (nx + 16.0 * xx * xx * xx * xx)) * r[j];
+      }
+      for (int jj = 0; jj <= i; ++jj) caxpy(-cdot(&X[(long)jj * npw], g.data(), npw), &X[(long)jj * npw], g.data(), npw);
+      const double zeta = cdot(g.data(), r.data(), npw).real();
+      if (k == 1) {
+        d = g;
+      } else {
+        const double gamma = (zeta - cdot(gp.data(), r.data(), npw).real()) / zeta_prev;
+        for (int j = 0; j < npw; ++j) d[j] = g[j] + gamma * d[j];
+      }
+      gp = g;
+      zeta_prev = zeta;
+      // d' = d - psi <psi|d>, normalised
+      dn = d;
+      caxpy(-cdot(x, dn.data(), npw), x, dn.data(), npw);
+      const double nd = nrm2(dn.data(), npw);
+      if (!(nd > 0.0)) { conv = true; break; }
+      for (int j = 0; j < npw; ++j) dn[j] /= nd;
+      kso_hpsi(c, dn.data(), h.data(), 1);
+      ++nh; ++steps;
+      const double a = 2.0 * cdot(x, h.data(), npw).real();
+      const double b = cdot(dn.data(), h.data(), npw).real();
+      const double theta = 0.5 * std::atan2(-a, b - lambda);
+      const double ct = std::cos(theta), st = std::sin(theta);
+      for (int j = 0; j < npw; ++j) {
+        x[j] = x[j] * ct + dn[j] * st;
+        p[j] = p[j] * ct + h[j] * st;
+      }
+      lambda = cdot(x, p.data(), npw).real();
+    }
+    if (!conv) status = 1;
+    std::copy(p.begin(), p.end(), &HX[(long)i * npw]);
+  }
+  // one Rayleigh-Ritz step over the nb vectors (H psi_i are the p_i: no extra H application)
+  std::vector<cplx> X2, HX2;
+  std::vector<double> eps(nb);
+  rayleigh_ritz(npw, nb, nb, X, HX, X2, HX2, eps);
+  for (int i = 0; i < nb; ++i) {
+    eig[i] = eps[i];
+    if (resid) {
+      for (int j = 0; j < npw; ++j) r[j] = HX2[(long)i * npw + j] - eps[i] * X2[(long)i * npw + j];
+      resid[i] = nrm2(r.data(), npw);
+    }
+  }
+  std::copy(X2.begin(), X2.end(), psi);
+  if (steps_out) *steps_out = steps;
   if (nhpsi_out) *nhpsi_out = nh;
   return status;
 }

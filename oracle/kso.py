@@ -41,6 +41,7 @@ def lib():
         _lib.kso_hpsi.argtypes = [_vp, _vp, _vp, C.c_int]
         _lib.kso_explicit_h.argtypes = [_vp, _vp]
         _lib.kso_density.argtypes = [_vp, _vp, _vp, C.c_int, _vp]
+        _lib.kso_cg.argtypes = [_vp, _vp, _vp, C.c_int, C.c_double, C.c_int, _vp, _vp, _vp]
         _lib.kso_chebyshev.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, C.c_double, C.c_double, _vp]
         _lib.kso_jacobi.argtypes = [C.c_int, _vp, _vp, _vp]
         _lib.kso_fft3d.argtypes = [C.c_int, C.c_int, C.c_int, _vp, C.c_int]
@@ -162,6 +163,16 @@ class Oracle:
         rc = lib().kso_chebyshev(self._h, _p(chi), chi.shape[0], coef.size, _p(coef), float(ebar), float(de), _p(out))
         assert rc == 0
         return out
+
+    def cg(self, psi0, tol=1e-8, kmaxiter=200):
+        """Band-by-band preconditioned CG (Fig. 10).  Returns dict(eig, psi, resid, steps, band_applications, converged)."""
+        psi = np.array(psi0, dtype=np.complex128, order="C")
+        nb = psi.shape[0]
+        eig = np.zeros(nb); res = np.zeros(nb)
+        steps = C.c_int(0); nh = C.c_longlong(0)
+        rc = lib().kso_cg(self._h, _p(psi), _p(eig), nb, float(tol), int(kmaxiter), _p(res), C.byref(steps), C.byref(nh))
+        assert rc >= 0, rc
+        return dict(eig=eig, psi=psi, resid=res, steps=steps.value, band_applications=nh.value, converged=(rc == 0))
 
     def explicit_h(self) -> np.ndarray:
         H = np.empty((self.npw, self.npw), dtype=np.complex128)

@@ -426,3 +426,42 @@ def test_chebyshev_sqrt_fermi_dirac(oracle_mod):
     got = o.chebyshev(chi, coef, ebar, de)
     want = (U @ (np.sqrt(1.0 / (1.0 + np.exp((w - mu) / kT)))[:, None] * (U.conj().T @ chi.T))).T
     assert np.abs(got - want).max() < 1e-9 * np.abs(want).max()
+
+
+# ----------------------------------------------------------------------------- band-by-band CG (Fig. 10)
+def test_cg_free_electron_exact(oracle_mod):
+    """V = 0, no projectors: the eigenvalues are the sorted |k+G|^2 exactly (north_star), degenerate shells included."""
+    p = I.make_problem(0, with_beta=False, with_vloc=False)
+    o = oracle_mod.Oracle.from_problem(p)
+    r = o.cg(p.psi0, tol=1e-9)
+    assert r["converged"] and np.abs(r["eig"] - np.sort(p.g2)[:p.nbands]).max() < 1e-12
+
+
+@pytest.mark.parametrize("name", ["cfg0", "s2"])
+def test_cg_vs_bruteforce_and_davidson(oracle_mod, name):
+    """Fig. 10's solver must reach the eigenpairs of the explicit H(G,G') (LAPACK on the definition) and agree with the
+    block-Davidson path; residuals <= tol after the closing Rayleigh-Ritz step, orthonormal vectors, and the Ritz value
+    of every band decreases monotonically inside its CG loop (theta is the energy minimiser)."""
+    p = I.make_problem(0) if name == "cfg0" else I.make_shrunk(name)
+    o = oracle_mod.Oracle.from_problem(p)
+    w = np.linalg.eigvalsh(o.explicit_h())
+    r = o.cg(p.psi0, tol=1e-8)
+    nb = p.nbands
+    assert r["converged"]
+    assert np.abs(r["eig"] - w[:nb]).max() < 1e-10
+    X = r["psi"]
+    assert np.abs(X.conj() @ X.T - np.eye(nb)).max() < 1e-12
+    res = np.linalg.norm(o.hpsi(X) - r["eig"][:, None] * X, axis=1)
+    assert res.max() <= 1e-8 and np.abs(res - r["resid"]).max() < 1e-12
+    d = o.davidson(p.psi0, tol=1e-8)
+    assert np.abs(d["eig"] - r["eig"]).max() < 1e-10
+    assert nb <= r["steps"] and r["band_applications"] == r["steps"] + nb
+
+
+def test_cg_reports_not_converged(oracle_mod):
+    p = I.make_problem(0)
+    o = oracle_mod.Oracle.from_problem(p)
+    r = o.cg(p.psi0, tol=1e-8, kmaxiter=2)
+    assert not r["converged"] and r["steps"] == 2 * p.nbands
+    w = np.linalg.eigvalsh(o.explicit_h())
+    assert (r["eig"] >= w[:p.nbands] - 1e-12).all()          # Ritz values bound the exact ones from above
