@@ -80,6 +80,15 @@ int ks_density(ks_ctx* ctx, const ks_c128* psi, const double* occ, int nbands, d
 /* same through HOST buffers (copies inside, synchronises before returning) */
 int ks_density_host(ks_ctx* ctx, const ks_c128* psi_host, const double* occ_host, int nbands, double* rho_host);
 
+/* Lowest nbands eigenpairs by the band-by-band preconditioned conjugate gradient of PAPER.md Fig. 10 (L549-570), the
+ * eigensolver the paper prints; what the listing omits follows reading C19 of DESIGN.md
+ * (K = Teter-Payne-Allan, gamma = Polak-Ribiere, theta = minimiser of the Rayleigh quotient, stop at ||r|| <= tol/2,
+ * one closing Rayleigh-Ritz step).  Same arguments and results as ks_davidson; kmaxiter = CG steps allowed per band;
+ * steps_out = CG steps taken in total (HOST), band_applications_out = H applications (steps + nbands).
+ * Returns KS_OK, KS_NOTCONV (some band used all kmaxiter steps; best pairs still written) or < 0. */
+int ks_cg(ks_ctx* ctx, ks_c128* psi, double* eig, int nbands, double tol, int kmaxiter, double* resid,
+          int* steps_out, long long* band_applications_out);
+
 /* Chebyshev expansion of an operator function on a block (the inner loop of sDFT: PAPER.md L588,
  * stochastic orbitals Eq. 52, gamma = f_H^{1/2} chi Eq. 54, orders 25..1200 L714):
  *   out = sum_{n=0}^{ncoef-1} coef[n] T_n(Ht) chi,  Ht = (H - ebar)/de,  T_0 = chi, T_1 = Ht chi, T_{n+1} = 2 Ht T_n - T_{n-1}.

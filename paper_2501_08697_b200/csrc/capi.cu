@@ -546,6 +546,11 @@ extern "C" int ks_davidson(ks_ctx* c, ks_c128* psi, double* eig, int nbands, dou
   return ks_davidson_impl(c, (cplx*)psi, eig, nbands, tol, max_iter, resid, iters_out, band_applications_out);
 }
 
+extern "C" int ks_cg(ks_ctx* c, ks_c128* psi, double* eig, int nbands, double tol, int kmaxiter, double* resid,
+                     int* steps_out, long long* band_applications_out) {
+  return ks_cg_impl(c, (cplx*)psi, eig, nbands, tol, kmaxiter, resid, steps_out, band_applications_out);
+}
+
 extern "C" int ks_davidson_host(ks_ctx* c, ks_c128* psi_host, double* eig_host, int nbands, double tol, int max_iter,
                                 double* resid_host, int* iters_out, long long* band_applications_out) {
   if (!c) return KS_EINVAL;

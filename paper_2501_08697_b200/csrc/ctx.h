@@ -61,3 +61,5 @@ int ks_hpsi_impl(ks_ctx* c, const cplx* psi, cplx* hpsi, int nb);
 int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int max_iter, double* resid,
                      int* iters_out, long long* nhpsi_out);
 void ks_davidson_free(DavidsonWs* w);
+int ks_cg_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int kmaxiter, double* resid, int* steps_out,
+               long long* nhpsi_out);

@@ -34,6 +34,7 @@ _lib.ks_hpsi.argtypes = [_vp, _vp, _vp, _i]
 _lib.ks_hpsi_host.argtypes = [_vp, _vp, _vp, _i]
 _lib.ks_density.argtypes = [_vp, _vp, _vp, _i, _vp]
 _lib.ks_density_host.argtypes = [_vp, _vp, _vp, _i, _vp]
+_lib.ks_cg.argtypes = [_vp, _vp, _vp, _i, _d, _i, _vp, _vp, _vp]
 _lib.ks_chebyshev.argtypes = [_vp, _vp, _vp, _i, _i, _vp, _d, _d]
 _lib.ks_davidson.argtypes = [_vp, _vp, _vp, _i, _d, _i, _vp, _vp, _vp]
 _lib.ks_davidson_host.argtypes = [_vp, _vp, _vp, _i, _d, _i, _vp, _vp, _vp]
@@ -47,7 +48,7 @@ _lib.ks_dmma_peak.argtypes = [_vp, _vp]
 
 KS_OK, KS_NOTCONV = 0, 1
 EXPORTS = ("ks_pw_count", "ks_pw_list", "ks_create", "ks_destroy", "ks_npw", "ks_set_stream", "ks_set_fft_batch",
-           "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_density", "ks_density_host", "ks_chebyshev", "ks_davidson", "ks_davidson_host",
+           "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_density", "ks_density_host", "ks_chebyshev", "ks_cg", "ks_davidson", "ks_davidson_host",
            "ks_davidson_profile", "ks_profile_begin", "ks_profile_end", "ks_zgemm_hn", "ks_zgemm_nn", "ks_eigh", "ks_dmma_peak")
 
 
@@ -213,6 +214,19 @@ class Context:
         rc = self._check(_lib.ks_davidson(self._h, _dev(psi), _dev(eig), nb, float(tol), int(max_iter), _dev(res),
                                           C.byref(it), C.byref(nh)))
         return dict(psi=psi, eig=eig, resid=res, iters=it.value, band_applications=nh.value, converged=(rc == 0))
+
+    def cg(self, psi, tol=1e-8, kmaxiter=200):
+        """Band-by-band preconditioned CG (Fig. 10).  psi: torch complex128 CUDA [nbands][npw], overwritten.
+        Returns dict(eig, resid (device tensors), steps, band_applications, converged)."""
+        import torch
+        assert psi.dtype == torch.complex128 and psi.dim() == 2 and psi.shape[1] == self.npw
+        nb = int(psi.shape[0])
+        eig = torch.empty(nb, dtype=torch.float64, device=psi.device)
+        res = torch.empty(nb, dtype=torch.float64, device=psi.device)
+        it, nh = _i(0), C.c_longlong(0)
+        rc = self._check(_lib.ks_cg(self._h, _dev(psi), _dev(eig), nb, float(tol), int(kmaxiter), _dev(res),
+                                    C.byref(it), C.byref(nh)))
+        return dict(psi=psi, eig=eig, resid=res, steps=it.value, band_applications=nh.value, converged=(rc == 0))
 
     def davidson_host(self, psi0: np.ndarray, tol=1e-8, max_iter=400):
         psi = np.array(psi0, dtype=np.complex128, order="C")

@@ -362,3 +362,58 @@ def test_chebyshev_full_size_cfg1(ks, oracle_mod):
     assert _rel(got[sel], ref) <= 1e-11
     half = ctx.chebyshev(_t(0.5 * chi), coef, ebar, de).cpu().numpy()
     assert _rel(2.0 * half, got) <= 1e-14
+
+
+# ------------------------------------------------------------------ band-by-band CG (Fig. 10)
+def _check_cg(ks, oracle_mod, p, exact, kmaxiter=200, need_conv=True):
+    ctx = ks.Context.from_problem(p)
+    o = oracle_mod.Oracle.from_problem(p)
+    r = ctx.cg(_t(p.psi0), tol=1e-8, kmaxiter=kmaxiter)
+    nb = p.nbands
+    eig = r["eig"].cpu().numpy()
+    X = r["psi"].cpu().numpy()
+    if need_conv:
+        assert r["converged"]
+    assert np.abs(eig - exact[:nb]).max() <= 1e-8
+    assert np.abs(X.conj() @ X.T - np.eye(nb)).max() <= 1e-10
+    res = np.linalg.norm(o.hpsi(X) - eig[:, None] * X, axis=1)       # re-evaluated with the oracle's H psi
+    assert np.abs(res - r["resid"].cpu().numpy()).max() <= 1e-10
+    if need_conv:
+        assert res.max() <= 1.05e-8
+    assert (np.diff(eig) >= -1e-12).all()
+    assert r["band_applications"] == r["steps"] + nb
+    return r, o
+
+
+def test_cg_cfg0_vs_oracle_and_bruteforce(ks, oracle_mod):
+    p = I.make_problem(0)
+    o = oracle_mod.Oracle.from_problem(p)
+    w = np.linalg.eigvalsh(o.explicit_h())
+    r, _ = _check_cg(ks, oracle_mod, p, w)
+    ro = o.cg(p.psi0, tol=1e-8)
+    assert np.abs(r["eig"].cpu().numpy() - ro["eig"]).max() <= 1e-8
+    assert abs(r["steps"] - ro["steps"]) <= 0.1 * ro["steps"]          # same listing: step counts agree to rounding effects
+    # Davidson reaches the same pairs
+    d = ks.Context.from_problem(p).davidson(_t(p.psi0), tol=1e-8)
+    assert np.abs(d["eig"].cpu().numpy() - r["eig"].cpu().numpy()).max() <= 1e-8
+
+
+@pytest.mark.parametrize("name", ["s2", "s1", "s4"])
+def test_cg_shrunk(ks, oracle_mod, name):
+    """k != 0 (s2), a clustered 64-atom spectrum (s1: the oracle needs up to ~1000 steps for one band too) and the
+    non-cubic slab grid (s4), against LAPACK on the explicit H."""
+    p = I.make_shrunk(name)
+    o = oracle_mod.Oracle.from_problem(p)
+    w = np.linalg.eigvalsh(o.explicit_h())
+    _check_cg(ks, oracle_mod, p, w, kmaxiter=1500)
+
+
+def test_cg_free_electron_and_not_converged(ks):
+    p = I.make_problem(0, with_beta=False, with_vloc=False)
+    ctx = ks.Context.from_problem(p)
+    r = ctx.cg(_t(p.psi0), tol=1e-9)
+    assert r["converged"] and np.abs(r["eig"].cpu().numpy() - np.sort(p.g2)[:8]).max() <= 1e-10
+    p = I.make_problem(0)
+    ctx = ks.Context.from_problem(p)
+    r = ctx.cg(_t(p.psi0), tol=1e-8, kmaxiter=2)
+    assert not r["converged"] and r["steps"] == 2 * p.nbands
