@@ -44,6 +44,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-density", action="store_true")
     ap.add_argument("--no-chebyshev", action="store_true")
+    ap.add_argument("--cg", type=int, default=0, metavar="KMAXITER",
+                    help="also time the band-by-band CG of PAPER.md Fig. 10 (ks_cg) with this many steps per band (0 = skip)")
     ap.add_argument("--davidson-max-iter", type=int, default=400)
     ap.add_argument("--fft-batch", type=int, default=0)
     ap.add_argument("--kbatch", action="store_true",
@@ -418,6 +420,17 @@ def main():
         cms = timed_steps(lambda: ctx.chebyshev(psi, coef, ebar, de, out=cout), 1)
         cheb = {"order": ncoef - 1, "ms": cms, "band_applications_per_s": nb * (ncoef - 1) / (cms * 1e-3),
                 "vs_plain_hpsi": (nb * (ncoef - 1) / (cms * 1e-3)) / (nb * args.steps / (ms * 1e-3))}
+    cgr = None
+    if args.cg > 0:
+        work = psi.clone()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        r = ctx.cg(work, tol=1e-8, kmaxiter=args.cg)
+        torch.cuda.synchronize()
+        csec = time.perf_counter() - t0
+        cgr = {"time_s": csec, "kmaxiter": args.cg, "steps": r["steps"], "band_applications": r["band_applications"],
+               "converged": bool(r["converged"]), "max_resid": float(r["resid"].max().item()),
+               "eig_min": float(r["eig"][0].item()), "eig_max": float(r["eig"][-1].item())}
     clk = clocks.stop() if rank == 0 else None
     ms, e2e_s = PL.max_over_ranks([ms, e2e_s])
     if rank != 0:
@@ -472,6 +485,7 @@ def main():
         "davidson": dav,
         "density": dens,
         "chebyshev": cheb,
+        "cg": cgr,
     }
     if not args.no_cpu_baseline and world == 1:
         from oracle import kso
