@@ -568,7 +568,7 @@ extern "C" int kso_davidson(const kso_ctx* c, cplx* psi, double* eig, int nb, do
 // DESIGN.md (the caption's prose, L570, and its ref 134 Teter-Payne-Allan):
 //   K      the Teter-Payne-Allan diagonal polynomial of the Davidson path (reading C11), x = |k+G|^2 / max(Ekin(psi_i), 1e-3)
 //   gamma  Polak-Ribiere ("by Polak-Ribiere method"):  gamma = Re<g_k - g_{k-1} | r_k> / Re<g_{k-1} | r_{k-1}>,
-//          r = (I - P)(p - lambda psi) the projected gradient, g = (I - P) K r the projected preconditioned one
+//          r = (I - P)(p - lambda psi) the projected gradient, g = (I - P) K (p - lambda psi) as the listing has it
 //   d      before the rotation d is made orthogonal to psi_i and normalised (the cos/sin update keeps ||psi|| = 1
 //          only then); the un-normalised d_k = g_k + gamma d_{k-1} is what the next step conjugates against
 //   theta  "optimal step size, ensuring maximal energy reduction": the minimiser of
@@ -601,19 +601,20 @@ extern "C" int kso_cg(const kso_ctx* c, cplx* psi, double* eig, int nb, double t
     double zeta_prev = 0.0;
     bool conv = false;
     for (int k = 1; k <= kmaxiter; ++k) {
-      // r = (I - P_{<=i}) (p - lambda psi)
-      for (int j = 0; j < npw; ++j) r[j] = p[j] - lambda * x[j];
-      for (int jj = 0; jj <= i; ++jj) caxpy(-cdot(&X[(long)jj * npw], r.data(), npw), &X[(long)jj * npw], r.data(), npw);
-      if (nrm2(r.data(), npw) <= 0.5 * tol) { conv = true; break; }
-      // g = (I - P_{<=i}) K r
+      // g_i = K (p_i - lambda psi_i)   (Fig. 10: K acts on the plain residual), then r = (I - P_{<=i}) (p - lambda psi)
+      // for the stopping rule and the Polak-Ribiere products
       double ekin = 0;
       for (int j = 0; j < npw; ++j) ekin += c->g2[j] * std::norm(x[j]);
       ekin = std::max(ekin, 1e-3);
       for (int j = 0; j < npw; ++j) {
+        r[j] = p[j] - lambda * x[j];
         const double xx = c->g2[j] / ekin;
         const double nx = 27.0 + 18.0 * xx + 12.0 * xx * xx + 8.0 * xx * xx * xx;
         g[j] = (nx / (nx + 16.0 * xx * xx * xx * xx)) * r[j];
       }
+      for (int jj = 0; jj <= i; ++jj) caxpy(-cdot(&X[(long)jj * npw], r.data(), npw), &X[(long)jj * npw], r.data(), npw);
+      if (nrm2(r.data(), npw) <= 0.5 * tol) { conv = true; break; }
+      // g_i = (I - sum_{j<=i} |psi_j><psi_j|) g_i
       for (int jj = 0; jj <= i; ++jj) caxpy(-cdot(&X[(long)jj * npw], g.data(), npw), &X[(long)jj * npw], g.data(), npw);
       const double zeta = cdot(g.data(), r.data(), npw).real();
       if (k == 1) {

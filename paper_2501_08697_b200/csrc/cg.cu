@@ -208,8 +208,10 @@ int ks_cg_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int kmaxit
     k_cg_dot3<<<2, CG_T, 0, st>>>(npw, dl, w.sc);
     bool conv = false;
     for (int k = 1; k <= kmaxiter; ++k) {
-      // r = (I - P_{<=i}) (p - lambda psi)
+      // g = K (p - lambda psi) (Fig. 10: K acts on the plain residual); r = (I - P_{<=i}) (p - lambda psi)
+      std::swap(g, gp);
       k_cg_resid<<<nblk, 256, 0, st>>>(npw, p, x, w.sc, r);
+      k_cg_precond<<<nblk, 256, 0, st>>>(npw, r, c->P.d_g2, w.sc, g);
       k_cg_dots_x<<<i + 1, CG_T, 0, st>>>(npw, X, r, w.s);
       k_cg_sub_x<<<nblk, 256, 0, st>>>(npw, i + 1, X, w.s, r);
       Dot3 dr;
@@ -218,9 +220,7 @@ int ks_cg_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int kmaxit
       KS_CUDA_CHECK(cudaMemcpyAsync(&hs[0], w.sc + S_R2, sizeof(double), cudaMemcpyDeviceToHost, st), c->err);
       KS_CUDA_CHECK(cudaStreamSynchronize(st), c->err);
       if (std::sqrt(hs[0]) <= 0.5 * tol) { conv = true; break; }
-      // g = (I - P_{<=i}) K r
-      std::swap(g, gp);
-      k_cg_precond<<<nblk, 256, 0, st>>>(npw, r, c->P.d_g2, w.sc, g);
+      // g = (I - P_{<=i}) g
       k_cg_dots_x<<<i + 1, CG_T, 0, st>>>(npw, X, g, w.s);
       k_cg_sub_x<<<nblk, 256, 0, st>>>(npw, i + 1, X, w.s, g);
       // zeta = Re<g|r>, <g_prev|r>; d = g + gamma d
