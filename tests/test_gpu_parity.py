@@ -178,6 +178,20 @@ def test_hpsi_full_size(ks, oracle_mod, c, k_index, nsample):
     assert np.abs(G - G.conj().T).max() <= 1e-11 * np.abs(G).max()
 
 
+def test_hpsi_full_symmetric_D_blocks(ks, oracle_mod):
+    """Per-atom D blocks that are full symmetric matrices of uneven sizes (Eq. 4 L221 allows D_ll' coupling)."""
+    p = I.make_problem(0)
+    rng = np.random.default_rng(21)
+    off = np.array([0, 5, 8], dtype=np.int32)
+    D = np.concatenate([(0.5 * (a + a.T)).ravel() for a in (rng.standard_normal((5, 5)), rng.standard_normal((3, 3)))])
+    ctx = ks.Context(p.cell, p.k_frac, p.ecutwfc, p.grid, p.vloc_g, p.beta, off, D)
+    o = oracle_mod.Oracle(p.cell, p.k_frac, p.ecutwfc, p.grid, p.vloc_g, p.beta, off, D)
+    assert _rel(ctx.hpsi(_t(p.psi0)).cpu().numpy(), o.hpsi(p.psi0)) <= HPSI_TOL
+    w = np.linalg.eigvalsh(o.explicit_h())
+    r = ctx.davidson(_t(p.psi0), tol=1e-8)
+    assert r["converged"] and np.abs(r["eig"].cpu().numpy() - w[:p.nbands]).max() <= 1e-8
+
+
 def test_hpsi_ragged_band_group(ks, oracle_mod):
     """cfg 1 geometry with 31 bands: the x kernel walks over band groups of 2, so the last group is ragged;
     a 7-band FFT batch adds a ragged last batch on top."""

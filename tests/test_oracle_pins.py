@@ -465,3 +465,28 @@ def test_cg_reports_not_converged(oracle_mod):
     assert not r["converged"] and r["steps"] == 2 * p.nbands
     w = np.linalg.eigvalsh(o.explicit_h())
     assert (r["eig"] >= w[:p.nbands] - 1e-12).all()          # Ritz values bound the exact ones from above
+
+
+def test_full_symmetric_D_blocks_uneven_sizes(oracle_mod):
+    """Eq. 4 L221 allows D_ll' coupling: per-atom blocks that are full real symmetric matrices of different sizes
+    (5 and 3 projectors).  Dual-space H psi must equal the explicit H, written here from the definition."""
+    p = I.make_problem(0)
+    rng = np.random.default_rng(21)
+    off = np.array([0, 5, 8], dtype=np.int32)
+    blocks = []
+    for n in (5, 3):
+        a = rng.standard_normal((n, n))
+        blocks.append(0.5 * (a + a.T))
+    D = np.concatenate([b.ravel() for b in blocks])
+    o = oracle_mod.Oracle(p.cell, p.k_frac, p.ecutwfc, p.grid, p.vloc_g, p.beta, off, D)
+    H = o.explicit_h()
+    assert np.abs(H - H.conj().T).max() < 1e-13
+    # the nonlocal part from the definition: sum_a beta_a^T-block D_a conj(beta_a)
+    o0 = oracle_mod.Oracle(p.cell, p.k_frac, p.ecutwfc, p.grid, p.vloc_g)
+    Hnl = np.zeros_like(H)
+    for a, b in enumerate(blocks):
+        ba = p.beta[off[a]:off[a + 1]]                    # [np_a][npw]
+        Hnl += ba.T @ b @ ba.conj()
+    assert np.abs(H - o0.explicit_h() - Hnl).max() < 1e-13
+    got = o.hpsi(p.psi0)
+    assert np.linalg.norm(got - p.psi0 @ H.T) <= 1e-13 * np.linalg.norm(got)
