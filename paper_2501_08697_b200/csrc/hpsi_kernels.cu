@@ -454,7 +454,9 @@ template <int NX> struct xcfg { static constexpr int ZC = 32, NT = 128, MINB = 4
 template <> struct xcfg<18> { static constexpr int ZC = 32, NT = 96, MINB = 4; };
 template <> struct xcfg<36> { static constexpr int ZC = 32, NT = 96, MINB = 4; };
 template <> struct xcfg<54> { static constexpr int ZC = 32, NT = 96, MINB = 4; };
-template <> struct xcfg<128> { static constexpr int ZC = 32, NT = 256, MINB = 2; };
+// 128: 16-column tiles and four 4-warp CTAs per SM beat 32-column tiles and two 8-warp CTAs (301 -> 283 us per 30-band launch);
+// the same halving for 96 (64-thread CTAs, eight per SM) is slightly slower (283 -> 289 us)
+template <> struct xcfg<128> { static constexpr int ZC = 16, NT = 128, MINB = 4; };
 
 // The CTA walks over bg bands with the same columns.  Thread (pz, g) owns the codelet lines j2 = g, g+G, ...
 // in the first AND the last pass, i.e. the tile rows {j1*R2 + j2}: once the last pass of band b has read a
