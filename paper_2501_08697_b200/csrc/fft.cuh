@@ -116,6 +116,8 @@ template <int N> struct fac;
 KS_FAC(16, 4, 4)   KS_FAC(18, 6, 3)   KS_FAC(24, 6, 4)   KS_FAC(32, 8, 4)   KS_FAC(36, 6, 6)
 KS_FAC(48, 8, 6)   KS_FAC(54, 9, 6)   KS_FAC(64, 8, 8)   KS_FAC(72, 9, 8)   KS_FAC(96, 12, 8)
 KS_FAC(128, 16, 8) KS_FAC(144, 12, 12) KS_FAC(192, 16, 12) KS_FAC(256, 16, 16) KS_FAC(288, 18, 16)
+// lengths with a factor 5 (grids with factors 2, 3, 5 are what plane-wave codes pick)
+KS_FAC(20, 5, 4)   KS_FAC(40, 8, 5)   KS_FAC(60, 10, 6)  KS_FAC(80, 10, 8)  KS_FAC(100, 10, 10) KS_FAC(120, 12, 10)
 #undef KS_FAC
 
 // twiddle w_n^{SIGN*t} from a shared-memory table tw[t] = e^{+2 pi i t/n}

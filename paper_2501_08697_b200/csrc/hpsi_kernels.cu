@@ -40,16 +40,16 @@ cudaError_t ks_fft_init_constants() {
 // ------------------------------------------------------------------------------------------------
 // supported sizes
 // ------------------------------------------------------------------------------------------------
-#define KS_X_SIZES(X) X(16) X(18) X(24) X(32) X(36) X(48) X(54) X(64) X(72) X(96) X(128)
+#define KS_X_SIZES(X) X(16) X(18) X(20) X(24) X(32) X(36) X(40) X(48) X(54) X(60) X(64) X(72) X(80) X(96) X(100) X(120) X(128)
 #define KS_YZ_PAIRS(X) \
   X(16, 16) X(18, 18) X(24, 24) X(32, 32) X(36, 36) X(48, 48) X(54, 54) X(64, 64) X(72, 72) \
-  X(96, 96) X(128, 128) X(18, 64) X(96, 288)
+  X(96, 96) X(128, 128) X(18, 64) X(96, 288) X(20, 20) X(40, 40) X(60, 60) X(80, 80) X(100, 100) X(120, 120)
 
 void ks_fft_factors(int n, int* R1, int* R2) {
   *R1 = 0; *R2 = 0;
   switch (n) {
 #define C_(N_) case N_: *R1 = fac<N_>::R1; *R2 = fac<N_>::R2; break;
-    C_(16) C_(18) C_(24) C_(32) C_(36) C_(48) C_(54) C_(64) C_(72) C_(96) C_(128) C_(144) C_(192) C_(256) C_(288)
+    C_(16) C_(18) C_(20) C_(24) C_(32) C_(36) C_(40) C_(48) C_(54) C_(60) C_(64) C_(72) C_(80) C_(96) C_(100) C_(120) C_(128) C_(144) C_(192) C_(256) C_(288)
 #undef C_
     default: break;
   }

@@ -178,6 +178,19 @@ def test_hpsi_full_size(ks, oracle_mod, c, k_index, nsample):
     assert np.abs(G - G.conj().T).max() <= 1e-11 * np.abs(G).max()
 
 
+@pytest.mark.parametrize("c,ecut,n,beta", [(0, 4.0, 20, True), (0, 25.0, 40, True), (0, 60.0, 60, True),
+                                           (1, 25.0, 80, False), (1, 40.0, 100, False), (3, 30.0, 120, False)])
+def test_hpsi_radix5_grids(ks, oracle_mod, c, ecut, n, beta):
+    """Grids with a factor 5 (20, 40, 60, 80, 100, 120): radix-5 codelets in all three kernels, plus the density."""
+    p = I.make_problem(c, ecutwfc=ecut, grid=(n, n, n), nbands=3, with_beta=beta)
+    ctx = ks.Context.from_problem(p)
+    o = oracle_mod.Oracle.from_problem(p)
+    assert _rel(ctx.hpsi(_t(p.psi0)).cpu().numpy(), o.hpsi(p.psi0)) <= HPSI_TOL
+    occ = np.array([2.0, 1.0, 0.5])
+    ref = o.density(p.psi0, occ)
+    assert np.abs(ctx.density(_t(p.psi0), _t(occ)).cpu().numpy() - ref).max() <= 1e-12 * ref.max()
+
+
 def test_hpsi_full_symmetric_D_blocks(ks, oracle_mod):
     """Per-atom D blocks that are full symmetric matrices of uneven sizes (Eq. 4 L221 allows D_ll' coupling)."""
     p = I.make_problem(0)
