@@ -601,10 +601,15 @@ struct RhoArgs {
   long ncol;
 };
 
+// tile geometry of k_rho: it has one staging buffer and waits for it once per band, so it wants more (smaller) CTAs per SM
+// than k_x: 16 columns x 64 threads, five CTAs per SM for 96 (cfg 1 density 217k -> 238k bands/s); k_x's geometry otherwise
+template <int NX> struct rcfg { static constexpr int ZC = xcfg<NX>::ZC, NT = xcfg<NX>::NT, MINB = xcfg<NX>::MINB > 3 ? 3 : xcfg<NX>::MINB; };
+template <> struct rcfg<96> { static constexpr int ZC = 16, NT = 64, MINB = 5; };
+
 template <int NX>
-__global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB > 3 ? 3 : xcfg<NX>::MINB) k_rho(RhoArgs a) {
+__global__ void __launch_bounds__(rcfg<NX>::NT, rcfg<NX>::MINB) k_rho(RhoArgs a) {
   constexpr int R1 = fac<NX>::R1, R2 = fac<NX>::R2;
-  constexpr int ZC = xcfg<NX>::ZC, NT = xcfg<NX>::NT, G = NT / ZC;
+  constexpr int ZC = rcfg<NX>::ZC, NT = rcfg<NX>::NT, G = NT / ZC;
   constexpr int IT2 = (R1 + G - 1) / G;       // pass-2 lines per thread
   constexpr int R1P = (R1 + 3) & ~3;
   extern __shared__ cplx sm[];
@@ -794,7 +799,7 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
 
 // ---- density build: launchers ----
 template <int NX> static size_t rho_smem(int L1) {
-  return sizeof(cplx) * ((size_t)NX + (size_t)NX * xcfg<NX>::ZC + (size_t)L1 * xcfg<NX>::ZC) +
+  return sizeof(cplx) * ((size_t)NX + (size_t)NX * rcfg<NX>::ZC + (size_t)L1 * rcfg<NX>::ZC) +
          sizeof(int) * (fac<NX>::R2 + 1) * ((fac<NX>::R1 + 3) & ~3);
 }
 
@@ -802,7 +807,11 @@ int ks_density_batch(HpsiPlan& P, const cplx* psi, const double* occ, int nb, in
   if (nb <= 0) return KS_OK;
   if (nb > P.batch_cap) { err = "internal: FFT batch larger than workspace"; return KS_EINVAL; }
   const long ncol = (long)P.n2 * P.n3;
-  const int nchunk = ceil_div(ncol, P.zc_x);
+  int zc_r = 0, nt_r = 0;
+#define C_(N_) if (P.n1 == N_) { zc_r = rcfg<N_>::ZC; nt_r = rcfg<N_>::NT; }
+  KS_X_SIZES(C_)
+#undef C_
+  const int nchunk = ceil_div(ncol, zc_r);
   if (!P.d_rho_part) {
     // band groups: enough CTAs for ~3 per resident slot, at most 8 partial copies of the grid
     P.rho_ng = std::max(1, std::min(8, ceil_div(3L * 148 * 3, nchunk)));
@@ -827,7 +836,7 @@ int ks_density_batch(HpsiPlan& P, const cplx* psi, const double* occ, int nb, in
     const size_t smem = rho_smem<N_>(P.L1);                                                             \
     if (smem > KS_SMEM_MAX) { err = "density kernel: tile + staging do not fit in shared memory"; return KS_ENOMEM; } \
     e = opt_in(k_rho<N_>, smem);                                                                        \
-    if (e == cudaSuccess) k_rho<N_><<<gr, xcfg<N_>::NT, smem, st>>>(r);                                 \
+    if (e == cudaSuccess) k_rho<N_><<<gr, nt_r, smem, st>>>(r);                                 \
   }
   KS_X_SIZES(C_)
 #undef C_
