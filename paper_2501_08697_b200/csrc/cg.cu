@@ -60,30 +60,62 @@ __global__ void k_cg_sub_x(int n, int nvec, const cplx* __restrict__ X, const cp
   }
   v[i] = cmake(re, im);
 }
-// up to three real parts of dot products in one launch (one CTA each): out[k] = Re <a_k | b_k>, weighted by w if given
+// up to three real parts of dot products in one launch: out[k] = Re <a_k | b_k>, weighted by w if given.
+// grid (CG_NB, count): CG_NB CTAs share one dot product, each writes its partial sum, and the CTA that arrives last adds
+// the partials in index order -- many CTAs' worth of loads in flight, and still one fixed summation order.
+#define CG_NB 32
 struct Dot3 { const cplx* a[3]; const cplx* b[3]; const double* w[3]; int out[3]; int count; };
-__global__ void __launch_bounds__(CG_T) k_cg_dot3(int n, Dot3 d, double* __restrict__ sc) {
-  const int k = blockIdx.x;
+__global__ void __launch_bounds__(CG_T) k_cg_dot3(int n, Dot3 d, double* __restrict__ sc, double* __restrict__ part,
+                                                  unsigned* __restrict__ ticket) {
+  const int k = blockIdx.y;
   const cplx *a = d.a[k], *b = d.b[k];
   const double* w = d.w[k];
   double re = 0;
-  for (int i = threadIdx.x; i < n; i += CG_T) {
+  for (int i = blockIdx.x * CG_T + threadIdx.x; i < n; i += CG_NB * CG_T) {
     const double t = a[i].x * b[i].x + a[i].y * b[i].y;
     re += w ? w[i] * t : t;
   }
   re = block_sum(re);
-  if (threadIdx.x == 0) sc[d.out[k]] = re;
+  __shared__ bool last;
+  if (threadIdx.x == 0) {
+    part[k * CG_NB + blockIdx.x] = re;
+    __threadfence();
+    last = (atomicAdd(&ticket[k], 1u) == CG_NB - 1);
+  }
+  __syncthreads();
+  if (last && threadIdx.x == 0) {
+    __threadfence();
+    double s = 0;
+    for (int j = 0; j < CG_NB; ++j) s += ((volatile double*)part)[k * CG_NB + j];
+    sc[d.out[k]] = s;
+    ticket[k] = 0;
+  }
 }
-// complex <x|d> -> sc[S_XD_RE], sc[S_XD_IM]
-__global__ void __launch_bounds__(CG_T) k_cg_cdot(int n, const cplx* __restrict__ x, const cplx* __restrict__ d, double* __restrict__ sc) {
+// complex <x|d> -> sc[S_XD_RE], sc[S_XD_IM]   (same scheme; partial slots 3 and 4)
+__global__ void __launch_bounds__(CG_T) k_cg_cdot(int n, const cplx* __restrict__ x, const cplx* __restrict__ d, double* __restrict__ sc,
+                                                  double* __restrict__ part, unsigned* __restrict__ ticket) {
   double re = 0, im = 0;
-  for (int i = threadIdx.x; i < n; i += CG_T) {
+  for (int i = blockIdx.x * CG_T + threadIdx.x; i < n; i += CG_NB * CG_T) {
     re += x[i].x * d[i].x + x[i].y * d[i].y;
     im += x[i].x * d[i].y - x[i].y * d[i].x;
   }
   re = block_sum(re);
   im = block_sum(im);
-  if (threadIdx.x == 0) { sc[S_XD_RE] = re; sc[S_XD_IM] = im; }
+  __shared__ bool last;
+  if (threadIdx.x == 0) {
+    part[3 * CG_NB + blockIdx.x] = re;
+    part[4 * CG_NB + blockIdx.x] = im;
+    __threadfence();
+    last = (atomicAdd(&ticket[3], 1u) == CG_NB - 1);
+  }
+  __syncthreads();
+  if (last && threadIdx.x == 0) {
+    __threadfence();
+    double sr = 0, si = 0;
+    for (int j = 0; j < CG_NB; ++j) { sr += ((volatile double*)part)[3 * CG_NB + j]; si += ((volatile double*)part)[4 * CG_NB + j]; }
+    sc[S_XD_RE] = sr; sc[S_XD_IM] = si;
+    ticket[3] = 0;
+  }
 }
 // g = K r, Teter-Payne-Allan with x = g2 / max(Ekin, 1e-3)
 __global__ void k_cg_precond(int n, const cplx* __restrict__ r, const double* __restrict__ g2, const double* __restrict__ sc,
@@ -151,8 +183,10 @@ __global__ void __launch_bounds__(CG_T) k_cg_resnorm(int n, const cplx* __restri
 
 struct CgBuf {     // freed on every exit path
   cplx *HX = nullptr, *X2 = nullptr, *HX2 = nullptr, *vec = nullptr, *s = nullptr, *Hc = nullptr, *Cm = nullptr;
-  double *sc = nullptr, *theta = nullptr, *rho = nullptr;
+  double *sc = nullptr, *theta = nullptr, *rho = nullptr, *part = nullptr;
+  unsigned* ticket = nullptr;
   ~CgBuf() {
+    cudaFree(part); cudaFree(ticket);
     cudaFree(HX); cudaFree(X2); cudaFree(HX2); cudaFree(vec); cudaFree(s); cudaFree(Hc); cudaFree(Cm);
     cudaFree(sc); cudaFree(theta); cudaFree(rho);
   }
@@ -174,6 +208,9 @@ int ks_cg_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int kmaxit
   KS_CUDA_CHECK(cudaMalloc(&w.Hc, sizeof(cplx) * (size_t)nb * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.Cm, sizeof(cplx) * (size_t)nb * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.sc, sizeof(double) * S_COUNT), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.part, sizeof(double) * 5 * CG_NB), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.ticket, sizeof(unsigned) * 4), c->err);
+  KS_CUDA_CHECK(cudaMemsetAsync(w.ticket, 0, sizeof(unsigned) * 4, st), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.theta, sizeof(double) * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.rho, sizeof(double) * nb), c->err);
   cplx *r = w.vec, *g = r + npw, *gp = g + npw, *d = gp + npw, *dn = d + npw, *h = dn + npw;
@@ -188,13 +225,13 @@ int ks_cg_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int kmaxit
     // psi_i = (I - sum_{j<i} |psi_j><psi_j|) psi_i (twice), normalised
     Dot3 dq;
     dq.count = 1; dq.a[0] = x; dq.b[0] = x; dq.w[0] = nullptr; dq.out[0] = S_DN2;
-    k_cg_dot3<<<1, CG_T, 0, st>>>(npw, dq, w.sc);
+    k_cg_dot3<<<dim3(CG_NB, 1), CG_T, 0, st>>>(npw, dq, w.sc, w.part, w.ticket);
     KS_CUDA_CHECK(cudaMemcpyAsync(&hs[0], w.sc + S_DN2, sizeof(double), cudaMemcpyDeviceToHost, st), c->err);
     for (int pass = 0; pass < 2 && i > 0; ++pass) {
       k_cg_dots_x<<<i, CG_T, 0, st>>>(npw, X, x, w.s);
       k_cg_sub_x<<<nblk, 256, 0, st>>>(npw, i, X, w.s, x);
     }
-    k_cg_dot3<<<1, CG_T, 0, st>>>(npw, dq, w.sc);
+    k_cg_dot3<<<dim3(CG_NB, 1), CG_T, 0, st>>>(npw, dq, w.sc, w.part, w.ticket);
     KS_CUDA_CHECK(cudaMemcpyAsync(&hs[1], w.sc + S_DN2, sizeof(double), cudaMemcpyDeviceToHost, st), c->err);
     KS_CUDA_CHECK(cudaStreamSynchronize(st), c->err);
     if (!(hs[1] > 1e-20 * hs[0]) || hs[0] == 0.0) { c->err = "ks_cg: start block is rank deficient"; return KS_EINVAL; }
@@ -205,7 +242,7 @@ int ks_cg_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int kmaxit
     Dot3 dl;
     dl.count = 2; dl.a[0] = x; dl.b[0] = p; dl.w[0] = nullptr; dl.out[0] = S_LAM;
     dl.a[1] = x; dl.b[1] = x; dl.w[1] = c->P.d_g2; dl.out[1] = S_EKIN;
-    k_cg_dot3<<<2, CG_T, 0, st>>>(npw, dl, w.sc);
+    k_cg_dot3<<<dim3(CG_NB, 2), CG_T, 0, st>>>(npw, dl, w.sc, w.part, w.ticket);
     bool conv = false;
     for (int k = 1; k <= kmaxiter; ++k) {
       // g = K (p - lambda psi) (Fig. 10: K acts on the plain residual); r = (I - P_{<=i}) (p - lambda psi)
@@ -216,7 +253,7 @@ int ks_cg_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int kmaxit
       k_cg_sub_x<<<nblk, 256, 0, st>>>(npw, i + 1, X, w.s, r);
       Dot3 dr;
       dr.count = 1; dr.a[0] = r; dr.b[0] = r; dr.w[0] = nullptr; dr.out[0] = S_R2;
-      k_cg_dot3<<<1, CG_T, 0, st>>>(npw, dr, w.sc);
+      k_cg_dot3<<<dim3(CG_NB, 1), CG_T, 0, st>>>(npw, dr, w.sc, w.part, w.ticket);
       KS_CUDA_CHECK(cudaMemcpyAsync(&hs[0], w.sc + S_R2, sizeof(double), cudaMemcpyDeviceToHost, st), c->err);
       KS_CUDA_CHECK(cudaStreamSynchronize(st), c->err);
       if (std::sqrt(hs[0]) <= 0.5 * tol) { conv = true; break; }
@@ -228,14 +265,14 @@ int ks_cg_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int kmaxit
       Dot3 dz;
       dz.count = 2; dz.a[0] = g; dz.b[0] = r; dz.w[0] = nullptr; dz.out[0] = S_ZETA;
       dz.a[1] = gp; dz.b[1] = r; dz.w[1] = nullptr; dz.out[1] = S_GPR;
-      k_cg_dot3<<<k > 1 ? 2 : 1, CG_T, 0, st>>>(npw, dz, w.sc);
+      k_cg_dot3<<<dim3(CG_NB, k > 1 ? 2 : 1), CG_T, 0, st>>>(npw, dz, w.sc, w.part, w.ticket);
       k_cg_dir<<<nblk, 256, 0, st>>>(npw, g, w.sc, k == 1, d);
       // dn = d - x <x|d>, normalised
-      k_cg_cdot<<<1, CG_T, 0, st>>>(npw, x, d, w.sc);
+      k_cg_cdot<<<CG_NB, CG_T, 0, st>>>(npw, x, d, w.sc, w.part, w.ticket);
       k_cg_orth<<<nblk, 256, 0, st>>>(npw, d, x, w.sc, dn);
       Dot3 dd;
       dd.count = 1; dd.a[0] = dn; dd.b[0] = dn; dd.w[0] = nullptr; dd.out[0] = S_DN2;
-      k_cg_dot3<<<1, CG_T, 0, st>>>(npw, dd, w.sc);
+      k_cg_dot3<<<dim3(CG_NB, 1), CG_T, 0, st>>>(npw, dd, w.sc, w.part, w.ticket);
       k_cg_scale<<<nblk, 256, 0, st>>>(npw, w.sc, dn);
       RC(ks_hpsi_impl(c, dn, h, 1));
       ++nh; ++steps;
@@ -243,9 +280,9 @@ int ks_cg_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int kmaxit
       Dot3 da;
       da.count = 2; da.a[0] = x; da.b[0] = h; da.w[0] = nullptr; da.out[0] = S_XH;
       da.a[1] = dn; da.b[1] = h; da.w[1] = nullptr; da.out[1] = S_DH;
-      k_cg_dot3<<<2, CG_T, 0, st>>>(npw, da, w.sc);
+      k_cg_dot3<<<dim3(CG_NB, 2), CG_T, 0, st>>>(npw, da, w.sc, w.part, w.ticket);
       k_cg_rotate<<<nblk, 256, 0, st>>>(npw, w.sc, x, p, dn, h);
-      k_cg_dot3<<<2, CG_T, 0, st>>>(npw, dl, w.sc);
+      k_cg_dot3<<<dim3(CG_NB, 2), CG_T, 0, st>>>(npw, dl, w.sc, w.part, w.ticket);
     }
     if (!conv) status = KS_NOTCONV;
   }

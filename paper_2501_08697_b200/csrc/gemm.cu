@@ -178,10 +178,98 @@ static int launch_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long l
   return KS_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// N <= 4 (one to four vectors: the band-by-band CG, the last Davidson iterations): matrix-vector forms that read A
+// once at memory speed instead of spending a 16/32-wide tensor tile on one column.  Fixed summation order.
+// ------------------------------------------------------------------------------------------------
+#define GEMV_T 256
+// C[m][n] = sum_k conj(A[k][m]) B[k][n]: one CTA per row m of A^H (column m of A), all N vectors at once
+template <int NV>
+__global__ void __launch_bounds__(GEMV_T) k_gemv_hn(int K, const cplx* __restrict__ A, long lda, const cplx* __restrict__ B, long ldb,
+                                                    cplx* __restrict__ C, long ldc) {
+  const cplx* a = A + (long)blockIdx.x * lda;
+  double re[NV], im[NV];
+#pragma unroll
+  for (int n = 0; n < NV; ++n) re[n] = im[n] = 0.0;
+  for (int k = threadIdx.x; k < K; k += GEMV_T) {
+    const cplx av = a[k];
+#pragma unroll
+    for (int n = 0; n < NV; ++n) {
+      const cplx bv = B[(long)n * ldb + k];
+      re[n] += av.x * bv.x + av.y * bv.y;
+      im[n] += av.x * bv.y - av.y * bv.x;
+    }
+  }
+  __shared__ double sh[2 * NV][GEMV_T / 32];
+#pragma unroll
+  for (int n = 0; n < NV; ++n) {
+    for (int o = 16; o > 0; o >>= 1) {
+      re[n] += __shfl_xor_sync(0xffffffffu, re[n], o);
+      im[n] += __shfl_xor_sync(0xffffffffu, im[n], o);
+    }
+    if ((threadIdx.x & 31) == 0) { sh[2 * n][threadIdx.x >> 5] = re[n]; sh[2 * n + 1][threadIdx.x >> 5] = im[n]; }
+  }
+  __syncthreads();
+  if (threadIdx.x < NV) {
+    double r = 0, i = 0;
+    for (int w = 0; w < GEMV_T / 32; ++w) { r += sh[2 * threadIdx.x][w]; i += sh[2 * threadIdx.x + 1][w]; }
+    C[(long)threadIdx.x * ldc + blockIdx.x] = cmake(r, i);
+  }
+}
+// C[m][n] (+)= sum_k A[m][k] B[k][n]: a CTA owns 32 rows; its 8 warps take every 8th k (32 rows x 16 B = one 512-byte
+// segment per load, 8 loads in flight per warp), partial sums meet in shared memory in a fixed order.  B (K x NV, tiny)
+// is read through the read-only cache.
+template <int NV>
+__global__ void __launch_bounds__(GEMV_T) k_gemv_nn(int M, int K, const cplx* __restrict__ A, long lda, const cplx* __restrict__ B, long ldb,
+                                                    cplx* __restrict__ C, long ldc, int accumulate) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int m = blockIdx.x * 32 + lane;
+  const bool ok = m < M;
+  double re[NV], im[NV];
+#pragma unroll
+  for (int n = 0; n < NV; ++n) re[n] = im[n] = 0.0;
+  const cplx* a = A + (ok ? m : 0);
+#pragma unroll 4
+  for (int k = w; k < K; k += GEMV_T / 32) {
+    const cplx av = a[(long)k * lda];
+#pragma unroll
+    for (int n = 0; n < NV; ++n) {
+      const cplx bv = __ldg(&B[(long)n * ldb + k]);
+      re[n] += av.x * bv.x - av.y * bv.y;
+      im[n] += av.x * bv.y + av.y * bv.x;
+    }
+  }
+  __shared__ double sh[GEMV_T / 32][2 * NV][32];
+#pragma unroll
+  for (int n = 0; n < NV; ++n) { sh[w][2 * n][lane] = re[n]; sh[w][2 * n + 1][lane] = im[n]; }
+  __syncthreads();
+  if (w == 0 && ok) {
+#pragma unroll
+    for (int n = 0; n < NV; ++n) {
+      double r = 0, i = 0;
+      for (int ww = 0; ww < GEMV_T / 32; ++ww) { r += sh[ww][2 * n][lane]; i += sh[ww][2 * n + 1][lane]; }
+      cplx* p = &C[(long)n * ldc + m];
+      cplx v = cmake(r, i);
+      if (accumulate) { const cplx o = *p; v.x += o.x; v.y += o.y; }
+      *p = v;
+    }
+  }
+}
+
 int ks_gemm_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
                long ldc, GemmWs* ws, std::string& err) {
   if (M <= 0 || N <= 0) return KS_OK;
   if (K < 0 || !ws) { err = "ks_gemm_hn: bad argument"; return KS_EINVAL; }
+  if (N <= 4 && K >= 1024) {
+    switch (N) {
+      case 1: k_gemv_hn<1><<<M, GEMV_T, 0, st>>>(K, A, lda, B, ldb, C, ldc); break;
+      case 2: k_gemv_hn<2><<<M, GEMV_T, 0, st>>>(K, A, lda, B, ldb, C, ldc); break;
+      case 3: k_gemv_hn<3><<<M, GEMV_T, 0, st>>>(K, A, lda, B, ldb, C, ldc); break;
+      default: k_gemv_hn<4><<<M, GEMV_T, 0, st>>>(K, A, lda, B, ldb, C, ldc); break;
+    }
+    KS_CUDA_CHECK(cudaGetLastError(), err);
+    return KS_OK;
+  }
   switch (pick_nj(N, 32)) {
     case 1: return launch_hn<1>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);
     case 2: return launch_hn<2>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);
@@ -302,6 +390,17 @@ int ks_gemm_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, co
                long ldc, int accumulate, std::string& err) {
   if (M <= 0 || N <= 0) return KS_OK;
   if (K < 0) { err = "ks_gemm_nn: bad argument"; return KS_EINVAL; }
+  if (N <= 4 && M >= 1024 && K >= 1) {
+    const int grid = ceil_div(M, 32);
+    switch (N) {
+      case 1: k_gemv_nn<1><<<grid, GEMV_T, 0, st>>>(M, K, A, lda, B, ldb, C, ldc, accumulate); break;
+      case 2: k_gemv_nn<2><<<grid, GEMV_T, 0, st>>>(M, K, A, lda, B, ldb, C, ldc, accumulate); break;
+      case 3: k_gemv_nn<3><<<grid, GEMV_T, 0, st>>>(M, K, A, lda, B, ldb, C, ldc, accumulate); break;
+      default: k_gemv_nn<4><<<grid, GEMV_T, 0, st>>>(M, K, A, lda, B, ldb, C, ldc, accumulate); break;
+    }
+    KS_CUDA_CHECK(cudaGetLastError(), err);
+    return KS_OK;
+  }
   switch (pick_nj(N, 16)) {
     case 1: return launch_nn<1>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
     case 2: return launch_nn<2>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);

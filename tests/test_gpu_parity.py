@@ -29,7 +29,8 @@ def _rel(a, b):
 
 
 # ------------------------------------------------------------------ building blocks (T1)
-@pytest.mark.parametrize("M,N,K", [(8, 8, 515), (160, 37, 1503), (70, 130, 4099), (1, 1, 1), (64, 64, 16), (5, 3, 0)])
+@pytest.mark.parametrize("M,N,K", [(8, 8, 515), (160, 37, 1503), (70, 130, 4099), (1, 1, 1), (64, 64, 16), (5, 3, 0),
+                                   (512, 1, 37073), (23, 2, 4099), (64, 3, 1503), (7, 4, 8459)])
 def test_zgemm_hn(ks, M, N, K):
     rng = np.random.default_rng(M * 1000 + N)
     A = rng.standard_normal((M, K)) + 1j * rng.standard_normal((M, K))
@@ -39,7 +40,8 @@ def test_zgemm_hn(ks, M, N, K):
     assert np.abs(Cm - ref).max() <= 1e-13 * max(1, K) ** 0.5 * (np.abs(ref).max() + 1)
 
 
-@pytest.mark.parametrize("M,N,K,acc", [(515, 8, 8, True), (1503, 23, 512, True), (4099, 70, 130, False), (1, 1, 1, False), (130, 65, 17, True)])
+@pytest.mark.parametrize("M,N,K,acc", [(515, 8, 8, True), (1503, 23, 512, True), (4099, 70, 130, False), (1, 1, 1, False), (130, 65, 17, True),
+                                       (37073, 1, 512, True), (4099, 2, 64, False), (1503, 3, 1728, True), (8459, 4, 1, True)])
 def test_zgemm_nn(ks, M, N, K, acc):
     rng = np.random.default_rng(M + N + K)
     A = rng.standard_normal((K, M)) + 1j * rng.standard_normal((K, M))
