@@ -21,6 +21,8 @@
 //                  waves -> 2 + 2 cos((G1-G2).r) closed form, non-negativity
 //   kso_chebyshev  U p(Lambda) U^H chi from numpy.linalg.eigh of the explicit H with p evaluated by
 //                  numpy.polynomial.chebyshev.chebval; T_n = cos(n arccos x) on an eigenvector; sqrt(Fermi-Dirac)
+//   kso_spsi / kso_explicit_s / kso_davidson_s   S rebuilt from its definition in numpy, scipy.linalg.eigh(H, S),
+//                  X^H S X = I, Q = 0 reduces to kso_davidson
 //   kso_cg         V=0: sorted |k+G|^2 exactly; numpy.linalg.eigvalsh of the explicit H; kso_davidson's eigenvalues;
 //                  residuals, orthonormality, Ritz values above the exact ones
 //   kso_davidson   V=0: sorted |k+G|^2 exactly; constant shift; brute-force Jacobi / eigvalsh of
@@ -171,6 +173,7 @@ struct kso_ctx {
   std::vector<int> off;         // [natom+1]
   std::vector<double> D;        // concatenated per-atom blocks
   std::vector<long> doff;       // offset of each atom's block in D
+  std::vector<double> Q;        // overlap blocks (same layout as D); empty: S = I
 };
 
 static inline int pmod(int a, int n) { int r = a % n; return r < 0 ? r + n : r; }
@@ -439,7 +442,8 @@ static inline double nrm2(const cplx* a, int n) {
 
 // Hc = V^H W (m x m), symmetrised, Jacobi; X = V C[:, :nb], HX = W C[:, :nb].
 static void rayleigh_ritz(int npw, int m, int nb, const std::vector<cplx>& V, const std::vector<cplx>& W,
-                          std::vector<cplx>& X, std::vector<cplx>& HX, std::vector<double>& eps) {
+                          std::vector<cplx>& X, std::vector<cplx>& HX, std::vector<double>& eps,
+                          const std::vector<cplx>* SV = nullptr, std::vector<cplx>* SX = nullptr) {
   std::vector<cplx> Hc((long)m * m), C((long)m * m);
   std::vector<double> th(m);
 #pragma omp parallel for collapse(2) schedule(static)
@@ -452,11 +456,13 @@ static void rayleigh_ritz(int npw, int m, int nb, const std::vector<cplx>& V, co
     }
   kso_jacobi(m, Hc.data(), th.data(), C.data());
   X.assign((long)nb * npw, cplx(0, 0)); HX.assign((long)nb * npw, cplx(0, 0));
+  if (SX) SX->assign((long)nb * npw, cplx(0, 0));
 #pragma omp parallel for schedule(static)
   for (int i = 0; i < nb; ++i)
     for (int r = 0; r < m; ++r) {
       caxpy(C[(long)r * m + i], &V[(long)r * npw], &X[(long)i * npw], npw);
       caxpy(C[(long)r * m + i], &W[(long)r * npw], &HX[(long)i * npw], npw);
+      if (SX) caxpy(C[(long)r * m + i], &(*SV)[(long)r * npw], &(*SX)[(long)i * npw], npw);   // S X = (S V) C
     }
   eps.assign(th.begin(), th.begin() + nb);
 }
@@ -659,6 +665,159 @@ extern "C" int kso_cg(const kso_ctx* c, cplx* psi, double* eig, int nb, double t
   }
   std::copy(X2.begin(), X2.end(), psi);
   if (steps_out) *steps_out = steps;
+  if (nhpsi_out) *nhpsi_out = nh;
+  return status;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Generalised problem H psi = eps S psi (ultrasoft pseudopotentials):
+//   S = 1 + sum_a sum_{p,p' in a} |beta_p> q^a_pp' <beta_p'|,  q^a real symmetric per atom (same layout as D).
+// kso_spsi applies S the way kso_hpsi applies the nonlocal term; kso_explicit_s is the definition; kso_davidson_s is
+// the listing of kso_davidson with every inner product taken in the S metric:
+//   X^H S X = I,  R_i = H X_i - eps_i S X_i,  T <- T - V ((S V)^H T),  T S-orthonormalised,  Hc = V^H H V (standard
+//   subspace problem because V^H S V = I).  Residual test: ||R_i||_2 <= tol.
+// ------------------------------------------------------------------------------------------------
+extern "C" int kso_set_overlap(kso_ctx* c, const double* Q) {
+  if (c->nproj == 0) return -1;
+  long o = 0;
+  for (int a = 0; a < c->natom; ++a) { const int np = c->off[a + 1] - c->off[a]; o += (long)np * np; }
+  c->Q.assign(Q, Q + o);
+  return 0;
+}
+
+extern "C" int kso_spsi(const kso_ctx* c, const cplx* psi, cplx* spsi, int nb) {
+  const int npw = c->npw;
+  std::copy(psi, psi + (long)nb * npw, spsi);
+  if (c->Q.empty()) return 0;
+  for (int b = 0; b < nb; ++b) {
+    const cplx* ps = psi + (long)b * npw;
+    cplx* out = spsi + (long)b * npw;
+    for (int a = 0; a < c->natom; ++a) {
+      const int p0 = c->off[a], np = c->off[a + 1] - p0;
+      const double* Qa = &c->Q[c->doff[a]];
+      std::vector<cplx> B(np), QB(np, cplx(0, 0));
+      for (int p = 0; p < np; ++p) B[p] = cdot(&c->beta[(long)(p0 + p) * npw], ps, npw);
+      for (int p = 0; p < np; ++p)
+        for (int q = 0; q < np; ++q) QB[p] += Qa[p * np + q] * B[q];
+      for (int p = 0; p < np; ++p) caxpy(QB[p], &c->beta[(long)(p0 + p) * npw], out, npw);
+    }
+  }
+  return 0;
+}
+
+extern "C" int kso_explicit_s(const kso_ctx* c, cplx* S) {
+  const int npw = c->npw;
+  for (int j = 0; j < npw; ++j)
+    for (int l = 0; l < npw; ++l) {
+      cplx sv = (j == l) ? cplx(1, 0) : cplx(0, 0);
+      for (int a = 0; a < c->natom && !c->Q.empty(); ++a) {
+        const int p0 = c->off[a], np = c->off[a + 1] - p0;
+        const double* Qa = &c->Q[c->doff[a]];
+        for (int p = 0; p < np; ++p)
+          for (int q = 0; q < np; ++q)
+            if (Qa[p * np + q] != 0.0)
+              sv += c->beta[(long)(p0 + p) * npw + j] * Qa[p * np + q] * std::conj(c->beta[(long)(p0 + q) * npw + l]);
+      }
+      S[(long)j * npw + l] = sv;
+    }
+  return 0;
+}
+
+// S-orthonormalise column t against basis vectors bv[0..nbv) (with their S images sb) by modified Gram-Schmidt, two
+// passes; returns the S-norm after the projections (t is then scaled to S-norm one and st = S t is returned).
+static double s_mgs(const kso_ctx* c, int npw, const std::vector<const cplx*>& bv, const std::vector<const cplx*>& sb, cplx* t,
+                    cplx* st) {
+  for (int pass = 0; pass < 2; ++pass)
+    for (size_t r = 0; r < bv.size(); ++r) caxpy(-cdot(sb[r], t, npw), bv[r], t, npw);
+  kso_spsi(c, t, st, 1);
+  const double n2 = cdot(t, st, npw).real();
+  const double n = std::sqrt(std::max(n2, 0.0));
+  if (n > 0)
+    for (int j = 0; j < npw; ++j) { t[j] /= n; st[j] /= n; }
+  return n;
+}
+
+extern "C" int kso_davidson_s(const kso_ctx* c, cplx* psi, double* eig, int nb, double tol, int max_iter, double* resid,
+                              int* iters_out, long long* nhpsi_out) {
+  const int npw = c->npw;
+  if (nb < 1 || nb > npw) return -1;
+  const int mmax = 2 * nb;
+  std::vector<cplx> X(psi, psi + (long)nb * npw), SX((long)nb * npw), HX, V, W, SV, R((long)nb * npw), T, ST;
+  std::vector<double> eps(nb), rho(nb);
+  // step 0: S-orthonormal start block
+  for (int i = 0; i < nb; ++i) {
+    std::vector<const cplx*> bv, sb;
+    for (int j = 0; j < i; ++j) { bv.push_back(&X[(long)j * npw]); sb.push_back(&SX[(long)j * npw]); }
+    const double n0 = nrm2(&X[(long)i * npw], npw);
+    const double n1 = s_mgs(c, npw, bv, sb, &X[(long)i * npw], &SX[(long)i * npw]);
+    if (!(n1 > 1e-10 * n0) || n0 == 0.0) return -3;
+  }
+  // step 1: Rayleigh-Ritz (V^H S V = I: standard subspace problem); S X rotates like H X
+  W.resize((long)nb * npw);
+  kso_hpsi(c, X.data(), W.data(), nb);
+  long long nh = nb;
+  V = X; SV = SX;
+  auto ritz = [&](int m) {
+    std::vector<cplx> X2, HX2, SX2;
+    rayleigh_ritz(npw, m, nb, V, W, X2, HX2, eps, &SV, &SX2);
+    X.swap(X2); HX.swap(HX2); SX.swap(SX2);
+  };
+  ritz(nb);
+  V = X; W = HX; SV = SX;
+  int m = nb, it = 0, status = 1;
+  for (;;) {
+    std::vector<int> U;
+    for (int i = 0; i < nb; ++i) {
+      for (int j = 0; j < npw; ++j) R[(long)i * npw + j] = HX[(long)i * npw + j] - eps[i] * SX[(long)i * npw + j];
+      rho[i] = nrm2(&R[(long)i * npw], npw);
+      if (rho[i] > tol) U.push_back(i);
+    }
+    int nu = (int)U.size();
+    if (nu == 0) { status = 0; break; }
+    if (it >= max_iter) break;
+    T.assign((long)nu * npw, cplx(0, 0));
+    ST.assign((long)nu * npw, cplx(0, 0));
+    std::vector<double> tn0(nu);
+    for (int u = 0; u < nu; ++u) {
+      const int i = U[u];
+      double ekin = 0;
+      for (int j = 0; j < npw; ++j) ekin += c->g2[j] * std::norm(X[(long)i * npw + j]);
+      ekin = std::max(ekin, 1e-3);
+      for (int j = 0; j < npw; ++j) {
+        const double x = c->g2[j] / ekin;
+        const double nx = 27.0 + 18.0 * x + 12.0 * x * x + 8.0 * x * x * x;
+        T[(long)u * npw + j] = (nx / (nx + 16.0 * x * x * x * x)) * R[(long)i * npw + j];
+      }
+      tn0[u] = nrm2(&T[(long)u * npw], npw);
+    }
+    if (m + nu > mmax) { V = X; W = HX; SV = SX; m = nb; }
+    int kept = 0;
+    for (int u = 0; u < nu; ++u) {
+      std::vector<const cplx*> bv, sb;
+      for (int r = 0; r < m; ++r) { bv.push_back(&V[(long)r * npw]); sb.push_back(&SV[(long)r * npw]); }
+      for (int r = 0; r < kept; ++r) { bv.push_back(&T[(long)r * npw]); sb.push_back(&ST[(long)r * npw]); }
+      std::vector<cplx> t(&T[(long)u * npw], &T[(long)u * npw] + npw), st(npw);
+      const double n1 = s_mgs(c, npw, bv, sb, t.data(), st.data());
+      if (!(n1 >= 1e-10 * tn0[u]) || tn0[u] == 0.0) continue;
+      std::copy(t.begin(), t.end(), &T[(long)kept * npw]);
+      std::copy(st.begin(), st.end(), &ST[(long)kept * npw]);
+      ++kept;
+    }
+    nu = kept;
+    if (nu == 0) break;
+    std::vector<cplx> HT((long)nu * npw);
+    kso_hpsi(c, T.data(), HT.data(), nu);
+    nh += nu;
+    V.insert(V.end(), T.begin(), T.begin() + (long)nu * npw);
+    SV.insert(SV.end(), ST.begin(), ST.begin() + (long)nu * npw);
+    W.insert(W.end(), HT.begin(), HT.end());
+    m += nu;
+    ritz(m);
+    ++it;
+  }
+  std::copy(X.begin(), X.end(), psi);
+  for (int i = 0; i < nb; ++i) { eig[i] = eps[i]; if (resid) resid[i] = rho[i]; }
+  if (iters_out) *iters_out = it;
   if (nhpsi_out) *nhpsi_out = nh;
   return status;
 }

@@ -42,6 +42,10 @@ def lib():
         _lib.kso_explicit_h.argtypes = [_vp, _vp]
         _lib.kso_density.argtypes = [_vp, _vp, _vp, C.c_int, _vp]
         _lib.kso_cg.argtypes = [_vp, _vp, _vp, C.c_int, C.c_double, C.c_int, _vp, _vp, _vp]
+        _lib.kso_set_overlap.argtypes = [_vp, _vp]
+        _lib.kso_spsi.argtypes = [_vp, _vp, _vp, C.c_int]
+        _lib.kso_explicit_s.argtypes = [_vp, _vp]
+        _lib.kso_davidson_s.argtypes = [_vp, _vp, _vp, C.c_int, C.c_double, C.c_int, _vp, _vp, _vp]
         _lib.kso_chebyshev.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, C.c_double, C.c_double, _vp]
         _lib.kso_jacobi.argtypes = [C.c_int, _vp, _vp, _vp]
         _lib.kso_fft3d.argtypes = [C.c_int, C.c_int, C.c_int, _vp, C.c_int]
@@ -173,6 +177,31 @@ class Oracle:
         rc = lib().kso_cg(self._h, _p(psi), _p(eig), nb, float(tol), int(kmaxiter), _p(res), C.byref(steps), C.byref(nh))
         assert rc >= 0, rc
         return dict(eig=eig, psi=psi, resid=res, steps=steps.value, band_applications=nh.value, converged=(rc == 0))
+
+    def set_overlap(self, Q: np.ndarray):
+        """S = 1 + sum_a beta_a q^a beta_a^H; Q: concatenated per-atom real symmetric blocks (layout of D)."""
+        Q = np.ascontiguousarray(Q, dtype=np.float64)
+        assert lib().kso_set_overlap(self._h, _p(Q)) == 0
+
+    def spsi(self, psi: np.ndarray) -> np.ndarray:
+        psi = np.ascontiguousarray(psi, dtype=np.complex128)
+        out = np.empty_like(psi)
+        assert lib().kso_spsi(self._h, _p(psi), _p(out), psi.shape[0]) == 0
+        return out
+
+    def explicit_s(self) -> np.ndarray:
+        S = np.empty((self.npw, self.npw), dtype=np.complex128)
+        lib().kso_explicit_s(self._h, _p(S))
+        return S
+
+    def davidson_s(self, psi0, tol=1e-8, max_iter=400):
+        psi = np.array(psi0, dtype=np.complex128, order="C")
+        nb = psi.shape[0]
+        eig = np.zeros(nb); res = np.zeros(nb)
+        it = C.c_int(0); nh = C.c_longlong(0)
+        rc = lib().kso_davidson_s(self._h, _p(psi), _p(eig), nb, float(tol), int(max_iter), _p(res), C.byref(it), C.byref(nh))
+        assert rc >= 0, rc
+        return dict(eig=eig, psi=psi, resid=res, iters=it.value, band_applications=nh.value, converged=(rc == 0))
 
     def explicit_h(self) -> np.ndarray:
         H = np.empty((self.npw, self.npw), dtype=np.complex128)

@@ -490,3 +490,51 @@ def test_full_symmetric_D_blocks_uneven_sizes(oracle_mod):
     assert np.abs(H - o0.explicit_h() - Hnl).max() < 1e-13
     got = o.hpsi(p.psi0)
     assert np.linalg.norm(got - p.psi0 @ H.T) <= 1e-13 * np.linalg.norm(got)
+
+
+# ----------------------------------------------------------------------------- generalised problem
+def _overlap_blocks(p, seed=3):
+    rng = np.random.default_rng(seed)
+    blocks = []
+    for a in range(len(p.proj_offset) - 1):
+        n = int(p.proj_offset[a + 1] - p.proj_offset[a])
+        m = rng.standard_normal((n, n))
+        blocks.append(0.3 * np.eye(n) + 0.05 * (m + m.T))
+    return blocks, np.concatenate([b.ravel() for b in blocks])
+
+
+@pytest.mark.parametrize("name", ["cfg0", "s2"])
+def test_generalised_problem_vs_scipy(oracle_mod, name):
+    """S = 1 + sum_a beta_a q^a beta_a^H (ultrasoft form): the explicit S equals its definition written
+    in numpy, S psi agrees with it, and the generalised Davidson reaches scipy.linalg.eigh(H, S) with X^H S X = I."""
+    import scipy.linalg
+    p = I.make_problem(0) if name == "cfg0" else I.make_shrunk(name)
+    o = oracle_mod.Oracle.from_problem(p)
+    blocks, Q = _overlap_blocks(p)
+    o.set_overlap(Q)
+    S = o.explicit_s()
+    want = np.eye(p.npw, dtype=complex)
+    for a, q in enumerate(blocks):
+        ba = p.beta[p.proj_offset[a]:p.proj_offset[a + 1]]
+        want += ba.T @ q @ ba.conj()
+    assert np.abs(S - want).max() < 1e-13
+    assert np.abs(o.spsi(p.psi0) - p.psi0 @ S.T).max() < 1e-12
+    w = scipy.linalg.eigh(o.explicit_h(), S, eigvals_only=True)
+    # the block must end at a gap of the GENERALISED spectrum (S moves the levels: s2's 10th level sits in a triplet
+    # 6e-5 Ry wide), as the shrunk variants do for the standard one
+    nb = 4 + int(np.argmax(np.diff(w[3:p.nbands + 1])))
+    r = o.davidson_s(p.psi0[:nb], tol=1e-8)
+    assert r["converged"] and np.abs(r["eig"] - w[:nb]).max() < 1e-10
+    X = r["psi"]
+    assert np.abs(X.conj() @ S @ X.T - np.eye(nb)).max() < 1e-11
+    res = np.linalg.norm(o.hpsi(X) - r["eig"][:, None] * o.spsi(X), axis=1)
+    assert res.max() <= 1e-8
+
+
+def test_generalised_problem_with_zero_q_is_the_standard_one(oracle_mod):
+    p = I.make_problem(0)
+    o = oracle_mod.Oracle.from_problem(p)
+    o.set_overlap(np.zeros(32))
+    r = o.davidson_s(p.psi0, tol=1e-8)
+    d = o.davidson(p.psi0, tol=1e-8)
+    assert np.abs(r["eig"] - d["eig"]).max() < 1e-12 and r["iters"] == d["iters"]
