@@ -80,6 +80,15 @@ int ks_density(ks_ctx* ctx, const ks_c128* psi, const double* occ, int nbands, d
 /* same through HOST buffers (copies inside, synchronises before returning) */
 int ks_density_host(ks_ctx* ctx, const ks_c128* psi_host, const double* occ_host, int nbands, double* rho_host);
 
+/* Generalised problem H psi = eps S psi (ultrasoft pseudopotentials):
+ *   S = 1 + sum_a sum_{p,p' in a} |beta_p> q^a_pp' <beta_p'|,   q^a real symmetric per atom.
+ * ks_set_overlap copies Q (HOST, concatenated per-atom blocks, the layout of D in ks_create); NULL restores S = I.
+ * With an overlap set, ks_davidson solves the generalised problem: the returned vectors satisfy X^H S X = I and the
+ * residuals are ||H x - eps S x||_2.  ks_hpsi, ks_density, ks_chebyshev and ks_cg are unaffected (they do not use S).
+ * ks_spsi: spsi = S psi for a block (DEVICE [nbands][npw], must not alias); a copy when S = I. */
+int ks_set_overlap(ks_ctx* ctx, const double* Q);
+int ks_spsi(ks_ctx* ctx, const ks_c128* psi, ks_c128* spsi, int nbands);
+
 /* Lowest nbands eigenpairs by the band-by-band preconditioned conjugate gradient of PAPER.md Fig. 10 (L549-570), the
  * eigensolver the paper prints; what the listing omits follows reading C19 of DESIGN.md
  * (K = Teter-Payne-Allan, gamma = Polak-Ribiere, theta = minimiser of the Rayleigh quotient, stop at ||r|| <= tol/2,

@@ -243,7 +243,7 @@ extern "C" void ks_destroy(ks_ctx* c) {
   cudaFree(P.d_plane_s0); cudaFree(P.d_plane_y0); cudaFree(P.d_stick);
   cudaFree(P.d_g2); cudaFree(P.d_vperm); cudaFree(P.d_planes); cudaFree(P.d_rho_part);
   for (int i = 0; i < 3; ++i) cudaFree(P.d_tw[i]);
-  cudaFree(c->d_beta); cudaFree(c->d_D); cudaFree(c->d_proj_atom); cudaFree(c->d_off); cudaFree(c->d_doff);
+  cudaFree(c->d_beta); cudaFree(c->d_D); cudaFree(c->d_Q); cudaFree(c->d_proj_atom); cudaFree(c->d_off); cudaFree(c->d_doff);
   cudaFree(c->d_B); cudaFree(c->d_DB); cudaFree(c->d_hin); cudaFree(c->d_hout);
   for (int i = 0; i < 3; ++i) cudaFree(c->d_cheb[i]);
   if (c->s_in) {
@@ -334,6 +334,57 @@ int ks_hpsi_impl(ks_ctx* c, const cplx* psi, cplx* hpsi, int nb) {
   }
   KS_CUDA_CHECK(cudaGetLastError(), c->err);
   return KS_OK;
+}
+
+// S psi = psi + beta q (beta^H psi); the same three kernels as the nonlocal term
+int ks_spsi_impl(ks_ctx* c, const cplx* psi, cplx* spsi, int nb) {
+  if (!c) return KS_EINVAL;
+  if (nb == 0) return KS_OK;
+  if (!psi || !spsi || nb < 0) { c->err = "ks_spsi: bad argument"; return KS_EINVAL; }
+  const HpsiPlan& P = c->P;
+  const size_t bytes = sizeof(cplx) * (size_t)nb * P.npw;
+  {
+    const char* a = (const char*)psi;
+    const char* b = (const char*)spsi;
+    if (a < b + bytes && b < a + bytes) { c->err = "ks_spsi: psi and spsi must not alias"; return KS_EINVAL; }
+  }
+  KS_CUDA_CHECK(cudaMemcpyAsync(spsi, psi, bytes, cudaMemcpyDeviceToDevice, c->stream), c->err);
+  if (!c->d_Q) return KS_OK;
+  if (nb > c->nl_cap) {
+    cudaFree(c->d_B); cudaFree(c->d_DB);
+    c->d_B = c->d_DB = nullptr; c->nl_cap = 0;
+    KS_CUDA_CHECK(cudaMalloc(&c->d_B, sizeof(cplx) * (size_t)c->nproj * nb), c->err);
+    KS_CUDA_CHECK(cudaMalloc(&c->d_DB, sizeof(cplx) * (size_t)c->nproj * nb), c->err);
+    c->nl_cap = nb;
+  }
+  int rc = ks_gemm_hn(c->stream, c->nproj, nb, P.npw, c->d_beta, P.npw, psi, P.npw, c->d_B, c->nproj, &c->gws, c->err);
+  if (rc) return rc;
+  k_apply_D<<<ceil_div((long)c->nproj * nb, 256), 256, 0, c->stream>>>(c->nproj, nb, c->d_B, c->d_DB, c->d_proj_atom, c->d_off,
+                                                                       c->d_doff, c->d_Q);
+  rc = ks_gemm_nn(c->stream, P.npw, nb, c->nproj, c->d_beta, P.npw, c->d_DB, c->nproj, spsi, P.npw, 1, c->err);
+  if (rc) return rc;
+  KS_CUDA_CHECK(cudaGetLastError(), c->err);
+  return KS_OK;
+}
+
+extern "C" int ks_set_overlap(ks_ctx* c, const double* Q) {
+  if (!c) return KS_EINVAL;
+  cudaStreamSynchronize(c->stream);
+  cudaFree(c->d_Q);
+  c->d_Q = nullptr;
+  if (!Q) return KS_OK;                       // back to S = I
+  if (c->nproj == 0) { c->err = "ks_set_overlap: the context has no projectors"; return KS_EINVAL; }
+  std::vector<int> off(c->natom + 1);
+  KS_CUDA_CHECK(cudaMemcpy(off.data(), c->d_off, sizeof(int) * (c->natom + 1), cudaMemcpyDeviceToHost), c->err);
+  size_t n = 0;
+  for (int a = 0; a < c->natom; ++a) n += (size_t)(off[a + 1] - off[a]) * (off[a + 1] - off[a]);
+  KS_CUDA_CHECK(cudaMalloc(&c->d_Q, sizeof(double) * n), c->err);
+  KS_CUDA_CHECK(cudaMemcpy(c->d_Q, Q, sizeof(double) * n, cudaMemcpyHostToDevice), c->err);
+  return KS_OK;
+}
+
+extern "C" int ks_spsi(ks_ctx* c, const ks_c128* psi, ks_c128* spsi, int nbands) {
+  return ks_spsi_impl(c, (const cplx*)psi, (cplx*)spsi, nbands);
 }
 
 // ---- per-kernel event timing (bench.py's roofline object) ----

@@ -7,6 +7,8 @@ struct DavidsonWs {
   cplx *V = nullptr, *W = nullptr;       // [2 nb][npw]
   cplx *X = nullptr, *HX = nullptr;      // [nb][npw]
   cplx *T = nullptr;                     // [nb][npw]
+  cplx *SV = nullptr, *SX = nullptr, *ST = nullptr;   // generalised problem only: S V [2nb], S X [nb], S T scratch [nb]
+  int s_cap = 0;
   cplx *Hc = nullptr, *Cm = nullptr;     // [2nb x 2nb] subspace matrix / eigenvectors (column-major)
   cplx *Hwork = nullptr;                 // [2nb x 2nb] copy destroyed by the eigensolver
   cplx *Cp = nullptr, *Cq = nullptr;     // [2nb x 2nb] eigenvectors of the previous iteration / of the rotated matrix
@@ -26,6 +28,7 @@ struct ks_ctx {
   int nproj = 0, natom = 0;
   cplx* d_beta = nullptr;        // [nproj][npw]
   double* d_D = nullptr;         // concatenated blocks
+  double* d_Q = nullptr;         // overlap blocks q^a (same layout); nullptr: S = I
   int* d_proj_atom = nullptr;    // [nproj]
   int* d_off = nullptr;          // [natom+1]
   long* d_doff = nullptr;        // [natom]
@@ -58,6 +61,7 @@ void ks_kprof_begin(ks_ctx* c, int phase, int launches);
 void ks_kprof_end(ks_ctx* c);
 
 int ks_hpsi_impl(ks_ctx* c, const cplx* psi, cplx* hpsi, int nb);
+int ks_spsi_impl(ks_ctx* c, const cplx* psi, cplx* spsi, int nb);   // S psi = psi + beta q (beta^H psi); a copy when S = I
 int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int max_iter, double* resid,
                      int* iters_out, long long* nhpsi_out);
 void ks_davidson_free(DavidsonWs* w);

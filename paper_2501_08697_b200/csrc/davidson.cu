@@ -40,18 +40,20 @@ __device__ __forceinline__ double block_sum(double v, double* sh) {
 }
 
 // D5: rho_i = ||HX_i - eps_i X_i||_2 , ekin_i = sum_G g2 |X_i|^2
-__global__ void __launch_bounds__(RED_THREADS) k_resid_norms(int npw, const cplx* __restrict__ X, const cplx* __restrict__ HX,
+__global__ void __launch_bounds__(RED_THREADS) k_resid_norms(int npw, const cplx* __restrict__ X, const cplx* __restrict__ SX,
+                                                             const cplx* __restrict__ HX,
                                                              const double* __restrict__ eps, const double* __restrict__ g2,
                                                              double* __restrict__ rho, double* __restrict__ ekin) {
   __shared__ double sh[RED_THREADS / 32];
   const int i = blockIdx.x;
   const cplx* x = X + (size_t)i * npw;
+  const cplx* sx = SX + (size_t)i * npw;       // = x when S = I
   const cplx* h = HX + (size_t)i * npw;
   const double e = eps[i];
   double r2 = 0, ek = 0;
   for (int j = threadIdx.x; j < npw; j += blockDim.x) {
-    const cplx a = x[j], b = h[j];
-    const double rx = b.x - e * a.x, ry = b.y - e * a.y;
+    const cplx a = x[j], s = sx[j], b = h[j];
+    const double rx = b.x - e * s.x, ry = b.y - e * s.y;
     r2 += rx * rx + ry * ry;
     ek += g2[j] * (a.x * a.x + a.y * a.y);
   }
@@ -62,7 +64,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_resid_norms(int npw, const cplx
 
 // D6: T_u = K_i (HX_i - eps_i X_i), i = idx[u];  K = n(x)/(n(x) + 16 x^4), n = 27 + 18x + 12x^2 + 8x^3,
 // x = g2 / max(ekin_i, 1e-3)   (Teter-Payne-Allan; reading C11)
-__global__ void k_precond(int npw, int nu, const int* __restrict__ idx, const cplx* __restrict__ X, const cplx* __restrict__ HX,
+__global__ void k_precond(int npw, int nu, const int* __restrict__ idx, const cplx* __restrict__ X /* S X when S != I */, const cplx* __restrict__ HX,
                           const double* __restrict__ eps, const double* __restrict__ ekin, const double* __restrict__ g2,
                           cplx* __restrict__ T) {
   const int u = blockIdx.y, i = idx[u];
@@ -295,6 +297,7 @@ __global__ void __launch_bounds__(128) k_trinv(int nu, const cplx* __restrict__ 
 void ks_davidson_free(DavidsonWs* w) {
   cudaFree(w->V); cudaFree(w->W); cudaFree(w->X); cudaFree(w->HX); cudaFree(w->T);
   cudaFree(w->Hc); cudaFree(w->Cm); cudaFree(w->Hwork); cudaFree(w->S); cudaFree(w->Us);
+  cudaFree(w->SV); cudaFree(w->SX); cudaFree(w->ST);
   cudaFree(w->Cp); cudaFree(w->Cq); cudaFree(w->thp); cudaFree(w->act); cudaFree(w->thf); cudaFree(w->lst); cudaFree(w->src);
   cudaFree(w->theta); cudaFree(w->rho); cudaFree(w->ekin); cudaFree(w->lam); cudaFree(w->idx);
   *w = DavidsonWs();
@@ -363,19 +366,24 @@ enum { PH_HPSI = 0, PH_PROJ = 1, PH_EIGH = 2, PH_ROT = 3, PH_RESID = 4, PH_ORTH 
 // unit column norms, Gram matrix G, Cholesky G = R^H R dropping columns whose remaining squared norm is
 // below 1e-12 of the original (norm ratio 1e-6; the Gram form cannot resolve the listing's 1e-10),
 // dst = src R_kept^{-1}.
-static int orth_pass(ks_ctx* c, cplx* src, int nu, cplx* dst, int m, int nproj_pass, int* nk_out, Phase& ph) {
+// Generalised problem (c->d_Q set): inner products in the S metric -- coefficients (S V)^H src, Gram matrix
+// src^H (S src) with S src from ks_spsi, and sdst = (S src) R_kept^{-1} = S dst comes out alongside dst.
+static int orth_pass(ks_ctx* c, cplx* src, int nu, cplx* dst, int m, int nproj_pass, int* nk_out, Phase& ph,
+                     cplx* sdst = nullptr) {
+  const bool gen = c->d_Q != nullptr;
   DavidsonWs& w = c->dws;
   const int npw = c->P.npw;
   cudaStream_t st = c->stream;
   ph.begin();
   for (int p = 0; p < nproj_pass && m > 0; ++p) {
-    RC(ks_gemm_hn(st, m, nu, npw, w.V, npw, src, npw, w.S, m, &c->gws, c->err));
+    RC(ks_gemm_hn(st, m, nu, npw, gen ? w.SV : w.V, npw, src, npw, w.S, m, &c->gws, c->err));
     k_negate<<<ceil_div((long)m * nu, 256), 256, 0, st>>>((long)m * nu, w.S);
     RC(ks_gemm_nn(st, npw, nu, m, w.V, npw, w.S, m, src, npw, 1, c->err));
   }
   k_col_norm2<<<nu, RED_THREADS, 0, st>>>(npw, src, w.lam);
   k_col_scale<<<dim3(std::max(1, std::min(64, ceil_div(npw, 1024))), nu), 256, 0, st>>>(npw, src, w.lam);
-  RC(ks_gemm_hn(st, nu, nu, npw, src, npw, src, npw, w.Us, nu, &c->gws, c->err));
+  if (gen) RC(ks_spsi_impl(c, src, w.ST, nu));
+  RC(ks_gemm_hn(st, nu, nu, npw, src, npw, gen ? w.ST : src, npw, w.Us, nu, &c->gws, c->err));
   ph.end(PH_ORTH);
   ph.begin();
   static bool opted = false;
@@ -393,6 +401,7 @@ static int orth_pass(ks_ctx* c, cplx* src, int nu, cplx* dst, int m, int nproj_p
   ph.end(PH_EIGH);
   ph.begin();
   RC(ks_gemm_nn(st, npw, nk, nu, src, npw, w.S, nu, dst, npw, 0, c->err));
+  if (gen && sdst) RC(ks_gemm_nn(st, npw, nk, nu, w.ST, npw, w.S, nu, sdst, npw, 0, c->err));
   ph.end(PH_ORTH);
   return KS_OK;
 }
@@ -406,6 +415,16 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
   DavidsonWs& w = c->dws;
   cudaStream_t st = c->stream;
   const size_t vb = sizeof(cplx) * (size_t)npw;
+  // generalised problem H x = eps S x (ks_set_overlap): S V, S X are carried next to H V, H X
+  const bool gen = c->d_Q != nullptr;
+  if (gen && w.s_cap < nb) {
+    cudaFree(w.SV); cudaFree(w.SX); cudaFree(w.ST);
+    w.SV = w.SX = w.ST = nullptr; w.s_cap = 0;
+    KS_CUDA_CHECK(cudaMalloc(&w.SV, vb * 2 * nb), c->err);
+    KS_CUDA_CHECK(cudaMalloc(&w.SX, vb * nb), c->err);
+    KS_CUDA_CHECK(cudaMalloc(&w.ST, vb * nb), c->err);
+    w.s_cap = nb;
+  }
   const long ldh = 2L * nb;
   Phase ph, tot;
   ph.init(st, c->prof_ms);
@@ -419,7 +438,7 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
   KS_CUDA_CHECK(cudaMemcpyAsync(w.T, psi, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
   RC(orth_pass(c, w.T, nb, w.X, 0, 0, &nk, ph));
   if (nk < nb) { c->err = "ks_davidson: start block is rank deficient"; return KS_EINVAL; }
-  RC(orth_pass(c, w.X, nb, w.V, 0, 0, &nk, ph));
+  RC(orth_pass(c, w.X, nb, w.V, 0, 0, &nk, ph, gen ? w.SV : nullptr));
   if (nk < nb) { c->err = "ks_davidson: start block is rank deficient"; return KS_EINVAL; }
   // D1-D4: initial Rayleigh-Ritz
   ph.begin();
@@ -435,8 +454,10 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
   ph.begin();
   RC(ks_gemm_nn(st, npw, nb, nb, w.V, npw, w.Cm, ldh, w.X, npw, 0, c->err));
   RC(ks_gemm_nn(st, npw, nb, nb, w.W, npw, w.Cm, ldh, w.HX, npw, 0, c->err));
+  if (gen) RC(ks_gemm_nn(st, npw, nb, nb, w.SV, npw, w.Cm, ldh, w.SX, npw, 0, c->err));
   KS_CUDA_CHECK(cudaMemcpyAsync(w.V, w.X, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
   KS_CUDA_CHECK(cudaMemcpyAsync(w.W, w.HX, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
+  if (gen) KS_CUDA_CHECK(cudaMemcpyAsync(w.SV, w.SX, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
   k_set_diag<<<ceil_div((long)nb * nb, 256), 256, 0, st>>>(nb, ldh, w.Hc, w.theta);
   ph.end(PH_ROT);
   // warm start of the subspace eigensolver (KSPW_WARM=0 switches it off): V = X, so C_prev = I, theta_prev = eps
@@ -461,13 +482,14 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
     const cplx* Cl = warm ? w.Cp : w.Cm;      // eigenvectors of the last eigensolve (after the end-of-iteration swap)
     RC(ks_gemm_nn(st, npw, nb, m, w.V, npw, Cl, ldh, w.X, npw, 0, c->err));
     RC(ks_gemm_nn(st, npw, nb, m, w.W, npw, Cl, ldh, w.HX, npw, 0, c->err));
+    if (gen) RC(ks_gemm_nn(st, npw, nb, m, w.SV, npw, Cl, ldh, w.SX, npw, 0, c->err));
     stale = false;
     return KS_OK;
   };
   for (;;) {
     // D5
     ph.begin();
-    k_resid_norms<<<nb, RED_THREADS, 0, st>>>(npw, w.X, w.HX, w.theta, c->P.d_g2, w.rho, w.ekin);
+    k_resid_norms<<<nb, RED_THREADS, 0, st>>>(npw, w.X, gen ? w.SX : w.X, w.HX, w.theta, c->P.d_g2, w.rho, w.ekin);
     KS_CUDA_CHECK(cudaMemcpyAsync(rho.data(), w.rho, sizeof(double) * nb, cudaMemcpyDeviceToHost, st), c->err);
     KS_CUDA_CHECK(cudaStreamSynchronize(st), c->err);
     ph.end(PH_RESID);
@@ -489,6 +511,7 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
       if (stale) { ph.begin(); RC(rotate_all()); ph.end(PH_ROT); }
       KS_CUDA_CHECK(cudaMemcpyAsync(w.V, w.X, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
       KS_CUDA_CHECK(cudaMemcpyAsync(w.W, w.HX, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
+      if (gen) KS_CUDA_CHECK(cudaMemcpyAsync(w.SV, w.SX, vb * nb, cudaMemcpyDeviceToDevice, st), c->err);
       k_set_diag<<<ceil_div((long)nb * nb, 256), 256, 0, st>>>(nb, ldh, w.Hc, w.theta);
       m = nb;
       if (warm) {   // V = X again: C_prev = I; theta_prev[0:nb] already holds eps
@@ -499,7 +522,7 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
     // D6
     ph.begin();
     KS_CUDA_CHECK(cudaMemcpyAsync(w.idx, idx.data(), sizeof(int) * nu, cudaMemcpyHostToDevice, st), c->err);
-    k_precond<<<dim3(std::max(1, std::min(64, ceil_div(npw, 1024))), nu), 256, 0, st>>>(npw, nu, w.idx, w.X, w.HX, w.theta, w.ekin,
+    k_precond<<<dim3(std::max(1, std::min(64, ceil_div(npw, 1024))), nu), 256, 0, st>>>(npw, nu, w.idx, gen ? w.SX : w.X, w.HX, w.theta, w.ekin,
                                                                                       c->P.d_g2, w.T);
     ph.end(PH_RESID);
     // D7: two passes; the result lands in V[m : m+nk]
@@ -508,7 +531,7 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
     RC(orth_pass(c, w.T, nu, Vnew, m, nproj_first, &nk, ph));
     if (nk == 0) break;
     int nk2 = 0;
-    RC(orth_pass(c, Vnew, nk, w.T, m, 1, &nk2, ph));
+    RC(orth_pass(c, Vnew, nk, w.T, m, 1, &nk2, ph, gen ? w.SV + (size_t)m * npw : nullptr));   // S V_new comes out of the second pass
     if (nk2 == 0) break;
     nk = nk2;
     KS_CUDA_CHECK(cudaMemcpyAsync(Vnew, w.T, vb * nk, cudaMemcpyDeviceToDevice, st), c->err);
@@ -578,6 +601,7 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
     if (!active_rot || 2 * nu > nb) {
       RC(ks_gemm_nn(st, npw, nb, m, w.V, npw, w.Cm, ldh, w.X, npw, 0, c->err));
       RC(ks_gemm_nn(st, npw, nb, m, w.W, npw, w.Cm, ldh, w.HX, npw, 0, c->err));
+      if (gen) RC(ks_gemm_nn(st, npw, nb, m, w.SV, npw, w.Cm, ldh, w.SX, npw, 0, c->err));
       stale = false;
     } else {
       // idx[0:nu] = the bands that were unconverged at this iteration's D5
@@ -588,6 +612,10 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
       k_scatter_bands<<<gs, 256, 0, st>>>(npw, nu, w.act, w.T, w.X);
       RC(ks_gemm_nn(st, npw, nu, m, w.W, npw, w.S, m, w.T, npw, 0, c->err));
       k_scatter_bands<<<gs, 256, 0, st>>>(npw, nu, w.act, w.T, w.HX);
+      if (gen) {
+        RC(ks_gemm_nn(st, npw, nu, m, w.SV, npw, w.S, m, w.T, npw, 0, c->err));
+        k_scatter_bands<<<gs, 256, 0, st>>>(npw, nu, w.act, w.T, w.SX);
+      }
       stale = true;
     }
     ph.end(PH_ROT);

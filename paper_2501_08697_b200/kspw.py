@@ -34,6 +34,8 @@ _lib.ks_hpsi.argtypes = [_vp, _vp, _vp, _i]
 _lib.ks_hpsi_host.argtypes = [_vp, _vp, _vp, _i]
 _lib.ks_density.argtypes = [_vp, _vp, _vp, _i, _vp]
 _lib.ks_density_host.argtypes = [_vp, _vp, _vp, _i, _vp]
+_lib.ks_set_overlap.argtypes = [_vp, _vp]
+_lib.ks_spsi.argtypes = [_vp, _vp, _vp, _i]
 _lib.ks_cg.argtypes = [_vp, _vp, _vp, _i, _d, _i, _vp, _vp, _vp]
 _lib.ks_chebyshev.argtypes = [_vp, _vp, _vp, _i, _i, _vp, _d, _d]
 _lib.ks_davidson.argtypes = [_vp, _vp, _vp, _i, _d, _i, _vp, _vp, _vp]
@@ -48,7 +50,7 @@ _lib.ks_dmma_peak.argtypes = [_vp, _vp]
 
 KS_OK, KS_NOTCONV = 0, 1
 EXPORTS = ("ks_pw_count", "ks_pw_list", "ks_create", "ks_destroy", "ks_npw", "ks_set_stream", "ks_set_fft_batch",
-           "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_density", "ks_density_host", "ks_chebyshev", "ks_cg", "ks_davidson", "ks_davidson_host",
+           "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_density", "ks_density_host", "ks_chebyshev", "ks_cg", "ks_set_overlap", "ks_spsi", "ks_davidson", "ks_davidson_host",
            "ks_davidson_profile", "ks_profile_begin", "ks_profile_end", "ks_zgemm_hn", "ks_zgemm_nn", "ks_eigh", "ks_dmma_peak")
 
 
@@ -214,6 +216,19 @@ class Context:
         rc = self._check(_lib.ks_davidson(self._h, _dev(psi), _dev(eig), nb, float(tol), int(max_iter), _dev(res),
                                           C.byref(it), C.byref(nh)))
         return dict(psi=psi, eig=eig, resid=res, iters=it.value, band_applications=nh.value, converged=(rc == 0))
+
+    def set_overlap(self, Q):
+        """S = 1 + sum_a beta_a q^a beta_a^H (Q: concatenated per-atom real symmetric blocks, layout of D); None: S = I."""
+        Q = None if Q is None else _np(Q, np.float64)
+        self._check(_lib.ks_set_overlap(self._h, _hp(Q)))
+
+    def spsi(self, psi, out=None):
+        import torch
+        assert psi.dtype == torch.complex128 and psi.dim() == 2 and psi.shape[1] == self.npw
+        if out is None:
+            out = torch.empty_like(psi)
+        self._check(_lib.ks_spsi(self._h, _dev(psi), _dev(out), int(psi.shape[0])))
+        return out
 
     def cg(self, psi, tol=1e-8, kmaxiter=200):
         """Band-by-band preconditioned CG (Fig. 10).  psi: torch complex128 CUDA [nbands][npw], overwritten.

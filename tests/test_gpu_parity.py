@@ -446,3 +446,46 @@ def test_cg_free_electron_and_not_converged(ks):
     ctx = ks.Context.from_problem(p)
     r = ctx.cg(_t(p.psi0), tol=1e-8, kmaxiter=2)
     assert not r["converged"] and r["steps"] == 2 * p.nbands
+
+
+# ------------------------------------------------------------------ generalised problem
+def _overlap_q(p, seed=3):
+    rng = np.random.default_rng(seed)
+    out = []
+    for a in range(len(p.proj_offset) - 1):
+        n = int(p.proj_offset[a + 1] - p.proj_offset[a])
+        m = rng.standard_normal((n, n))
+        out.append((0.3 * np.eye(n) + 0.05 * (m + m.T)).ravel())
+    return np.concatenate(out)
+
+
+@pytest.mark.parametrize("name", ["cfg0", "s2", "s4"])
+def test_generalised_davidson(ks, oracle_mod, name):
+    """H x = eps S x with S = 1 + sum_a beta_a q^a beta_a^H: S psi against the oracle, eigenvalues against
+    scipy.linalg.eigh(H, S) of the explicit matrices, X^H S X = I, residuals ||H x - eps S x|| re-evaluated with the
+    oracle's operators; the block ends at a gap of the generalised spectrum."""
+    import scipy.linalg
+    p = I.make_problem(0) if name == "cfg0" else I.make_shrunk(name)
+    Q = _overlap_q(p)
+    o = oracle_mod.Oracle.from_problem(p)
+    o.set_overlap(Q)
+    ctx = ks.Context.from_problem(p)
+    ctx.set_overlap(Q)
+    assert _rel(ctx.spsi(_t(p.psi0)).cpu().numpy(), o.spsi(p.psi0)) <= 1e-13
+    S = o.explicit_s()
+    w = scipy.linalg.eigh(o.explicit_h(), S, eigvals_only=True)
+    nb = 4 + int(np.argmax(np.diff(w[3:p.nbands + 1])))
+    r = ctx.davidson(_t(p.psi0[:nb].copy()), tol=1e-8)
+    assert r["converged"]
+    eig = r["eig"].cpu().numpy()
+    X = r["psi"].cpu().numpy()
+    assert np.abs(eig - w[:nb]).max() <= 1e-8
+    assert np.abs(X.conj() @ S @ X.T - np.eye(nb)).max() <= 1e-10
+    res = np.linalg.norm(o.hpsi(X) - eig[:, None] * o.spsi(X), axis=1)
+    assert res.max() <= 1.05e-8 and np.abs(res - r["resid"].cpu().numpy()).max() <= 1e-10
+    # S = I again: the standard problem, untouched
+    ctx.set_overlap(None)
+    o2 = oracle_mod.Oracle.from_problem(p)
+    w2 = np.linalg.eigvalsh(o2.explicit_h())
+    r2 = ctx.davidson(_t(p.psi0), tol=1e-8)
+    assert r2["converged"] and np.abs(r2["eig"].cpu().numpy() - w2[:p.nbands]).max() <= 1e-8
