@@ -96,22 +96,30 @@ static int upload(T** dst, const std::vector<T>& src, std::string& err) {
   return KS_OK;
 }
 
-static int alloc_planes(ks_ctx* c, int batch) {
-  HpsiPlan& P = c->P;
-  if (P.d_planes) { cudaFree(P.d_planes); P.d_planes = nullptr; P.batch_cap = 0; }
-  const size_t per = sizeof(cplx) * (size_t)P.L1 * P.n2 * P.n3;
-  KS_CUDA_CHECK(cudaMalloc(&P.d_planes, per * batch), c->err);
-  P.batch_cap = batch;
-  c->fft_batch = batch;
-  return KS_OK;
-}
-
+// Live-plane workspace: c->fft_batch is the batch LIMIT (bands per launch of the three FFT kernels); the buffer itself is
+// sized at first use to min(limit, bands actually applied) and grows when a larger block arrives, so a context that only
+// ever sees 32 bands does not hold gigabytes.
 static int auto_batch(const HpsiPlan& P) {
   const char* env = getenv("KSPW_FFT_BATCH");
   if (env && atoi(env) > 0) return atoi(env);
   const double per = 16.0 * P.L1 * P.n2 * P.n3;
-  int b = (int)(512.0e6 / per);    // several waves of CTAs per launch; the planes stream through HBM (L2 cannot hold a useful batch)
-  return std::max(2, std::min(b, 1024));
+  int b = (int)(2.0e9 / per);      // as many waves of CTAs per launch as 2 GB of planes allow (cfg 1: the whole 160-band
+  return std::max(2, std::min(b, 1024));   // block; measured 80 -> 160 bands: FFT path 51 -> 54 % of HBM); L2 cannot hold a useful batch
+}
+
+static int ensure_planes(ks_ctx* c, int nb) {
+  HpsiPlan& P = c->P;
+  const int want = std::min(c->fft_batch, std::max(nb, 1));
+  if (want <= P.batch_cap) return KS_OK;
+  if (P.d_planes) {
+    cudaStreamSynchronize(c->stream);
+    cudaFree(P.d_planes);
+    P.d_planes = nullptr; P.batch_cap = 0;
+  }
+  const size_t per = sizeof(cplx) * (size_t)P.L1 * P.n2 * P.n3;
+  KS_CUDA_CHECK(cudaMalloc(&P.d_planes, per * want), c->err);
+  P.batch_cap = want;
+  return KS_OK;
 }
 
 extern "C" void ks_destroy(ks_ctx* c);
@@ -190,7 +198,7 @@ static int create_impl(ks_ctx* c, const double* cell, const double* kf, double e
   if ((rc = ks_hpsi_configure(P, err))) return rc;
   KS_CUDA_CHECK(cudaMalloc(&P.d_vperm, sizeof(double) * P.N), err);
   if ((rc = ks_build_vperm(P, vloc, c->stream, err))) return rc;
-  if ((rc = alloc_planes(c, auto_batch(P)))) return rc;
+  c->fft_batch = auto_batch(P);
   // nonlocal part (Eq. 4)
   c->nproj = nproj; c->natom = natom;
   if (nproj > 0) {
@@ -267,7 +275,12 @@ extern "C" int ks_set_stream(ks_ctx* c, void* s) {
 extern "C" int ks_set_fft_batch(ks_ctx* c, int nbatch) {
   if (!c || nbatch < 0) return KS_EINVAL;
   cudaStreamSynchronize(c->stream);
-  return alloc_planes(c, nbatch > 0 ? nbatch : auto_batch(c->P));
+  c->fft_batch = nbatch > 0 ? nbatch : auto_batch(c->P);
+  if (c->P.d_planes && c->P.batch_cap > c->fft_batch) {      // shrink on request
+    cudaFree(c->P.d_planes);
+    c->P.d_planes = nullptr; c->P.batch_cap = 0;
+  }
+  return KS_OK;
 }
 extern "C" const char* ks_last_error(const ks_ctx* c) { return c ? c->err.c_str() : ks_global_error().c_str(); }
 
@@ -301,6 +314,10 @@ int ks_hpsi_impl(ks_ctx* c, const cplx* psi, cplx* hpsi, int nb) {
     const char* b = (const char*)hpsi;
     const size_t bytes = sizeof(cplx) * (size_t)nb * P.npw;
     if (a < b + bytes && b < a + bytes) { c->err = "ks_hpsi: psi and hpsi must not alias"; return KS_EINVAL; }
+  }
+  {
+    const int rc = ensure_planes(c, nb);
+    if (rc) return rc;
   }
   for (int b0 = 0; b0 < nb; b0 += c->fft_batch) {
     const int n = std::min(c->fft_batch, nb - b0);
@@ -492,6 +509,10 @@ extern "C" int ks_density(ks_ctx* c, const ks_c128* psi, const double* occ, int 
   if (nbands == 0) {
     KS_CUDA_CHECK(cudaMemsetAsync(rho, 0, sizeof(double) * P.N, c->stream), c->err);
     return KS_OK;
+  }
+  {
+    const int rc = ensure_planes(c, nbands);
+    if (rc) return rc;
   }
   for (int b0 = 0; b0 < nbands; b0 += c->fft_batch) {
     const int n = std::min(c->fft_batch, nbands - b0);
