@@ -160,10 +160,6 @@ __global__ void k_cg_rotate(int n, const double* __restrict__ sc, cplx* __restri
   x[i] = cmake(x[i].x * ct + dn[i].x * st, x[i].y * ct + dn[i].y * st);
   p[i] = cmake(p[i].x * ct + h[i].x * st, p[i].y * ct + h[i].y * st);
 }
-__global__ void k_cg_scale_by(int n, double f, cplx* __restrict__ v) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) v[i] = cmake(f * v[i].x, f * v[i].y);
-}
 __global__ void k_cg_shift_scalar(double* sc) { sc[S_ZETAP] = sc[S_ZETA]; }
 // closing residual norms: rho[b] = || HX_b - eps_b X_b ||
 __global__ void __launch_bounds__(CG_T) k_cg_resnorm(int n, const cplx* __restrict__ X, const cplx* __restrict__ HX,
