@@ -130,9 +130,9 @@ __device__ __forceinline__ cplx mul_tw(cplx a, const cplx* tw, int t) {
 
 // ---- type A ------------------------------------------------------------------------------------
 // line: pointer to element 0 of the line; es: element stride (in cplx); tw: n-entry table (smem).
-template <int N, int SIGN>
+template <int N, int SIGN, class F = fac<N>>
 __device__ __forceinline__ void lineA_stage1(cplx* line, int es, int j2, const cplx* tw) {
-  constexpr int R1 = fac<N>::R1, R2 = fac<N>::R2;
+  constexpr int R1 = F::R1, R2 = F::R2;
   cplx v[R1];
 #pragma unroll
   for (int j1 = 0; j1 < R1; ++j1) v[j1] = line[(j1 * R2 + j2) * es];
@@ -140,9 +140,9 @@ __device__ __forceinline__ void lineA_stage1(cplx* line, int es, int j2, const c
 #pragma unroll
   for (int k1 = 0; k1 < R1; ++k1) line[(k1 * R2 + j2) * es] = (k1 == 0) ? v[0] : mul_tw<SIGN>(v[k1], tw, j2 * k1);
 }
-template <int N, int SIGN>
+template <int N, int SIGN, class F = fac<N>>
 __device__ __forceinline__ void lineA_stage2(cplx* line, int es, int k1) {
-  constexpr int R2 = fac<N>::R2;
+  constexpr int R2 = F::R2;
   cplx v[R2];
 #pragma unroll
   for (int j2 = 0; j2 < R2; ++j2) v[j2] = line[(k1 * R2 + j2) * es];
@@ -151,9 +151,9 @@ __device__ __forceinline__ void lineA_stage2(cplx* line, int es, int k1) {
   for (int k2 = 0; k2 < R2; ++k2) line[(k1 * R2 + k2) * es] = v[k2];
 }
 // ---- type B ------------------------------------------------------------------------------------
-template <int N, int SIGN>
+template <int N, int SIGN, class F = fac<N>>
 __device__ __forceinline__ void lineB_stage1(cplx* line, int es, int k1, const cplx* tw) {
-  constexpr int R2 = fac<N>::R2;
+  constexpr int R2 = F::R2;
   cplx v[R2];
 #pragma unroll
   for (int k2 = 0; k2 < R2; ++k2) v[k2] = line[(k1 * R2 + k2) * es];
@@ -161,9 +161,9 @@ __device__ __forceinline__ void lineB_stage1(cplx* line, int es, int k1, const c
 #pragma unroll
   for (int q2 = 0; q2 < R2; ++q2) line[(k1 * R2 + q2) * es] = (q2 == 0) ? v[0] : mul_tw<SIGN>(v[q2], tw, k1 * q2);
 }
-template <int N, int SIGN>
+template <int N, int SIGN, class F = fac<N>>
 __device__ __forceinline__ void lineB_stage2(cplx* line, int es, int q2) {
-  constexpr int R1 = fac<N>::R1, R2 = fac<N>::R2;
+  constexpr int R1 = F::R1, R2 = F::R2;
   cplx v[R1];
 #pragma unroll
   for (int k1 = 0; k1 < R1; ++k1) v[k1] = line[(k1 * R2 + q2) * es];
@@ -171,6 +171,12 @@ __device__ __forceinline__ void lineB_stage2(cplx* line, int es, int q2) {
 #pragma unroll
   for (int q1 = 0; q1 < R1; ++q1) line[(q1 * R2 + q2) * es] = v[q1];
 }
+
+// z axis of the yz kernels (sticks): the split whose line counts fill 256 threads best.  96 = 16 x 6: a plane of S <= 41
+// sticks gives S*6 <= 246 DFT-16 lines (one round) and S*16 DFT-6 lines, instead of S*8 DFT-12 (two rounds, the second
+// nearly empty) and S*12 DFT-8.
+template <int N> struct facz : fac<N> {};
+template <> struct facz<96> { static constexpr int R1 = 16, R2 = 6; };
 
 // position -> natural index of a type-A output (host + device)
 __host__ __device__ __forceinline__ int perm_index(int p, int R1, int R2) { return p / R2 + R1 * (p % R2); }

@@ -45,10 +45,10 @@ cudaError_t ks_fft_init_constants() {
   X(16, 16) X(18, 18) X(24, 24) X(32, 32) X(36, 36) X(48, 48) X(54, 54) X(64, 64) X(72, 72) \
   X(96, 96) X(128, 128) X(18, 64) X(96, 288) X(20, 20) X(40, 40) X(60, 60) X(80, 80) X(100, 100) X(120, 120)
 
-void ks_fft_factors(int n, int* R1, int* R2) {
+void ks_fft_factors(int n, int* R1, int* R2, int axis) {
   *R1 = 0; *R2 = 0;
   switch (n) {
-#define C_(N_) case N_: *R1 = fac<N_>::R1; *R2 = fac<N_>::R2; break;
+#define C_(N_) case N_: *R1 = (axis == 2) ? facz<N_>::R1 : fac<N_>::R1; *R2 = (axis == 2) ? facz<N_>::R2 : fac<N_>::R2; break;
     C_(16) C_(18) C_(20) C_(24) C_(32) C_(36) C_(40) C_(48) C_(54) C_(60) C_(64) C_(72) C_(80) C_(96) C_(100) C_(120) C_(128) C_(144) C_(192) C_(256) C_(288)
 #undef C_
     default: break;
@@ -136,7 +136,7 @@ int ks_build_vperm(HpsiPlan& P, const cplx* vhat_host, cudaStream_t st, std::str
     std::swap(a, b);
   }
   int f[6];
-  for (int ax = 0; ax < 3; ++ax) ks_fft_factors(nn[ax], &f[2 * ax], &f[2 * ax + 1]);
+  for (int ax = 0; ax < 3; ++ax) ks_fft_factors(nn[ax], &f[2 * ax], &f[2 * ax + 1], ax);
   k_vperm<<<nblk, 256, 0, st>>>(a, P.d_vperm, P.n1, P.n2, P.n3, f[0], f[1], f[2], f[3], f[4], f[5], mx);
   double h[2];
   KS_CUDA_CHECK(cudaMemcpyAsync(h, mx, sizeof h, cudaMemcpyDeviceToHost, st), err);
@@ -214,7 +214,7 @@ struct StickWalk {
 
 template <int NY, int NZ>
 __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_inv_yz(YzArgs a) {
-  constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = fac<NZ>::R1, R2z = fac<NZ>::R2;
+  constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = facz<NZ>::R1, R2z = facz<NZ>::R2;
   constexpr int SZ = NZ | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
   extern __shared__ cplx sm[];
   cplx* tw_y = sm;
@@ -256,7 +256,7 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_inv_yz(YzArgs a) {
     }
   }
   __syncthreads();
-  for (StickWalk w(tid, NT, S); w.j < R1z; w.next()) lineA_stage2<NZ, +1>(stile + w.s * SZ, 1, w.j);
+  for (StickWalk w(tid, NT, S); w.j < R1z; w.next()) lineA_stage2<NZ, +1, facz<NZ>>(stile + w.s * SZ, 1, w.j);
   __syncthreads();
   // H2 (y): for each chunk of z' positions, type-A inverse FFT along y; output straight to HBM
   cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ);
@@ -297,7 +297,7 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_inv_yz(YzArgs a) {
 
 template <int NY, int NZ>
 __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_fwd_yz(YzArgs a) {
-  constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = fac<NZ>::R1, R2z = fac<NZ>::R2;
+  constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = facz<NZ>::R1, R2z = facz<NZ>::R2;
   constexpr int SZ = NZ | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
   extern __shared__ cplx sm[];
   cplx* tw_y = sm;
@@ -407,7 +407,7 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_fwd_yz(YzArgs a) {
   }
   }
   // H4 (z): type-B forward FFT on each stick
-  for (StickWalk w(tid, NT, S); w.j < R1z; w.next()) lineB_stage1<NZ, -1>(stile + w.s * SZ, 1, w.j, tw_z);
+  for (StickWalk w(tid, NT, S); w.j < R1z; w.next()) lineB_stage1<NZ, -1, facz<NZ>>(stile + w.s * SZ, 1, w.j, tw_z);
   __syncthreads();
   // last pass + H5: DFT-R1z, then hpsi = |k+G|^2 psi + (.)/N written straight to the stick's run of hpsi
   const cplx* psi = a.psi + (size_t)b * a.npw;
@@ -848,7 +848,7 @@ int ks_density_batch(HpsiPlan& P, const cplx* psi, const double* occ, int nb, in
 int ks_density_finish(const HpsiPlan& P, double* rho, cudaStream_t st, std::string& err) {
   int f[6];
   const int nn[3] = {P.n1, P.n2, P.n3};
-  for (int ax = 0; ax < 3; ++ax) ks_fft_factors(nn[ax], &f[2 * ax], &f[2 * ax + 1]);
+  for (int ax = 0; ax < 3; ++ax) ks_fft_factors(nn[ax], &f[2 * ax], &f[2 * ax + 1], ax);
   k_rho_finish<<<ceil_div(P.N, 256), 256, 0, st>>>(P.d_rho_part, P.rho_ng, rho, P.n1, P.n2, P.n3, f[0], f[1], f[2], f[3], f[4], f[5]);
   KS_CUDA_CHECK(cudaGetLastError(), err);
   return KS_OK;

@@ -30,7 +30,7 @@ struct HpsiPlan {
 bool ks_fft_size_supported(int n);
 bool ks_fft_yz_supported(int n2, int n3);
 int ks_fft_sizes(int* out, int cap);
-void ks_fft_factors(int n, int* R1, int* R2);
+void ks_fft_factors(int n, int* R1, int* R2, int axis = 0);   // axis 2 (z sticks) may use its own split
 cudaError_t ks_fft_init_constants();
 
 // V(r) = Re sum_m vhat[m] e^{+2 pi i m.j/n} on the device by a plain O(N n) DFT per axis (create time
