@@ -550,3 +550,21 @@ def test_davidson_large_configs_sampled(ks, oracle_mod, c):
     res = np.linalg.norm(o.hpsi(Xs) - eig[sel, None] * Xs, axis=1)
     assert res.max() <= 1.05e-8
     assert np.abs(res - r["resid"].cpu().numpy()[sel]).max() <= 1e-10
+
+
+def test_davidson_cfg1_vs_stored_oracle_solve(ks):
+    """cfg 1 at full size against the ORACLE's own Davidson solve of the same inputs, stored once by
+    tests/golden/make_oracle_davidson.py (minutes of CPU time): all 160 eigenvalues within north_star's 1e-8 Ry."""
+    import json, os
+    path = os.path.join(os.path.dirname(__file__), "golden", "oracle_davidson_cfg1.json")
+    if not os.path.exists(path):
+        pytest.skip("tests/golden/oracle_davidson_cfg1.json has not been generated")
+    g = json.load(open(path))
+    p = I.make_problem(1)
+    assert p.npw == g["npw"] and p.nbands == g["nbands"] and g["converged"]
+    r = ks.Context.from_problem(p).davidson(_t(p.psi0), tol=1e-8)
+    assert r["converged"]
+    assert np.abs(r["eig"].cpu().numpy() - np.array(g["eig"])).max() <= 1e-8
+    # same listing on both sides: iteration and band-application counts agree to a few per cent
+    assert abs(r["iters"] - g["iterations"]) <= 0.1 * g["iterations"]
+    assert abs(r["band_applications"] - g["band_applications"]) <= 0.1 * g["band_applications"]
