@@ -1,19 +1,25 @@
-// hpsi_kernels.cu -- the dual-space local part of H*psi (DESIGN.md steps H1-H5) as three kernels:
+// hpsi_kernels.cu -- the dual-space local part of H*psi (DESIGN.md steps H1-H5) as three kernels, and the density
+// build that reuses the first one and a half of them:
 //
-//   k_inv_yz  per (band, live x-plane): scatter the plane's G-sphere coefficients onto its z-sticks in
-//             shared memory (H1), inverse FFT along z on the sticks only, then along y for the plane
-//             (H2, pruned: PAPER.md Eq. 31, e^{+i}); writes the live plane [y'][z'] once.
-//   k_x       per (band, y', z'-chunk): inverse FFT along x from the live planes (zero fill in shared
-//             memory), multiply by V(r) (H3, Eq. 32), forward FFT along x, write the live planes
-//             back in place.  The full n1*n2*n3 cube never exists in HBM.
+//   k_inv_yz  per (band, live x-plane): the first z codelet pass reads each stick's contiguous run of psi straight
+//             from global memory (H1: no zero fill, no scatter pass), inverse FFT along z on the sticks only, then
+//             along y for the plane (H2, pruned: PAPER.md Eq. 31, e^{+i}); the last y pass writes the live plane
+//             [y'][z'] from registers.
+//   k_x       per (32 (y',z') columns, group of bands): inverse FFT along x from the live planes (dead rows are zeros
+//             in registers), multiply by V(r) (H3, Eq. 32), forward FFT along x, live planes written back in
+//             place from registers; the next band's live rows are prefetched by cp.async into the tile rows the same
+//             thread owns.  The full n1*n2*n3 cube never exists in HBM.
 //   k_fwd_yz  per (band, live x-plane): forward FFT along y, keep the stick columns, forward FFT along z
-//             (H4, Eq. 36, e^{-i} and 1/N), gather + kinetic term  hpsi = |k+G|^2 psi + (.)/N  (H5).
+//             (H4, Eq. 36, e^{-i} and 1/N); the last z pass writes hpsi = |k+G|^2 psi + (.)/N straight to the
+//             stick's run of hpsi (H5: gather and kinetic term fused).
+//   k_rho     the first half of k_x with occ |psi(r)|^2 accumulated over bands (ks_density).
 //
-// All intermediates are in "position" order (fft.cuh): type-A transforms leave their output
-// transposed, type-B transforms consume exactly that order, and V(r) is stored permuted once at
-// ks_create, so no reordering pass exists.  Thread mapping is lines-first: consecutive threads work
-// on consecutive lines, whose stride in shared memory is odd (or 1), so the 16-byte accesses of a
-// quarter-warp fall in distinct banks.
+// All intermediates are in "position" order (fft.cuh): type-A transforms leave their output transposed, type-B
+// transforms consume exactly that order, and V(r) is stored permuted once at ks_create, so no reordering pass exists.
+// A tile crosses shared memory only between codelet passes; thread t works on column t % ZC and codelet lines
+// t / ZC, t / ZC + G, ... (stick passes: lines-first over (stick, line) with an odd stick stride), so every
+// shared-memory offset is a compile-time multiple of the chunk width plus one per-thread base and the 16-byte accesses
+// of a quarter-warp fall in distinct banks.
 #include "fft.cuh"
 #include "plan.h"
 #include <algorithm>
