@@ -1,4 +1,5 @@
-// davidson.cu -- block Davidson for the lowest nbands eigenpairs of H psi = eps psi, S = I
+// davidson.cu -- block Davidson for the lowest nbands eigenpairs of H psi = eps psi (S = I), or of H psi = eps S psi when
+// ks_set_overlap gave an overlap (S V, S X carried next to H V, H X; S-metric projections and CholQR)
 // (DESIGN.md §3 listing, steps D0-D9; the paper names the method at PAPER.md L326, L547, L578 and prints
 // no listing; the residual p - lambda psi and the preconditioner K are Fig. 10, `vecdiv` L578).
 //
@@ -15,6 +16,9 @@
 //       T <- T R^{-1} ; twice (CholQR2)
 //   D8  V <- [V, T], restart V <- X when m + nu > 2 nb
 //   D9  psi <- X, eig, residuals
+// On top of the listing, none of which changes the converged pairs: D3 is warm-started in the basis of the
+// previous Ritz vectors, converged pairs are locked out of the subspace eigenproblem, and D4 rotates only the
+// unconverged bands (all bands before a restart and before returning).
 // Difference from the oracle listing (reading C10): the orthonormalisation is Gram/Cholesky based (CholQR2,
 // the BLAS-3 form of Gram-Schmidt, same column order and the same kind of drop rule) instead of modified
 // Gram-Schmidt.  Both span the same space; the converged pairs agree.

@@ -5,12 +5,15 @@
 //
 //   n <= 64   one CTA: A and the accumulated rotations V live in shared memory; every round applies
 //             n/2 disjoint complex Givens rotations (two-sided), n-1 rounds per sweep.
-//   n  > 64   two-sided BLOCK Jacobi with 32-wide blocks: every round solves nblk/2 independent 64x64
-//             pair problems with the one-CTA kernel (a few inner sweeps), then applies the 64x64
-//             unitary blocks U to the columns of A and V and the rows of A as 64x64x64 complex GEMM
-//             tiles on the FP64 tensor path (DMMA).
+//   n  > 64   two-sided BLOCK Jacobi with 16-wide blocks: every round solves nblk/2 independent 32x32 pair problems
+//             with the one-CTA solver (one inner sweep; after round 0 of an outer sweep only the pivots that couple the
+//             two blocks), then applies the 32x32 unitary blocks: one CTA per 32x32 tile computes U_a^H A U_b (or V U_b)
+//             in place (k_jac_upd32).  For n >= 512 one launch per round does both (k_jac_round32): the solver CTAs of
+//             the NEXT round rebuild their pair matrices from the old A and this round's U and run next to the tile
+//             CTAs (A double buffered).  (The older 64x64 pair / column + row DMMA kernels remain behind KSPW_JAC_PAIR=64.)
 // Rotation for pivot (p,q), a_pq = |a_pq| e^{i phi}:  J = diag(1, e^{-i phi}) [[c, s], [-s, c]],
-// tau = (a_qq - a_pp)/(2|a_pq|), t = sign(tau)/(|tau| + sqrt(1 + tau^2))  (same formula as the oracle).
+// tau = (a_qq - a_pp)/(2|a_pq|), t = sign(tau)/(|tau| + sqrt(1 + tau^2))  (the oracle's rotation, evaluated here in the
+// division-free form c = sqrt((1 + |d|/r)/2), sg = sign(d) a_pq/(2 r c), d = (a_qq - a_pp)/2, r = sqrt(d^2 + |a_pq|^2)).
 #include "mma.cuh"
 #include "plan.h"
 #include <algorithm>

@@ -7,6 +7,9 @@
 //   ks_gemm_nn:  C[M x N] (+)= A B  A: M x K, C: M x N column-major, M (= npw) long and contiguous.
 //                Used for hpsi += beta (D B) (H8), X = V C, HX = W C (D4), T -= V (V^H T) (D7).
 //
+// The N-tile width is a template parameter (NJ = 1..5 MMA tiles per warp) picked per call for the least padding of N;
+// N <= 4 takes matrix-vector kernels instead (k_gemv_hn / k_gemv_nn: A is read once at memory speed).
+//
 // A complex product is four real DMMAs on split re/im fragments:
 //   C_re += A_re B_re - A_im B_im ,  C_im += A_re B_im + A_im B_re     (signs folded into one negated
 // fragment; for A^H the imaginary part of A is negated instead).
