@@ -27,7 +27,7 @@ def main():
         "_citation": "oracle/kso.cpp kso_davidson (DESIGN.md §3 listing) on BASELINE config %d, k-point %d, seed %d, tol 1e-8; "
                      "written by tests/golden/make_oracle_davidson.py" % (c, k, 1000 + c),
         "config": c, "k_index": k, "npw": int(p.npw), "nbands": int(p.nbands),
-        "converged": bool(r["converged"]), "iterations": int(r["iters"]), "band_applications": int(r["band_applications"]),
+        "converged": bool(r["converged"]), "iterations": int(r["iters"]), "band_applications": int(r["nhpsi"]),
         "max_resid": float(r["resid"].max()), "wall_s": wall, "threads": kso.num_threads(),
         "eig": [float(x) for x in r["eig"]],
     }
