@@ -552,15 +552,16 @@ def test_davidson_large_configs_sampled(ks, oracle_mod, c):
     assert np.abs(res - r["resid"].cpu().numpy()[sel]).max() <= 1e-10
 
 
-def test_davidson_cfg1_vs_stored_oracle_solve(ks):
-    """cfg 1 at full size against the ORACLE's own Davidson solve of the same inputs, stored once by
-    tests/golden/make_oracle_davidson.py (minutes of CPU time): all 160 eigenvalues within north_star's 1e-8 Ry."""
+@pytest.mark.parametrize("c", [1, 4])
+def test_davidson_vs_stored_oracle_solve(ks, c):
+    """Full-size configs against the ORACLE's own Davidson solve of the same inputs, stored once by
+    tests/golden/make_oracle_davidson.py (minutes of CPU time): every eigenvalue within north_star's 1e-8 Ry."""
     import json, os
-    path = os.path.join(os.path.dirname(__file__), "golden", "oracle_davidson_cfg1.json")
+    path = os.path.join(os.path.dirname(__file__), "golden", "oracle_davidson_cfg%d.json" % c)
     if not os.path.exists(path):
-        pytest.skip("tests/golden/oracle_davidson_cfg1.json has not been generated")
+        pytest.skip("tests/golden/oracle_davidson_cfg%d.json has not been generated" % c)
     g = json.load(open(path))
-    p = I.make_problem(1)
+    p = I.make_problem(c)
     assert p.npw == g["npw"] and p.nbands == g["nbands"] and g["converged"]
     r = ks.Context.from_problem(p).davidson(_t(p.psi0), tol=1e-8)
     assert r["converged"]
