@@ -266,6 +266,124 @@ __global__ void __launch_bounds__(CHOL_THREADS) k_chol_drop(int n, cplx* __restr
   }
 }
 
+// Blocked form of the same factorisation (same column order, same drop rule, sums in a different order): panels of
+// CB columns; per panel one CTA factors the CB x CB diagonal block in shared memory, a row-panel kernel solves
+// R11^H R12 = G12 (one thread per trailing column), and a tiled rank-CB update takes R12^H R12 off the trailing
+// upper triangle.  A dropped column's row of R is zero, so the later panels skip it by arithmetic.  n = 520 (cfg 3):
+// 17 ms in the single-CTA kernel above, 51 short launches here.
+#define CB 32
+__global__ void __launch_bounds__(CB * CB) k_chol_diag(int n, int j0, cplx* __restrict__ G, long ld, double thr) {
+  __shared__ cplx D[CB][CB + 1];
+  __shared__ double s_inv;
+  __shared__ int s_keep;
+  const int i = threadIdx.x % CB, k = threadIdx.x / CB;     // D[i][k] = element (row j0+i, column j0+k), i <= k
+  const int w = min(CB, n - j0);
+  const bool in = (i <= k && k < w);
+  if (in) D[i][k] = G[(long)(j0 + k) * ld + j0 + i];
+  __syncthreads();
+  for (int j = 0; j < w; ++j) {
+    if (threadIdx.x == 0) {
+      const double d = D[j][j].x;
+      s_keep = (d > thr) ? 1 : 0;
+      const double r = s_keep ? sqrt(d) : 0.0;
+      D[j][j] = cmake(r, 0.0);                 // 0 marks the column as dropped
+      s_inv = s_keep ? 1.0 / r : 0.0;          // a dropped column's row of R becomes zero
+    }
+    __syncthreads();
+    if (i == j && k > j && k < w) D[j][k] = cscale(s_inv, D[j][k]);
+    __syncthreads();
+    if (in && i > j) {
+      const cplx a = D[j][i], b = D[j][k];
+      D[i][k].x -= a.x * b.x + a.y * b.y;
+      D[i][k].y -= a.x * b.y - a.y * b.x;
+    }
+    __syncthreads();
+  }
+  if (in) G[(long)(j0 + k) * ld + j0 + i] = D[i][k];
+}
+// R12 = R11^{-H} G12: thread per trailing column k, forward substitution in registers (right-looking)
+__global__ void __launch_bounds__(64) k_chol_trsm(int n, int j0, cplx* __restrict__ G, long ld) {
+  __shared__ cplx R[CB][CB + 1];
+  const int w = min(CB, n - j0);
+  for (int e = threadIdx.x; e < CB * CB; e += blockDim.x) {
+    const int i = e % CB, k = e / CB;
+    R[i][k] = (i <= k && k < w) ? G[(long)(j0 + k) * ld + j0 + i] : cmake(0.0, 0.0);
+  }
+  __syncthreads();
+  const int k = j0 + w + blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  cplx* col = G + (long)k * ld + j0;
+  cplx x[CB];
+#pragma unroll
+  for (int j = 0; j < CB; ++j) x[j] = (j < w) ? col[j] : cmake(0.0, 0.0);
+#pragma unroll
+  for (int j = 0; j < CB; ++j) {
+    const double d = R[j][j].x;
+    const double inv = (d > 0.0) ? 1.0 / d : 0.0;
+    x[j] = cscale(inv, x[j]);
+#pragma unroll
+    for (int q = j + 1; q < CB; ++q) {        // x_q -= conj(R[j][q]) x_j
+      const cplx r = R[j][q];
+      x[q].x -= r.x * x[j].x + r.y * x[j].y;
+      x[q].y -= r.x * x[j].y - r.y * x[j].x;
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < CB; ++j)
+    if (j < w) col[j] = x[j];
+}
+// trailing update of the upper triangle: G[i][k] -= sum_j conj(R[j][i]) R[j][k], j in the panel, j0+w <= i <= k < n
+__global__ void __launch_bounds__(256) k_chol_update(int n, int j0, cplx* __restrict__ G, long ld) {
+  if (blockIdx.x > blockIdx.y) return;        // tiles below the diagonal
+  __shared__ cplx Pi[CB][CB + 1], Pk[CB][CB + 1];          // [column in tile][panel row]
+  const int w = min(CB, n - j0), t0 = j0 + w;
+  const int i0 = t0 + blockIdx.x * CB, k0 = t0 + blockIdx.y * CB;
+  for (int e = threadIdx.x; e < CB * CB; e += 256) {
+    const int j = e % CB, cidx = e / CB;
+    Pi[cidx][j] = (j < w && i0 + cidx < n) ? G[(long)(i0 + cidx) * ld + j0 + j] : cmake(0.0, 0.0);
+    Pk[cidx][j] = (j < w && k0 + cidx < n) ? G[(long)(k0 + cidx) * ld + j0 + j] : cmake(0.0, 0.0);
+  }
+  __syncthreads();
+  const int ii = threadIdx.x % CB;
+  for (int kk = threadIdx.x / CB; kk < CB; kk += 256 / CB) {
+    const int gi = i0 + ii, gk = k0 + kk;
+    if (gi > gk || gk >= n) continue;
+    double sr = 0.0, si = 0.0;
+#pragma unroll
+    for (int j = 0; j < CB; ++j) {
+      const cplx a = Pi[ii][j], b = Pk[kk][j];
+      sr += a.x * b.x + a.y * b.y;
+      si += a.x * b.y - a.y * b.x;
+    }
+    cplx* g = G + (long)gk * ld + gi;
+    g->x -= sr;
+    g->y -= si;
+  }
+}
+__global__ void __launch_bounds__(256) k_chol_kept(int n, const cplx* __restrict__ G, long ld, int* __restrict__ kept,
+                                                  int* __restrict__ nk_out) {
+  extern __shared__ int s_flag[];
+  for (int j = threadIdx.x; j < n; j += blockDim.x) s_flag[j] = G[(long)j * ld + j].x > 0.0;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int nk = 0;
+    for (int j = 0; j < n; ++j)
+      if (s_flag[j]) kept[nk++] = j;
+    *nk_out = nk;
+  }
+}
+static void chol_drop_blocked(cudaStream_t st, int n, cplx* G, long ld, double thr, int* kept, int* nk_out) {
+  for (int j0 = 0; j0 < n; j0 += CB) {
+    k_chol_diag<<<1, CB * CB, 0, st>>>(n, j0, G, ld, thr);
+    const int m = n - j0 - CB;                 // trailing columns
+    if (m <= 0) break;
+    k_chol_trsm<<<ceil_div(m, 64), 64, 0, st>>>(n, j0, G, ld);
+    const int nt = ceil_div(m, CB);
+    k_chol_update<<<dim3(nt, nt), 256, 0, st>>>(n, j0, G, ld);
+  }
+  k_chol_kept<<<1, 256, sizeof(int) * n, st>>>(n, G, ld, kept, nk_out);
+}
+
 // one warp per kept column jj: x = R_kept^{-1} e_jj by back substitution; M[:, jj] (nu rows) = scatter(x)
 __global__ void __launch_bounds__(128) k_trinv(int nu, const cplx* __restrict__ R, long ld, const int* __restrict__ kept, int nk,
                                                cplx* __restrict__ M, long ldm) {
@@ -395,7 +513,9 @@ static int orth_pass(ks_ctx* c, cplx* src, int nu, cplx* dst, int m, int nproj_p
     KS_CUDA_CHECK(cudaFuncSetAttribute(k_trinv, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 16 * 2048), c->err);
     opted = true;
   }
-  k_chol_drop<<<1, CHOL_THREADS, sizeof(cplx) * nu, st>>>(nu, w.Us, nu, 1e-12, w.idx, w.idx + nu);
+  static const bool chol_blocked = !(getenv("KSPW_CHOL_BLOCKED") && atoi(getenv("KSPW_CHOL_BLOCKED")) == 0);
+  if (chol_blocked) chol_drop_blocked(st, nu, w.Us, nu, 1e-12, w.idx, w.idx + nu);
+  else k_chol_drop<<<1, CHOL_THREADS, sizeof(cplx) * nu, st>>>(nu, w.Us, nu, 1e-12, w.idx, w.idx + nu);
   int nk = 0;
   KS_CUDA_CHECK(cudaMemcpyAsync(&nk, w.idx + nu, sizeof(int), cudaMemcpyDeviceToHost, st), c->err);
   KS_CUDA_CHECK(cudaStreamSynchronize(st), c->err);
