@@ -26,6 +26,8 @@
 #include <cmath>
 #include <cstdlib>
 #include <vector>
+#include <cooperative_groups.h>
+namespace cg = cooperative_groups;
 
 
 cudaError_t ks_fft_init_constants() {
@@ -187,9 +189,23 @@ constexpr int yz_pick_zc(int nz) {
 }
 // DBF: the forward kernel splits the y tile into two half-width buffers filled by cp.async one chunk ahead (pays
 // when two CTAs fit per SM; measured: 96x96 213 -> 201 us; 128x128 224 -> 254 us and 96x288 337 -> 376 us, where one CTA fills the SM: off there)
-template <int NY, int NZ> struct yzcfg { static constexpr int ZC = yz_pick_zc(NZ), NT = 256; static constexpr bool DBF = (ZC % 2 == 0); };
-template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 512; static constexpr bool DBF = false; };
-template <> struct yzcfg<96, 288> { static constexpr int ZC = 16, NT = 256; static constexpr bool DBF = false; };
+// ZS > 1: the z' positions of a plane are split over ZS CTAs (blockIdx.x = lx * ZS + h).  Position p = k1 * R2z + k2, so
+// CTA h owns the codelet lines k1 in [h, h + 1) * R1z / ZS and holds only that part of every stick: the stick tile shrinks by
+// ZS and two CTAs fit per SM where the whole plane's sticks filled it (128 x 128: 126 KB, 96 x 288: 190 KB of sticks).
+// The inverse kernel repeats the first z codelet pass in every CTA of the plane (it needs no exchange); the forward kernel's
+// last z pass needs all k1, so its ZS CTAs form a thread-block cluster and read each other's stick tiles through
+// distributed shared memory.
+template <int NY, int NZ> struct yzcfg { static constexpr int ZC = yz_pick_zc(NZ), NT = 256, ZS = 1; static constexpr bool DBF = (ZC % 2 == 0); };
+#ifdef KSPW_ZSPLIT128   // measured on cfg 3: k_inv_yz unchanged (0.589 ms), k_fwd_yz slower (0.712 -> 0.843 ms): off
+template <> struct yzcfg<128, 128> { static constexpr int ZC = 16, NT = 256, ZS = 2; static constexpr bool DBF = false; };
+#else
+template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 512, ZS = 1; static constexpr bool DBF = false; };
+#endif
+#ifndef KSPW_NO_ZSPLIT288
+template <> struct yzcfg<96, 288> { static constexpr int ZC = 16, NT = 256, ZS = 3; static constexpr bool DBF = false; };
+#else
+template <> struct yzcfg<96, 288> { static constexpr int ZC = 16, NT = 256, ZS = 1; static constexpr bool DBF = false; };
+#endif
 
 // 16-byte global -> shared async copy (LDGSTS), ordered against the surrounding shared-memory accesses
 __device__ __forceinline__ void cp16m(cplx* smem, const cplx* gmem) {
@@ -219,16 +235,18 @@ struct StickWalk {
 };
 
 template <int NY, int NZ>
-__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_inv_yz(YzArgs a) {
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 1) k_inv_yz(YzArgs a) {
   constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = facz<NZ>::R1, R2z = facz<NZ>::R2;
-  constexpr int SZ = NZ | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
+  constexpr int ZS = yzcfg<NY, NZ>::ZS, NZH = NZ / ZS, K1H = R1z / ZS;   // this CTA's z' positions and codelet lines
+  static_assert(R1z % ZS == 0 && NZH % yzcfg<NY, NZ>::ZC == 0, "z' split must cut between codelet lines and chunks");
+  constexpr int SZ = NZH | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
   extern __shared__ cplx sm[];
   cplx* tw_y = sm;
   cplx* tw_z = (NY == NZ) ? tw_y : tw_y + NY;     // equal lengths share one twiddle table
   cplx* stile = tw_z + NZ;
   cplx* ytile = stile + (size_t)a.smax * SZ;
   const int tid = threadIdx.x;
-  const int lx = blockIdx.x, b = blockIdx.y;
+  const int lx = blockIdx.x / ZS, h = blockIdx.x % ZS, b = blockIdx.y;
   const int s0 = a.plane_s0[lx], S = a.plane_s0[lx + 1] - s0;
   const int y0 = a.plane_y0[lx];
   const cplx* psi = a.psi + (size_t)b * a.npw;
@@ -256,18 +274,19 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_inv_yz(YzArgs a) {
       cplx* o = stile + w.s * SZ + w.j;
       const int j2 = w.j;
 #pragma unroll
-      for (int k1 = 0; k1 < R1z; ++k1) o[k1 * R2z] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw_z, j2 * k1);
+      for (int k1 = 0; k1 < R1z; ++k1)
+        if (ZS == 1 || k1 / K1H == h) o[(k1 % K1H) * R2z] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw_z, j2 * k1);
       w.next();
       if (w.j < R2z) load_in();
     }
   }
   __syncthreads();
-  for (StickWalk w(tid, NT, S); w.j < R1z; w.next()) lineA_stage2<NZ, +1, facz<NZ>>(stile + w.s * SZ, 1, w.j);
+  for (StickWalk w(tid, NT, S); w.j < K1H; w.next()) lineA_stage2<NZ, +1, facz<NZ>>(stile + w.s * SZ, 1, w.j);
   __syncthreads();
   // H2 (y): for each chunk of z' positions, type-A inverse FFT along y; output straight to HBM
-  cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ);
+  cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ) + h * NZH;
   const int pz = tid % ZC, g = tid / ZC;
-  for (int c = 0; c < NZ / ZC; ++c) {
+  for (int c = 0; c < NZH / ZC; ++c) {
     if (g < G) {
       for (int j2 = g; j2 < R2y; j2 += G) {
         cplx v[R1y];
@@ -302,19 +321,21 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_inv_yz(YzArgs a) {
 }
 
 template <int NY, int NZ>
-__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_fwd_yz(YzArgs a) {
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 1) k_fwd_yz(YzArgs a) {
   constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = facz<NZ>::R1, R2z = facz<NZ>::R2;
-  constexpr int SZ = NZ | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
+  constexpr int ZS = yzcfg<NY, NZ>::ZS, NZH = NZ / ZS, K1H = R1z / ZS;   // this CTA's z' positions and codelet lines
+  static_assert(ZS == 1 || !yzcfg<NY, NZ>::DBF, "the z' split uses the single-buffer y transform");
+  constexpr int SZ = NZH | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
   extern __shared__ cplx sm[];
   cplx* tw_y = sm;
   cplx* tw_z = (NY == NZ) ? tw_y : tw_y + NY;     // equal lengths share one twiddle table
   cplx* stile = tw_z + NZ;
   cplx* ytile = stile + (size_t)a.smax * SZ;
   const int tid = threadIdx.x;
-  const int lx = blockIdx.x, b = blockIdx.y;
+  const int lx = blockIdx.x / ZS, h = blockIdx.x % ZS, b = blockIdx.y;   // h = rank in the cluster of ZS CTAs
   const int s0 = a.plane_s0[lx], S = a.plane_s0[lx + 1] - s0;
   const int y0 = a.plane_y0[lx];
-  const cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ);
+  const cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ) + h * NZH;
   const int pz = tid % ZC, g = tid / ZC;
   // H4 (y), type B, forward.  The y tile is split into two half-width buffers: while chunk c (ZF = ZC/2 columns) is
   // transformed in place in one of them, chunk c+1 streams into the other by cp.async, so the plane loads are
@@ -381,10 +402,10 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_fwd_yz(YzArgs a) {
     if (NY != NZ)
       for (int i = tid; i < NZ; i += NT) tw_z[i] = a.tw_z[i];
     __syncthreads();
-    for (int c = 0; c < NZ / ZC; ++c) {
+    for (int c = 0; c < NZH / ZC; ++c) {
       if (g < G) {
         for (int k1 = g; k1 < R1y; k1 += G) {
-          if (k1 != g || c != 0) load_in(v, c, k1);
+          if (k1 != g) load_in(v, c, k1);          // the thread's first line of a chunk is already in registers
           dft<R2y, -1>(v);
           cplx* o = ytile + k1 * R2y * ZC + pz;
 #pragma unroll
@@ -392,6 +413,7 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_fwd_yz(YzArgs a) {
         }
       }
       __syncthreads();
+      if (g < G && g < R1y && c + 1 < NZH / ZC) load_in(v, c + 1, g);   // next chunk's loads fly during pass 2
       if (g < G) {
         for (int q2 = g; q2 < R2y; q2 += G) {
           cplx u[R1y];
@@ -413,29 +435,69 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT) k_fwd_yz(YzArgs a) {
   }
   }
   // H4 (z): type-B forward FFT on each stick
-  for (StickWalk w(tid, NT, S); w.j < R1z; w.next()) lineB_stage1<NZ, -1, facz<NZ>>(stile + w.s * SZ, 1, w.j, tw_z);
-  __syncthreads();
-  // last pass + H5: DFT-R1z, then hpsi = |k+G|^2 psi + (.)/N written straight to the stick's run of hpsi
   const cplx* psi = a.psi + (size_t)b * a.npw;
   cplx* hpsi = a.hpsi + (size_t)b * a.npw;
-  for (StickWalk w(tid, NT, S); w.j < R2z; w.next()) {
-    const int4 si = __ldg(a.stick + s0 + w.s);
-    cplx v[R1z];
-    const cplx* t = stile + w.s * SZ + w.j;
+  if constexpr (ZS == 1) {
+    for (StickWalk w(tid, NT, S); w.j < R1z; w.next()) lineB_stage1<NZ, -1, facz<NZ>>(stile + w.s * SZ, 1, w.j, tw_z);
+    __syncthreads();
+    // last pass + H5: DFT-R1z, then hpsi = |k+G|^2 psi + (.)/N written straight to the stick's run of hpsi
+    for (StickWalk w(tid, NT, S); w.j < R2z; w.next()) {
+      const int4 si = __ldg(a.stick + s0 + w.s);
+      cplx v[R1z];
+      const cplx* t = stile + w.s * SZ + w.j;
 #pragma unroll
-    for (int k1 = 0; k1 < R1z; ++k1) v[k1] = t[k1 * R2z];
-    dft<R1z, -1>(v);
+      for (int k1 = 0; k1 < R1z; ++k1) v[k1] = t[k1 * R2z];
+      dft<R1z, -1>(v);
 #pragma unroll
-    for (int q1 = 0; q1 < R1z; ++q1) {       // natural z = q1*R2z + q2
-      int idx = q1 * R2z + w.j - si.y;
-      if (idx < 0) idx += NZ;
-      if (idx < si.z) {
-        const int j = si.x + idx;
-        const cplx p = psi[j];
-        const double k = __ldg(a.g2 + j);
-        hpsi[j] = cmake(fma(k, p.x, v[q1].x * a.invN), fma(k, p.y, v[q1].y * a.invN));
+      for (int q1 = 0; q1 < R1z; ++q1) {       // natural z = q1*R2z + q2
+        int idx = q1 * R2z + w.j - si.y;
+        if (idx < 0) idx += NZ;
+        if (idx < si.z) {
+          const int j = si.x + idx;
+          const cplx p = psi[j];
+          const double k = __ldg(a.g2 + j);
+          hpsi[j] = cmake(fma(k, p.x, v[q1].x * a.invN), fma(k, p.y, v[q1].y * a.invN));
+        }
       }
     }
+  } else {
+    // first z pass on this CTA's lines k1 = h*K1H + k1l (local offset k1l, twiddle index from the global k1)
+    for (StickWalk w(tid, NT, S); w.j < K1H; w.next()) {
+      cplx* line = stile + w.s * SZ + w.j * R2z;
+      const int k1 = h * K1H + w.j;
+      cplx v[R2z];
+#pragma unroll
+      for (int k2 = 0; k2 < R2z; ++k2) v[k2] = line[k2];
+      dft<R2z, -1>(v);
+#pragma unroll
+      for (int q2 = 0; q2 < R2z; ++q2) line[q2] = (q2 == 0) ? v[0] : mul_tw<-1>(v[q2], tw_z, k1 * q2);
+    }
+    cg::cluster_group cl = cg::this_cluster();
+    cl.sync();                                   // every CTA of the plane has finished its part of the sticks
+    const cplx* peer[ZS];
+#pragma unroll
+    for (int r = 0; r < ZS; ++r) peer[r] = (const cplx*)cl.map_shared_rank((void*)stile, r);
+    // last pass + H5: the (stick, q2) items of the plane are dealt over the ZS CTAs; line k1 lives in CTA k1 / K1H
+    for (StickWalk w(h * NT + tid, ZS * NT, S); w.j < R2z; w.next()) {
+      const int4 si = __ldg(a.stick + s0 + w.s);
+      cplx v[R1z];
+      const int off = w.s * SZ + w.j;
+#pragma unroll
+      for (int k1 = 0; k1 < R1z; ++k1) v[k1] = peer[k1 / K1H][off + (k1 % K1H) * R2z];
+      dft<R1z, -1>(v);
+#pragma unroll
+      for (int q1 = 0; q1 < R1z; ++q1) {       // natural z = q1*R2z + q2
+        int idx = q1 * R2z + w.j - si.y;
+        if (idx < 0) idx += NZ;
+        if (idx < si.z) {
+          const int j = si.x + idx;
+          const cplx p = psi[j];
+          const double k = __ldg(a.g2 + j);
+          hpsi[j] = cmake(fma(k, p.x, v[q1].x * a.invN), fma(k, p.y, v[q1].y * a.invN));
+        }
+      }
+    }
+    cl.sync();                                   // no CTA leaves while its stick tile is still being read
   }
 }
 
@@ -720,11 +782,27 @@ __global__ void k_rho_finish(const double* __restrict__ part, int ng, double* __
 static const size_t KS_SMEM_MAX = 227 * 1024;
 
 static size_t yz_smem(const HpsiPlan& P, int zc) {
-  const size_t SZ = (size_t)(P.n3 | 1);
+  const size_t SZ = (size_t)((P.n3 / P.zs_yz) | 1);
   return sizeof(cplx) * ((size_t)P.n2 + (P.n2 == P.n3 ? 0 : P.n3) + (size_t)P.smax * SZ + (size_t)P.n2 * zc);
 }
 template <int NX> static constexpr size_t x_smem() {
   return sizeof(cplx) * ((size_t)NX + (size_t)NX * xcfg<NX>::ZC) + sizeof(unsigned) * (fac<NX>::R2 + 1) * ((fac<NX>::R1 + 3) & ~3);
+}
+
+// the forward yz kernel runs as clusters of ZS CTAs along x when the plane's z' positions are split (yzcfg)
+template <int NY, int NZ>
+static void launch_fwd_yz(dim3 grid, size_t smem, cudaStream_t st, const YzArgs& a) {
+  if (yzcfg<NY, NZ>::ZS == 1) {
+    k_fwd_yz<NY, NZ><<<grid, yzcfg<NY, NZ>::NT, smem, st>>>(a);
+    return;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = dim3(yzcfg<NY, NZ>::NT); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = yzcfg<NY, NZ>::ZS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, k_fwd_yz<NY, NZ>, a);
 }
 
 template <typename K>
@@ -745,6 +823,7 @@ int ks_hpsi_configure(HpsiPlan& P, std::string& err) {
 #define C_(A_, B_)                                                              \
   if (P.n2 == A_ && P.n3 == B_) {                                               \
     P.zc_yz = yzcfg<A_, B_>::ZC;                                                \
+    P.zs_yz = yzcfg<A_, B_>::ZS;                                                \
     P.smem_yz = yz_smem(P, P.zc_yz);                                            \
     if (P.smem_yz > KS_SMEM_MAX) { err = "yz kernels: stick tile does not fit in 227 KB of shared memory"; return KS_ENOMEM; } \
     e = opt_in(k_inv_yz<A_, B_>, P.smem_yz);                                    \
@@ -783,7 +862,7 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
   x.planes = P.d_planes; x.vperm = P.d_vperm; x.tw_x = P.d_tw[0];
   x.L1 = P.L1; x.x0 = P.x0; x.ncol = (long)P.n2 * P.n3;
   x.nb = nb; x.bg = ks_x_band_group(ceil_div(x.ncol, P.zc_x), nb);
-  const dim3 gyz(P.L1, nb), gx(ceil_div(x.ncol, P.zc_x), ceil_div(nb, x.bg));
+  const dim3 gyz(P.L1 * P.zs_yz, nb), gx(ceil_div(x.ncol, P.zc_x), ceil_div(nb, x.bg));
   if (stage < 0 || stage == 0) {
 #define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_inv_yz<A_, B_><<<gyz, yzcfg<A_, B_>::NT, P.smem_yz, st>>>(a);
     KS_YZ_PAIRS(C_)
@@ -795,7 +874,7 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
 #undef C_
   }
   if (stage < 0 || stage == 2) {
-#define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_fwd_yz<A_, B_><<<gyz, yzcfg<A_, B_>::NT, P.smem_yz, st>>>(a);
+#define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) launch_fwd_yz<A_, B_>(gyz, P.smem_yz, st, a);
     KS_YZ_PAIRS(C_)
 #undef C_
   }
@@ -828,7 +907,7 @@ int ks_density_batch(HpsiPlan& P, const cplx* psi, const double* occ, int nb, in
   a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.stick = P.d_stick;
   a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
   a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.invN = 1.0 / (double)P.N;
-  const dim3 gyz(P.L1, nb);
+  const dim3 gyz(P.L1 * P.zs_yz, nb);
 #define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_inv_yz<A_, B_><<<gyz, yzcfg<A_, B_>::NT, P.smem_yz, st>>>(a);
   KS_YZ_PAIRS(C_)
 #undef C_

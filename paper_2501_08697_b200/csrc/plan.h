@@ -12,6 +12,7 @@ struct HpsiPlan {
   int nsticks = 0;     // z-sticks (distinct (m1,m2)) of the sphere
   int smax = 0;        // max sticks in one plane
   int zc_yz = 0, zc_x = 0;        // z-chunk sizes of the yz kernels and of the x kernel
+  int zs_yz = 1;                  // CTAs that share one (band, plane) of the yz kernels, each owning n3/zs_yz z' positions
   size_t smem_yz = 0, smem_x = 0;
   // device arrays
   int* d_plane_s0 = nullptr;   // [L1+1] first stick of each plane
