@@ -273,6 +273,15 @@ int ks_gemm_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, co
     KS_CUDA_CHECK(cudaGetLastError(), err);
     return KS_OK;
   }
+  // N beyond the widest tile and not a multiple of a wide one (N = 520 -> 17 tiles of 32 by the least-padding rule): whole
+  // 160-wide tiles first, the remainder in a second launch with its own least-padding tile
+  static const bool nsplit_on = !(getenv("KSPW_GEMM_NSPLIT") && atoi(getenv("KSPW_GEMM_NSPLIT")) == 0);
+  if (nsplit_on && N > 160 && N % 160 != 0 && pick_nj(N, 32) < 4) {
+    const int main_n = N / 160 * 160;
+    const int rc = launch_hn<5>(st, M, main_n, K, A, lda, B, ldb, C, ldc, ws, err);
+    if (rc != KS_OK) return rc;
+    return ks_gemm_hn(st, M, N - main_n, K, A, lda, B + (long)main_n * ldb, ldb, C + (long)main_n * ldc, ldc, ws, err);
+  }
   switch (pick_nj(N, 32)) {
     case 1: return launch_hn<1>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);
     case 2: return launch_hn<2>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);

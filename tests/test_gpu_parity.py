@@ -30,7 +30,8 @@ def _rel(a, b):
 
 # ------------------------------------------------------------------ building blocks (T1)
 @pytest.mark.parametrize("M,N,K", [(8, 8, 515), (160, 37, 1503), (70, 130, 4099), (1, 1, 1), (64, 64, 16), (5, 3, 0),
-                                   (512, 1, 37073), (23, 2, 4099), (64, 3, 1503), (7, 4, 8459)])
+                                   (512, 1, 37073), (23, 2, 4099), (64, 3, 1503), (7, 4, 8459),
+                                   (70, 200, 4099), (33, 520, 2050), (9, 163, 1503)])   # N > 160: whole 160-wide tiles + a remainder launch
 def test_zgemm_hn(ks, M, N, K):
     rng = np.random.default_rng(M * 1000 + N)
     A = rng.standard_normal((M, K)) + 1j * rng.standard_normal((M, K))
