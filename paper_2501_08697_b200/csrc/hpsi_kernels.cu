@@ -235,7 +235,7 @@ struct StickWalk {
 };
 
 template <int NY, int NZ>
-__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 1) k_inv_yz(YzArgs a) {
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 0) k_inv_yz(YzArgs a) {
   constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = facz<NZ>::R1, R2z = facz<NZ>::R2;
   constexpr int ZS = yzcfg<NY, NZ>::ZS, NZH = NZ / ZS, K1H = R1z / ZS;   // this CTA's z' positions and codelet lines
   static_assert(R1z % ZS == 0 && NZH % yzcfg<NY, NZ>::ZC == 0, "z' split must cut between codelet lines and chunks");
@@ -274,8 +274,13 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 :
       cplx* o = stile + w.s * SZ + w.j;
       const int j2 = w.j;
 #pragma unroll
-      for (int k1 = 0; k1 < R1z; ++k1)
-        if (ZS == 1 || k1 / K1H == h) o[(k1 % K1H) * R2z] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw_z, j2 * k1);
+      for (int k1 = 0; k1 < R1z; ++k1) {
+        if constexpr (ZS == 1) {
+          o[k1 * R2z] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw_z, j2 * k1);
+        } else {
+          if (k1 / K1H == h) o[(k1 % K1H) * R2z] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw_z, j2 * k1);
+        }
+      }
       w.next();
       if (w.j < R2z) load_in();
     }
@@ -321,7 +326,7 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 :
 }
 
 template <int NY, int NZ>
-__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 1) k_fwd_yz(YzArgs a) {
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 0) k_fwd_yz(YzArgs a) {
   constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = facz<NZ>::R1, R2z = facz<NZ>::R2;
   constexpr int ZS = yzcfg<NY, NZ>::ZS, NZH = NZ / ZS, K1H = R1z / ZS;   // this CTA's z' positions and codelet lines
   static_assert(ZS == 1 || !yzcfg<NY, NZ>::DBF, "the z' split uses the single-buffer y transform");
