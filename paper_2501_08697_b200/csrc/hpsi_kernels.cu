@@ -196,8 +196,11 @@ constexpr int yz_pick_zc(int nz) {
 // last z pass needs all k1, so its ZS CTAs form a thread-block cluster and read each other's stick tiles through
 // distributed shared memory.
 template <int NY, int NZ> struct yzcfg { static constexpr int ZC = yz_pick_zc(NZ), NT = 256, ZS = 1; static constexpr bool DBF = (ZC % 2 == 0); };
-#ifdef KSPW_ZSPLIT128   // measured on cfg 3: k_inv_yz unchanged (0.589 ms), k_fwd_yz slower (0.712 -> 0.843 ms): off
-template <> struct yzcfg<128, 128> { static constexpr int ZC = 16, NT = 256, ZS = 2; static constexpr bool DBF = false; };
+#ifdef KSPW_ZSPLIT128   // measured on cfg 3 (104-band launches; unsplit: k_inv_yz 0.589 ms, k_fwd_yz 0.688 ms):
+                        //   ZS = 2, ZC = 16, 256 threads: k_inv_yz 0.589 ms, k_fwd_yz 0.843 ms
+                        //   ZS = 4, ZC = 32, 256 threads (both y passes fill the CTA): k_inv_yz 0.794 ms (the repeated first
+                        //   z pass), k_fwd_yz 1.439 ms (clusters of 4 with two cluster barriers each)  -> off
+template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 256, ZS = 4; static constexpr bool DBF = false; };
 #else
 template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 512, ZS = 1; static constexpr bool DBF = false; };
 #endif

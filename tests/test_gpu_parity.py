@@ -194,6 +194,21 @@ def test_hpsi_radix5_grids(ks, oracle_mod, c, ecut, n, beta):
     assert np.abs(ctx.density(_t(p.psi0), _t(occ)).cpu().numpy() - ref).max() <= 1e-12 * ref.max()
 
 
+@pytest.mark.parametrize("c,ecut,grid", [(4, 3.0, (96, 96, 288)), (4, 12.0, (96, 96, 288)), (3, 2.5, (128, 128, 128))])
+def test_hpsi_large_planes_small_sphere(ks, oracle_mod, c, ecut, grid):
+    """The 96 x 288 planes are split over three CTAs per (band, plane) (forward kernel: a cluster exchanging stick tiles
+    through distributed shared memory), the 128 x 128 ones use 512-thread CTAs: small spheres on the full grids leave
+    planes with a handful of sticks (fewer work items than threads, ranks of the cluster with little to do) and let the
+    oracle check every element of every band."""
+    p = I.make_problem(c, ecutwfc=ecut, grid=grid, nbands=3, with_beta=False)
+    ctx = ks.Context.from_problem(p)
+    o = oracle_mod.Oracle.from_problem(p)
+    assert _rel(ctx.hpsi(_t(p.psi0)).cpu().numpy(), o.hpsi(p.psi0)) <= HPSI_TOL
+    occ = np.array([2.0, 1.0, 0.5])
+    ref = o.density(p.psi0, occ)
+    assert np.abs(ctx.density(_t(p.psi0), _t(occ)).cpu().numpy() - ref).max() <= 1e-12 * ref.max()
+
+
 def test_hpsi_full_symmetric_D_blocks(ks, oracle_mod):
     """Per-atom D blocks that are full symmetric matrices of uneven sizes (Eq. 4 L221 allows D_ll' coupling)."""
     p = I.make_problem(0)
