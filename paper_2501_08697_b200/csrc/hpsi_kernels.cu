@@ -202,7 +202,11 @@ template <int NY, int NZ> struct yzcfg { static constexpr int ZC = yz_pick_zc(NZ
                         //   z pass), k_fwd_yz 1.439 ms (clusters of 4 with two cluster barriers each)  -> off
 template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 256, ZS = 4; static constexpr bool DBF = false; };
 #else
+#ifdef KSPW_YZ128_NT256   // 8 warps, both y passes fill the CTA: k_inv_yz 0.605 ms (0.589 with 512 threads), k_fwd_yz 0.819 ms (0.688): off
+template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 256, ZS = 1; static constexpr bool DBF = false; };
+#else
 template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 512, ZS = 1; static constexpr bool DBF = false; };
+#endif
 #endif
 #ifndef KSPW_NO_ZSPLIT288
 template <> struct yzcfg<96, 288> { static constexpr int ZC = 16, NT = 256, ZS = 3; static constexpr bool DBF = false; };
