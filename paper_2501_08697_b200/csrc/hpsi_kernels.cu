@@ -247,6 +247,11 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 :
   constexpr int ZS = yzcfg<NY, NZ>::ZS, NZH = NZ / ZS, K1H = R1z / ZS;   // this CTA's z' positions and codelet lines
   static_assert(R1z % ZS == 0 && NZH % yzcfg<NY, NZ>::ZC == 0, "z' split must cut between codelet lines and chunks");
   constexpr int SZ = NZH | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
+#ifdef KSPW_YHALF_INV   // measured on cfg 3: k_inv_yz 0.589 -> 0.607 ms (twice the stick-tile reads in the pass, 128 registers): off
+  constexpr bool YHALF = (G == 2 * R2y) && (R1y % 2 == 0) && (NT == G * ZC) && (ZC == 32);
+#else
+  constexpr bool YHALF = false;
+#endif
   extern __shared__ cplx sm[];
   cplx* tw_y = sm;
   cplx* tw_z = (NY == NZ) ? tw_y : tw_y + NY;     // equal lengths share one twiddle table
@@ -299,7 +304,36 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 :
   cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ) + h * NZH;
   const int pz = tid % ZC, g = tid / ZC;
   for (int c = 0; c < NZH / ZC; ++c) {
-    if (g < G) {
+    if constexpr (YHALF) {
+      // twice as many line groups as DFT-R1y lines: two groups share a line, one takes the even outputs (DFT-R1y/2 of
+      // x[n] + x[n + R1y/2]), the other the odd ones (DFT-R1y/2 of (x[n] - x[n + R1y/2]) w^n): every warp works in this pass
+      constexpr int H = R1y / 2;
+      const int j2 = g % R2y, half = g / R2y;
+      cplx v[R1y];
+      const cplx* src = stile + c * ZC + pz;
+#pragma unroll
+      for (int j1 = 0; j1 < R1y; ++j1) {
+        int s = j1 * R2y + j2 - y0;
+        if (s < 0) s += NY;
+        v[j1] = (s < S) ? src[s * SZ] : cmake(0.0, 0.0);
+      }
+      cplx u[H];
+      if (half == 0) {
+#pragma unroll
+        for (int n = 0; n < H; ++n) u[n] = cmake(v[n].x + v[n + H].x, v[n].y + v[n + H].y);
+      } else {
+#pragma unroll
+        for (int n = 0; n < H; ++n) {
+          const cplx d = cmake(v[n].x - v[n + H].x, v[n].y - v[n + H].y);
+          u[n] = (n == 0) ? d : mul_tw<+1>(d, tw_y, n * (NY / R1y));
+        }
+      }
+      dft<H, +1>(u);
+      cplx* o = ytile + j2 * ZC + pz + half * (R2y * ZC);
+#pragma unroll
+      for (int kh = 0; kh < H; ++kh)      // k1 = 2 kh + half
+        o[2 * kh * R2y * ZC] = (kh == 0 && half == 0) ? u[0] : mul_tw<+1>(u[kh], tw_y, j2 * (2 * kh + half));
+    } else if (g < G) {
       for (int j2 = g; j2 < R2y; j2 += G) {
         cplx v[R1y];
         const cplx* src = stile + c * ZC + pz;
@@ -338,6 +372,11 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 :
   constexpr int ZS = yzcfg<NY, NZ>::ZS, NZH = NZ / ZS, K1H = R1z / ZS;   // this CTA's z' positions and codelet lines
   static_assert(ZS == 1 || !yzcfg<NY, NZ>::DBF, "the z' split uses the single-buffer y transform");
   constexpr int SZ = NZH | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
+#ifndef KSPW_NO_YHALF    // measured on cfg 3: k_fwd_yz 0.688 -> 0.665 ms
+  constexpr bool YHALF = (G == 2 * R2y) && (R1y % 2 == 0) && (NT == G * ZC) && (ZC == 32);   // 128 x 128: 16 warps, 8 DFT-16 lines
+#else
+  constexpr bool YHALF = false;
+#endif
   extern __shared__ cplx sm[];
   cplx* tw_y = sm;
   cplx* tw_z = (NY == NZ) ? tw_y : tw_y + NY;     // equal lengths share one twiddle table
@@ -426,7 +465,34 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 :
       }
       __syncthreads();
       if (g < G && g < R1y && c + 1 < NZH / ZC) load_in(v, c + 1, g);   // next chunk's loads fly during pass 2
-      if (g < G) {
+      if constexpr (YHALF) {
+        // two line groups per DFT-R1y line: even outputs from one, odd outputs from the other (see k_inv_yz)
+        constexpr int H = R1y / 2;
+        const int q2 = g % R2y, half = g / R2y;
+        cplx u[R1y];
+        const cplx* t = ytile + q2 * ZC + pz;
+#pragma unroll
+        for (int k1 = 0; k1 < R1y; ++k1) u[k1] = t[k1 * R2y * ZC];
+        cplx w[H];
+        if (half == 0) {
+#pragma unroll
+          for (int n = 0; n < H; ++n) w[n] = cmake(u[n].x + u[n + H].x, u[n].y + u[n + H].y);
+        } else {
+#pragma unroll
+          for (int n = 0; n < H; ++n) {
+            const cplx d = cmake(u[n].x - u[n + H].x, u[n].y - u[n + H].y);
+            w[n] = (n == 0) ? d : mul_tw<-1>(d, tw_y, n * (NY / R1y));
+          }
+        }
+        dft<H, -1>(w);
+        cplx* o = stile + c * ZC + pz;
+#pragma unroll
+        for (int qh = 0; qh < H; ++qh) {     // q1 = 2 qh + half; natural y = q1*R2y + q2; keep the stick columns only
+          int s = (2 * qh + half) * R2y + q2 - y0;
+          if (s < 0) s += NY;
+          if (s < S) o[s * SZ] = w[qh];
+        }
+      } else if (g < G) {
         for (int q2 = g; q2 < R2y; q2 += G) {
           cplx u[R1y];
           const cplx* t = ytile + q2 * ZC + pz;
