@@ -229,6 +229,15 @@ __device__ __forceinline__ void cp_wait_n(int n) {   // n = groups allowed to st
   }
 }
 
+// plane elements are written once by k_inv_yz and read once by k_fwd_yz: streaming (evict-first) accesses
+#ifdef KSPW_PLANE_CS
+#define KS_ST_PLANE(p, v) __stcs((p), (v))
+#define KS_LD_PLANE(p) __ldcs(p)
+#else
+#define KS_ST_PLANE(p, v) (*(p) = (v))
+#define KS_LD_PLANE(p) (*(p))
+#endif
+
 // lines-first walk over (stick s, line j) pairs: item it = j*S + s, it = tid, tid + NT, ...
 struct StickWalk {
   int s, j, ds, dj, S;
@@ -359,7 +368,7 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 :
         dft<R2y, +1>(v);
         cplx* o = plane + (size_t)(k1 * R2y) * NZ + c * ZC + pz;
 #pragma unroll
-        for (int k2 = 0; k2 < R2y; ++k2) o[k2 * NZ] = v[k2];
+        for (int k2 = 0; k2 < R2y; ++k2) KS_ST_PLANE(o + k2 * NZ, v[k2]);
       }
     }
     __syncthreads();
@@ -444,7 +453,7 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 :
   auto load_in = [&](cplx (&v)[R2y], int c, int k1) {
     const cplx* src = plane + (size_t)(k1 * R2y) * NZ + c * ZC + pz;
 #pragma unroll
-    for (int k2 = 0; k2 < R2y; ++k2) v[k2] = src[k2 * NZ];
+    for (int k2 = 0; k2 < R2y; ++k2) v[k2] = KS_LD_PLANE(src + k2 * NZ);
   };
   {
     cplx v[R2y];
