@@ -477,21 +477,23 @@ extern "C" int ks_hpsi_host(ks_ctx* c, const ks_c128* psi_host, ks_c128* hpsi_ho
       KS_CUDA_CHECK(cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming), c->err);
     }
   }
-  // chunks of >= 32 bands (the GEMM tiles want some width), at most 8 of them
-  const int nchunk = std::max(1, std::min(8, nbands / 32));
-  const int per = ceil_div(nbands, nchunk);
+  // chunk = a multiple of 32 bands (the GEMM tile unit: no padded columns inside a chunk), about eight chunks per block.
+  // Measured (band-applications/s through host buffers): cfg 1, 160 bands: 32 -> 39.2k, 64 -> 37.9k, 40 -> 33.7k;
+  // cfg 3, 520 bands: 64 -> 6.78k, 96 -> 6.58k, 128 -> 6.56k, 160 -> 6.62k, 65 (the old nbands/8 rule) -> 5.41k.
+  static const int env_per = getenv("KSPW_HOST_CHUNK_BANDS") ? atoi(getenv("KSPW_HOST_CHUNK_BANDS")) : 0;
+  const int per = env_per > 0 ? env_per : std::max(32, nbands / 8 / 32 * 32);
   KS_CUDA_CHECK(cudaEventRecord(c->ev_start, c->stream), c->err);          // order after earlier work on the stream
   KS_CUDA_CHECK(cudaStreamWaitEvent(c->s_in, c->ev_start, 0), c->err);
   for (int i = 0, b0 = 0; b0 < nbands; ++i, b0 += per) {
     const int n = std::min(per, nbands - b0);
     const size_t off = (size_t)b0 * npw, cb = sizeof(cplx) * (size_t)n * npw;
     KS_CUDA_CHECK(cudaMemcpyAsync(c->d_hin + off, (const cplx*)psi_host + off, cb, cudaMemcpyHostToDevice, c->s_in), c->err);
-    KS_CUDA_CHECK(cudaEventRecord(c->ev_in[i], c->s_in), c->err);
-    KS_CUDA_CHECK(cudaStreamWaitEvent(c->stream, c->ev_in[i], 0), c->err);
+    KS_CUDA_CHECK(cudaEventRecord(c->ev_in[i & 7], c->s_in), c->err);
+    KS_CUDA_CHECK(cudaStreamWaitEvent(c->stream, c->ev_in[i & 7], 0), c->err);
     rc = ks_hpsi_impl(c, c->d_hin + off, c->d_hout + off, n);
     if (rc) return rc;
-    KS_CUDA_CHECK(cudaEventRecord(c->ev_done[i], c->stream), c->err);
-    KS_CUDA_CHECK(cudaStreamWaitEvent(c->s_out, c->ev_done[i], 0), c->err);
+    KS_CUDA_CHECK(cudaEventRecord(c->ev_done[i & 7], c->stream), c->err);
+    KS_CUDA_CHECK(cudaStreamWaitEvent(c->s_out, c->ev_done[i & 7], 0), c->err);
     KS_CUDA_CHECK(cudaMemcpyAsync((cplx*)hpsi_host + off, c->d_hout + off, cb, cudaMemcpyDeviceToHost, c->s_out), c->err);
   }
   KS_CUDA_CHECK(cudaStreamSynchronize(c->s_out), c->err);

@@ -239,6 +239,22 @@ def test_hpsi_ragged_band_group(ks, oracle_mod):
     assert np.array_equal(got, got2)          # batching never changes a bit: bands are independent
 
 
+def test_hpsi_host_chunked_pipeline(ks, oracle_mod):
+    """ks_hpsi_host on 300 bands of the cfg 1 geometry: ten chunks of 32 bands with a ragged last one (12 bands) run through
+    the copy-in / compute / copy-out pipeline, more chunks than the eight event pairs; against the device-resident call on
+    the whole block (another split of the projector products, so equal to rounding, not bit for bit) and the oracle."""
+    p = I.make_problem(1)
+    ctx = ks.Context.from_problem(p)
+    psi = np.ascontiguousarray(np.concatenate([p.psi0, 0.5j * p.psi0[::-1][:140]]))
+    assert psi.shape[0] == 300
+    dev = ctx.hpsi(_t(psi)).cpu().numpy()
+    host = ctx.hpsi_host(psi)
+    assert _rel(host, dev) <= 1e-13
+    sel = np.array([0, 31, 32, 159, 160, 287, 288, 299])
+    ref = oracle_mod.Oracle.from_problem(p).hpsi(psi[sel])
+    assert _rel(host[sel], ref) <= HPSI_TOL
+
+
 # ------------------------------------------------------------------ Davidson (T3)
 def _check_davidson(ks, oracle_mod, p, tol=1e-8, exact=None, oracle_run=True):
     ctx = ks.Context.from_problem(p)
