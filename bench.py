@@ -37,7 +37,8 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1: Si64-like)")
+    ap.add_argument("--config", type=int, default=3,
+                    help="BASELINE.json configs index (default 3: Si216-like, the largest single-GPU config, on which north_star sets its roofline targets)")
     ap.add_argument("--k-index", type=int, default=0)
     ap.add_argument("--impl", default="kspw", choices=["kspw", "reference"])
     ap.add_argument("--no-davidson", action="store_true")
@@ -189,16 +190,17 @@ def ncu_traffic(kernel, cfg, bands_per_launch):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed `ncu --set full` capture
     (profiles/r1_traffic.csv: kernel,cfg,bands_per_launch,dram_read_bytes,dram_write_bytes), scaled to this run's
     bands per launch; None when no capture of that kernel and config is committed."""
-    path = os.path.join(ROOT, "profiles", "r1_traffic.csv")
-    if not os.path.exists(path):
-        return None
-    for ln in open(path):
-        f = ln.strip().split(",")
-        if len(f) >= 5 and f[0] == kernel.split("+")[0] and f[1] == str(cfg):
-            try:
-                return (float(f[3]) + float(f[4])) * bands_per_launch / float(f[2])
-            except ValueError:
-                return None
+    for name in ("r2_traffic.csv", "r1_traffic.csv"):       # the latest round's capture of a kernel wins
+        path = os.path.join(ROOT, "profiles", name)
+        if not os.path.exists(path):
+            continue
+        for ln in open(path):
+            f = ln.strip().split(",")
+            if len(f) >= 5 and f[0] == kernel.split("+")[0] and f[1] == str(cfg):
+                try:
+                    return (float(f[3]) + float(f[4])) * bands_per_launch / float(f[2])
+                except ValueError:
+                    break
     return None
 
 
@@ -471,6 +473,22 @@ def main():
             ach, peak, unit = 0.0, 1.0, ""
         rows[name] = {"bound": kind, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak if peak else None,
                       "avg_launch_ms": avg_ms, "launches": nlaunch, "share_of_step": tms / ms}
+    # north_star's two fractions, each over the kernels it names: (sum of algorithmic bytes | flops per step) / (sum of
+    # their event times per step) / peak
+    def group(names, kind):
+        ks_ = [k for k in names if k in rows]
+        tot_ms = sum(prof[k][0] for k in ks_) / args.steps
+        work = sum((models if kind == "hbm" else gmodels)[k][1] * rows[k]["launches"] for k in ks_) / args.steps
+        if tot_ms <= 0:
+            return None
+        if kind == "hbm":
+            ach, peak, unit = work / (tot_ms * 1e-3) / 1e9, pk["hbm_gbs"], "GB/s"
+        else:
+            ach, peak, unit = work / (tot_ms * 1e-3) / 1e12, dmma_tf, "TFLOP/s"
+        return {"bound": kind, "kernels": ks_, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
+                "ms_per_step": tot_ms, "algorithmic_per_step": work, "share_of_step": tot_ms * args.steps / ms}
+    roof_fft = group(("k_inv_yz", "k_x", "k_fwd_yz"), "hbm")
+    roof_gemm = group(("k_gemm_hn+reduce", "k_gemm_nn"), "tensor")
     dom = max((k for k in rows if rows[k]["bound"] != "alu"), key=lambda k: rows[k]["share_of_step"])
     roof = dict(rows[dom])
     for name, r in rows.items():
@@ -492,6 +510,8 @@ def main():
                 "d2h_bytes_per_step": nb * npw * 16, "api": "ks_hpsi_host (pinned host buffers)"},
         "gpu_launches": int(sum(v[1] for v in prof.values())),
         "roofline": roof,
+        "roofline_fft": roof_fft,
+        "roofline_gemm": roof_gemm,
         "roofline_all": rows,
         "peaks": {"hbm_gbs": pk["hbm_gbs"], "source": pk["src"], "dmma_tflops_live": dmma_tf, "dfma_tflops_live": dfma_tf},
         "davidson": dav,

@@ -57,7 +57,8 @@ int ks_create(ks_ctx** out, const double cell[9], const double k_frac[3], double
 void ks_destroy(ks_ctx* ctx);
 int ks_npw(const ks_ctx* ctx);
 int ks_set_stream(ks_ctx* ctx, void* cuda_stream /* cudaStream_t; NULL = default stream */);
-/* number of bands per FFT batch (0 = automatic, sized so one batch of planes stays L2-resident) */
+/* bands per launch of the three FFT kernels (0 = automatic: as many as 2 GB of live-plane workspace hold, at most 1024;
+ * the planes stream through HBM -- a batch small enough to stay in L2 measured slower) */
 int ks_set_fft_batch(ks_ctx* ctx, int nbatch);
 const char* ks_last_error(const ks_ctx* ctx);   /* ctx may be NULL: last ks_create failure */
 /* writes up to cap supported FFT lengths to sizes (HOST), returns how many exist */
@@ -140,7 +141,8 @@ int ks_zgemm_hn(void* stream, int M, int N, int K, const ks_c128* A, long lda, c
 int ks_zgemm_nn(void* stream, int M, int N, int K, const ks_c128* A, long lda, const ks_c128* B,
                 long ldb, ks_c128* C, long ldc, int accumulate);
 /* Hermitian eigenproblem A = C diag(theta) C^H by (block) Jacobi.  A: DEVICE n x n column-major (lda),
- * destroyed; theta: DEVICE [n] ascending; C: DEVICE n x n column-major (ldc), column i <-> theta[i]. */
+ * destroyed; theta: DEVICE [n] ascending; C: DEVICE n x n column-major (ldc), column i <-> theta[i].
+ * Returns KS_NOTCONV (best pairs still written) if 40 sweeps did not reach off_F(A) <= 1e-14 ||A||_F (n > 64 only). */
 int ks_eigh(void* stream, int n, ks_c128* A, long lda, double* theta, ks_c128* C, long ldc,
             int* sweeps_out /*HOST, may be NULL*/);
 /* register-resident DMMA m8n8k4 microbenchmark: achieved FP64 tensor TFLOP/s (roofline denominator) */

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 extern "C" {
@@ -653,11 +654,14 @@ extern "C" int ks_davidson_profile(const ks_ctx* c, double* ms) {
 // ------------------------------------------------------------------------------------------------
 // building blocks (unit tests, microbenchmarks)
 // ------------------------------------------------------------------------------------------------
+// one process-wide workspace behind a lock: these exports have no context to keep it in
 static GemmWs g_gws;
 static EighWs g_ews;
+static std::mutex g_ws_lock;
 
 extern "C" int ks_zgemm_hn(void* stream, int M, int N, int K, const ks_c128* A, long lda, const ks_c128* B, long ldb,
                            ks_c128* C, long ldc) {
+  std::lock_guard<std::mutex> lk(g_ws_lock);
   return ks_gemm_hn((cudaStream_t)stream, M, N, K, (const cplx*)A, lda, (const cplx*)B, ldb, (cplx*)C, ldc, &g_gws, ks_global_error());
 }
 extern "C" int ks_zgemm_nn(void* stream, int M, int N, int K, const ks_c128* A, long lda, const ks_c128* B, long ldb,
@@ -665,6 +669,7 @@ extern "C" int ks_zgemm_nn(void* stream, int M, int N, int K, const ks_c128* A, 
   return ks_gemm_nn((cudaStream_t)stream, M, N, K, (const cplx*)A, lda, (const cplx*)B, ldb, (cplx*)C, ldc, accumulate, ks_global_error());
 }
 extern "C" int ks_eigh(void* stream, int n, ks_c128* A, long lda, double* theta, ks_c128* C, long ldc, int* sweeps_out) {
+  std::lock_guard<std::mutex> lk(g_ws_lock);
   return ks_eigh_run((cudaStream_t)stream, n, (cplx*)A, lda, theta, (cplx*)C, ldc, &g_ews, sweeps_out, ks_global_error());
 }
 extern "C" int ks_dmma_peak(double* tflops_out, double* dfma_tflops_out) {

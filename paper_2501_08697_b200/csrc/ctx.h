@@ -19,6 +19,7 @@ struct DavidsonWs {
   cplx *S = nullptr, *Us = nullptr;      // [2nb x nb] projections / [nb x nb] Gram matrices
   double *theta = nullptr;               // [2nb]
   double *rho = nullptr, *ekin = nullptr, *lam = nullptr;   // [nb]
+  double *lam0 = nullptr, *thr = nullptr;                   // [nb] squared column norms before the projection; drop thresholds
   int *idx = nullptr;                    // [nb] unconverged band list / kept column list
   int *act = nullptr;                    // [nb] bands whose Ritz vectors are rotated this iteration
 };

@@ -24,6 +24,7 @@
 // Gram-Schmidt.  Both span the same space; the converged pairs agree.
 #include "ctx.h"
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdlib>
 #include <vector>
@@ -97,6 +98,19 @@ __global__ void k_col_scale(int npw, cplx* __restrict__ T, const double* __restr
   const double sc = nn > 0.0 ? s * (1.5 - 0.5 * nn * s * s) : 0.0;   // one Newton step on rsqrt: full FP64 accuracy
   cplx* t = T + (size_t)blockIdx.y * npw;
   for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < npw; j += gridDim.x * blockDim.x) t[j] = cscale(sc, t[j]);
+}
+
+// Drop thresholds of the Cholesky (D7): the Gram matrix is built from columns scaled to unit norm AFTER the projection
+// against V, so its remaining diagonal d_j measures the shrinkage against the earlier T columns only.  The listing's
+// rule compares the norm after ALL projections with the norm before any: d_j n1_j^2 / n0_j^2 < thr2, i.e. a column is
+// dropped when d_j <= thr2 n0_j^2 / n1_j^2 (n0, n1: squared norms before / after the projection against V; a column that
+// the projection wiped out, n1 = 0, gets +inf).  n0 == nullptr: no projection happened, plain thr2.
+__global__ void k_drop_thresholds(int nu, const double* __restrict__ n0, const double* __restrict__ n1, double thr2,
+                                  double* __restrict__ thrv) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= nu) return;
+  if (!n0) { thrv[j] = thr2; return; }
+  thrv[j] = (n1[j] > 0.0) ? thr2 * n0[j] / n1[j] : __longlong_as_double(0x7ff0000000000000LL);
 }
 
 // small-matrix helpers (column-major)
@@ -217,7 +231,7 @@ __global__ void k_copy_mat(int m, int n, const cplx* __restrict__ a, long lda, c
 // triangle is overwritten by R (R[j][k] at G[k*ld + j], k >= j).
 // ------------------------------------------------------------------------------------------------
 #define CHOL_THREADS 1024
-__global__ void __launch_bounds__(CHOL_THREADS) k_chol_drop(int n, cplx* __restrict__ G, long ld, double thr,
+__global__ void __launch_bounds__(CHOL_THREADS) k_chol_drop(int n, cplx* __restrict__ G, long ld, const double* __restrict__ thrv,
                                                           int* __restrict__ kept, int* __restrict__ nk_out) {
   extern __shared__ cplx rowj[];          // [n] current row of R
   __shared__ double s_inv;
@@ -226,7 +240,7 @@ __global__ void __launch_bounds__(CHOL_THREADS) k_chol_drop(int n, cplx* __restr
   for (int j = 0; j < n; ++j) {
     if (tid == 0) {
       const double d = G[(long)j * ld + j].x;
-      s_keep = (d > thr) ? 1 : 0;
+      s_keep = (d > thrv[j]) ? 1 : 0;
       if (s_keep) {
         const double r = sqrt(d);
         G[(long)j * ld + j] = cmake(r, 0.0);
@@ -236,8 +250,10 @@ __global__ void __launch_bounds__(CHOL_THREADS) k_chol_drop(int n, cplx* __restr
       }
     }
     __syncthreads();
-    if (!s_keep) continue;
+    const int keep = s_keep;
     const double inv = s_inv;
+    __syncthreads();                       // everyone has read s_keep / s_inv before thread 0 writes the next column's
+    if (!keep) continue;
     for (int k = j + 1 + tid; k < n; k += nt) {
       const cplx v = cscale(inv, G[(long)k * ld + j]);
       G[(long)k * ld + j] = v;
@@ -272,7 +288,7 @@ __global__ void __launch_bounds__(CHOL_THREADS) k_chol_drop(int n, cplx* __restr
 // upper triangle.  A dropped column's row of R is zero, so the later panels skip it by arithmetic.  n = 520 (cfg 3):
 // 17 ms in the single-CTA kernel above, 51 short launches here.
 #define CB 32
-__global__ void __launch_bounds__(CB * CB) k_chol_diag(int n, int j0, cplx* __restrict__ G, long ld, double thr) {
+__global__ void __launch_bounds__(CB * CB) k_chol_diag(int n, int j0, cplx* __restrict__ G, long ld, const double* __restrict__ thrv) {
   __shared__ cplx D[CB][CB + 1];
   __shared__ double s_inv;
   __shared__ int s_keep;
@@ -284,7 +300,7 @@ __global__ void __launch_bounds__(CB * CB) k_chol_diag(int n, int j0, cplx* __re
   for (int j = 0; j < w; ++j) {
     if (threadIdx.x == 0) {
       const double d = D[j][j].x;
-      s_keep = (d > thr) ? 1 : 0;
+      s_keep = (d > thrv[j0 + j]) ? 1 : 0;
       const double r = s_keep ? sqrt(d) : 0.0;
       D[j][j] = cmake(r, 0.0);                 // 0 marks the column as dropped
       s_inv = s_keep ? 1.0 / r : 0.0;          // a dropped column's row of R becomes zero
@@ -372,9 +388,9 @@ __global__ void __launch_bounds__(256) k_chol_kept(int n, const cplx* __restrict
     *nk_out = nk;
   }
 }
-static void chol_drop_blocked(cudaStream_t st, int n, cplx* G, long ld, double thr, int* kept, int* nk_out) {
+static void chol_drop_blocked(cudaStream_t st, int n, cplx* G, long ld, const double* thrv, int* kept, int* nk_out) {
   for (int j0 = 0; j0 < n; j0 += CB) {
-    k_chol_diag<<<1, CB * CB, 0, st>>>(n, j0, G, ld, thr);
+    k_chol_diag<<<1, CB * CB, 0, st>>>(n, j0, G, ld, thrv);
     const int m = n - j0 - CB;                 // trailing columns
     if (m <= 0) break;
     k_chol_trsm<<<ceil_div(m, 64), 64, 0, st>>>(n, j0, G, ld);
@@ -384,6 +400,7 @@ static void chol_drop_blocked(cudaStream_t st, int n, cplx* G, long ld, double t
   k_chol_kept<<<1, 256, sizeof(int) * n, st>>>(n, G, ld, kept, nk_out);
 }
 
+#define TRINV_MAX 3584     // columns k_trinv can hold: 4 warps x TRINV_MAX x 16 B = 224 KB of shared memory
 // one warp per kept column jj: x = R_kept^{-1} e_jj by back substitution; M[:, jj] (nu rows) = scatter(x)
 __global__ void __launch_bounds__(128) k_trinv(int nu, const cplx* __restrict__ R, long ld, const int* __restrict__ kept, int nk,
                                                cplx* __restrict__ M, long ldm) {
@@ -421,7 +438,7 @@ void ks_davidson_free(DavidsonWs* w) {
   cudaFree(w->Hc); cudaFree(w->Cm); cudaFree(w->Hwork); cudaFree(w->S); cudaFree(w->Us);
   cudaFree(w->SV); cudaFree(w->SX); cudaFree(w->ST);
   cudaFree(w->Cp); cudaFree(w->Cq); cudaFree(w->thp); cudaFree(w->act); cudaFree(w->thf); cudaFree(w->lst); cudaFree(w->src);
-  cudaFree(w->theta); cudaFree(w->rho); cudaFree(w->ekin); cudaFree(w->lam); cudaFree(w->idx);
+  cudaFree(w->theta); cudaFree(w->rho); cudaFree(w->ekin); cudaFree(w->lam); cudaFree(w->lam0); cudaFree(w->thr); cudaFree(w->idx);
   *w = DavidsonWs();
 }
 
@@ -451,6 +468,8 @@ static int reserve(ks_ctx* c, int nb) {
   KS_CUDA_CHECK(cudaMalloc(&w.rho, sizeof(double) * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.ekin, sizeof(double) * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.lam, sizeof(double) * nb), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.lam0, sizeof(double) * nb), c->err);
+  KS_CUDA_CHECK(cudaMalloc(&w.thr, sizeof(double) * nb), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.idx, sizeof(int) * (nb + 1)), c->err);
   KS_CUDA_CHECK(cudaMalloc(&w.act, sizeof(int) * nb), c->err);
   w.nb_cap = nb;
@@ -497,25 +516,29 @@ static int orth_pass(ks_ctx* c, cplx* src, int nu, cplx* dst, int m, int nproj_p
   const int npw = c->P.npw;
   cudaStream_t st = c->stream;
   ph.begin();
+  const bool projected = nproj_pass > 0 && m > 0;
+  if (projected) k_col_norm2<<<nu, RED_THREADS, 0, st>>>(npw, src, w.lam0);
   for (int p = 0; p < nproj_pass && m > 0; ++p) {
     RC(ks_gemm_hn(st, m, nu, npw, gen ? w.SV : w.V, npw, src, npw, w.S, m, &c->gws, c->err));
     k_negate<<<ceil_div((long)m * nu, 256), 256, 0, st>>>((long)m * nu, w.S);
     RC(ks_gemm_nn(st, npw, nu, m, w.V, npw, w.S, m, src, npw, 1, c->err));
   }
   k_col_norm2<<<nu, RED_THREADS, 0, st>>>(npw, src, w.lam);
+  k_drop_thresholds<<<ceil_div(nu, 128), 128, 0, st>>>(nu, projected ? w.lam0 : nullptr, w.lam, 1e-12, w.thr);
   k_col_scale<<<dim3(std::max(1, std::min(64, ceil_div(npw, 1024))), nu), 256, 0, st>>>(npw, src, w.lam);
   if (gen) RC(ks_spsi_impl(c, src, w.ST, nu));
   RC(ks_gemm_hn(st, nu, nu, npw, src, npw, gen ? w.ST : src, npw, w.Us, nu, &c->gws, c->err));
   ph.end(PH_ORTH);
   ph.begin();
-  static bool opted = false;
-  if (!opted) {
-    KS_CUDA_CHECK(cudaFuncSetAttribute(k_trinv, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 16 * 2048), c->err);
-    opted = true;
+  static std::atomic<bool> opted{false};
+  if (!opted.load()) {
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_trinv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(cplx) * 4 * TRINV_MAX)), c->err);
+    opted.store(true);
   }
+  if (nu > TRINV_MAX) { c->err = "ks_davidson: more than 3584 columns in one orthonormalisation block"; return KS_EINVAL; }
   static const bool chol_blocked = !(getenv("KSPW_CHOL_BLOCKED") && atoi(getenv("KSPW_CHOL_BLOCKED")) == 0);
-  if (chol_blocked) chol_drop_blocked(st, nu, w.Us, nu, 1e-12, w.idx, w.idx + nu);
-  else k_chol_drop<<<1, CHOL_THREADS, sizeof(cplx) * nu, st>>>(nu, w.Us, nu, 1e-12, w.idx, w.idx + nu);
+  if (chol_blocked) chol_drop_blocked(st, nu, w.Us, nu, w.thr, w.idx, w.idx + nu);
+  else k_chol_drop<<<1, CHOL_THREADS, sizeof(cplx) * nu, st>>>(nu, w.Us, nu, w.thr, w.idx, w.idx + nu);
   int nk = 0;
   KS_CUDA_CHECK(cudaMemcpyAsync(&nk, w.idx + nu, sizeof(int), cudaMemcpyDeviceToHost, st), c->err);
   KS_CUDA_CHECK(cudaStreamSynchronize(st), c->err);
@@ -610,6 +633,14 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
     stale = false;
     return KS_OK;
   };
+  // leaving the loop with no correction left (every one was dropped as dependent): D9 must return X, HX, rho that
+  // belong to the last eigensolve, so the bands that were not rotated since they converged are brought up to date
+  auto refresh_if_stale = [&]() -> int {
+    if (!stale) return KS_OK;
+    RC(rotate_all());
+    k_resid_norms<<<nb, RED_THREADS, 0, st>>>(npw, w.X, gen ? w.SX : w.X, w.HX, w.theta, c->P.d_g2, w.rho, w.ekin);
+    return KS_OK;
+  };
   for (;;) {
     // D5
     ph.begin();
@@ -653,10 +684,10 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
     cplx* Vnew = w.V + (size_t)m * npw;
     static const int nproj_first = (getenv("KSPW_ORTH_PROJ") && atoi(getenv("KSPW_ORTH_PROJ")) > 0) ? atoi(getenv("KSPW_ORTH_PROJ")) : 1;   // + one projection in the second pass = the listing's "twice"
     RC(orth_pass(c, w.T, nu, Vnew, m, nproj_first, &nk, ph));
-    if (nk == 0) break;
+    if (nk == 0) { RC(refresh_if_stale()); break; }
     int nk2 = 0;
     RC(orth_pass(c, Vnew, nk, w.T, m, 1, &nk2, ph, gen ? w.SV + (size_t)m * npw : nullptr));   // S V_new comes out of the second pass
-    if (nk2 == 0) break;
+    if (nk2 == 0) { RC(refresh_if_stale()); break; }
     nk = nk2;
     KS_CUDA_CHECK(cudaMemcpyAsync(Vnew, w.T, vb * nk, cudaMemcpyDeviceToDevice, st), c->err);
     // D1

@@ -19,6 +19,7 @@
 #include "mma.cuh"
 #include "plan.h"
 #include <algorithm>
+#include <atomic>
 #include <cstdlib>
 
 #define GEMM_THREADS 256
@@ -142,7 +143,7 @@ template <int NJ>
 static int launch_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
                      long ldc, GemmWs* ws, std::string& err) {
   constexpr int HN_NT = 32 * NJ;
-  static bool opted = false;
+  static std::atomic<bool> opted{false};
   const size_t smem = sizeof(cplx) * GEMM_STAGES * (HN_MT + HN_NT) * LDK;
   if (!opted) {
     KS_CUDA_CHECK(cudaFuncSetAttribute(k_gemm_hn<NJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err);
@@ -386,7 +387,7 @@ template <int NJ>
 static int launch_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
                      long ldc, int accumulate, std::string& err) {
   constexpr int NN_NT = 16 * NJ;
-  static bool opted = false;
+  static std::atomic<bool> opted{false};
   const size_t smem = sizeof(cplx) * GEMM_STAGES * (KT * LDM + NN_NT * LDK);
   if (!opted) {
     KS_CUDA_CHECK(cudaFuncSetAttribute(k_gemm_nn<NJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err);

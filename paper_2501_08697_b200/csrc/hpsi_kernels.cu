@@ -127,10 +127,17 @@ __global__ void k_vperm(const cplx* __restrict__ v, double* __restrict__ vperm, 
   }
 }
 
-int ks_build_vperm(HpsiPlan& P, const cplx* vhat_host, cudaStream_t st, std::string& err) {
-  const long N = P.N;
+struct VpermTmp {     // create-time temporaries, released on every return path
   cplx *a = nullptr, *b = nullptr;
   double* mx = nullptr;
+  ~VpermTmp() { cudaFree(a); cudaFree(b); cudaFree(mx); }
+};
+
+int ks_build_vperm(HpsiPlan& P, const cplx* vhat_host, cudaStream_t st, std::string& err) {
+  const long N = P.N;
+  VpermTmp tmp;
+  cplx *&a = tmp.a, *&b = tmp.b;
+  double*& mx = tmp.mx;
   KS_CUDA_CHECK(cudaMalloc(&a, N * sizeof(cplx)), err);
   KS_CUDA_CHECK(cudaMalloc(&b, N * sizeof(cplx)), err);
   KS_CUDA_CHECK(cudaMalloc(&mx, 2 * sizeof(double)), err);
@@ -149,7 +156,6 @@ int ks_build_vperm(HpsiPlan& P, const cplx* vhat_host, cudaStream_t st, std::str
   double h[2];
   KS_CUDA_CHECK(cudaMemcpyAsync(h, mx, sizeof h, cudaMemcpyDeviceToHost, st), err);
   KS_CUDA_CHECK(cudaStreamSynchronize(st), err);
-  cudaFree(a); cudaFree(b); cudaFree(mx);
   if (h[1] > 1e-12 * h[0] && h[1] > 0.0) {
     char buf[160];
     snprintf(buf, sizeof buf, "V(r) is not real: max|Im| = %.3e, max|Re| = %.3e", h[1], h[0]);
@@ -878,10 +884,10 @@ template <int NX> static constexpr size_t x_smem() {
 
 // the forward yz kernel runs as clusters of ZS CTAs along x when the plane's z' positions are split (yzcfg)
 template <int NY, int NZ>
-static void launch_fwd_yz(dim3 grid, size_t smem, cudaStream_t st, const YzArgs& a) {
+static cudaError_t launch_fwd_yz(dim3 grid, size_t smem, cudaStream_t st, const YzArgs& a) {
   if (yzcfg<NY, NZ>::ZS == 1) {
     k_fwd_yz<NY, NZ><<<grid, yzcfg<NY, NZ>::NT, smem, st>>>(a);
-    return;
+    return cudaSuccess;
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = grid; cfg.blockDim = dim3(yzcfg<NY, NZ>::NT); cfg.dynamicSmemBytes = smem; cfg.stream = st;
@@ -889,7 +895,7 @@ static void launch_fwd_yz(dim3 grid, size_t smem, cudaStream_t st, const YzArgs&
   at[0].id = cudaLaunchAttributeClusterDimension;
   at[0].val.clusterDim.x = yzcfg<NY, NZ>::ZS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
   cfg.attrs = at; cfg.numAttrs = 1;
-  cudaLaunchKernelEx(&cfg, k_fwd_yz<NY, NZ>, a);
+  return cudaLaunchKernelEx(&cfg, k_fwd_yz<NY, NZ>, a);
 }
 
 template <typename K>
@@ -913,8 +919,10 @@ int ks_hpsi_configure(HpsiPlan& P, std::string& err) {
     P.zs_yz = yzcfg<A_, B_>::ZS;                                                \
     P.smem_yz = yz_smem(P, P.zc_yz);                                            \
     if (P.smem_yz > KS_SMEM_MAX) { err = "yz kernels: stick tile does not fit in 227 KB of shared memory"; return KS_ENOMEM; } \
-    e = opt_in(k_inv_yz<A_, B_>, P.smem_yz);                                    \
-    if (e == cudaSuccess) e = opt_in(k_fwd_yz<A_, B_>, P.smem_yz);              \
+    /* the attribute belongs to the kernel, not to the context: opt in to the hardware maximum once, so contexts  \
+       with different spheres (stick tiles) on the same plane size never lower each other's limit */               \
+    e = opt_in(k_inv_yz<A_, B_>, KS_SMEM_MAX);                                  \
+    if (e == cudaSuccess) e = opt_in(k_fwd_yz<A_, B_>, KS_SMEM_MAX);            \
   }
   KS_YZ_PAIRS(C_)
 #undef C_
@@ -961,9 +969,11 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
 #undef C_
   }
   if (stage < 0 || stage == 2) {
-#define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) launch_fwd_yz<A_, B_>(gyz, P.smem_yz, st, a);
+    cudaError_t le = cudaSuccess;
+#define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) le = launch_fwd_yz<A_, B_>(gyz, P.smem_yz, st, a);
     KS_YZ_PAIRS(C_)
 #undef C_
+    KS_CUDA_CHECK(le, err);
   }
   KS_CUDA_CHECK(cudaGetLastError(), err);
   return KS_OK;

@@ -6,7 +6,7 @@ CPU time (plain loops, OpenMP over bands), so its result is stored once and the 
 
 With `nbands` the full-size problem (same cell, sphere, grid, projectors) is solved for its lowest `nbands` levels only,
 start block drawn by the recipe with that nbands (inputs.make_problem(c, k, nbands=nbands)); the file is then
-oracle_davidson_cfg<C>_nb<nbands>.json.
+oracle_davidson_cfg<C>_nb<nbands>.json.  Configs with several k-points (cfg 2) write oracle_davidson_cfg<C>_k<k_index>.json.
 
 --lapack GUARD SUBFACTOR: the one-off route SURVEY.md §8(d)(4) allows for the largest config: the same listing with
 library primitives as steps (oracle/davidson_lapack.py: LAPACK eigh / QR, zgemm, the oracle's own H psi), GUARD extra
@@ -61,7 +61,7 @@ def main():
         "max_resid": float(r["resid"].max()), "wall_s": wall, "threads": kso.num_threads(),
         "eig": [float(x) for x in r["eig"]],
     }
-    name = "oracle_davidson_cfg%d.json" % c if nbo is None else "oracle_davidson_cfg%d_nb%d.json" % (c, nbo)
+    name = "oracle_davidson_cfg%d%s%s.json" % (c, "_k%d" % k if len(I.config(c).kpts) > 1 else "", "" if nbo is None else "_nb%d" % nbo)
     dst = os.path.join(os.path.dirname(os.path.abspath(__file__)), name)
     if os.environ.get("KSO_GOLDEN_OUT"):
         dst = os.environ["KSO_GOLDEN_OUT"]

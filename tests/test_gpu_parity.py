@@ -119,11 +119,11 @@ def test_hpsi_small(ks, oracle_mod, name):
     else:
         p = I.make_shrunk(name)
     got, ref, ctx, o = _hpsi_pair(ks, oracle_mod, p, p.psi0)
-    assert _rel(got, ref) <= HPSI_TOL
+    assert _rel(got, ref) <= HPSI_TOL and _elementwise_ok(got, ref)
     # local + kinetic only and kinetic only (degenerate cases)
     p2 = I.make_problem(p.cfg.index, p.k_index, ecutwfc=p.ecutwfc, grid=tuple(p.grid), nbands=2, with_beta=False)
     got, ref, _, _ = _hpsi_pair(ks, oracle_mod, p2, p2.psi0)
-    assert _rel(got, ref) <= HPSI_TOL
+    assert _rel(got, ref) <= HPSI_TOL and _elementwise_ok(got, ref)
     # host-buffer entry point gives the same bits as the device one
     h = ctx.hpsi_host(p.psi0)
     assert np.array_equal(h, ctx.hpsi(_t(p.psi0)).cpu().numpy())
@@ -165,17 +165,36 @@ def test_hpsi_edge_cases(ks, oracle_mod):
     assert _rel(out.cpu().numpy(), ref) <= HPSI_TOL
 
 
-@pytest.mark.parametrize("c,k_index,nsample", [(2, 0, 32), (2, 21, 32), (2, 63, 32), (1, 0, 6), (3, 0, 3), (4, 0, 3)])
-def test_hpsi_full_size(ks, oracle_mod, c, k_index, nsample):
-    """Full-size configs in the launch configuration bench.py times (whole block in one call);
-    the oracle recomputes a sample of the bands one by one (bands are independent in H psi)."""
+def _elementwise_ok(got, ref):
+    """next to every norm-wise comparison: no single element off by more than 1e-12 of the largest one (measured ~1e-15)"""
+    return np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max()
+
+
+def _boundary_bands(nb, batch, bg=8):
+    """bands at both ends of every FFT batch (`batch` bands per launch of the three FFT kernels) and at both ends of a
+    k_x band group (bg bands walked by one CTA), plus the middle of the block"""
+    s = {0, nb - 1, nb // 2, bg - 1, bg}
+    for b0 in range(batch, nb, batch):
+        s |= {b0 - 1, b0, b0 + bg - 1, b0 + bg}
+    return np.array(sorted(i for i in s if 0 <= i < nb))
+
+
+# FFT batch limits ks_create picks (2 GB of live planes): cfg 1 and cfg 2 whole block, cfg 3 125 bands, cfg 4 110 bands
+@pytest.mark.parametrize("c,k_index,batch", [(2, 0, 32), (2, 21, 32), (2, 63, 32), (1, 0, 160), (3, 0, 125), (4, 0, 110)])
+def test_hpsi_full_size(ks, oracle_mod, c, k_index, batch):
+    """Full-size configs in the launch configuration bench.py times (whole block in one call); the oracle recomputes
+    bands one by one (bands are independent in H psi): every band of cfg 2, and for cfg 1 / 3 / 4 the bands on both sides
+    of every FFT-batch boundary and at both ends of a k_x band group."""
     p = I.make_problem(c, k_index)
     ctx = ks.Context.from_problem(p)
     got = ctx.hpsi(_t(p.psi0)).cpu().numpy()
     o = oracle_mod.Oracle.from_problem(p)
-    sel = np.unique(np.linspace(0, p.nbands - 1, nsample).astype(int))
+    sel = np.arange(p.nbands) if c == 2 else _boundary_bands(p.nbands, batch)
     ref = o.hpsi(p.psi0[sel])
     assert _rel(got[sel], ref) <= HPSI_TOL
+    assert _elementwise_ok(got[sel], ref)
+    for i, b in enumerate(sel):                     # band by band too: a wrong band cannot hide in the block norm
+        assert _rel(got[b], ref[i]) <= HPSI_TOL
     # property at any size: Hermiticity <phi|H psi> = conj <psi|H phi> over the whole block
     G = p.psi0.conj() @ got.T
     assert np.abs(G - G.conj().T).max() <= 1e-11 * np.abs(G).max()
@@ -188,7 +207,8 @@ def test_hpsi_radix5_grids(ks, oracle_mod, c, ecut, n, beta):
     p = I.make_problem(c, ecutwfc=ecut, grid=(n, n, n), nbands=3, with_beta=beta)
     ctx = ks.Context.from_problem(p)
     o = oracle_mod.Oracle.from_problem(p)
-    assert _rel(ctx.hpsi(_t(p.psi0)).cpu().numpy(), o.hpsi(p.psi0)) <= HPSI_TOL
+    got, ref = ctx.hpsi(_t(p.psi0)).cpu().numpy(), o.hpsi(p.psi0)
+    assert _rel(got, ref) <= HPSI_TOL and _elementwise_ok(got, ref)
     occ = np.array([2.0, 1.0, 0.5])
     ref = o.density(p.psi0, occ)
     assert np.abs(ctx.density(_t(p.psi0), _t(occ)).cpu().numpy() - ref).max() <= 1e-12 * ref.max()
@@ -203,7 +223,8 @@ def test_hpsi_large_planes_small_sphere(ks, oracle_mod, c, ecut, grid):
     p = I.make_problem(c, ecutwfc=ecut, grid=grid, nbands=3, with_beta=False)
     ctx = ks.Context.from_problem(p)
     o = oracle_mod.Oracle.from_problem(p)
-    assert _rel(ctx.hpsi(_t(p.psi0)).cpu().numpy(), o.hpsi(p.psi0)) <= HPSI_TOL
+    got, ref = ctx.hpsi(_t(p.psi0)).cpu().numpy(), o.hpsi(p.psi0)
+    assert _rel(got, ref) <= HPSI_TOL and _elementwise_ok(got, ref)
     occ = np.array([2.0, 1.0, 0.5])
     ref = o.density(p.psi0, occ)
     assert np.abs(ctx.density(_t(p.psi0), _t(occ)).cpu().numpy() - ref).max() <= 1e-12 * ref.max()
@@ -233,7 +254,7 @@ def test_hpsi_ragged_band_group(ks, oracle_mod):
     sel = np.array([0, 1, 14, 29, 30])
     ref = o.hpsi(psi[sel])
     got = ctx.hpsi(_t(psi)).cpu().numpy()
-    assert _rel(got[sel], ref) <= HPSI_TOL
+    assert _rel(got[sel], ref) <= HPSI_TOL and _elementwise_ok(got[sel], ref)
     ctx.set_fft_batch(7)
     got2 = ctx.hpsi(_t(psi)).cpu().numpy()
     assert np.array_equal(got, got2)          # batching never changes a bit: bands are independent
@@ -252,7 +273,7 @@ def test_hpsi_host_chunked_pipeline(ks, oracle_mod):
     assert _rel(host, dev) <= 1e-13
     sel = np.array([0, 31, 32, 159, 160, 287, 288, 299])
     ref = oracle_mod.Oracle.from_problem(p).hpsi(psi[sel])
-    assert _rel(host[sel], ref) <= HPSI_TOL
+    assert _rel(host[sel], ref) <= HPSI_TOL and _elementwise_ok(host[sel], ref)
 
 
 # ------------------------------------------------------------------ Davidson (T3)
@@ -326,6 +347,99 @@ def test_davidson_cfg2_kpoint(ks, oracle_mod):
     r = _check_davidson(ks, oracle_mod, p, oracle_run=True)
     eig = r["eig"].cpu().numpy()
     assert abs(eig[15] - eig[16]) < 1e-8            # degenerate pair; compare values only
+
+
+# ------------------------------------------------------------------ Davidson edge paths (drop rule, rank deficiency)
+def _drop_problem():
+    # cfg 0 cell at ecutwfc 1.5 Ry: npw = 27 on the 16^3 grid; 16 bands -> 2 nbands = 32 > npw, so the corrections of the
+    # first expansion MUST become linearly dependent (at most 27 - 16 = 11 new directions exist)
+    return I.make_problem(0, ecutwfc=1.5, grid=(16, 16, 16), nbands=16)
+
+
+def test_davidson_drop_rule_forced(ks, oracle_mod):
+    """D7's drop rule (DESIGN.md §2 'Drop rule'): with 2 nbands > npw the projected corrections are dependent and both
+    sides must drop columns; eigenvalues against LAPACK on the explicit 27 x 27 H and against the oracle's own solve."""
+    p = _drop_problem()
+    assert p.npw == 27
+    o = oracle_mod.Oracle.from_problem(p)
+    w = np.linalg.eigvalsh(o.explicit_h())
+    ro = o.davidson(p.psi0, tol=1e-8)
+    assert ro["converged"] and np.abs(ro["eig"] - w[:16]).max() <= 1e-8
+    r = ks.Context.from_problem(p).davidson(_t(p.psi0), tol=1e-8)
+    assert r["converged"]
+    assert np.abs(r["eig"].cpu().numpy() - w[:16]).max() <= 1e-8
+    # a drop happened on both sides: fewer band applications than nbands * (iterations + 1) and never more than npw directions
+    assert r["band_applications"] < 16 * (r["iters"] + 1) and ro["nhpsi"] < 16 * (ro["iters"] + 1)
+    X = r["psi"].cpu().numpy()
+    assert np.abs(X.conj() @ X.T - np.eye(16)).max() <= 1e-10
+    res = np.linalg.norm(o.hpsi(X) - r["eig"].cpu().numpy()[:, None] * X, axis=1)
+    assert res.max() <= 1.05e-8
+
+
+def test_davidson_whole_space(ks, oracle_mod):
+    """nbands = npw (degenerate): the start block spans the whole space, the initial Rayleigh-Ritz step is exact and no
+    correction is ever built: nbands band applications, zero iterations -- as in the oracle."""
+    p = I.make_problem(0, ecutwfc=1.5, grid=(16, 16, 16), nbands=27)
+    o = oracle_mod.Oracle.from_problem(p)
+    w = np.linalg.eigvalsh(o.explicit_h())
+    r = ks.Context.from_problem(p).davidson(_t(p.psi0), tol=1e-8)
+    assert r["converged"] and r["band_applications"] == 27 and r["iters"] == 0
+    assert np.abs(r["eig"].cpu().numpy() - w).max() <= 1e-8
+
+
+def test_davidson_rank_deficient_start_block(ks):
+    p = I.make_problem(0)
+    psi = p.psi0.copy()
+    psi[5] = 2.0 * psi[1] - 0.5j * psi[3]            # a dependent start vector
+    ctx = ks.Context.from_problem(p)
+    with pytest.raises(ks.KsError) as ei:
+        ctx.davidson(_t(psi), tol=1e-8)
+    assert ei.value.rc == -1 and "rank deficient" in str(ei.value)
+    # the context is still usable
+    r = ctx.davidson(_t(p.psi0), tol=1e-8)
+    assert r["converged"]
+
+
+def test_davidson_single_cta_cholesky_path_in_subprocess():
+    """KSPW_CHOL_BLOCKED=0 selects the one-CTA Cholesky (k_chol_drop); the switch is read once per process, so the forced-drop
+    problem and the rank-deficient start block run in a child process with it set."""
+    import os, subprocess, sys
+    code = (
+        "import numpy as np, torch\n"
+        "from paper_2501_08697_b200 import inputs as I, kspw\n"
+        "p = I.make_problem(0, ecutwfc=1.5, grid=(16, 16, 16), nbands=16)\n"
+        "r = kspw.Context.from_problem(p).davidson(torch.from_numpy(p.psi0).cuda(), tol=1e-8)\n"
+        "assert r['converged'] and r['band_applications'] < 16 * (r['iters'] + 1)\n"
+        "np.save(__import__('sys').argv[1], r['eig'].cpu().numpy())\n"
+        "p = I.make_problem(0); psi = p.psi0.copy(); psi[5] = psi[1]\n"
+        "try:\n"
+        "    kspw.Context.from_problem(p).davidson(torch.from_numpy(psi).cuda(), tol=1e-8)\n"
+        "    raise SystemExit('no error for a rank-deficient start block')\n"
+        "except kspw.KsError as e:\n"
+        "    assert e.rc == -1\n")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = os.path.join("/tmp", "kspw_chol_single_%d.npy" % os.getpid())
+    env = dict(os.environ, KSPW_CHOL_BLOCKED="0", PYTHONPATH=root)
+    subprocess.run([sys.executable, "-c", code, out], check=True, env=env, cwd=root, timeout=600)
+    eig = np.load(out)
+    os.remove(out)
+    p = _drop_problem()
+    from oracle import kso
+    w = np.linalg.eigvalsh(kso.Oracle.from_problem(p).explicit_h())
+    assert np.abs(eig - w[:16]).max() <= 1e-8
+
+
+def test_two_contexts_same_plane_size_different_spheres(ks, oracle_mod):
+    """The yz kernels' dynamic shared memory depends on the context's sticks per plane, the opt-in attribute belongs to the
+    kernel: a small-sphere context created AFTER a large-sphere one on the same 96 x 96 planes must not break the first."""
+    big = I.make_problem(1, nbands=3)
+    ctx_big = ks.Context.from_problem(big)
+    small = I.make_problem(1, ecutwfc=6.0, grid=(96, 96, 96), nbands=3)
+    ctx_small = ks.Context.from_problem(small)
+    for p, ctx in ((big, ctx_big), (small, ctx_small), (big, ctx_big)):
+        got = ctx.hpsi(_t(p.psi0)).cpu().numpy()
+        ref = oracle_mod.Oracle.from_problem(p).hpsi(p.psi0)
+        assert _rel(got, ref) <= HPSI_TOL and _elementwise_ok(got, ref)
 
 
 # ------------------------------------------------------------------ density build (SURVEY 8(f) rank 2)
@@ -561,11 +675,18 @@ def test_davidson_cfg2_kpoints_vs_survey_values(ks, key):
         assert abs(eig[i] - g[name]) <= 1e-8
 
 
+def _golden(name):
+    import json, os
+    path = os.path.join(os.path.dirname(__file__), "golden", name)
+    return json.load(open(path)) if os.path.exists(path) else None
+
+
 @pytest.mark.parametrize("c", [4, 3])
-def test_davidson_large_configs_sampled(ks, oracle_mod, c):
+def test_davidson_large_configs_all_residuals(ks, oracle_mod, c):
     """cfg 4 (slab, 96x96x288) and cfg 3 (216 atoms, 520 bands, subspace up to 1040: the one-launch-per-round Jacobi
-    path) at full size.  No external eigenvalues exist for them (parity unpinned at full size), so: the solve
-    converges, a sample of the eigenpairs has residual <= tol under the ORACLE's H psi, the block is orthonormal."""
+    path) at full size: the solve converges, EVERY eigenpair has residual <= tol under the ORACLE's H psi (one oracle
+    block apply of all nbands vectors), the block is orthonormal.  The eigenvalues themselves are compared with the
+    oracle's stored solves in test_davidson_vs_stored_oracle_solve / test_davidson_cfg3_lowest64_vs_stored_oracle_solve."""
     import torch
     p = I.make_problem(c)
     ctx = ks.Context.from_problem(p)
@@ -576,28 +697,78 @@ def test_davidson_large_configs_sampled(ks, oracle_mod, c):
     G = X.conj() @ X.T
     assert float((G - torch.eye(p.nbands, dtype=G.dtype, device=G.device)).abs().max()) <= 1e-10
     assert (np.diff(eig) >= -1e-12).all()
-    sel = np.unique(np.linspace(0, p.nbands - 1, 4).astype(int))
-    Xs = X[torch.as_tensor(sel, device=X.device)].cpu().numpy()
+    Xh = X.cpu().numpy()
     o = oracle_mod.Oracle.from_problem(p)
-    res = np.linalg.norm(o.hpsi(Xs) - eig[sel, None] * Xs, axis=1)
+    res = np.linalg.norm(o.hpsi(Xh) - eig[:, None] * Xh, axis=1)
     assert res.max() <= 1.05e-8
-    assert np.abs(res - r["resid"].cpu().numpy()[sel]).max() <= 1e-10
+    assert np.abs(res - r["resid"].cpu().numpy()).max() <= 1e-10
 
 
-@pytest.mark.parametrize("c", [1, 4])
+def test_davidson_cfg3_lowest64_vs_stored_oracle_solve(ks):
+    """The FULL-SIZE cfg 3 problem (npw 124 289, 128^3 grid, 1728 projectors) solved for its lowest 64 bands: the
+    oracle's own kso_davidson (the listing, subspace <= 2 nbands) stored by tests/golden/make_oracle_davidson.py 3 0 64.
+    Same listing and same start block on both sides: all 64 eigenvalues to 1e-8 Ry, counts to 10 %."""
+    g = _golden("oracle_davidson_cfg3_nb64.json")
+    if g is None:
+        pytest.skip("tests/golden/oracle_davidson_cfg3_nb64.json has not been generated")
+    p = I.make_problem(3, nbands=64)
+    assert p.npw == g["npw"] and g["nbands"] == 64 and g["converged"]
+    r = ks.Context.from_problem(p).davidson(_t(p.psi0), tol=1e-8)
+    assert r["converged"]
+    assert np.abs(r["eig"].cpu().numpy() - np.array(g["eig"])).max() <= 1e-8
+    assert abs(r["iters"] - g["iterations"]) <= 0.1 * g["iterations"]
+    assert abs(r["band_applications"] - g["band_applications"]) <= 0.1 * g["band_applications"]
+
+
+@pytest.mark.parametrize("c", [1, 4, 3])
 def test_davidson_vs_stored_oracle_solve(ks, c):
-    """Full-size configs against the ORACLE's own Davidson solve of the same inputs, stored once by
-    tests/golden/make_oracle_davidson.py (minutes of CPU time): every eigenvalue within north_star's 1e-8 Ry."""
-    import json, os
-    path = os.path.join(os.path.dirname(__file__), "golden", "oracle_davidson_cfg%d.json" % c)
-    if not os.path.exists(path):
+    """Full-size configs against the ORACLE's own Davidson solve of the same problem, stored once by
+    tests/golden/make_oracle_davidson.py (minutes to hours of CPU time): every eigenvalue within north_star's 1e-8 Ry.
+    cfg 1 and cfg 4 were solved by kso_davidson (the listing as it stands: counts comparable); cfg 3's 520 bands by the
+    library-routed statement of the same listing (oracle/davidson_lapack.py, guard bands, larger subspace: SURVEY.md
+    8(d)(4)) -- converged eigenvalues do not depend on the route, its counts are not compared."""
+    g = _golden("oracle_davidson_cfg%d.json" % c)
+    if g is None:
         pytest.skip("tests/golden/oracle_davidson_cfg%d.json has not been generated" % c)
-    g = json.load(open(path))
     p = I.make_problem(c)
     assert p.npw == g["npw"] and p.nbands == g["nbands"] and g["converged"]
     r = ks.Context.from_problem(p).davidson(_t(p.psi0), tol=1e-8)
     assert r["converged"]
     assert np.abs(r["eig"].cpu().numpy() - np.array(g["eig"])).max() <= 1e-8
-    # same listing on both sides: iteration and band-application counts agree to a few per cent
-    assert abs(r["iters"] - g["iterations"]) <= 0.1 * g["iterations"]
-    assert abs(r["band_applications"] - g["band_applications"]) <= 0.1 * g["band_applications"]
+    if g.get("route", "listing") == "listing":
+        # same listing on both sides: iteration and band-application counts agree to a few per cent
+        assert abs(r["iters"] - g["iterations"]) <= 0.1 * g["iterations"]
+        assert abs(r["band_applications"] - g["band_applications"]) <= 0.1 * g["band_applications"]
+
+
+# ------------------------------------------------------------------ cfg 2: all 64 k-points
+CFG2_STORED_K = (0, 1, 5, 21, 26, 37, 42, 63)      # two k-points from each of the four |k| shells of the 4x4x4 mesh
+
+
+def test_davidson_cfg2_all_kpoints_time_reversal_and_stored_oracle_solves(ks):
+    """Every k-point of the Monkhorst-Pack mesh: the mesh is inversion symmetric, k_{63-i} = -k_i, and
+    H(-k) = conj(H(k)) for a real local potential and the real-harmonic projectors, so eps(k_i) = eps(k_{63-i}) band by
+    band (time reversal) -- a pin that needs no oracle run.  Eight k-points (two per |k| shell) are
+    compared with the oracle's stored kso_davidson solves (tests/golden/oracle_davidson_cfg2_k<i>.json)."""
+    eig = []
+    for k in range(64):
+        p = I.make_problem(2, k)
+        ctx = ks.Context.from_problem(p)
+        r = ctx.davidson(_t(p.psi0), tol=1e-8)
+        assert r["converged"], "k-point %d" % k
+        eig.append(r["eig"].cpu().numpy())
+        del ctx
+    eig = np.array(eig)
+    kp = np.array(I.config(2).kpts)
+    for i in range(32):
+        assert np.allclose(kp[i], -kp[63 - i])
+        assert np.abs(eig[i] - eig[63 - i]).max() <= 1e-8, "time reversal broken at k-point %d" % i
+    seen = 0
+    for k in CFG2_STORED_K:
+        g = _golden("oracle_davidson_cfg2_k%d.json" % k)
+        if g is None:
+            continue
+        seen += 1
+        assert g["converged"] and g["k_index"] == k
+        assert np.abs(eig[k] - np.array(g["eig"])).max() <= 1e-8, "k-point %d vs the oracle's solve" % k
+    assert seen >= 1, "no stored oracle solve of a cfg 2 k-point found under tests/golden/"
