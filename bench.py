@@ -50,9 +50,8 @@ def parse():
     ap.add_argument("--davidson-max-iter", type=int, default=400)
     ap.add_argument("--fft-batch", type=int, default=0)
     ap.add_argument("--kbatch", action="store_true",
-                    help="config 2 only: a step = one H psi block apply on EVERY k-point of the 4x4x4 mesh (64 contexts on a "
-                         "pool of CUDA streams), k-points sharded over the ranks")
-    ap.add_argument("--streams", type=int, default=8)
+                    help="config 2 only: a step = one ks_hpsi_batch call, H psi on EVERY k-point of the 4x4x4 mesh (64 contexts), "
+                         "k-points sharded over the ranks")
     return ap.parse_args()
 
 
@@ -205,9 +204,10 @@ def ncu_traffic(kernel, cfg, bands_per_launch):
 
 
 def run_kbatch(args):
-    """BASELINE config 2 as a k-point batch: every k-point is an independent unit (its own G sphere, beta and ks_ctx);
-    the k-points of this rank's share run on a pool of CUDA streams so that the small kernels of different k overlap.
-    N > 1: the 64 k-points are sharded over the ranks (strong scaling: total work fixed), no data-path collective."""
+    """BASELINE config 2 as a k-point batch through ks_hpsi_batch / ks_davidson_batch: every k-point is an independent unit
+    (its own G sphere, beta and ks_ctx); one call applies H on all k-points of this rank's share, each kernel of the path as
+    one launch per group of k-points.  N > 1: the 64 k-points are sharded over the ranks (strong scaling: total work
+    fixed), no data-path collective."""
     import torch
     from paper_2501_08697_b200 import parallel as PL
     rank, world, local = PL.env_world()
@@ -219,106 +219,127 @@ def run_kbatch(args):
     nk_total = 64
     mine = PL.shard_units(nk_total, rank, world)
     main = torch.cuda.current_stream()
-    pool = [torch.cuda.Stream() for _ in range(max(1, args.streams))]
-    items = []
-    for i, k in enumerate(mine):
-        p = I.make_problem(2, k)
-        ctx = kspw.Context.from_problem(p)
-        ctx.set_fft_batch(p.nbands)
-        st = pool[i % len(pool)]
-        ctx.set_stream(st)
-        psi = torch.from_numpy(p.psi0).cuda()
-        items.append((p, ctx, st, psi, torch.empty_like(psi)))
-    nb = items[0][0].nbands
+    ps = [I.make_problem(2, k) for k in mine]
+    ctxs = [kspw.Context.from_problem(p) for p in ps]
+    for c in ctxs:
+        c.set_stream(main)
+    psis = [torch.from_numpy(p.psi0).cuda() for p in ps]
+    outs = [torch.empty_like(t) for t in psis]
+    nb = ps[0].nbands
     torch.cuda.synchronize()
 
     def step():
-        ev = torch.cuda.Event()
-        ev.record(main)
-        for st in pool:
-            st.wait_event(ev)
-        for p, ctx, st, psi, out in items:
-            ctx.hpsi(psi, out=out)
-        for st in pool:
-            main.wait_stream(st)
+        kspw.hpsi_batch(ctxs, psis, outs)
+
+    def step_single():
+        for c, t, o in zip(ctxs, psis, outs):
+            c.hpsi(t, out=o)
+
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")
+
+    def timed(fn, k):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
+        for a, b in ev:
+            flush.fill_(1.0)
+            a.record(main)
+            fn()
+            b.record(main)
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in ev)
 
     for _ in range(max(args.warmup, 3)):
         step()
+        step_single()
     PL.barrier()
     clocks = ClockSampler(local)
     if rank == 0:
         clocks.start()
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")
-    ms = 0.0
-    for _ in range(args.steps):
-        flush.fill_(1.0)
-        a.record(main)
-        step()
-        b.record(main)
-        torch.cuda.synchronize()
-        ms += a.elapsed_time(b)
+    ctxs[0].profile_begin()
+    ms = timed(step, args.steps)
+    prof = ctxs[0].profile_end()
+    ms_single = timed(step_single, args.steps)
     PL.barrier()
-    # end to end: pinned host buffers through ks_hpsi_host, k after k
-    hbuf = [(torch.from_numpy(i[0].psi0).pin_memory().numpy(), torch.empty(i[0].psi0.shape, dtype=torch.complex128).pin_memory().numpy())
-            for i in items]
-    for (p, ctx, st, psi, out), (hi, ho) in zip(items, hbuf):
-        ctx.hpsi_host(hi, ho)                      # warm-up: staging buffers
-    torch.cuda.synchronize()
+    # end to end: pinned host buffers -> device, one ks_hpsi_batch call, device -> pinned host buffers, all inside the timed region
+    hin = [torch.from_numpy(p.psi0).pin_memory() for p in ps]
+    hout = [torch.empty_like(t).pin_memory() for t in hin]
+
+    def e2e_step():
+        for d, h in zip(psis, hin):
+            d.copy_(h, non_blocking=True)
+        kspw.hpsi_batch(ctxs, psis, outs)
+        for d, h in zip(outs, hout):
+            h.copy_(d, non_blocking=True)
+        torch.cuda.synchronize()
+
+    e2e_step()
+    e2e_steps = max(1, min(args.steps, 5))
     t0 = time.perf_counter()
-    for (p, ctx, st, psi, out), (hi, ho) in zip(items, hbuf):
-        ctx.hpsi_host(hi, ho)
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    # Davidson on every k-point of the share (sequential: each solve syncs with the host once per iteration)
+    for _ in range(e2e_steps):
+        e2e_step()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
     dav = None
     if not args.no_davidson:
-        # the solves are independent: one host thread per stream of the pool drives its k-points (ctypes releases the GIL
-        # inside the C calls), so the per-iteration host syncs of one solve overlap the kernels of the others
-        from concurrent.futures import ThreadPoolExecutor
-
-        def solve(item):
-            p_, ctx_, st_, psi_, _ = item
-            torch.cuda.set_device(local)
-            with torch.cuda.stream(st_):
-                work_ = psi_.clone()
-                r_ = ctx_.davidson(work_, tol=1e-8, max_iter=args.davidson_max_iter)
-                return (r_["iters"], r_["band_applications"], bool(r_["converged"]), float(r_["eig"][0].item()), float(r_["eig"][-1].item()))
-
-        groups = [[it_ for j, it_ in enumerate(items) if j % len(pool) == g_] for g_ in range(len(pool))]
+        work = [t.clone() for t in psis]
+        kspw.davidson_batch(ctxs, work, tol=1e-8, max_iter=args.davidson_max_iter)      # warm-up: workspaces
+        for w_, t in zip(work, psis):
+            w_.copy_(t)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        with ThreadPoolExecutor(max_workers=len(pool)) as ex:
-            results = sum(ex.map(lambda grp: [solve(it_) for it_ in grp], groups), [])
+        rs = kspw.davidson_batch(ctxs, work, tol=1e-8, max_iter=args.davidson_max_iter)
         torch.cuda.synchronize()
         dsec = time.perf_counter() - t0
-        its = sum(r_[0] for r_ in results); bas = sum(r_[1] for r_ in results); conv = all(r_[2] for r_ in results)
-        emin = min(r_[3] for r_ in results); emax = max(r_[4] for r_ in results)
-        dav = {"time_to_converge_s": dsec, "k_points": len(items), "iterations_total": its, "band_applications": bas,
-               "converged": conv, "tol": 1e-8, "eig_min": emin, "eig_max": emax, "timer": "host wall clock around the share, %d host threads (one per stream)" % len(pool)}
+        eig = np.array([r["eig"].cpu().numpy() for r in rs])
+        trev = None
+        if world == 1:        # time reversal eps(k_i) = eps(k_{63-i}) over the 32 +-k pairs of the mesh
+            trev = float(max(np.abs(eig[i] - eig[63 - i]).max() for i in range(32)))
+        dav = {"time_to_converge_s": dsec, "k_points": len(ctxs), "iterations_total": int(sum(r["iters"] for r in rs)),
+               "band_applications": int(sum(r["band_applications"] for r in rs)), "converged": all(r["converged"] for r in rs),
+               "max_resid": float(max(float(r["resid"].max()) for r in rs)), "tol": 1e-8, "eig_min": float(eig.min()),
+               "eig_max": float(eig.max()), "max_time_reversal_violation": trev,
+               "api": "ks_davidson_batch (worker threads inside the library, one stream each)", "timer": "host wall clock around the call"}
     clk = clocks.stop() if rank == 0 else None
-    ms, e2e_s, dsec = PL.max_over_ranks([ms, e2e_s, dav["time_to_converge_s"] if dav else 0.0])
+    ms, ms_single, e2e_s, dsec = PL.max_over_ranks([ms, ms_single, e2e_s, dav["time_to_converge_s"] if dav else 0.0])
     if rank != 0:
         PL.finalize()
         return 0
     if dav:
         dav["time_to_converge_s"] = dsec
-    p0 = items[0][0]
+    pk = peaks()
+    dmma_tf, _ = kspw.ks_dmma_peak()
+    # algorithmic work of the share per step, DESIGN.md §5 byte model per k-point (4 L + 48 npw per band; 8 P npw nb per GEMM)
+    fft_bytes = sum(kernel_models(p, nb)[k][1] for p in ps for k in ("k_inv_yz", "k_x", "k_fwd_yz"))
+    gemm_flops = sum(2 * kernel_models(p, nb)["k_gemm_nn"][1] for p in ps)
+    fft_ms = sum(prof[k][0] for k in ("k_inv_yz", "k_x", "k_fwd_yz")) / args.steps
+    gemm_ms = sum(prof[k][0] for k in ("k_gemm_hn+reduce", "k_apply_D", "k_gemm_nn")) / args.steps
+    roof_fft = {"bound": "hbm", "kernels": ["k_inv_yz_k", "k_x_k", "k_fwd_yz_k"], "achieved": fft_bytes / (fft_ms * 1e-3) / 1e9,
+                "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": fft_bytes / (fft_ms * 1e-3) / 1e9 / pk["hbm_gbs"], "ms_per_step": fft_ms,
+                "algorithmic_per_step": fft_bytes, "traffic": ncu_traffic("kbatch_fft", 2, nb * len(ps)),
+                "note": "pass-model EFFECTIVE bandwidth: a group's live planes are sized to stay in the 126 MB L2 between the three "
+                        "kernels, so DRAM traffic (ncu dram__bytes, `traffic`) is well below the algorithmic bytes -- SURVEY.md L535-538"}
+    roof_gemm = {"bound": "tensor", "kernels": ["k_gemm_hn_g", "k_reduce_applyD_g", "k_gemm_nn_g"], "achieved": gemm_flops / (gemm_ms * 1e-3) / 1e12,
+                 "peak": dmma_tf, "unit": "TFLOP/s", "frac": gemm_flops / (gemm_ms * 1e-3) / 1e12 / dmma_tf, "ms_per_step": gemm_ms,
+                 "algorithmic_per_step": gemm_flops}
+    dom = roof_fft if fft_ms >= gemm_ms else roof_gemm
+    p0 = ps[0]
+    nbytes = sum(p.npw for p in ps) * nb * 16
     line = {
         "metric": METRIC, "value": nk_total * nb * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong",
         "vs_baseline": None, "dtype": "f64 (complex128)", "data": "synthetic",
         "config": {"workload": "cfg2 k-point batch: 4x4x4 Monkhorst-Pack mesh (64 k), 8-atom diamond cell 10.26 bohr, ecutwfc 60 Ry, "
                                "npw %d..%d per k, grid 54x54x54, nproj %d, nbands %d per k" % (
-                                   min(i[0].npw for i in items), max(i[0].npw for i in items), p0.nproj, nb),
-                   "step": "one ks_hpsi block apply of %d bands on each of the 64 k-points (H1-H8)" % nb,
-                   "l2": "flushed between timed iterations", "streams": len(pool),
+                                   min(p.npw for p in ps), max(p.npw for p in ps), p0.nproj, nb),
+                   "step": "one ks_hpsi_batch call: H psi on %d bands of each of the 64 k-points (H1-H8)" % nb,
+                   "l2": "flushed between timed iterations",
                    "parallelism": "k-points sharded over %d rank(s), no collective on the data path" % world},
         "clocks": clk,
-        "e2e": {"value": len(items) * world * nb / e2e_s, "unit": UNIT, "h2d_bytes_per_step": sum(i[0].npw for i in items) * nb * 16,
-                "d2h_bytes_per_step": sum(i[0].npw for i in items) * nb * 16, "api": "ks_hpsi_host, one call per k-point"},
-        "gpu_launches": len(items) * 7 * args.steps,
-        "roofline": None, "davidson": dav, "cpu_baseline": None,
+        "e2e": {"value": nk_total * nb / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                "api": "pinned host -> device copies, ks_hpsi_batch, device -> pinned host copies"},
+        "gpu_launches": int(sum(v[1] for v in prof.values())),
+        "roofline": dict(dom, kernel="+".join(dom["kernels"])), "roofline_fft": roof_fft, "roofline_gemm": roof_gemm,
+        "single_k_calls": {"value": nk_total * nb * args.steps / (ms_single * 1e-3), "unit": UNIT,
+                           "what": "the same work as 64 ks_hpsi calls, k after k, on one stream"},
+        "davidson": dav, "cpu_baseline": None,
     }
     print(json.dumps(line))
     PL.finalize()

@@ -71,6 +71,30 @@ int ks_hpsi(ks_ctx* ctx, const ks_c128* psi, ks_c128* hpsi, int nbands);
 /* same through HOST buffers (copies H2D / D2H inside, synchronises before returning) */
 int ks_hpsi_host(ks_ctx* ctx, const ks_c128* psi_host, ks_c128* hpsi_host, int nbands);
 
+/* ---- many k-points at once (the batched multi-k entry point) ------------------------------
+ * The KS equation is solved independently for every k-point of the Monkhorst-Pack mesh (ref 128; Eq. 32
+ * L507 holds per k; "independently for each k point" L900).  One context = one k-point; these calls take the contexts of
+ * nk k-points that share the FFT grid (the same cell and grid, different k: different spheres, beta, |k+G|^2).
+ *
+ * ks_hpsi_batch: hpsi[i] = H(k_i) psi[i] for every i, the same arithmetic as nk ks_hpsi calls (bit for bit in the local
+ * and kinetic part; the projector sums are split differently over K, so equal to rounding).  Every kernel of the path is
+ * ONE launch over (plane | column chunk | tile, band, k-point) per group of k-points; a group is sized so that its live
+ * planes stay in L2 between the three FFT kernels.
+ *   ctxs    HOST [nk]  contexts, all distinct, same grid; work is enqueued on the stream of ctxs[0]
+ *   psi     HOST [nk]  of DEVICE pointers, psi[i] is [nbands[i]][npw_i]
+ *   hpsi    HOST [nk]  of DEVICE pointers, same shapes, must not alias psi[i]
+ *   nbands  HOST [nk]  (entries may be 0; then psi[i] / hpsi[i] may be NULL)
+ * Asynchronous on the stream.  Errors: KS_EINVAL (NULL, aliasing, mixed grids, a context twice), KS_ENOMEM, KS_ECUDA;
+ * the text is ks_last_error(ctxs[0]). */
+int ks_hpsi_batch(ks_ctx* const* ctxs, int nk, const ks_c128* const* psi, ks_c128* const* hpsi, const int* nbands);
+/* ks_davidson_batch: ks_davidson on every k-point (arguments per k as in ks_davidson; resid, iters_out,
+ * band_applications_out, status_out may be NULL).  The solves are independent host-driven iterations: they run on
+ * internal worker threads, one CUDA stream each, after the work already enqueued on ctxs[0]'s stream, and the call
+ * returns when all have finished.  status_out[i] = that solve's return value; the call returns the first error (< 0)
+ * if any, else KS_NOTCONV if some solve hit max_iter, else KS_OK. */
+int ks_davidson_batch(ks_ctx* const* ctxs, int nk, ks_c128* const* psi, double* const* eig, const int* nbands, double tol,
+                      int max_iter, double* const* resid, int* iters_out, long long* band_applications_out, int* status_out);
+
 /* Density build (the step after diagonalisation in the SCF loop, Fig. 3):
  *   rho(r) = sum_b occ[b] |psi_b(r)|^2,  psi_b(r) = sum_G psi_b(G) e^{+i G.r}  (Eq. 31, unnormalised; the caller
  *   owns 1/Omega and k weights).  Reuses the scatter + inverse-FFT half of ks_hpsi.

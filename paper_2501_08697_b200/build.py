@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libkspw.so")
-SOURCES = ["capi.cu", "hpsi_kernels.cu", "gemm.cu", "eigh.cu", "davidson.cu", "cg.cu"]
+SOURCES = ["capi.cu", "hpsi_kernels.cu", "gemm.cu", "eigh.cu", "davidson.cu", "cg.cu", "batch.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-Wno-deprecated-gpu-targets"]

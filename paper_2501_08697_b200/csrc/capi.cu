@@ -108,12 +108,12 @@ static int auto_batch(const HpsiPlan& P) {
   return std::max(2, std::min(b, 1024));   // block; measured 80 -> 160 bands: FFT path 51 -> 54 % of HBM); L2 cannot hold a useful batch
 }
 
-static int ensure_planes(ks_ctx* c, int nb) {
+int ks_ensure_planes(ks_ctx* c, int nb, cudaStream_t sync_stream) {
   HpsiPlan& P = c->P;
   const int want = std::min(c->fft_batch, std::max(nb, 1));
   if (want <= P.batch_cap) return KS_OK;
   if (P.d_planes) {
-    cudaStreamSynchronize(c->stream);
+    cudaStreamSynchronize(sync_stream);
     cudaFree(P.d_planes);
     P.d_planes = nullptr; P.batch_cap = 0;
   }
@@ -262,6 +262,7 @@ extern "C" void ks_destroy(ks_ctx* c) {
   cudaFree(c->gws.part);
   ks_eigh_free(&c->ews);
   ks_davidson_free(&c->dws);
+  ks_kbatch_free(&c->kb);
   for (auto& r : c->krecs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (auto e : c->kpool) cudaEventDestroy(e);
   delete c;
@@ -305,6 +306,25 @@ __global__ void k_apply_D(int nproj, int nb, const cplx* __restrict__ B, cplx* _
   DB[e] = cmake(sr, si);
 }
 
+int ks_ensure_nl(ks_ctx* c, int nb, int nsplit) {
+  if (c->nproj == 0 || nb <= 0) return KS_OK;
+  if (nb > c->nl_cap) {
+    cudaFree(c->d_B); cudaFree(c->d_DB);
+    c->d_B = c->d_DB = nullptr; c->nl_cap = 0;
+    KS_CUDA_CHECK(cudaMalloc(&c->d_B, sizeof(cplx) * (size_t)c->nproj * nb), c->err);
+    KS_CUDA_CHECK(cudaMalloc(&c->d_DB, sizeof(cplx) * (size_t)c->nproj * nb), c->err);
+    c->nl_cap = nb;
+  }
+  const size_t need = sizeof(cplx) * (size_t)nsplit * c->nproj * nb;
+  if (c->gws.bytes < need) {
+    cudaFree(c->gws.part);
+    c->gws.part = nullptr; c->gws.bytes = 0;
+    KS_CUDA_CHECK(cudaMalloc(&c->gws.part, need), c->err);
+    c->gws.bytes = need;
+  }
+  return KS_OK;
+}
+
 int ks_hpsi_impl(ks_ctx* c, const cplx* psi, cplx* hpsi, int nb) {
   if (!c) return KS_EINVAL;
   if (nb == 0) return KS_OK;   // empty block: nothing to do (pointers may be NULL)
@@ -317,7 +337,7 @@ int ks_hpsi_impl(ks_ctx* c, const cplx* psi, cplx* hpsi, int nb) {
     if (a < b + bytes && b < a + bytes) { c->err = "ks_hpsi: psi and hpsi must not alias"; return KS_EINVAL; }
   }
   {
-    const int rc = ensure_planes(c, nb);
+    const int rc = ks_ensure_planes(c, nb, c->stream);
     if (rc) return rc;
   }
   for (int b0 = 0; b0 < nb; b0 += c->fft_batch) {
@@ -514,7 +534,7 @@ extern "C" int ks_density(ks_ctx* c, const ks_c128* psi, const double* occ, int 
     return KS_OK;
   }
   {
-    const int rc = ensure_planes(c, nbands);
+    const int rc = ks_ensure_planes(c, nbands, c->stream);
     if (rc) return rc;
   }
   for (int b0 = 0; b0 < nbands; b0 += c->fft_batch) {

@@ -24,6 +24,16 @@ struct DavidsonWs {
   int *act = nullptr;                    // [nb] bands whose Ritz vectors are rotated this iteration
 };
 
+struct KBatchWs {     // ks_hpsi_batch / ks_davidson_batch state kept in the FIRST context of the batch
+  char* h = nullptr;                 // pinned host descriptor block
+  char* d = nullptr;                 // its device copy
+  size_t bytes = 0;
+  cudaEvent_t ev = nullptr;          // recorded after the descriptor copy of the last call
+  bool ev_pending = false;
+  std::vector<cudaStream_t> pool;    // ks_davidson_batch: one stream per worker thread
+  std::vector<cudaEvent_t> pool_ev;
+};
+
 struct ks_ctx {
   HpsiPlan P;
   int nproj = 0, natom = 0;
@@ -42,6 +52,7 @@ struct ks_ctx {
   GemmWs gws;
   EighWs ews;
   DavidsonWs dws;
+  KBatchWs kb;
   cudaStream_t stream = 0;
   // ks_hpsi_host pipeline: copy-in / copy-out streams and per-chunk events (created at first use)
   cudaStream_t s_in = nullptr, s_out = nullptr;
@@ -62,6 +73,9 @@ void ks_kprof_begin(ks_ctx* c, int phase, int launches);
 void ks_kprof_end(ks_ctx* c);
 
 int ks_hpsi_impl(ks_ctx* c, const cplx* psi, cplx* hpsi, int nb);
+int ks_ensure_planes(ks_ctx* c, int nb, cudaStream_t sync_stream);   // live-plane workspace for min(fft_batch, nb) bands
+int ks_ensure_nl(ks_ctx* c, int nb, int nsplit);                     // d_DB [nproj x nb] and split-K partials [nsplit][nb][nproj]
+void ks_kbatch_free(KBatchWs* w);
 int ks_spsi_impl(ks_ctx* c, const cplx* psi, cplx* spsi, int nb);   // S psi = psi + beta q (beta^H psi); a copy when S = I
 int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int max_iter, double* resid,
                      int* iters_out, long long* nhpsi_out);

@@ -34,18 +34,16 @@
 // ------------------------------------------------------------------------------------------------
 #define HN_MT 64
 
+// one CTA tile of C = A^H B over the K range [kbeg, kend): the partial tile goes to out (column-major M x N)
 template <int NJ>
-__global__ void __launch_bounds__(GEMM_THREADS) k_gemm_hn(int M, int N, int K, const cplx* __restrict__ A, long lda,
-                                                          const cplx* __restrict__ B, long ldb, cplx* __restrict__ part,
-                                                          int kchunk) {
+__device__ __forceinline__ void gemm_hn_tile(int M, int N, const cplx* __restrict__ A, long lda, const cplx* __restrict__ B,
+                                             long ldb, cplx* __restrict__ out, int m0, int n0, int kbeg, int kend) {
   constexpr int HN_NT = 32 * NJ;
   extern __shared__ cplx sm[];
   cplx* sA = sm;                                     // [stage][HN_MT][LDK]
   cplx* sB = sm + GEMM_STAGES * HN_MT * LDK;         // [stage][HN_NT][LDK]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = warp & 1, wn = warp >> 1;
-  const int m0 = blockIdx.y * HN_MT, n0 = blockIdx.x * HN_NT;
-  const int kbeg = blockIdx.z * kchunk, kend = min(K, kbeg + kchunk);
   const int ntile = (kend - kbeg + KT - 1) / KT;
 
   auto load_stage = [&](int st, int kt) {
@@ -104,8 +102,6 @@ __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_hn(int M, int N, int K, c
     }
   }
   cp_wait<0>();
-  // partial tile -> part[z][n][m] (column-major M x N per split)
-  cplx* out = part + (size_t)blockIdx.z * M * N;
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
@@ -115,6 +111,30 @@ __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_hn(int M, int N, int K, c
         const int m = m0 + wm * 32 + i * 8 + fr, n = n0 + wn * 8 * NJ + j * 8 + 2 * fk + h;
         if (m < M && n < N) out[(size_t)n * M + m] = cmake(cre[i][j][h], cim[i][j][h]);
       }
+}
+
+template <int NJ>
+__global__ void __launch_bounds__(GEMM_THREADS) k_gemm_hn(int M, int N, int K, const cplx* __restrict__ A, long lda,
+                                                          const cplx* __restrict__ B, long ldb, cplx* __restrict__ part,
+                                                          int kchunk) {
+  const int kbeg = blockIdx.z * kchunk;
+  // partial tile -> part[z][n][m] (column-major M x N per split)
+  gemm_hn_tile<NJ>(M, N, A, lda, B, ldb, part + (size_t)blockIdx.z * M * N, blockIdx.y * HN_MT, blockIdx.x * 32 * NJ, kbeg,
+                   min(K, kbeg + kchunk));
+}
+
+// Grouped form (ks_hpsi_batch): blockIdx.z = problem * nsplit + split; every problem has its own operands and sizes, the
+// grid covers the largest one.  part of problem g: [nsplit][N_g][M_g].
+template <int NJ>
+__global__ void __launch_bounds__(GEMM_THREADS) k_gemm_hn_g(const GemmProb* __restrict__ probs, int nsplit) {
+  const int g = blockIdx.z / nsplit, z = blockIdx.z % nsplit;
+  const GemmProb p = probs[g];
+  const int m0 = blockIdx.y * HN_MT, n0 = blockIdx.x * 32 * NJ;
+  if (m0 >= p.M || n0 >= p.N) return;
+  int kchunk = (p.K + nsplit - 1) / nsplit;
+  kchunk = (kchunk + KT - 1) / KT * KT;
+  const int kbeg = z * kchunk, kend = min(p.K, kbeg + kchunk);
+  gemm_hn_tile<NJ>(p.M, p.N, p.A, p.lda, p.B, p.ldb, p.C + (size_t)z * p.M * p.N, m0, n0, kbeg, max(kend, kbeg));
 }
 
 __global__ void k_splitk_reduce(int M, int N, int nsplit, const cplx* __restrict__ part, cplx* __restrict__ C, long ldc) {
@@ -300,16 +320,14 @@ int ks_gemm_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, co
 #define LDM (NN_MT + 2)   // "m-contiguous" tile leading dimension: == 2 (mod 8)
 
 template <int NJ>
-__global__ void __launch_bounds__(GEMM_THREADS) k_gemm_nn(int M, int N, int K, const cplx* __restrict__ A, long lda,
-                                                          const cplx* __restrict__ B, long ldb, cplx* __restrict__ C,
-                                                          long ldc, int accumulate) {
+__device__ __forceinline__ void gemm_nn_tile(int M, int N, int K, const cplx* __restrict__ A, long lda, const cplx* __restrict__ B,
+                                             long ldb, cplx* __restrict__ C, long ldc, int accumulate, int m0, int n0) {
   constexpr int NN_NT = 16 * NJ;
   extern __shared__ cplx sm[];
   cplx* sA = sm;                                   // [stage][KT][LDM]
   cplx* sB = sm + GEMM_STAGES * KT * LDM;          // [stage][NN_NT][LDK]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = warp & 3, wn = warp >> 2;
-  const int m0 = blockIdx.x * NN_MT, n0 = blockIdx.y * NN_NT;
   const int ntile = (K + KT - 1) / KT;
 
   auto load_stage = [&](int st, int kt) {
@@ -384,6 +402,20 @@ __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_nn(int M, int N, int K, c
 }
 
 template <int NJ>
+__global__ void __launch_bounds__(GEMM_THREADS) k_gemm_nn(int M, int N, int K, const cplx* __restrict__ A, long lda,
+                                                          const cplx* __restrict__ B, long ldb, cplx* __restrict__ C,
+                                                          long ldc, int accumulate) {
+  gemm_nn_tile<NJ>(M, N, K, A, lda, B, ldb, C, ldc, accumulate, blockIdx.x * NN_MT, blockIdx.y * 16 * NJ);
+}
+template <int NJ>
+__global__ void __launch_bounds__(GEMM_THREADS) k_gemm_nn_g(const GemmProb* __restrict__ probs, int accumulate) {
+  const GemmProb p = probs[blockIdx.z];
+  const int m0 = blockIdx.x * NN_MT, n0 = blockIdx.y * 16 * NJ;
+  if (m0 >= p.M || n0 >= p.N) return;
+  gemm_nn_tile<NJ>(p.M, p.N, p.K, p.A, p.lda, p.B, p.ldb, p.C, p.ldc, accumulate, m0, n0);
+}
+
+template <int NJ>
 static int launch_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
                      long ldc, int accumulate, std::string& err) {
   constexpr int NN_NT = 16 * NJ;
@@ -420,6 +452,71 @@ int ks_gemm_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, co
     case 3: return launch_nn<3>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
     case 4: return launch_nn<4>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
     default: return launch_nn<5>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Grouped launches (ks_hpsi_batch): ng independent problems of similar size in ONE launch each.  dev_probs: DEVICE [ng].
+// ------------------------------------------------------------------------------------------------
+// split count for ng problems of (about) M x N x K: enough CTAs for two waves of the resident slots, >= 8 k-tiles per split
+int ks_gemm_hn_group_nsplit(int ng, int M, int N, int K) {
+  const int nj = pick_nj(N, 32);
+  const size_t smem = sizeof(cplx) * GEMM_STAGES * (HN_MT + 32 * nj) * LDK;
+  const int per_sm = std::max(1, (int)((227 * 1024) / (smem + 1024)));
+  const long slots = 148L * per_sm, tiles = (long)ng * ceil_div(M, HN_MT) * ceil_div(N, 32 * nj);
+  const int max_split = std::max(1, K / (8 * KT));
+  return (int)std::max(1L, std::min((long)max_split, (2 * slots + tiles - 1) / tiles));
+}
+
+template <int NJ>
+static int launch_hn_g(cudaStream_t st, const GemmProb* dev_probs, int ng, int M, int N, int nsplit, std::string& err) {
+  static std::atomic<bool> opted{false};
+  const size_t smem = sizeof(cplx) * GEMM_STAGES * (HN_MT + 32 * NJ) * LDK;
+  if (!opted.load()) {
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_gemm_hn_g<NJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err);
+    opted.store(true);
+  }
+  const dim3 grid(ceil_div(N, 32 * NJ), ceil_div(M, HN_MT), ng * nsplit);
+  k_gemm_hn_g<NJ><<<grid, GEMM_THREADS, smem, st>>>(dev_probs, nsplit);
+  KS_CUDA_CHECK(cudaGetLastError(), err);
+  return KS_OK;
+}
+// partial sums C_g[z] = A_g^H B_g over split z of K_g; M, N: the largest of the group (sizes the grid and the tile width)
+int ks_gemm_hn_group(cudaStream_t st, const GemmProb* dev_probs, int ng, int M, int N, int nsplit, std::string& err) {
+  if (ng <= 0 || M <= 0 || N <= 0) return KS_OK;
+  if ((long)ng * nsplit > 65535) { err = "ks_gemm_hn_group: too many problems x splits for one launch"; return KS_EINVAL; }
+  switch (pick_nj(N, 32)) {
+    case 1: return launch_hn_g<1>(st, dev_probs, ng, M, N, nsplit, err);
+    case 2: return launch_hn_g<2>(st, dev_probs, ng, M, N, nsplit, err);
+    case 3: return launch_hn_g<3>(st, dev_probs, ng, M, N, nsplit, err);
+    case 4: return launch_hn_g<4>(st, dev_probs, ng, M, N, nsplit, err);
+    default: return launch_hn_g<5>(st, dev_probs, ng, M, N, nsplit, err);
+  }
+}
+
+template <int NJ>
+static int launch_nn_g(cudaStream_t st, const GemmProb* dev_probs, int ng, int M, int N, int accumulate, std::string& err) {
+  static std::atomic<bool> opted{false};
+  const size_t smem = sizeof(cplx) * GEMM_STAGES * (KT * LDM + 16 * NJ * LDK);
+  if (!opted.load()) {
+    KS_CUDA_CHECK(cudaFuncSetAttribute(k_gemm_nn_g<NJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err);
+    opted.store(true);
+  }
+  const dim3 grid(ceil_div(M, NN_MT), ceil_div(N, 16 * NJ), ng);
+  k_gemm_nn_g<NJ><<<grid, GEMM_THREADS, smem, st>>>(dev_probs, accumulate);
+  KS_CUDA_CHECK(cudaGetLastError(), err);
+  return KS_OK;
+}
+// C_g (+)= A_g B_g for every problem of the group
+int ks_gemm_nn_group(cudaStream_t st, const GemmProb* dev_probs, int ng, int M, int N, int accumulate, std::string& err) {
+  if (ng <= 0 || M <= 0 || N <= 0) return KS_OK;
+  if (ng > 65535) { err = "ks_gemm_nn_group: too many problems for one launch"; return KS_EINVAL; }
+  switch (pick_nj(N, 16)) {
+    case 1: return launch_nn_g<1>(st, dev_probs, ng, M, N, accumulate, err);
+    case 2: return launch_nn_g<2>(st, dev_probs, ng, M, N, accumulate, err);
+    case 3: return launch_nn_g<3>(st, dev_probs, ng, M, N, accumulate, err);
+    case 4: return launch_nn_g<4>(st, dev_probs, ng, M, N, accumulate, err);
+    default: return launch_nn_g<5>(st, dev_probs, ng, M, N, accumulate, err);
   }
 }
 

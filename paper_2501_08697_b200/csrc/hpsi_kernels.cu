@@ -185,6 +185,7 @@ struct YzArgs {
   const cplx* tw_y;
   const cplx* tw_z;
   int npw, L1, smax;
+  int nb;               // bands of this k-point (k-batched launches: CTAs beyond it leave at once)
   double invN;
 };
 
@@ -257,7 +258,7 @@ struct StickWalk {
 };
 
 template <int NY, int NZ>
-__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 0) k_inv_yz(YzArgs a) {
+__device__ __forceinline__ void inv_yz_body(const YzArgs& a, const int bx, const int b) {
   constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = facz<NZ>::R1, R2z = facz<NZ>::R2;
   constexpr int ZS = yzcfg<NY, NZ>::ZS, NZH = NZ / ZS, K1H = R1z / ZS;   // this CTA's z' positions and codelet lines
   static_assert(R1z % ZS == 0 && NZH % yzcfg<NY, NZ>::ZC == 0, "z' split must cut between codelet lines and chunks");
@@ -273,7 +274,7 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 :
   cplx* stile = tw_z + NZ;
   cplx* ytile = stile + (size_t)a.smax * SZ;
   const int tid = threadIdx.x;
-  const int lx = blockIdx.x / ZS, h = blockIdx.x % ZS, b = blockIdx.y;
+  const int lx = bx / ZS, h = bx % ZS;
   const int s0 = a.plane_s0[lx], S = a.plane_s0[lx + 1] - s0;
   const int y0 = a.plane_y0[lx];
   const cplx* psi = a.psi + (size_t)b * a.npw;
@@ -382,7 +383,21 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 :
 }
 
 template <int NY, int NZ>
-__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 0) k_fwd_yz(YzArgs a) {
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 0) k_inv_yz(const __grid_constant__ YzArgs a) {
+  inv_yz_body<NY, NZ>(a, blockIdx.x, blockIdx.y);
+}
+// k-batched form (ks_hpsi_batch): blockIdx.z picks the k-point's descriptor; the grid is sized for the largest k of the group
+template <int NY, int NZ>
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 0) k_inv_yz_k(const YzArgs* __restrict__ arr) {
+  __shared__ YzArgs a;
+  if (threadIdx.x == 0) a = arr[blockIdx.z];
+  __syncthreads();
+  if ((int)blockIdx.x >= a.L1 * yzcfg<NY, NZ>::ZS || (int)blockIdx.y >= a.nb) return;
+  inv_yz_body<NY, NZ>(a, blockIdx.x, blockIdx.y);
+}
+
+template <int NY, int NZ>
+__device__ __forceinline__ void fwd_yz_body(const YzArgs& a, const int bx, const int b) {
   constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = facz<NZ>::R1, R2z = facz<NZ>::R2;
   constexpr int ZS = yzcfg<NY, NZ>::ZS, NZH = NZ / ZS, K1H = R1z / ZS;   // this CTA's z' positions and codelet lines
   static_assert(ZS == 1 || !yzcfg<NY, NZ>::DBF, "the z' split uses the single-buffer y transform");
@@ -398,7 +413,7 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 :
   cplx* stile = tw_z + NZ;
   cplx* ytile = stile + (size_t)a.smax * SZ;
   const int tid = threadIdx.x;
-  const int lx = blockIdx.x / ZS, h = blockIdx.x % ZS, b = blockIdx.y;   // h = rank in the cluster of ZS CTAs
+  const int lx = bx / ZS, h = bx % ZS;   // h = rank in the cluster of ZS CTAs
   const int s0 = a.plane_s0[lx], S = a.plane_s0[lx + 1] - s0;
   const int y0 = a.plane_y0[lx];
   const cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ) + h * NZH;
@@ -594,6 +609,20 @@ __global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 :
   }
 }
 
+template <int NY, int NZ>
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 0) k_fwd_yz(const __grid_constant__ YzArgs a) {
+  fwd_yz_body<NY, NZ>(a, blockIdx.x, blockIdx.y);
+}
+template <int NY, int NZ>
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 0) k_fwd_yz_k(const YzArgs* __restrict__ arr) {
+  __shared__ YzArgs a;
+  if (threadIdx.x == 0) a = arr[blockIdx.z];
+  __syncthreads();
+  // whole clusters leave together: lx = blockIdx.x / ZS is the same for the ZS CTAs of a cluster
+  if ((int)blockIdx.x >= a.L1 * yzcfg<NY, NZ>::ZS || (int)blockIdx.y >= a.nb) return;
+  fwd_yz_body<NY, NZ>(a, blockIdx.x, blockIdx.y);
+}
+
 // ------------------------------------------------------------------------------------------------
 // x pass: inverse FFT, V(r) multiply, forward FFT in one kernel
 // ------------------------------------------------------------------------------------------------
@@ -625,7 +654,7 @@ template <> struct xcfg<128> { static constexpr int ZC = 16, NT = 128, MINB = 4;
 // first pass of band b+1 picks them up with no barrier in between (only its own cp.async group to wait for).
 // The global-load latency of a band is hidden behind the last pass of the band before it.
 template <int NX>
-__global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB) k_x(XArgs a) {
+__device__ __forceinline__ void x_body(const XArgs& a, const int bx, const int by) {
   constexpr int R1 = fac<NX>::R1, R2 = fac<NX>::R2;
   constexpr int ZC = xcfg<NX>::ZC, NT = xcfg<NX>::NT, G = NT / ZC;
   constexpr int ITEMS = (R2 + G - 1) / G;     // first/last-pass lines per thread
@@ -639,9 +668,9 @@ __global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB) k_x(XArgs a) {
   unsigned* rofs = reinterpret_cast<unsigned*>(tile + NX * ZC);   // [R2+1][R1P]: element offset of row j1*R2+j2, or DEAD
   const int tid = threadIdx.x, pz = tid % ZC, g = tid / ZC;
   const unsigned ncol = (unsigned)a.ncol;      // one band's live planes (L1*ncol elements) fit 32-bit offsets
-  const unsigned col = blockIdx.x * ZC + pz;
+  const unsigned col = bx * ZC + pz;
   const bool colok = col < ncol;              // ragged last chunk: such threads use the all-dead table line
-  const int b0 = blockIdx.y * a.bg, b1 = min(b0 + a.bg, a.nb);
+  const int b0 = by * a.bg, b1 = min(b0 + a.bg, a.nb);
   const size_t bstride = (size_t)a.L1 * a.ncol;
   cplx* base = a.planes + (size_t)b0 * bstride + (colok ? col : 0);
   const double* vbase = a.vperm + (colok ? col : 0);
@@ -743,6 +772,19 @@ __global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB) k_x(XArgs a) {
         if (o[q1] != DEAD) base[o[q1]] = v[q1];
     }
   }
+}
+
+template <int NX>
+__global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB) k_x(const __grid_constant__ XArgs a) {
+  x_body<NX>(a, blockIdx.x, blockIdx.y);
+}
+template <int NX>
+__global__ void __launch_bounds__(xcfg<NX>::NT, xcfg<NX>::MINB) k_x_k(const XArgs* __restrict__ arr) {
+  __shared__ XArgs a;
+  if (threadIdx.x == 0) a = arr[blockIdx.z];
+  __syncthreads();
+  if ((int)blockIdx.y * a.bg >= a.nb) return;
+  x_body<NX>(a, blockIdx.x, blockIdx.y);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -873,6 +915,7 @@ __global__ void k_rho_finish(const double* __restrict__ part, int ng, double* __
 // host: configuration and launch
 // ------------------------------------------------------------------------------------------------
 static const size_t KS_SMEM_MAX = 227 * 1024;
+static const size_t KS_SMEM_MAX_K = 226 * 1024;   // the k-batched kernels keep their descriptor in static shared memory
 
 static size_t yz_smem(const HpsiPlan& P, int zc) {
   const size_t SZ = (size_t)((P.n3 / P.zs_yz) | 1);
@@ -923,11 +966,13 @@ int ks_hpsi_configure(HpsiPlan& P, std::string& err) {
        with different spheres (stick tiles) on the same plane size never lower each other's limit */               \
     e = opt_in(k_inv_yz<A_, B_>, KS_SMEM_MAX);                                  \
     if (e == cudaSuccess) e = opt_in(k_fwd_yz<A_, B_>, KS_SMEM_MAX);            \
+    if (e == cudaSuccess) e = opt_in(k_inv_yz_k<A_, B_>, KS_SMEM_MAX_K);        \
+    if (e == cudaSuccess) e = opt_in(k_fwd_yz_k<A_, B_>, KS_SMEM_MAX_K);        \
   }
   KS_YZ_PAIRS(C_)
 #undef C_
   KS_CUDA_CHECK(e, err);
-#define C_(N_) if (P.n1 == N_) { P.zc_x = xcfg<N_>::ZC; P.smem_x = x_smem<N_>(); e = opt_in(k_x<N_>, P.smem_x); }
+#define C_(N_) if (P.n1 == N_) { P.zc_x = xcfg<N_>::ZC; P.smem_x = x_smem<N_>(); e = opt_in(k_x<N_>, P.smem_x); if (e == cudaSuccess) e = opt_in(k_x_k<N_>, P.smem_x); }
   KS_X_SIZES(C_)
 #undef C_
   KS_CUDA_CHECK(e, err);
@@ -952,7 +997,7 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
   a.psi = psi; a.hpsi = hpsi; a.planes = P.d_planes;
   a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.stick = P.d_stick;
   a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
-  a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.invN = 1.0 / (double)P.N;
+  a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.nb = nb; a.invN = 1.0 / (double)P.N;
   XArgs x;
   x.planes = P.d_planes; x.vperm = P.d_vperm; x.tw_x = P.d_tw[0];
   x.L1 = P.L1; x.x0 = P.x0; x.ncol = (long)P.n2 * P.n3;
@@ -971,6 +1016,84 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
   if (stage < 0 || stage == 2) {
     cudaError_t le = cudaSuccess;
 #define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) le = launch_fwd_yz<A_, B_>(gyz, P.smem_yz, st, a);
+    KS_YZ_PAIRS(C_)
+#undef C_
+    KS_CUDA_CHECK(le, err);
+  }
+  KS_CUDA_CHECK(cudaGetLastError(), err);
+  return KS_OK;
+}
+
+// ---- k-batched launch (ks_hpsi_batch): one grid over (plane | column chunk, band, k-point) per kernel ----
+// Descriptor block of a group of nk k-points, built on the host and copied to the device by the caller:
+// [YzArgs x nk][XArgs x nk].  All k-points of a group share the grid size (same kernel instantiation).
+size_t ks_kdesc_bytes(int nk) { return (sizeof(YzArgs) + sizeof(XArgs)) * (size_t)nk; }
+
+void ks_kdesc_fill(void* host_desc, const KItem* items, int nk) {
+  YzArgs* ya = (YzArgs*)host_desc;
+  XArgs* xa = (XArgs*)(ya + nk);
+  int nbmax = 0;
+  for (int i = 0; i < nk; ++i) nbmax = std::max(nbmax, items[i].nb);
+  const HpsiPlan& P0 = *items[0].P;
+  const long ncol = (long)P0.n2 * P0.n3;
+  const int bg = ks_x_band_group(ceil_div(ncol, P0.zc_x) * nk, nbmax);
+  for (int i = 0; i < nk; ++i) {
+    const HpsiPlan& P = *items[i].P;
+    YzArgs& a = ya[i];
+    a.psi = items[i].psi; a.hpsi = items[i].hpsi; a.planes = P.d_planes;
+    a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.stick = P.d_stick;
+    a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
+    a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.nb = items[i].nb; a.invN = 1.0 / (double)P.N;
+    XArgs& x = xa[i];
+    x.planes = P.d_planes; x.vperm = P.d_vperm; x.tw_x = P.d_tw[0];
+    x.L1 = P.L1; x.x0 = P.x0; x.ncol = ncol; x.nb = items[i].nb; x.bg = std::min(bg, std::max(1, items[i].nb));
+  }
+}
+
+int ks_hpsi_local_launch_k(const KItem* items, int nk, const void* dev_desc, cudaStream_t st, std::string& err, int stage) {
+  if (nk <= 0) return KS_OK;
+  const HpsiPlan& P0 = *items[0].P;
+  int nbmax = 0, l1max = 0;
+  size_t smem_yz = 0;
+  for (int i = 0; i < nk; ++i) {
+    const HpsiPlan& P = *items[i].P;
+    if (P.n1 != P0.n1 || P.n2 != P0.n2 || P.n3 != P0.n3) { err = "ks_hpsi_batch: the k-points of a batch must share the FFT grid"; return KS_EINVAL; }
+    if (items[i].nb > P.batch_cap) { err = "internal: FFT batch larger than workspace"; return KS_EINVAL; }
+    nbmax = std::max(nbmax, items[i].nb); l1max = std::max(l1max, P.L1);
+    smem_yz = std::max(smem_yz, P.smem_yz);
+  }
+  if (nbmax == 0) return KS_OK;
+  if (smem_yz > KS_SMEM_MAX_K) { err = "ks_hpsi_batch: stick tile does not fit next to the descriptor in shared memory"; return KS_ENOMEM; }
+  const YzArgs* ya = (const YzArgs*)dev_desc;
+  const XArgs* xa = (const XArgs*)(ya + nk);
+  const long ncol = (long)P0.n2 * P0.n3;
+  const int bg = ks_x_band_group(ceil_div(ncol, P0.zc_x) * nk, nbmax);
+  const dim3 gyz(l1max * P0.zs_yz, nbmax, nk), gx(ceil_div(ncol, P0.zc_x), ceil_div(nbmax, bg), nk);
+  if (stage < 0 || stage == 0) {
+#define C_(A_, B_) if (P0.n2 == A_ && P0.n3 == B_) k_inv_yz_k<A_, B_><<<gyz, yzcfg<A_, B_>::NT, smem_yz, st>>>(ya);
+    KS_YZ_PAIRS(C_)
+#undef C_
+  }
+  if (stage < 0 || stage == 1) {
+#define C_(N_) if (P0.n1 == N_) k_x_k<N_><<<gx, xcfg<N_>::NT, P0.smem_x, st>>>(xa);
+    KS_X_SIZES(C_)
+#undef C_
+  }
+  if (stage < 0 || stage == 2) {
+    cudaError_t le = cudaSuccess;
+#define C_(A_, B_)                                                                                      \
+    if (P0.n2 == A_ && P0.n3 == B_) {                                                                   \
+      if (yzcfg<A_, B_>::ZS == 1) k_fwd_yz_k<A_, B_><<<gyz, yzcfg<A_, B_>::NT, smem_yz, st>>>(ya);      \
+      else {                                                                                            \
+        cudaLaunchConfig_t cfg = {};                                                                    \
+        cfg.gridDim = gyz; cfg.blockDim = dim3(yzcfg<A_, B_>::NT); cfg.dynamicSmemBytes = smem_yz; cfg.stream = st; \
+        cudaLaunchAttribute at[1];                                                                      \
+        at[0].id = cudaLaunchAttributeClusterDimension;                                                 \
+        at[0].val.clusterDim.x = yzcfg<A_, B_>::ZS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1; \
+        cfg.attrs = at; cfg.numAttrs = 1;                                                               \
+        le = cudaLaunchKernelEx(&cfg, k_fwd_yz_k<A_, B_>, ya);                                          \
+      }                                                                                                 \
+    }
     KS_YZ_PAIRS(C_)
 #undef C_
     KS_CUDA_CHECK(le, err);
@@ -1003,7 +1126,7 @@ int ks_density_batch(HpsiPlan& P, const cplx* psi, const double* occ, int nb, in
   a.psi = psi; a.hpsi = nullptr; a.planes = P.d_planes;
   a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.stick = P.d_stick;
   a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
-  a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.invN = 1.0 / (double)P.N;
+  a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.nb = nb; a.invN = 1.0 / (double)P.N;
   const dim3 gyz(P.L1 * P.zs_yz, nb);
 #define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_inv_yz<A_, B_><<<gyz, yzcfg<A_, B_>::NT, P.smem_yz, st>>>(a);
   KS_YZ_PAIRS(C_)

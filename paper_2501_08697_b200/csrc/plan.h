@@ -47,6 +47,14 @@ int ks_hpsi_configure(HpsiPlan& P, std::string& err);
 int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb, cudaStream_t st,
                          std::string& err, int stage = -1);
 
+// k-batched form of the same three launches (ks_hpsi_batch): the k-points of one group share the FFT grid; every kernel is
+// ONE launch over (plane | column chunk, band, k-point).  The caller owns the descriptor block: ks_kdesc_fill writes
+// ks_kdesc_bytes(nk) bytes on the host, the caller copies them to the device (dev_desc) before the launch.
+struct KItem { const HpsiPlan* P; const cplx* psi; cplx* hpsi; int nb; };
+size_t ks_kdesc_bytes(int nk);
+void ks_kdesc_fill(void* host_desc, const KItem* items, int nk);
+int ks_hpsi_local_launch_k(const KItem* items, int nk, const void* dev_desc, cudaStream_t st, std::string& err, int stage = -1);
+
 // density build: rho(r) += occ_b |psi_b(r)|^2 for one batch of bands (k_inv_yz + k_rho; first != 0 starts a new sum),
 // then ks_density_finish adds the band groups in order and writes rho[n1][n2][n3] in natural order.
 int ks_density_batch(HpsiPlan& P, const cplx* psi, const double* occ, int nb, int first, cudaStream_t st, std::string& err);
@@ -61,6 +69,17 @@ int ks_gemm_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, co
                cplx* C, long ldc, GemmWs* ws, std::string& err);
 int ks_gemm_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb,
                cplx* C, long ldc, int accumulate, std::string& err);
+
+// grouped launches (ks_hpsi_batch): ng independent problems of similar size in one launch; dev_probs is a DEVICE array
+struct GemmProb {
+  const cplx* A; const cplx* B;     // hn: A is K x M, B is K x N ; nn: A is M x K, B is K x N (column-major)
+  cplx* C;                          // hn: partial sums [nsplit][N][M] ; nn: M x N with ldc
+  int M, N, K;
+  long lda, ldb, ldc;
+};
+int ks_gemm_hn_group_nsplit(int ng, int M, int N, int K);
+int ks_gemm_hn_group(cudaStream_t st, const GemmProb* dev_probs, int ng, int M, int N, int nsplit, std::string& err);
+int ks_gemm_nn_group(cudaStream_t st, const GemmProb* dev_probs, int ng, int M, int N, int accumulate, std::string& err);
 
 int ks_peak_run(double* dmma_tf, double* dfma_tf, std::string& err);
 

@@ -32,6 +32,8 @@ _lib.ks_last_error.restype = C.c_char_p
 _lib.ks_supported_sizes.argtypes = [_vp, _i]
 _lib.ks_hpsi.argtypes = [_vp, _vp, _vp, _i]
 _lib.ks_hpsi_host.argtypes = [_vp, _vp, _vp, _i]
+_lib.ks_hpsi_batch.argtypes = [_vp, _i, _vp, _vp, _vp]
+_lib.ks_davidson_batch.argtypes = [_vp, _i, _vp, _vp, _vp, _d, _i, _vp, _vp, _vp, _vp]
 _lib.ks_density.argtypes = [_vp, _vp, _vp, _i, _vp]
 _lib.ks_density_host.argtypes = [_vp, _vp, _vp, _i, _vp]
 _lib.ks_set_overlap.argtypes = [_vp, _vp]
@@ -50,7 +52,7 @@ _lib.ks_dmma_peak.argtypes = [_vp, _vp]
 
 KS_OK, KS_NOTCONV = 0, 1
 EXPORTS = ("ks_pw_count", "ks_pw_list", "ks_create", "ks_destroy", "ks_npw", "ks_set_stream", "ks_set_fft_batch",
-           "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_density", "ks_density_host", "ks_chebyshev", "ks_cg", "ks_set_overlap", "ks_spsi", "ks_davidson", "ks_davidson_host",
+           "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_hpsi_batch", "ks_davidson_batch", "ks_density", "ks_density_host", "ks_chebyshev", "ks_cg", "ks_set_overlap", "ks_spsi", "ks_davidson", "ks_davidson_host",
            "ks_davidson_profile", "ks_profile_begin", "ks_profile_end", "ks_zgemm_hn", "ks_zgemm_nn", "ks_eigh", "ks_dmma_peak")
 
 
@@ -269,6 +271,53 @@ class Context:
         self._check(_lib.ks_davidson_profile(self._h, _hp(ms)))
         keys = ("hpsi", "proj_gemm", "eigh", "rot_gemm", "resid_precond", "orth_gemm", "total")
         return {k: float(ms[i]) for i, k in enumerate(keys)}
+
+
+def _ptr_array(tensors):
+    return (_vp * len(tensors))(*[t.data_ptr() if t is not None and t.numel() else None for t in tensors])
+
+
+def hpsi_batch(ctxs, psis, outs=None):
+    """ks_hpsi_batch: ctxs[i].hpsi(psis[i]) for every k-point in one call (work goes to ctxs[0]'s stream)."""
+    import torch
+    nk = len(ctxs)
+    assert len(psis) == nk
+    if outs is None:
+        outs = [torch.empty_like(t) for t in psis]
+    for c, t, o in zip(ctxs, psis, outs):
+        assert t.is_cuda and t.is_contiguous() and t.dtype == torch.complex128 and t.shape[1] == c.npw
+        assert o.is_cuda and o.is_contiguous() and o.dtype == torch.complex128 and o.shape == t.shape
+    if nk == 0:
+        return outs
+    h = (_vp * nk)(*[c._h for c in ctxs])
+    nb = np.array([t.shape[0] for t in psis], dtype=np.int32)
+    rc = _lib.ks_hpsi_batch(h, nk, _ptr_array(psis), _ptr_array(outs), _hp(nb))
+    if rc < 0:
+        raise KsError(rc, (_lib.ks_last_error(ctxs[0]._h) or b"").decode())
+    return outs
+
+
+def davidson_batch(ctxs, psis, tol=1e-8, max_iter=400):
+    """ks_davidson_batch: psis[i] is overwritten with the eigenvectors of k-point i.  Returns a list of dicts as
+    Context.davidson does."""
+    import torch
+    nk = len(ctxs)
+    assert len(psis) == nk and nk > 0
+    eig = [torch.empty(t.shape[0], dtype=torch.float64, device=t.device) for t in psis]
+    res = [torch.empty(t.shape[0], dtype=torch.float64, device=t.device) for t in psis]
+    for c, t in zip(ctxs, psis):
+        assert t.is_cuda and t.is_contiguous() and t.dtype == torch.complex128 and t.shape[1] == c.npw
+    h = (_vp * nk)(*[c._h for c in ctxs])
+    nb = np.array([t.shape[0] for t in psis], dtype=np.int32)
+    its = np.zeros(nk, dtype=np.int32)
+    nh = np.zeros(nk, dtype=np.int64)
+    st = np.zeros(nk, dtype=np.int32)
+    rc = _lib.ks_davidson_batch(h, nk, _ptr_array(psis), _ptr_array(eig), _hp(nb), float(tol), int(max_iter), _ptr_array(res),
+                                _hp(its), _hp(nh), _hp(st))
+    if rc < 0:
+        raise KsError(rc, (_lib.ks_last_error(ctxs[0]._h) or b"").decode())
+    return [dict(psi=psis[i], eig=eig[i], resid=res[i], iters=int(its[i]), band_applications=int(nh[i]),
+                 converged=(st[i] == KS_OK)) for i in range(nk)]
 
 
 def _stream_ptr(stream):

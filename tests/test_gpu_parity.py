@@ -772,3 +772,94 @@ def test_davidson_cfg2_all_kpoints_time_reversal_and_stored_oracle_solves(ks):
         assert g["converged"] and g["k_index"] == k
         assert np.abs(eig[k] - np.array(g["eig"])).max() <= 1e-8, "k-point %d vs the oracle's solve" % k
     assert seen >= 1, "no stored oracle solve of a cfg 2 k-point found under tests/golden/"
+
+
+# ------------------------------------------------------------------ batched multi-k entry points
+def test_hpsi_batch_all_64_kpoints_of_cfg2(ks, oracle_mod):
+    """ks_hpsi_batch over the whole 4x4x4 Monkhorst-Pack mesh of cfg 2 (Eq. 32 L507 per k): every element of
+    every band of every k-point against the oracle's H psi, and against 64 single ks_hpsi calls."""
+    ps = [I.make_problem(2, k) for k in range(64)]
+    ctxs = [ks.Context.from_problem(p) for p in ps]
+    psis = [_t(p.psi0) for p in ps]
+    outs = ks.hpsi_batch(ctxs, psis)
+    for k, (p, ctx) in enumerate(zip(ps, ctxs)):
+        got = outs[k].cpu().numpy()
+        ref = oracle_mod.Oracle.from_problem(p).hpsi(p.psi0)
+        assert _rel(got, ref) <= HPSI_TOL and _elementwise_ok(got, ref), "k-point %d" % k
+        one = ctx.hpsi(psis[k]).cpu().numpy()
+        assert _rel(got, one) <= 1e-13, "k-point %d vs the single-k call" % k
+    # the call is repeatable bit for bit (fixed summation orders, no atomics)
+    again = ks.hpsi_batch(ctxs, psis)
+    assert all(bool((a == b).all()) for a, b in zip(outs, again))
+
+
+def test_hpsi_batch_ragged_and_edge_cases(ks, oracle_mod):
+    import torch
+    ps = [I.make_problem(2, k, nbands=nb) for k, nb in ((0, 5), (21, 32), (42, 1), (63, 17))]
+    ctxs = [ks.Context.from_problem(p) for p in ps]
+    psis = [_t(p.psi0) for p in ps]
+    # ragged band counts, one empty entry, a group size that does not divide the batch, band slabs smaller than a block
+    p5 = I.make_problem(2, 5, nbands=3)
+    ctxs.append(ks.Context.from_problem(p5))
+    ps.append(p5)
+    psis.append(torch.empty((0, ctxs[4].npw), dtype=torch.complex128, device="cuda"))
+    for ctx in ctxs:
+        ctx.set_fft_batch(7)
+    outs = ks.hpsi_batch(ctxs, psis)
+    for k in range(4):
+        ref = oracle_mod.Oracle.from_problem(ps[k]).hpsi(ps[k].psi0)
+        got = outs[k].cpu().numpy()
+        assert _rel(got, ref) <= HPSI_TOL and _elementwise_ok(got, ref)
+    assert outs[4].shape[0] == 0
+    assert ks.hpsi_batch([], []) == []
+    # no projectors, local + kinetic only: bit-identical to the single-k path (same kernels' arithmetic, no GEMM)
+    q = [I.make_problem(2, k, nbands=4, with_beta=False) for k in (3, 60)]
+    cq = [ks.Context.from_problem(p) for p in q]
+    tq = [_t(p.psi0) for p in q]
+    oq = ks.hpsi_batch(cq, tq)
+    for c, t, o in zip(cq, tq, oq):
+        assert bool((c.hpsi(t) == o).all())
+    # refused: a context twice, mixed grids, aliasing
+    with pytest.raises(ks.KsError):
+        ks.hpsi_batch([ctxs[0], ctxs[0]], [psis[0], psis[0]])
+    other = ks.Context.from_problem(I.make_problem(0))
+    with pytest.raises(ks.KsError):
+        ks.hpsi_batch([ctxs[0], other], [psis[0], _t(I.make_problem(0).psi0)])
+    with pytest.raises(ks.KsError):
+        ks.hpsi_batch([ctxs[1]], [psis[1]], outs=[psis[1]])
+
+
+def test_hpsi_batch_large_grid_cluster_path(ks, oracle_mod):
+    """Two contexts on the 96 x 96 x 288 slab grid (different small spheres): the k-batched forward kernel runs as clusters of
+    three CTAs with the descriptor picked by blockIdx.z."""
+    ps = [I.make_problem(4, ecutwfc=e, grid=(96, 96, 288), nbands=nb, with_beta=False) for e, nb in ((3.0, 3), (6.0, 2))]
+    ctxs = [ks.Context.from_problem(p) for p in ps]
+    outs = ks.hpsi_batch(ctxs, [_t(p.psi0) for p in ps])
+    for p, o in zip(ps, outs):
+        ref = oracle_mod.Oracle.from_problem(p).hpsi(p.psi0)
+        assert _rel(o.cpu().numpy(), ref) <= HPSI_TOL and _elementwise_ok(o.cpu().numpy(), ref)
+
+
+def test_davidson_batch_cfg2(ks):
+    """ks_davidson_batch on 16 k-points of cfg 2 (worker threads, one stream each) against single ks_davidson solves of
+    the same contexts, the survey's printed values, and time reversal between k_i and k_{63-i}."""
+    sel = [0, 1, 5, 21, 26, 31, 32, 37, 42, 58, 62, 63, 10, 53, 7, 56]
+    ps = [I.make_problem(2, k) for k in sel]
+    ctxs = [ks.Context.from_problem(p) for p in ps]
+    rs = ks.davidson_batch(ctxs, [_t(p.psi0) for p in ps], tol=1e-8)
+    eig = {}
+    for k, p, ctx, r in zip(sel, ps, ctxs, rs):
+        assert r["converged"] and float(r["resid"].max()) <= 1e-8
+        eig[k] = r["eig"].cpu().numpy()
+        if k in (0, 21, 63):
+            one = ctx.davidson(_t(p.psi0), tol=1e-8)
+            assert np.abs(one["eig"].cpu().numpy() - eig[k]).max() <= 1e-8
+            assert one["iters"] == r["iters"] and one["band_applications"] == r["band_applications"]
+    g = _gold()["cfg2"]
+    for key in ("k_m38", "k_m18"):
+        e = eig[g[key]["k_index"]]
+        for i, name in ((0, "eps0"), (15, "eps15"), (16, "eps16"), (31, "eps31")):
+            assert abs(e[i] - g[key][name]) <= 1e-8
+    for a in sel:
+        if 63 - a in eig:
+            assert np.abs(eig[a] - eig[63 - a]).max() <= 1e-8
