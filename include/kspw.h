@@ -78,8 +78,7 @@ int ks_hpsi_host(ks_ctx* ctx, const ks_c128* psi_host, ks_c128* hpsi_host, int n
  *
  * ks_hpsi_batch: hpsi[i] = H(k_i) psi[i] for every i, the same arithmetic as nk ks_hpsi calls (bit for bit in the local
  * and kinetic part; the projector sums are split differently over K, so equal to rounding).  Every kernel of the path is
- * ONE launch over (plane | column chunk | tile, band, k-point) per group of k-points; a group is sized so that its live
- * planes stay in L2 between the three FFT kernels.
+ * ONE launch over (plane | column chunk | tile, band, k-point) per group of k-points (default: one group).
  *   ctxs    HOST [nk]  contexts, all distinct, same grid; work is enqueued on the stream of ctxs[0]
  *   psi     HOST [nk]  of DEVICE pointers, psi[i] is [nbands[i]][npw_i]
  *   hpsi    HOST [nk]  of DEVICE pointers, same shapes, must not alias psi[i]
@@ -171,6 +170,10 @@ int ks_eigh(void* stream, int n, ks_c128* A, long lda, double* theta, ks_c128* C
             int* sweeps_out /*HOST, may be NULL*/);
 /* register-resident DMMA m8n8k4 microbenchmark: achieved FP64 tensor TFLOP/s (roofline denominator) */
 int ks_dmma_peak(double* tflops_out /*HOST*/, double* dfma_tflops_out /*HOST, plain DFMA, may be NULL*/);
+/* DMMA result latency probe: SM clocks per DMMA of ONE warp per SM sub-partition that keeps 1, 2, 3, 4, 6, 8 independent
+ * accumulator tiles in flight (HOST out [6]); the first entry is the dependent-issue latency, the last the issue interval.
+ * sm_ghz: the SM clock the times are converted with (bench.py passes the clock it sampled). */
+int ks_dmma_latency(double* clk_per_dmma, double sm_ghz);
 #ifdef __cplusplus
 }
 #endif

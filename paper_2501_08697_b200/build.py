@@ -17,6 +17,9 @@ FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-li
          "-Xcompiler", "-fPIC", "-Wno-deprecated-gpu-targets"]
 
 
+FLAGS += os.environ.get("KSPW_NVCC_FLAGS", "").split()      # e.g. -DKSPW_NO_YHALF (compile-time switches of DESIGN.md §9)
+
+
 def _newest_header() -> float:
     return max(os.path.getmtime(os.path.join(CSRC, f)) for f in os.listdir(CSRC) if f.endswith((".h", ".cuh")))
 

@@ -6,8 +6,7 @@
 // ks_hpsi_batch takes the contexts of all k-points and runs H psi as ONE grid per kernel over (plane | column chunk | tile,
 // band, k-point) for a GROUP of k-points at a time: the three FFT kernels read a per-k descriptor (their own sticks, live
 // planes, |k+G|^2, workspace), the projector products are grouped GEMMs (one launch for beta^H psi of every k of the group,
-// a fused split-K reduction + D apply, one launch for hpsi += beta (D B)).  A group is sized so that its live planes stay
-// in the 126 MB L2 between the three FFT kernels (they are written once, read and written once, read once).
+// a fused split-K reduction + D apply, one launch for hpsi += beta (D B)).  By default all k-points form one group.
 #include "ctx.h"
 #include <algorithm>
 #include <cstdlib>
@@ -67,12 +66,16 @@ void ks_kbatch_free(KBatchWs* w) {
   *w = KBatchWs();
 }
 
-// k-points per group: as many as keep the group's live planes within the L2 budget (KSPW_KBATCH_L2_MB, default 80 MB of the
-// 126 MB L2: the rest holds psi, beta tiles and V(r)); KSPW_KBATCH_GROUP fixes the count.
+// k-points per group.  Measured on cfg 2 (64 k x 32 bands, 54^3; band-applications/s): groups sized to keep their live
+// planes in L2 (2 k-points, 76 MB) 273k; 4 k 335k; 8 k 387k; all 64 k in one group 467k -- a group small enough for L2 is a
+// fraction of a wave per kernel and pays the drain / fill between dependent launches 3 x 32 times, so the default is ONE
+// group (the planes stream through HBM as in the single-k path).  KSPW_KBATCH_GROUP fixes the count, KSPW_KBATCH_L2_MB
+// sizes groups by the planes they hold.
 static int group_size(ks_ctx* const* ctxs, int nk, const int* nbands) {
   static const int env_g = getenv("KSPW_KBATCH_GROUP") ? atoi(getenv("KSPW_KBATCH_GROUP")) : 0;
   if (env_g > 0) return std::min(env_g, nk);
-  static const double l2_mb = getenv("KSPW_KBATCH_L2_MB") ? atof(getenv("KSPW_KBATCH_L2_MB")) : 80.0;
+  static const double l2_mb = getenv("KSPW_KBATCH_L2_MB") ? atof(getenv("KSPW_KBATCH_L2_MB")) : 0.0;
+  if (!(l2_mb > 0)) return std::min(nk, 4096);
   double per = 0;
   for (int i = 0; i < nk; ++i) {
     const HpsiPlan& P = ctxs[i]->P;

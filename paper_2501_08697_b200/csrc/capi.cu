@@ -692,6 +692,10 @@ extern "C" int ks_eigh(void* stream, int n, ks_c128* A, long lda, double* theta,
   std::lock_guard<std::mutex> lk(g_ws_lock);
   return ks_eigh_run((cudaStream_t)stream, n, (cplx*)A, lda, theta, (cplx*)C, ldc, &g_ews, sweeps_out, ks_global_error());
 }
+extern "C" int ks_dmma_latency(double* clk_per_dmma, double sm_ghz) {
+  if (!clk_per_dmma || !(sm_ghz > 0)) return KS_EINVAL;
+  return ks_dmma_latency_run(clk_per_dmma, sm_ghz, ks_global_error());
+}
 extern "C" int ks_dmma_peak(double* tflops_out, double* dfma_tflops_out) {
   return ks_peak_run(tflops_out, dfma_tflops_out, ks_global_error());
 }

@@ -476,14 +476,23 @@ static int reserve(ks_ctx* c, int nb) {
   return KS_OK;
 }
 
-struct Phase {   // optional per-phase timing (KSPW_PROFILE=1): adds a stream sync per phase
+struct Phase {   // optional per-phase timing (KSPW_PROFILE=1; 2 also prints one line per iteration): adds a stream sync per phase
   bool on = false;
+  int level = 0;
+  double mark[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  void iter_line(int it, int m, int nu, int nk, int nl, int sweeps) {     // per-iteration phase times since the last line
+    if (level < 2) return;
+    fprintf(stderr, "dav it %d m %d nu %d nk %d locked %d sweeps %d | hpsi %.3f proj %.3f eigh %.3f rot %.3f resid %.3f orth %.3f ms\n", it, m, nu, nk,
+            nl, sweeps, acc[0] - mark[0], acc[1] - mark[1], acc[2] - mark[2], acc[3] - mark[3], acc[4] - mark[4], acc[5] - mark[5]);
+    for (int i = 0; i < 8; ++i) mark[i] = acc[i];
+  }
   cudaEvent_t a = nullptr, b = nullptr;
   cudaStream_t st = 0;
   double* acc = nullptr;
   void init(cudaStream_t s, double* ms) {
     const char* e = getenv("KSPW_PROFILE");
     on = e && atoi(e) > 0;
+    level = e ? atoi(e) : 0;
     st = s; acc = ms;
     for (int i = 0; i < 8; ++i) ms[i] = 0;
     if (on) { cudaEventCreate(&a); cudaEventCreate(&b); }
@@ -625,6 +634,7 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
   std::vector<int> lockL, lockF, rowF;
   static const bool active_rot = !(getenv("KSPW_ACTIVE_ROT") && atoi(getenv("KSPW_ACTIVE_ROT")) == 0);
   bool stale = false;
+  int dbg_nl = 0, dbg_sw = 0;
   auto rotate_all = [&]() -> int {
     const cplx* Cl = warm ? w.Cp : w.Cm;      // eigenvectors of the last eigensolve (after the end-of-iteration swap)
     RC(ks_gemm_nn(st, npw, nb, m, w.V, npw, Cl, ldh, w.X, npw, 0, c->err));
@@ -726,6 +736,7 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
         nl = (int)lockL.size();
       }
       int sw = 0;
+      dbg_nl = nl;
       if (nl == 0) {
         RC(ks_eigh_run(st, m, w.Hwork, m, w.theta, w.Cq, ldh, &c->ews, &sw, c->err));
         if (getenv("KSPW_DEBUG_SWEEPS")) fprintf(stderr, "it %d m %d nk %d sweeps %d\n", it, m, nk, sw);
@@ -749,6 +760,7 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
         k_copy_mat<<<ceil_div((long)(m - mp) * m, 256), 256, 0, st>>>(m - mp, m, w.Hwork + mp, m, w.Cm + mp, ldh);
       }
       KS_CUDA_CHECK(cudaMemcpyAsync(w.thp, w.theta, sizeof(double) * m, cudaMemcpyDeviceToDevice, st), c->err);
+      dbg_sw = sw;
     }
     ph.end(PH_EIGH);
     // D4
@@ -775,6 +787,7 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
     }
     ph.end(PH_ROT);
     if (warm) { std::swap(w.Cm, w.Cp); mp = m; }   // C of this iteration is C_prev of the next
+    ph.iter_line(it, m, nu, nk, dbg_nl, dbg_sw);
     ++it;
   }
   // D9

@@ -88,11 +88,14 @@ __device__ __forceinline__ void gemm_hn_tile(int M, int N, const cplx* __restric
       for (int i = 0; i < 4; ++i) af[i] = a[(i * 8 + fr) * LDK + ks + fk];
 #pragma unroll
       for (int j = 0; j < NJ; ++j) bf[j] = b[(j * 8 + fr) * LDK + ks + fk];
+      // conj(a) b = (ar br + ai bi) + i (ar bi - ai br).  The two products of one accumulator are two DMMAs apart: enough,
+      // the DMMA result latency is 27 clk against an issue interval of 16 (ks_dmma_latency); spreading them 8 NJ apart
+      // measured no difference (cfg 3: 30.24 vs 30.29 ms)
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
         const double nai = -af[i].y;
 #pragma unroll
-        for (int j = 0; j < NJ; ++j) {   // conj(a) b = (ar br + ai bi) + i (ar bi - ai br)
+        for (int j = 0; j < NJ; ++j) {
           dmma(cre[i][j][0], cre[i][j][1], af[i].x, bf[j].x);
           dmma(cim[i][j][0], cim[i][j][1], af[i].x, bf[j].y);
           dmma(cre[i][j][0], cre[i][j][1], af[i].y, bf[j].y);
@@ -175,15 +178,18 @@ static int launch_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long l
   // (Measured on cfg 1, 8 output tiles: 148 splits 0.84 ms, 37 splits = exactly two waves 0.78 ms.)
   const int per_sm = std::max(1, (int)((227 * 1024) / (smem + 1024)));
   const long slots = 148L * per_sm, tiles = (long)tm * tn;
-  const int max_split = std::max(1, K / (8 * KT));
+  // CTAs of one launch take equal time, so they run as lockstep waves of `slots`: take the split count with the fullest
+  // last wave among those that give at least two waves and keep >= 48 k-tiles per split (the pipeline prologue and the
+  // partial-tile store stay < 1 %).  cfg 3 beta^H psi (81 tiles of 64 x 160): 7 splits = 3.83 waves (ncu: tensor pipe 68 %
+  // active on the SMs that got three CTAs, 91 % on those with four) -> 20 splits = 10.95 waves.
+  const int max_split = std::max(1, K / (48 * KT));
   int nsplit = max_split;
   double best_eff = 0.0;
   for (int sp = 1; sp <= max_split; ++sp) {
     const long total = tiles * sp;
     if (total < 2 * slots && sp < max_split) continue;
     const double eff = (double)total / (double)(ceil_div(total, slots) * slots);
-    if (eff >= 0.93) { nsplit = sp; best_eff = eff; break; }
-    if (eff > best_eff) { best_eff = eff; nsplit = sp; }
+    if (eff > best_eff + 1e-9) { best_eff = eff; nsplit = sp; }
   }
   int kchunk = ceil_div(std::max(K, 1), nsplit);
   kchunk = ceil_div(kchunk, KT) * KT;
@@ -557,6 +563,54 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters) {
 #pragma unroll
   for (int i = 0; i < 16; ++i) s += c[i];
   if (s == 12345.678) out[0] = s;
+}
+
+// DMMA result latency probe: NACC independent accumulators per warp, each DMMA depends on the one NACC issues earlier.
+// 8 warps per SM sub-partition would hide it; ONE warp per sub-partition (128-thread CTA, one CTA per SM) shows it.
+template <int NACC>
+__global__ void __launch_bounds__(128) k_dmma_chain(double* out, int iters) {
+  double c[NACC][2];
+#pragma unroll
+  for (int i = 0; i < NACC; ++i) c[i][0] = c[i][1] = 0.0;
+  const double a = 1.0 + 1e-9 * threadIdx.x, b = 1.0 - 1e-9 * threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) dmma(c[i][0], c[i][1], a, b);
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < NACC; ++i) s += c[i][0] + c[i][1];
+  if (s == 12345.678) out[0] = s;
+}
+// clocks per DMMA of one warp on its sub-partition with NACC = 1, 2, 3, 4, 6, 8 independent accumulators (HOST out [6])
+int ks_dmma_latency_run(double* clk_per_dmma, double sm_ghz, std::string& err) {
+  double* d = nullptr;
+  KS_CUDA_CHECK(cudaMalloc(&d, 8), err);
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int iters = 20000;
+  for (int v = 0; v < 6; ++v) {
+    float best = 1e30f;
+    const int nacc[6] = {1, 2, 3, 4, 6, 8};
+    for (int rep = 0; rep < 3; ++rep) {
+      cudaEventRecord(e0);
+      switch (v) {
+        case 0: k_dmma_chain<1><<<148, 128>>>(d, iters); break;
+        case 1: k_dmma_chain<2><<<148, 128>>>(d, iters); break;
+        case 2: k_dmma_chain<3><<<148, 128>>>(d, iters); break;
+        case 3: k_dmma_chain<4><<<148, 128>>>(d, iters); break;
+        case 4: k_dmma_chain<6><<<148, 128>>>(d, iters); break;
+        default: k_dmma_chain<8><<<148, 128>>>(d, iters); break;
+      }
+      cudaEventRecord(e1);
+      KS_CUDA_CHECK(cudaEventSynchronize(e1), err);
+      float ms; cudaEventElapsedTime(&ms, e0, e1);
+      if (rep) best = std::min(best, ms);
+    }
+    clk_per_dmma[v] = best * 1e-3 * sm_ghz * 1e9 / ((double)iters * nacc[v]);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+  return KS_OK;
 }
 
 int ks_peak_run(double* dmma_tf, double* dfma_tf, std::string& err) {

@@ -23,6 +23,7 @@
 #include "fft.cuh"
 #include "plan.h"
 #include <algorithm>
+#include <type_traits>
 #include <cmath>
 #include <cstdlib>
 #include <vector>
@@ -245,6 +246,7 @@ __device__ __forceinline__ void cp_wait_n(int n) {   // n = groups allowed to st
 #define KS_LD_PLANE(p) (*(p))
 #endif
 
+
 // lines-first walk over (stick s, line j) pairs: item it = j*S + s, it = tid, tid + NT, ...
 struct StickWalk {
   int s, j, ds, dj, S;
@@ -256,6 +258,22 @@ struct StickWalk {
     if (s >= S) { s -= S; ++j; }
   }
 };
+
+// line-first walk over (stick s, line j) pairs, j fastest: item it = s*L + j, it = start, start + step, ...  Used where a
+// thread's line touches GLOBAL memory at psi[first + j1*L + j - z0]: the L lanes of one stick read or write consecutive
+// plane waves (one or two 128-byte lines per stick instead of one line per lane)
+template <int L>
+struct JWalk {
+  int s, j, it, step;
+  __device__ __forceinline__ JWalk(int start, int step_) : it(start), step(step_) { s = it / L; j = it % L; }
+  __device__ __forceinline__ void next() { it += step; s = it / L; j = it % L; }
+};
+
+template <bool JFAST, int L>
+__device__ __forceinline__ typename std::conditional<JFAST, JWalk<L>, StickWalk>::type make_walk(int tid, int nt, int S) {
+  if constexpr (JFAST) return JWalk<L>(tid, nt);
+  else return StickWalk(tid, nt, S);
+}
 
 template <int NY, int NZ>
 __device__ __forceinline__ void inv_yz_body(const YzArgs& a, const int bx, const int b) {
@@ -280,7 +298,13 @@ __device__ __forceinline__ void inv_yz_body(const YzArgs& a, const int bx, const
   const cplx* psi = a.psi + (size_t)b * a.npw;
   // H1 + H2 (z) pass 1: psi -> registers -> DFT-R1z -> twiddle -> stick tile (type A, inverse)
   {
-    StickWalk w(tid, NT, S);
+    // walk over the (stick, line) items of the pass that touches psi: lines-first (StickWalk) or j-fastest (JWalk, the
+    // lanes of a stick read consecutive plane waves).  Measured: 128 x 128 lines-first 0.592 / j-fastest 0.599 ms, 96 x 96
+    // 0.272 / 0.276 ms -- but on the z'-split 96 x 288 planes, where the (stick, line) items of a plane are dealt over the
+    // three CTAs of a cluster, j-fastest took the forward kernel from 33 to 42 % of HBM.  So: j-fastest iff ZS > 1.
+    constexpr bool JFAST = (ZS > 1);
+    typename std::conditional<JFAST, JWalk<R2z>, StickWalk>::type w = make_walk<JFAST, R2z>(tid, NT, S);
+#define KS_W_OK(w_) (JFAST ? ((w_).s < S) : ((w_).j < R2z))
     cplx v[R1z];
     auto load_in = [&]() {
       const int4 si = __ldg(a.stick + s0 + w.s);
@@ -292,12 +316,12 @@ __device__ __forceinline__ void inv_yz_body(const YzArgs& a, const int bx, const
         v[j1] = (idx < si.z) ? src[idx] : cmake(0.0, 0.0);
       }
     };
-    if (w.j < R2z) load_in();
+    if (KS_W_OK(w)) load_in();
     for (int i = tid; i < NY; i += NT) tw_y[i] = a.tw_y[i];
     if (NY != NZ)
       for (int i = tid; i < NZ; i += NT) tw_z[i] = a.tw_z[i];
     __syncthreads();
-    while (w.j < R2z) {
+    while (KS_W_OK(w)) {
       dft<R1z, +1>(v);
       cplx* o = stile + w.s * SZ + w.j;
       const int j2 = w.j;
@@ -310,7 +334,7 @@ __device__ __forceinline__ void inv_yz_body(const YzArgs& a, const int bx, const
         }
       }
       w.next();
-      if (w.j < R2z) load_in();
+      if (KS_W_OK(w)) load_in();
     }
   }
   __syncthreads();
@@ -586,7 +610,7 @@ __device__ __forceinline__ void fwd_yz_body(const YzArgs& a, const int bx, const
 #pragma unroll
     for (int r = 0; r < ZS; ++r) peer[r] = (const cplx*)cl.map_shared_rank((void*)stile, r);
     // last pass + H5: the (stick, q2) items of the plane are dealt over the ZS CTAs; line k1 lives in CTA k1 / K1H
-    for (StickWalk w(h * NT + tid, ZS * NT, S); w.j < R2z; w.next()) {
+    for (JWalk<R2z> w(h * NT + tid, ZS * NT); w.s < S; w.next()) {   // j-fastest: see k_inv_yz
       const int4 si = __ldg(a.stick + s0 + w.s);
       cplx v[R1z];
       const int off = w.s * SZ + w.j;

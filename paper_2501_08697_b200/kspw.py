@@ -49,11 +49,12 @@ _lib.ks_zgemm_hn.argtypes = [_vp, _i, _i, _i, _vp, _l, _vp, _l, _vp, _l]
 _lib.ks_zgemm_nn.argtypes = [_vp, _i, _i, _i, _vp, _l, _vp, _l, _vp, _l, _i]
 _lib.ks_eigh.argtypes = [_vp, _i, _vp, _l, _vp, _vp, _l, _vp]
 _lib.ks_dmma_peak.argtypes = [_vp, _vp]
+_lib.ks_dmma_latency.argtypes = [_vp, _d]
 
 KS_OK, KS_NOTCONV = 0, 1
 EXPORTS = ("ks_pw_count", "ks_pw_list", "ks_create", "ks_destroy", "ks_npw", "ks_set_stream", "ks_set_fft_batch",
            "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_hpsi_batch", "ks_davidson_batch", "ks_density", "ks_density_host", "ks_chebyshev", "ks_cg", "ks_set_overlap", "ks_spsi", "ks_davidson", "ks_davidson_host",
-           "ks_davidson_profile", "ks_profile_begin", "ks_profile_end", "ks_zgemm_hn", "ks_zgemm_nn", "ks_eigh", "ks_dmma_peak")
+           "ks_davidson_profile", "ks_profile_begin", "ks_profile_end", "ks_zgemm_hn", "ks_zgemm_nn", "ks_eigh", "ks_dmma_peak", "ks_dmma_latency")
 
 
 class KsError(RuntimeError):
@@ -365,6 +366,15 @@ def ks_eigh(A, stream=None):
     if rc:
         raise KsError(rc, _glob_err())
     return th, Cm, sw.value
+
+
+def ks_dmma_latency(sm_ghz=1.965):
+    """clocks per DMMA of one warp per sub-partition with 1, 2, 3, 4, 6, 8 independent accumulators"""
+    out = np.zeros(6)
+    rc = _lib.ks_dmma_latency(_hp(out), float(sm_ghz))
+    if rc:
+        raise KsError(rc, _glob_err())
+    return dict(zip((1, 2, 3, 4, 6, 8), (float(x) for x in out)))
 
 
 def ks_dmma_peak():

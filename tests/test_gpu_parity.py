@@ -863,3 +863,82 @@ def test_davidson_batch_cfg2(ks):
     for a in sel:
         if 63 - a in eig:
             assert np.abs(eig[a] - eig[63 - a]).max() <= 1e-8
+
+
+# ------------------------------------------------------------------ stand-ins for compute-sanitizer (profiles/r2_sanitizer.md)
+def _disturber(stream, n):
+    """a bandwidth-heavy kernel on another stream: changes which CTAs are co-resident and when"""
+    import torch
+    with torch.cuda.stream(stream):
+        a = torch.empty(n, dtype=torch.float32, device="cuda")
+        a.fill_(1.0)
+        a.mul_(1.0001)
+    return a
+
+
+@pytest.mark.parametrize("which", ["cfg1_bg8", "cfg1_ragged31", "slab288_cluster", "cube128", "cfg2_kbatch", "slab288_kbatch"])
+def test_hpsi_repeatability_stress(ks, which):
+    """200 repeats of one block apply must give the same BITS every time (fixed summation orders, no atomics), also while
+    another stream keeps the SMs and HBM busy: a shared-memory or cp.async hazard (k_x's barrier-free refill, the DSMEM
+    exchange of the cluster kernel) would show up as a repeat that differs."""
+    import torch
+    if which == "cfg1_bg8":
+        ps = [I.make_problem(1, nbands=64, with_beta=False)]
+    elif which == "cfg1_ragged31":
+        ps = [I.make_problem(1, nbands=31)]
+    elif which == "slab288_cluster":
+        ps = [I.make_problem(4, ecutwfc=12.0, grid=(96, 96, 288), nbands=6, with_beta=False)]
+    elif which == "cube128":
+        ps = [I.make_problem(3, ecutwfc=6.0, grid=(128, 128, 128), nbands=6, with_beta=False)]
+    elif which == "cfg2_kbatch":
+        ps = [I.make_problem(2, k, nbands=8) for k in (0, 21, 42, 63, 5)]
+    else:
+        ps = [I.make_problem(4, ecutwfc=e, grid=(96, 96, 288), nbands=3, with_beta=False) for e in (3.0, 6.0)]
+    ctxs = [ks.Context.from_problem(p) for p in ps]
+    psis = [_t(p.psi0) for p in ps]
+    batch = which.endswith("kbatch")
+
+    def apply():
+        return ks.hpsi_batch(ctxs, psis) if batch else [ctxs[0].hpsi(psis[0])]
+
+    first = [o.clone() for o in apply()]
+    side = torch.cuda.Stream()
+    keep = []
+    for rep in range(200):
+        if rep % 3 != 2:
+            keep.append(_disturber(side, (1 + rep % 7) * (1 << 22)))
+        outs = apply()
+        for a, b in zip(first, outs):
+            assert bool((a == b).all()), "repeat %d differs" % rep
+        keep = keep[-2:]
+    torch.cuda.synchronize()
+
+
+def test_hpsi_guard_zones(ks):
+    """psi / hpsi are slices of larger buffers; the borders hold a pattern that every entry point must leave alone."""
+    import torch
+    pat = complex(1.25e300, -7.5e-300)
+    for ps, batch in (([I.make_problem(0)], False), ([I.make_problem(1, nbands=31)], False),
+                      ([I.make_problem(2, k, nbands=nb) for k, nb in ((0, 5), (21, 32), (63, 17))], True),
+                      ([I.make_problem(4, ecutwfc=3.0, grid=(96, 96, 288), nbands=3, with_beta=False)], False)):
+        ctxs = [ks.Context.from_problem(p) for p in ps]
+        G = 4096
+        bufs_in, bufs_out, psis, outs = [], [], [], []
+        for p in ps:
+            n = p.nbands * p.npw
+            bi = torch.full((n + 2 * G,), pat, dtype=torch.complex128, device="cuda")
+            bo = torch.full((n + 2 * G,), pat, dtype=torch.complex128, device="cuda")
+            bi[G:G + n] = _t(p.psi0).reshape(-1)
+            bufs_in.append(bi); bufs_out.append(bo)
+            psis.append(bi[G:G + n].view(p.nbands, p.npw)); outs.append(bo[G:G + n].view(p.nbands, p.npw))
+        if batch:
+            ks.hpsi_batch(ctxs, psis, outs)
+        else:
+            ctxs[0].hpsi(psis[0], out=outs[0])
+        torch.cuda.synchronize()
+        for p, bi, bo, o in zip(ps, bufs_in, bufs_out, outs):
+            n = p.nbands * p.npw
+            for b in (bi, bo):
+                assert bool((b[:G] == pat).all()) and bool((b[G + n:] == pat).all()), "guard zone overwritten"
+            assert bool((bi[G:G + n].view(p.nbands, p.npw) == _t(p.psi0)).all()), "input block modified"
+            assert bool(torch.isfinite(o.real).all()) and float(o.abs().max()) < 1e6
