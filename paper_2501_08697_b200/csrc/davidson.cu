@@ -48,9 +48,10 @@ __device__ __forceinline__ double block_sum(double v, double* sh) {
 __global__ void __launch_bounds__(RED_THREADS) k_resid_norms(int npw, const cplx* __restrict__ X, const cplx* __restrict__ SX,
                                                              const cplx* __restrict__ HX,
                                                              const double* __restrict__ eps, const double* __restrict__ g2,
-                                                             double* __restrict__ rho, double* __restrict__ ekin) {
+                                                             double* __restrict__ rho, double* __restrict__ ekin,
+                                                             const int* __restrict__ list) {
   __shared__ double sh[RED_THREADS / 32];
-  const int i = blockIdx.x;
+  const int i = list ? list[blockIdx.x] : blockIdx.x;      // list: only the bands whose Ritz vectors changed
   const cplx* x = X + (size_t)i * npw;
   const cplx* sx = SX + (size_t)i * npw;       // = x when S = I
   const cplx* h = HX + (size_t)i * npw;
@@ -634,6 +635,7 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
   std::vector<int> lockL, lockF, rowF;
   static const bool active_rot = !(getenv("KSPW_ACTIVE_ROT") && atoi(getenv("KSPW_ACTIVE_ROT")) == 0);
   bool stale = false;
+  int n_changed = -1;        // bands whose X, HX changed since the last residual evaluation (-1: all)
   int dbg_nl = 0, dbg_sw = 0;
   auto rotate_all = [&]() -> int {
     const cplx* Cl = warm ? w.Cp : w.Cm;      // eigenvectors of the last eigensolve (after the end-of-iteration swap)
@@ -641,6 +643,7 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
     RC(ks_gemm_nn(st, npw, nb, m, w.W, npw, Cl, ldh, w.HX, npw, 0, c->err));
     if (gen) RC(ks_gemm_nn(st, npw, nb, m, w.SV, npw, Cl, ldh, w.SX, npw, 0, c->err));
     stale = false;
+    n_changed = -1;
     return KS_OK;
   };
   // leaving the loop with no correction left (every one was dropped as dependent): D9 must return X, HX, rho that
@@ -648,13 +651,18 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
   auto refresh_if_stale = [&]() -> int {
     if (!stale) return KS_OK;
     RC(rotate_all());
-    k_resid_norms<<<nb, RED_THREADS, 0, st>>>(npw, w.X, gen ? w.SX : w.X, w.HX, w.theta, c->P.d_g2, w.rho, w.ekin);
+    k_resid_norms<<<nb, RED_THREADS, 0, st>>>(npw, w.X, gen ? w.SX : w.X, w.HX, w.theta, c->P.d_g2, w.rho, w.ekin, nullptr);
     return KS_OK;
   };
   for (;;) {
     // D5
     ph.begin();
-    k_resid_norms<<<nb, RED_THREADS, 0, st>>>(npw, w.X, gen ? w.SX : w.X, w.HX, w.theta, c->P.d_g2, w.rho, w.ekin);
+    // a locked band keeps its Ritz value and its (not rotated) vectors, so its residual cannot have changed: after an
+    // active-band rotation only the nu rotated bands (w.act) are re-evaluated
+    if (n_changed >= 0 && lock_on)
+      k_resid_norms<<<n_changed, RED_THREADS, 0, st>>>(npw, w.X, gen ? w.SX : w.X, w.HX, w.theta, c->P.d_g2, w.rho, w.ekin, w.act);
+    else
+      k_resid_norms<<<nb, RED_THREADS, 0, st>>>(npw, w.X, gen ? w.SX : w.X, w.HX, w.theta, c->P.d_g2, w.rho, w.ekin, nullptr);
     KS_CUDA_CHECK(cudaMemcpyAsync(rho.data(), w.rho, sizeof(double) * nb, cudaMemcpyDeviceToHost, st), c->err);
     KS_CUDA_CHECK(cudaStreamSynchronize(st), c->err);
     ph.end(PH_RESID);
@@ -736,10 +744,13 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
         nl = (int)lockL.size();
       }
       int sw = 0;
+      // the sweep count costs a blocking read: only when somebody looks at it
+      static const bool dbg_sweeps = getenv("KSPW_DEBUG_SWEEPS") != nullptr;
+      int* swp = (dbg_sweeps || ph.level >= 2) ? &sw : nullptr;
       dbg_nl = nl;
       if (nl == 0) {
-        RC(ks_eigh_run(st, m, w.Hwork, m, w.theta, w.Cq, ldh, &c->ews, &sw, c->err));
-        if (getenv("KSPW_DEBUG_SWEEPS")) fprintf(stderr, "it %d m %d nk %d sweeps %d\n", it, m, nk, sw);
+        RC(ks_eigh_run(st, m, w.Hwork, m, w.theta, w.Cq, ldh, &c->ews, swp, c->err));
+        if (dbg_sweeps) fprintf(stderr, "it %d m %d nk %d sweeps %d\n", it, m, nk, sw);
         // C = Q C'
         RC(ks_gemm_nn(st, mp, m, mp, w.Cp, ldh, w.Cq, ldh, w.Cm, ldh, 0, c->err));
         k_copy_mat<<<ceil_div((long)(m - mp) * m, 256), 256, 0, st>>>(m - mp, m, w.Cq + mp, ldh, w.Cm + mp, ldh);
@@ -751,8 +762,8 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
         KS_CUDA_CHECK(cudaMemcpyAsync(dR, rowF.data(), sizeof(int) * m, cudaMemcpyHostToDevice, st), c->err);
         // Hc is not needed again before the next D2, but it must survive: the gathered problem goes to Cm (free until D4)
         k_gather_sub<<<ceil_div((long)mf * mf, 256), 256, 0, st>>>(mf, dF, w.Hwork, m, w.Cm);
-        RC(ks_eigh_run(st, mf, w.Cm, mf, w.thf, w.Cq, ldh, &c->ews, &sw, c->err));
-        if (getenv("KSPW_DEBUG_SWEEPS")) fprintf(stderr, "it %d m %d nk %d locked %d sweeps %d\n", it, m, nk, nl, sw);
+        RC(ks_eigh_run(st, mf, w.Cm, mf, w.thf, w.Cq, ldh, &c->ews, swp, c->err));
+        if (dbg_sweeps) fprintf(stderr, "it %d m %d nk %d locked %d sweeps %d\n", it, m, nk, nl, sw);
         k_merge_order<<<ceil_div(m, 128), 128, 0, st>>>(nl, dL, w.thp, mf, w.thf, w.theta, w.src);
         k_assemble_cprime<<<ceil_div((long)m * m, 256), 256, 0, st>>>(m, w.src, dL, dR, w.Cq, ldh, w.Hwork);
         // C = Q C'  (C' in Hwork, leading dimension m)
@@ -770,6 +781,7 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
       RC(ks_gemm_nn(st, npw, nb, m, w.W, npw, w.Cm, ldh, w.HX, npw, 0, c->err));
       if (gen) RC(ks_gemm_nn(st, npw, nb, m, w.SV, npw, w.Cm, ldh, w.SX, npw, 0, c->err));
       stale = false;
+      n_changed = -1;
     } else {
       // idx[0:nu] = the bands that were unconverged at this iteration's D5
       KS_CUDA_CHECK(cudaMemcpyAsync(w.act, idx.data(), sizeof(int) * nu, cudaMemcpyHostToDevice, st), c->err);
@@ -784,6 +796,7 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
         k_scatter_bands<<<gs, 256, 0, st>>>(npw, nu, w.act, w.T, w.SX);
       }
       stale = true;
+      n_changed = nu;
     }
     ph.end(PH_ROT);
     if (warm) { std::swap(w.Cm, w.Cp); mp = m; }   // C of this iteration is C_prev of the next

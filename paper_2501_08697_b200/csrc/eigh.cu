@@ -20,6 +20,8 @@
 #include <atomic>
 #include <cstdlib>
 #include <vector>
+#include <cooperative_groups.h>
+namespace cg = cooperative_groups;
 
 #define JB 32            // block size of the block method
 #define JS (2 * JB)      // pair problem size
@@ -362,7 +364,7 @@ __global__ void k_gather_cols(const cplx* __restrict__ Vp, int np, const int* __
 
 void ks_eigh_free(EighWs* ws) {
   cudaFree(ws->U); cudaFree(ws->Ap); cudaFree(ws->Vp); cudaFree(ws->diag); cudaFree(ws->red);
-  cudaFree(ws->order); cudaFree(ws->pairs); cudaFree(ws->where); cudaFree(ws->Ap2);
+  cudaFree(ws->order); cudaFree(ws->pairs); cudaFree(ws->where); cudaFree(ws->Ap2); cudaFree(ws->red_sweeps);
   *ws = EighWs();
 }
 
@@ -393,8 +395,8 @@ static int eigh_reserve(EighWs* ws, int np, std::string& err) {
 // leading dimension (33) in shared memory: a half-warp reads one row segment, conflict-free.
 // ------------------------------------------------------------------------------------------------
 #define JU_LD 33
-__device__ __forceinline__ void jac_upd_tile(cplx* sm, cplx* __restrict__ Ap, cplx* __restrict__ Vp, long ld, int npair,
-                                             const int2* __restrict__ pairs, const cplx* __restrict__ U, int b, int ay) {
+__device__ __forceinline__ void jac_upd_tile(cplx* sm, cplx* Ap, cplx* Vp, long ld, int npair,
+                                             const int2* __restrict__ pairs, const cplx* U, int b, int ay) {
   cplx *sT = sm, *sUa = sm + 32 * JU_LD, *sUb = sm + 64 * JU_LD;
   const int tid = threadIdx.x;
   const bool isA = ay < npair;
@@ -453,6 +455,74 @@ __global__ void __launch_bounds__(256) k_jac_upd32(cplx* __restrict__ Ap, cplx* 
                                                    const int2* __restrict__ pairs, const cplx* __restrict__ U) {
   extern __shared__ cplx sm[];
   jac_upd_tile(sm, Ap, Vp, ld, npair, pairs, U, blockIdx.x, blockIdx.y);
+}
+
+// ------------------------------------------------------------------------------------------------
+// The whole solve in ONE cooperative launch (64 < n, padded size < 512): every sweep tests the off-diagonal norm on the
+// device and every round is [pair solves] grid.sync [tile updates] grid.sync, with the pairs and tiles dealt over the
+// resident CTAs.  Launch by launch the same rounds cost ~37 us each at n = 320 (two launches of a few microseconds of work
+// plus one blocking host read per sweep); here a round is two grid barriers plus the pair solve.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_jac_coop32(cplx* Ap, cplx* Vp, int np, int n, int nblk, const int2* __restrict__ pairs_all,
+                                                    cplx* U, double* red /* [2 * max_sweeps], zeroed */, int inner, int cross_rounds,
+                                                    double tol2, int max_sweeps, int* __restrict__ sweeps_out) {
+  cg::grid_group grid = cg::this_grid();
+  extern __shared__ cplx sm[];
+  const int tid = threadIdx.x, npair = nblk / 2, nbk = JB / 2;
+  const int ntile = npair * (npair + np / 32);
+  int sweep = 0;
+  for (; sweep < max_sweeps; ++sweep) {
+    // off(A)_F^2 and ||A||_F^2 of the n x n part, fixed partition of the elements over the grid
+    double off = 0, tot = 0;
+    for (long e = blockIdx.x * 256L + tid; e < (long)np * np; e += (long)gridDim.x * 256) {
+      const int i = (int)(e % np), j = (int)(e / np);
+      if (i < n && j < n) {
+        const cplx a = Ap[e];
+        const double v = a.x * a.x + a.y * a.y;
+        tot += v;
+        if (i != j) off += v;
+      }
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+      off += __shfl_xor_sync(0xffffffffu, off, o);
+      tot += __shfl_xor_sync(0xffffffffu, tot, o);
+    }
+    if ((tid & 31) == 0 && tot != 0.0) { atomicAdd(&red[2 * sweep], off); atomicAdd(&red[2 * sweep + 1], tot); }
+    grid.sync();
+    const double goff = __ldcg(&red[2 * sweep]), gtot = __ldcg(&red[2 * sweep + 1]);
+    if (goff <= tol2 * gtot) break;              // the same two numbers in every CTA: a uniform decision
+    for (int r = 0; r < nblk - 1; ++r) {
+      const int2* pr = pairs_all + (size_t)r * npair;
+      const int cross = (r > 0 && cross_rounds) ? 1 : 0;
+      for (int p = blockIdx.x; p < npair; p += gridDim.x) {
+        // pair problem p: gather the 32 x 32 block, one inner sweep, rotations to U[p]
+        const int ns = 2 * nbk, LD = ns + 1;
+        cplx* As = sm;
+        cplx* Vs = As + ns * LD;
+        const int2 pq = pr[p];
+        __syncthreads();
+        for (int e = tid; e < ns * ns; e += 256) {
+          const int i = e % ns, j = e / ns;
+          const int gi = (i < nbk ? pq.x * nbk + i : pq.y * nbk + i - nbk);
+          const int gj = (j < nbk ? pq.x * nbk + j : pq.y * nbk + j - nbk);
+          As[i * LD + j] = Ap[(long)gj * np + gi];
+        }
+        jac_solve_smem(As, Vs, Vs + ns * LD, nbk, inner, 1e-30, cross);
+        cplx* Uo = U + (size_t)p * ns * ns;
+        for (int e = tid; e < ns * ns; e += 256) {
+          const int i = e % ns, j = e / ns;
+          Uo[(size_t)j * ns + i] = Vs[i * LD + j];
+        }
+      }
+      grid.sync();
+      for (int t = blockIdx.x; t < ntile; t += gridDim.x) {
+        __syncthreads();
+        jac_upd_tile(sm, Ap, Vp, np, npair, pr, U, t % npair, t / npair);
+      }
+      grid.sync();
+    }
+  }
+  if (blockIdx.x == 0 && tid == 0) *sweeps_out = sweep;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -592,7 +662,7 @@ __global__ void __launch_bounds__(256) k_jac_round32(const cplx* __restrict__ Ao
 
 template <int JSZ>
 static int block_sweeps(cudaStream_t st, int n, const cplx* A, long lda, EighWs* ws, double tol2, int inner, int* sweeps_out,
-                        std::string& err) {
+                        bool want_sweeps, std::string& err) {
   constexpr int JBK = JSZ / 2;
   constexpr int WNc = JSZ / 16, MT = (8 / WNc) * 32;          // k_jac_col tile rows
   constexpr int WMr = JSZ / 32, NT = (8 / WMr) * 16;          // k_jac_row tile columns
@@ -640,6 +710,41 @@ static int block_sweeps(cudaStream_t st, int n, const cplx* A, long lda, EighWs*
   static const bool cross_rounds = !(getenv("KSPW_JAC_CROSS") && atoi(getenv("KSPW_JAC_CROSS")) == 0);
   static const bool one_launch = !(getenv("KSPW_JAC_ROUND") && atoi(getenv("KSPW_JAC_ROUND")) == 0);
   int sweeps = 0;
+  static const bool coop_on = !(getenv("KSPW_JAC_COOP") && atoi(getenv("KSPW_JAC_COOP")) == 0);
+  if (JSZ == 32 && fused_upd && coop_on && np < 512) {
+    // one cooperative launch for the whole solve; the sweep count comes back with the next blocking read of the caller
+    const size_t smem_coop = std::max(sizeof(cplx) * 96 * JU_LD, smem_cta);
+    static std::atomic<int> coop_ctas{0};
+    if (coop_ctas.load() == 0) {
+      KS_CUDA_CHECK(cudaFuncSetAttribute(k_jac_coop32, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_coop), err);
+      int per_sm = 0, dev = 0, nsm = 0, coop = 0;
+      KS_CUDA_CHECK(cudaGetDevice(&dev), err);
+      KS_CUDA_CHECK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev), err);
+      KS_CUDA_CHECK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev), err);
+      KS_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_jac_coop32, 256, smem_coop), err);
+      coop_ctas.store(coop ? std::max(1, per_sm * nsm) : -1);
+    }
+    if (coop_ctas.load() > 0) {
+      if (!ws->red_sweeps) KS_CUDA_CHECK(cudaMalloc(&ws->red_sweeps, sizeof(double) * 2 * 40 + sizeof(int) * 2), err);
+      KS_CUDA_CHECK(cudaMemsetAsync(ws->red_sweeps, 0, sizeof(double) * 2 * 40 + sizeof(int) * 2, st), err);
+      int* d_sweeps = (int*)(ws->red_sweeps + 2 * 40);
+      const int ntile = npair * (npair + np / 32);
+      const int grid = std::min(coop_ctas.load(), std::max(ntile, npair));
+      cplx *Ap_ = ws->Ap, *Vp_ = ws->Vp, *U_ = ws->U;
+      const int2* pairs_ = ws->pairs;
+      double* red_ = ws->red_sweeps;
+      int np_ = np, n_ = n, nblk_ = nblk, inner_ = inner, cross_ = cross_rounds ? 1 : 0, maxs = 40;
+      double tol2_ = tol2;
+      void* args[] = {&Ap_, &Vp_, &np_, &n_, &nblk_, &pairs_, &U_, &red_, &inner_, &cross_, &tol2_, &maxs, &d_sweeps};
+      KS_CUDA_CHECK(cudaLaunchCooperativeKernel((void*)k_jac_coop32, dim3(grid), dim3(256), args, smem_coop, st), err);
+      if (want_sweeps) {
+        KS_CUDA_CHECK(cudaMemcpyAsync(&sweeps, d_sweeps, sizeof(int), cudaMemcpyDeviceToHost, st), err);
+        KS_CUDA_CHECK(cudaStreamSynchronize(st), err);
+      }
+      *sweeps_out = sweeps;
+      return sweeps >= 40 ? KS_NOTCONV : KS_OK;
+    }
+  }
   if (JSZ == 32 && fused_upd && one_launch && np >= 512) {   // below ~500 the solver CTAs' own tile products outweigh the overlap
     // one launch per round: the launch that applies round r also solves the pair problems of round r+1
     const size_t smem_round = sizeof(cplx) * 128 * JU_LD + 2048;
@@ -741,8 +846,8 @@ int ks_eigh_run(cudaStream_t st, int n, cplx* A, long lda, double* theta, cplx* 
     force_blk = e ? atoi(e) : 0;
   }
   const bool use32 = force_blk != 64;   // 32-wide pairs win at every size measured (n = 320 .. 1040)
-  if (use32) rc = block_sweeps<32>(st, n, A, lda, ws, tol2, inner, &sweeps, err);
-  else rc = block_sweeps<64>(st, n, A, lda, ws, tol2, inner, &sweeps, err);
+  if (use32) rc = block_sweeps<32>(st, n, A, lda, ws, tol2, inner, &sweeps, sweeps_out != nullptr, err);
+  else rc = block_sweeps<64>(st, n, A, lda, ws, tol2, inner, &sweeps, sweeps_out != nullptr, err);
   if (rc < 0) return rc;
   const int notconv = rc;      // KS_NOTCONV: 40 sweeps did not reach off_F <= 1e-14 ||A||_F; the best pairs are still written
   const int np = ws->np;

@@ -182,14 +182,21 @@ static int launch_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long l
   // last wave among those that give at least two waves and keep >= 48 k-tiles per split (the pipeline prologue and the
   // partial-tile store stay < 1 %).  cfg 3 beta^H psi (81 tiles of 64 x 160): 7 splits = 3.83 waves (ncu: tensor pipe 68 %
   // active on the SMs that got three CTAs, 91 % on those with four) -> 20 splits = 10.95 waves.
-  const int max_split = std::max(1, K / (48 * KT));
-  int nsplit = max_split;
-  double best_eff = 0.0;
-  for (int sp = 1; sp <= max_split; ++sp) {
-    const long total = tiles * sp;
-    if (total < 2 * slots && sp < max_split) continue;
-    const double eff = (double)total / (double)(ceil_div(total, slots) * slots);
-    if (eff > best_eff + 1e-9) { best_eff = eff; nsplit = sp; }
+  const int cap_long = std::max(1, K / (48 * KT)), cap_short = std::max(1, K / (8 * KT));
+  int nsplit;
+  if (tiles * cap_long >= 2 * slots) {
+    nsplit = cap_long;
+    double best_eff = 0.0;
+    for (int sp = 1; sp <= cap_long; ++sp) {
+      const long total = tiles * sp;
+      if (total < 2 * slots) continue;
+      const double eff = (double)total / (double)(ceil_div(total, slots) * slots);
+      if (eff > best_eff + 1e-9) { best_eff = eff; nsplit = sp; }
+    }
+  } else {
+    // a small product (few tiles, short K): it cannot fill two waves with long splits, so fill ONE wave as far as splits of
+    // at least 8 k-tiles allow (cfg 2: 1 tile x 66 splits; with 48-tile splits it ran on 11 CTAs and cost 50 us more per call)
+    nsplit = (int)std::max(1L, std::min((long)cap_short, (slots + tiles - 1) / tiles));
   }
   int kchunk = ceil_div(std::max(K, 1), nsplit);
   kchunk = ceil_div(kchunk, KT) * KT;

@@ -90,6 +90,7 @@ struct EighWs {
   cplx* Vp = nullptr;      // padded eigenvector accumulator [np*np]
   double* diag = nullptr;  // [np]
   double* red = nullptr;   // [2] off^2, tot^2
+  double* red_sweeps = nullptr;   // cooperative solve: [2 x 40] off^2, tot^2 per sweep, then the sweep count (int)
   int* order = nullptr;    // [np]
   int2* pairs = nullptr;   // [(nblk-1)][nblk/2] block pairs of every round
   int2* where = nullptr;   // [(nblk-1)][nblk] block -> (index of its pair in the round, 0/1 = first/second of the pair)
