@@ -23,6 +23,12 @@
 #include <cstdlib>
 
 #define GEMM_THREADS 256
+#ifndef KS_EARLY
+#define KS_EARLY 8      // k-step (0, 4, 8, 12) before which warps 0..3 / 4..7 issue their cp.async of the stage after next
+#endif
+#ifndef KS_LATE
+#define KS_LATE 4
+#endif
 #define GEMM_STAGES 3
 #define KT 16          // complex K elements per stage
 #define LDK (KT + 4)   // "k-contiguous" tile leading dimension: == 4 (mod 8) -> conflict-free fragment loads
@@ -74,15 +80,33 @@ __device__ __forceinline__ void gemm_hn_tile(int M, int N, const cplx* __restric
     cp_commit();
   }
   const int fr = lane >> 2, fk = lane & 3;
+  // The two warps of an SM sub-partition (w, w + 4) leave the barrier together.  If both then spend ~130 instructions on
+  // the addresses and cp.async of the stage after next, the DMMA pipe of that sub-partition idles for that long at every
+  // k-tile (ncu, cfg 3: pipe 87 % active inside a CTA).  So warps 4..7 start their DMMAs at once and issue their share of the
+  // loads after the first k-step, when warps 0..3 are computing: one warp alone keeps the pipe full (ks_dmma_latency).
+#ifdef KSPW_GEMM_NO_STAGGER
+  const bool late = false;
+#else
+  const bool late = warp >= 4;
+#endif
   for (int kt = 0; kt < ntile; ++kt) {
     cp_wait<GEMM_STAGES - 2>();
     __syncthreads();
-    if (kt + GEMM_STAGES - 1 < ntile) load_stage((kt + GEMM_STAGES - 1) % GEMM_STAGES, kt + GEMM_STAGES - 1);
+    const bool more = kt + GEMM_STAGES - 1 < ntile;
+#ifdef KSPW_GEMM_NO_STAGGER
+    if (more) load_stage((kt + GEMM_STAGES - 1) % GEMM_STAGES, kt + GEMM_STAGES - 1);
     cp_commit();
+#endif
     const cplx* a = sA + ((kt % GEMM_STAGES) * HN_MT + wm * 32) * LDK;
     const cplx* b = sB + ((kt % GEMM_STAGES) * HN_NT + wn * 8 * NJ) * LDK;
 #pragma unroll
     for (int ks = 0; ks < KT; ks += 4) {
+#ifndef KSPW_GEMM_NO_STAGGER
+      if (ks == (late ? KS_LATE : KS_EARLY)) {
+        if (more) load_stage((kt + GEMM_STAGES - 1) % GEMM_STAGES, kt + GEMM_STAGES - 1);
+        cp_commit();
+      }
+#endif
       cplx af[4], bf[NJ];
 #pragma unroll
       for (int i = 0; i < 4; ++i) af[i] = a[(i * 8 + fr) * LDK + ks + fk];
@@ -370,15 +394,29 @@ __device__ __forceinline__ void gemm_nn_tile(int M, int N, int K, const cplx* __
     cp_commit();
   }
   const int fr = lane >> 2, fk = lane & 3;
+#ifdef KSPW_GEMM_NO_STAGGER
+  const bool late = false;
+#else
+  const bool late = warp >= 4;      // see gemm_hn_tile: the two warps of a sub-partition issue their loads at different times
+#endif
   for (int kt = 0; kt < ntile; ++kt) {
     cp_wait<GEMM_STAGES - 2>();
     __syncthreads();
-    if (kt + GEMM_STAGES - 1 < ntile) load_stage((kt + GEMM_STAGES - 1) % GEMM_STAGES, kt + GEMM_STAGES - 1);
+    const bool more = kt + GEMM_STAGES - 1 < ntile;
+#ifdef KSPW_GEMM_NO_STAGGER
+    if (more) load_stage((kt + GEMM_STAGES - 1) % GEMM_STAGES, kt + GEMM_STAGES - 1);
     cp_commit();
+#endif
     const cplx* a = sA + (kt % GEMM_STAGES) * KT * LDM + wm * 32;
     const cplx* b = sB + ((kt % GEMM_STAGES) * NN_NT + wn * 8 * NJ) * LDK;
 #pragma unroll
     for (int ks = 0; ks < KT; ks += 4) {
+#ifndef KSPW_GEMM_NO_STAGGER
+      if (ks == (late ? KS_LATE : KS_EARLY)) {
+        if (more) load_stage((kt + GEMM_STAGES - 1) % GEMM_STAGES, kt + GEMM_STAGES - 1);
+        cp_commit();
+      }
+#endif
       cplx af[4], bf[NJ];
 #pragma unroll
       for (int i = 0; i < 4; ++i) af[i] = a[(ks + fk) * LDM + i * 8 + fr];
@@ -458,6 +496,15 @@ int ks_gemm_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, co
     }
     KS_CUDA_CHECK(cudaGetLastError(), err);
     return KS_OK;
+  }
+  // N beyond the widest tile and not a multiple of it (N = 520 -> eleven 48-wide tiles by the least-padding rule): whole 80-wide
+  // tiles first (more DMMAs per fragment load, A re-read 7 instead of 11 times), the remainder in a second launch
+  static const bool nsplit_on = !(getenv("KSPW_GEMM_NSPLIT") && atoi(getenv("KSPW_GEMM_NSPLIT")) == 0);
+  if (nsplit_on && N > 80 && N % 80 != 0 && pick_nj(N, 16) < 5) {
+    const int main_n = N / 80 * 80;
+    const int rc = launch_nn<5>(st, M, main_n, K, A, lda, B, ldb, C, ldc, accumulate, err);
+    if (rc != KS_OK) return rc;
+    return ks_gemm_nn(st, M, N - main_n, K, A, lda, B + (long)main_n * ldb, ldb, C + (long)main_n * ldc, ldc, accumulate, err);
   }
   switch (pick_nj(N, 16)) {
     case 1: return launch_nn<1>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
