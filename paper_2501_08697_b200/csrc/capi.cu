@@ -120,7 +120,7 @@ int ks_ensure_planes(ks_ctx* c, int nb, cudaStream_t sync_stream) {
   const size_t per = sizeof(cplx) * (size_t)P.L1 * P.n2 * P.n3;
   KS_CUDA_CHECK(cudaMalloc(&P.d_planes, per * want), c->err);
   P.batch_cap = want;
-  return KS_OK;
+  return ks_hpsi_make_tmap(P, c->err);
 }
 
 extern "C" void ks_destroy(ks_ctx* c);
@@ -280,7 +280,7 @@ extern "C" int ks_set_fft_batch(ks_ctx* c, int nbatch) {
   c->fft_batch = nbatch > 0 ? nbatch : auto_batch(c->P);
   if (c->P.d_planes && c->P.batch_cap > c->fft_batch) {      // shrink on request
     cudaFree(c->P.d_planes);
-    c->P.d_planes = nullptr; c->P.batch_cap = 0;
+    c->P.d_planes = nullptr; c->P.batch_cap = 0; c->P.tmap_ok = false;
   }
   return KS_OK;
 }

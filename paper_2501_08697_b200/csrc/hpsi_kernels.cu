@@ -22,6 +22,7 @@
 // of a quarter-warp fall in distinct banks.
 #include "fft.cuh"
 #include "plan.h"
+#include <cuda.h>          // CUtensorMap and its enums only; the driver entry point is looked up at run time
 #include <algorithm>
 #include <type_traits>
 #include <cmath>
@@ -203,23 +204,40 @@ constexpr int yz_pick_zc(int nz) {
 // The inverse kernel repeats the first z codelet pass in every CTA of the plane (it needs no exchange); the forward kernel's
 // last z pass needs all k1, so its ZS CTAs form a thread-block cluster and read each other's stick tiles through
 // distributed shared memory.
-template <int NY, int NZ> struct yzcfg { static constexpr int ZC = yz_pick_zc(NZ), NT = 256, ZS = 1; static constexpr bool DBF = (ZC % 2 == 0); };
+// NG > 1: during the y transform the CTA's warps form NG independent groups of NT / NG threads; group q transforms the chunks
+// q, q + NG, ... in its own y tile and synchronises with a named barrier of its own, so the groups drift apart and one
+// group's global loads / stores overlap another's codelets (a single CTA per SM otherwise moves through load, compute and
+// store phases in lockstep).  ZC is the chunk width of ONE group; the y tiles of all groups take NY * ZC * NG elements.
+// TMA: the inverse kernel's last y pass runs in place in the y tile and the tile leaves for HBM as bulk asynchronous copies
+// (one per plane row, issued by NY threads, SASS UBLKCP) instead of 16-byte stores from registers: the per-thread stores kept
+// the CTA in a store phase for a third of its time (measured with clock64: 9.5k of 26.8k clocks per 128 x 128 plane) during
+// which the LSU queue was full and nothing else progressed; the bulk copies drain while the next chunk is transformed.
+template <int NY, int NZ> struct yzcfg { static constexpr int ZC = yz_pick_zc(NZ), NT = 256, ZS = 1, NG = 1; static constexpr bool DBF = (ZC % 2 == 0), TMA = false; };
 #ifdef KSPW_ZSPLIT128   // measured on cfg 3 (104-band launches; unsplit: k_inv_yz 0.589 ms, k_fwd_yz 0.688 ms):
                         //   ZS = 2, ZC = 16, 256 threads: k_inv_yz 0.589 ms, k_fwd_yz 0.843 ms
                         //   ZS = 4, ZC = 32, 256 threads (both y passes fill the CTA): k_inv_yz 0.794 ms (the repeated first
                         //   z pass), k_fwd_yz 1.439 ms (clusters of 4 with two cluster barriers each)  -> off
-template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 256, ZS = 4; static constexpr bool DBF = false; };
+template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 256, ZS = 4, NG = 1; static constexpr bool DBF = false, TMA = false; };
 #else
 #ifdef KSPW_YZ128_NT256   // 8 warps, both y passes fill the CTA: k_inv_yz 0.605 ms (0.589 with 512 threads), k_fwd_yz 0.819 ms (0.688): off
-template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 256, ZS = 1; static constexpr bool DBF = false; };
+template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 256, ZS = 1, NG = 1; static constexpr bool DBF = false, TMA = false; };
 #else
-template <> struct yzcfg<128, 128> { static constexpr int ZC = 32, NT = 512, ZS = 1; static constexpr bool DBF = false; };
+#ifndef KSPW_YZ128_NG
+#define KSPW_YZ128_NG 4
+#endif
+#ifndef KSPW_NO_YHALF_INV
+#define KSPW_YHALF_INV       // with four y groups the even/odd split of the DFT-16 pass pays in the inverse kernel too (0.628 -> 0.574 ms)
+#endif
+#ifndef KSPW_YZ128_TMA
+#define KSPW_YZ128_TMA 0     // measured (cfg 3, k_inv_yz per 104 bands): register stores 0.574 ms; one tensor store per chunk 0.600-0.649 ms;
+#endif                       // 128 row-wise cp.async.bulk per chunk 0.687-0.745 ms -- see DESIGN.md section 5
+template <> struct yzcfg<128, 128> { static constexpr int NG = KSPW_YZ128_NG, ZC = 32 / NG, NT = 512, ZS = 1; static constexpr bool DBF = false, TMA = (KSPW_YZ128_TMA != 0); };
 #endif
 #endif
 #ifndef KSPW_NO_ZSPLIT288
-template <> struct yzcfg<96, 288> { static constexpr int ZC = 16, NT = 256, ZS = 3; static constexpr bool DBF = false; };
+template <> struct yzcfg<96, 288> { static constexpr int ZC = 16, NT = 256, ZS = 3, NG = 1; static constexpr bool DBF = false, TMA = false; };
 #else
-template <> struct yzcfg<96, 288> { static constexpr int ZC = 16, NT = 256, ZS = 1; static constexpr bool DBF = false; };
+template <> struct yzcfg<96, 288> { static constexpr int ZC = 16, NT = 256, ZS = 1, NG = 1; static constexpr bool DBF = false, TMA = false; };
 #endif
 
 // 16-byte global -> shared async copy (LDGSTS), ordered against the surrounding shared-memory accesses
@@ -246,6 +264,44 @@ __device__ __forceinline__ void cp_wait_n(int n) {   // n = groups allowed to st
 #define KS_LD_PLANE(p) (*(p))
 #endif
 
+
+#ifdef KSPW_PHASE_CLOCKS   // experiment: SM clocks per phase of the yz kernels, summed over CTAs (thread 0 of each CTA)
+__device__ unsigned long long g_phase[16];
+#define KS_PH_INIT() unsigned long long ph_t = clock64()
+#define KS_PH(i_) do { if (threadIdx.x == 0) { const unsigned long long t_ = clock64(); atomicAdd(&g_phase[i_], t_ - ph_t); ph_t = t_; } } while (0)
+extern "C" int ks_debug_phase_clocks(unsigned long long* out, int reset) {
+  cudaMemcpyFromSymbol(out, g_phase, sizeof(g_phase));
+  if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_phase, z, sizeof(z)); }
+  return 0;
+}
+#else
+#define KS_PH_INIT()
+#define KS_PH(i_)
+#endif
+
+// ---- bulk asynchronous copies (TMA engine, SASS UBLKCP): shared -> global stores tracked by bulk async-groups ----
+__device__ __forceinline__ void bulk_store(void* gmem, const void* smem, unsigned bytes) {     // 16-byte aligned, bytes % 16 == 0
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;\n" ::"l"(gmem), "r"(s), "r"(bytes) : "memory");
+}
+// one 2-D box [rows][cols] of a tensor map, shared -> global (SASS UTMASTG); x = column (fastest), y = row coordinate
+__device__ __forceinline__ void tensor_store_2d(const void* tmap, const void* smem, int x, int y) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];\n" ::"l"(tmap), "r"(s), "r"(x), "r"(y) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;\n" ::: "memory"); }
+// the issuing thread's bulk groups have finished READING their shared-memory source (the buffer may be overwritten)
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;\n" ::: "memory"); }
+// generic-proxy writes to shared memory made visible to the async proxy (before a barrier that precedes the bulk copy)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
+
+// barrier of one y group (named barrier 1 + q over GT threads) or of the whole CTA when there is one group
+template <int NG, int GT>
+__device__ __forceinline__ void ygroup_sync(int q) {
+  if constexpr (NG == 1) __syncthreads();
+  else asm volatile("bar.sync %0, %1;" ::"r"(1 + q), "n"(GT) : "memory");
+}
 
 // lines-first walk over (stick s, line j) pairs: item it = j*S + s, it = tid, tid + NT, ...
 struct StickWalk {
@@ -275,28 +331,30 @@ __device__ __forceinline__ typename std::conditional<JFAST, JWalk<L>, StickWalk>
   else return StickWalk(tid, nt, S);
 }
 
-template <int NY, int NZ>
-__device__ __forceinline__ void inv_yz_body(const YzArgs& a, const int bx, const int b) {
+template <int NY, int NZ, bool USE_TMA>
+__device__ __forceinline__ void inv_yz_body(const YzArgs& a, const int bx, const int b, const void* tmap) {
   constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = facz<NZ>::R1, R2z = facz<NZ>::R2;
   constexpr int ZS = yzcfg<NY, NZ>::ZS, NZH = NZ / ZS, K1H = R1z / ZS;   // this CTA's z' positions and codelet lines
   static_assert(R1z % ZS == 0 && NZH % yzcfg<NY, NZ>::ZC == 0, "z' split must cut between codelet lines and chunks");
-  constexpr int SZ = NZH | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
+  constexpr int SZ = NZH | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, NG = yzcfg<NY, NZ>::NG, GT = NT / NG, G = GT / ZC;
+  static_assert(NT % NG == 0 && GT % 32 == 0 && (NZH / ZC) % NG == 0, "y groups: whole warps, equal numbers of chunks");
 #ifdef KSPW_YHALF_INV   // measured on cfg 3: k_inv_yz 0.589 -> 0.607 ms (twice the stick-tile reads in the pass, 128 registers): off
-  constexpr bool YHALF = (G == 2 * R2y) && (R1y % 2 == 0) && (NT == G * ZC) && (ZC == 32);
+  constexpr bool YHALF = (G == 2 * R2y) && (R1y % 2 == 0) && (GT == G * ZC) && (ZC * NG == 32);
 #else
   constexpr bool YHALF = false;
 #endif
-  extern __shared__ cplx sm[];
-  cplx* tw_y = sm;
+  extern __shared__ __align__(128) cplx sm[];
+  cplx* ytile = sm;                               // first: the source of the tensor stores must be 128-byte aligned
+  cplx* tw_y = ytile + NY * ZC * NG;
   cplx* tw_z = (NY == NZ) ? tw_y : tw_y + NY;     // equal lengths share one twiddle table
   cplx* stile = tw_z + NZ;
-  cplx* ytile = stile + (size_t)a.smax * SZ;
   const int tid = threadIdx.x;
   const int lx = bx / ZS, h = bx % ZS;
   const int s0 = a.plane_s0[lx], S = a.plane_s0[lx + 1] - s0;
   const int y0 = a.plane_y0[lx];
   const cplx* psi = a.psi + (size_t)b * a.npw;
   // H1 + H2 (z) pass 1: psi -> registers -> DFT-R1z -> twiddle -> stick tile (type A, inverse)
+  KS_PH_INIT();
   {
     // walk over the (stick, line) items of the pass that touches psi: lines-first (StickWalk) or j-fastest (JWalk, the
     // lanes of a stick read consecutive plane waves).  Measured: 128 x 128 lines-first 0.592 / j-fastest 0.599 ms, 96 x 96
@@ -338,12 +396,66 @@ __device__ __forceinline__ void inv_yz_body(const YzArgs& a, const int bx, const
     }
   }
   __syncthreads();
+  KS_PH(0);
   for (StickWalk w(tid, NT, S); w.j < K1H; w.next()) lineA_stage2<NZ, +1, facz<NZ>>(stile + w.s * SZ, 1, w.j);
   __syncthreads();
+  KS_PH(1);
   // H2 (y): for each chunk of z' positions, type-A inverse FFT along y; output straight to HBM
   cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ) + h * NZH;
-  const int pz = tid % ZC, g = tid / ZC;
-  for (int c = 0; c < NZH / ZC; ++c) {
+  const int grp = tid / GT, gt = tid % GT;
+  const int pz = gt % ZC, g = gt / ZC;
+  ytile += grp * (NY * ZC);
+  if constexpr (USE_TMA) {
+    static_assert(G >= R2y && G >= R1y, "TMA variant: at most one codelet line per thread and pass");
+    static_assert(ZS == 1, "TMA variant: whole planes");
+    for (int c = grp; c < NZH / ZC; c += NG) {
+      // pass 1 in registers (reads the stick tile only)
+      cplx v[R1y];
+      const bool p1 = g < R2y;
+      if (p1) {
+        const cplx* src = stile + c * ZC + pz;
+#pragma unroll
+        for (int j1 = 0; j1 < R1y; ++j1) {
+          int s = j1 * R2y + g - y0;
+          if (s < 0) s += NY;
+          v[j1] = (s < S) ? src[s * SZ] : cmake(0.0, 0.0);
+        }
+        dft<R1y, +1>(v);
+#pragma unroll
+        for (int k1 = 1; k1 < R1y; ++k1) v[k1] = mul_tw<+1>(v[k1], tw_y, g * k1);
+      }
+      // the bulk copies of the group's previous chunk have read the y tile (they drained during pass 1)
+      if (gt == 0) bulk_wait_read();
+      ygroup_sync<NG, GT>(grp);
+      if (p1) {
+        cplx* o = ytile + g * ZC + pz;
+#pragma unroll
+        for (int k1 = 0; k1 < R1y; ++k1) o[k1 * R2y * ZC] = v[k1];
+      }
+      ygroup_sync<NG, GT>(grp);
+      KS_PH(2);
+      if (g < R1y) {            // pass 2 in place: thread (g, pz) owns rows g*R2y .. g*R2y + R2y - 1 of column pz
+        cplx u[R2y];
+        cplx* t = ytile + g * R2y * ZC + pz;
+#pragma unroll
+        for (int j2 = 0; j2 < R2y; ++j2) u[j2] = t[j2 * ZC];
+        dft<R2y, +1>(u);
+#pragma unroll
+        for (int k2 = 0; k2 < R2y; ++k2) t[k2 * ZC] = u[k2];
+      }
+      fence_proxy_async();
+      ygroup_sync<NG, GT>(grp);
+      // plane row r = k1*R2y + k2 is y-tile row r: the whole [NY][ZC] tile leaves as ONE tensor store (box = 2 ZC doubles x NY rows)
+      if (gt == 0) {
+        tensor_store_2d(tmap, ytile, 2 * (c * ZC), (b * a.L1 + lx) * NY);
+        bulk_commit();
+      }
+      KS_PH(3);
+    }
+    if (gt == 0) bulk_wait_all();
+    return;
+  }
+  for (int c = grp; c < NZH / ZC; c += NG) {
     if constexpr (YHALF) {
       // twice as many line groups as DFT-R1y lines: two groups share a line, one takes the even outputs (DFT-R1y/2 of
       // x[n] + x[n + R1y/2]), the other the odd ones (DFT-R1y/2 of (x[n] - x[n + R1y/2]) w^n): every warp works in this pass
@@ -389,7 +501,8 @@ __device__ __forceinline__ void inv_yz_body(const YzArgs& a, const int bx, const
         for (int k1 = 0; k1 < R1y; ++k1) o[k1 * R2y * ZC] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw_y, j2 * k1);
       }
     }
-    __syncthreads();
+    ygroup_sync<NG, GT>(grp);
+    KS_PH(2);
     if (g < G) {
       for (int k1 = g; k1 < R1y; k1 += G) {
         cplx v[R2y];
@@ -402,22 +515,29 @@ __device__ __forceinline__ void inv_yz_body(const YzArgs& a, const int bx, const
         for (int k2 = 0; k2 < R2y; ++k2) KS_ST_PLANE(o + k2 * NZ, v[k2]);
       }
     }
-    __syncthreads();
+    ygroup_sync<NG, GT>(grp);
+    KS_PH(3);
   }
 }
 
 template <int NY, int NZ>
-__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 0) k_inv_yz(const __grid_constant__ YzArgs a) {
-  inv_yz_body<NY, NZ>(a, blockIdx.x, blockIdx.y);
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::NT <= 256 ? 2 : 1) k_inv_yz(const __grid_constant__ YzArgs a) {
+  inv_yz_body<NY, NZ, false>(a, blockIdx.x, blockIdx.y, nullptr);
+}
+// the same with the planes leaving through the tensor map `tm` of the live-plane workspace (yzcfg::TMA)
+template <int NY, int NZ>
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::NT <= 256 ? 2 : 1) k_inv_yz_tma(const __grid_constant__ YzArgs a,
+                                                                                                const __grid_constant__ CUtensorMap tm) {
+  inv_yz_body<NY, NZ, yzcfg<NY, NZ>::TMA>(a, blockIdx.x, blockIdx.y, &tm);
 }
 // k-batched form (ks_hpsi_batch): blockIdx.z picks the k-point's descriptor; the grid is sized for the largest k of the group
 template <int NY, int NZ>
-__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 0) k_inv_yz_k(const YzArgs* __restrict__ arr) {
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::NT <= 256 ? 2 : 1) k_inv_yz_k(const YzArgs* __restrict__ arr) {
   __shared__ YzArgs a;
   if (threadIdx.x == 0) a = arr[blockIdx.z];
   __syncthreads();
   if ((int)blockIdx.x >= a.L1 * yzcfg<NY, NZ>::ZS || (int)blockIdx.y >= a.nb) return;
-  inv_yz_body<NY, NZ>(a, blockIdx.x, blockIdx.y);
+  inv_yz_body<NY, NZ, false>(a, blockIdx.x, blockIdx.y, nullptr);
 }
 
 template <int NY, int NZ>
@@ -425,23 +545,27 @@ __device__ __forceinline__ void fwd_yz_body(const YzArgs& a, const int bx, const
   constexpr int R1y = fac<NY>::R1, R2y = fac<NY>::R2, R1z = facz<NZ>::R1, R2z = facz<NZ>::R2;
   constexpr int ZS = yzcfg<NY, NZ>::ZS, NZH = NZ / ZS, K1H = R1z / ZS;   // this CTA's z' positions and codelet lines
   static_assert(ZS == 1 || !yzcfg<NY, NZ>::DBF, "the z' split uses the single-buffer y transform");
-  constexpr int SZ = NZH | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, G = NT / ZC;
+  constexpr int SZ = NZH | 1, ZC = yzcfg<NY, NZ>::ZC, NT = yzcfg<NY, NZ>::NT, NG = yzcfg<NY, NZ>::NG, GT = NT / NG, G = GT / ZC;
+  static_assert(NG == 1 || !yzcfg<NY, NZ>::DBF, "y groups use the single-buffer y transform");
 #ifndef KSPW_NO_YHALF    // measured on cfg 3: k_fwd_yz 0.688 -> 0.665 ms
-  constexpr bool YHALF = (G == 2 * R2y) && (R1y % 2 == 0) && (NT == G * ZC) && (ZC == 32);   // 128 x 128: 16 warps, 8 DFT-16 lines
+  constexpr bool YHALF = (G == 2 * R2y) && (R1y % 2 == 0) && (GT == G * ZC) && (ZC * NG == 32);   // 128 x 128: twice as many line groups as DFT-16 lines (on 96 x 288, ZC 16, it measured slower: 0.636 -> 0.688 ms)
 #else
   constexpr bool YHALF = false;
 #endif
-  extern __shared__ cplx sm[];
-  cplx* tw_y = sm;
+  extern __shared__ __align__(128) cplx sm[];
+  cplx* ytile = sm;                               // same layout as the inverse kernel
+  cplx* const ytile0 = sm;                        // all groups' y tiles: NY * ZC * NG elements (reused for psi after the y phase)
+  cplx* tw_y = ytile + NY * ZC * NG;
   cplx* tw_z = (NY == NZ) ? tw_y : tw_y + NY;     // equal lengths share one twiddle table
   cplx* stile = tw_z + NZ;
-  cplx* ytile = stile + (size_t)a.smax * SZ;
   const int tid = threadIdx.x;
   const int lx = bx / ZS, h = bx % ZS;   // h = rank in the cluster of ZS CTAs
   const int s0 = a.plane_s0[lx], S = a.plane_s0[lx + 1] - s0;
   const int y0 = a.plane_y0[lx];
   const cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ) + h * NZH;
-  const int pz = tid % ZC, g = tid / ZC;
+  const int grp = tid / GT, gt = tid % GT;
+  const int pz = gt % ZC, g = gt / ZC;
+  KS_PH_INIT();
   // H4 (y), type B, forward.  The y tile is split into two half-width buffers: while chunk c (ZF = ZC/2 columns) is
   // transformed in place in one of them, chunk c+1 streams into the other by cp.async, so the plane loads are
   // in flight during both codelet passes.  (Odd ZC: single buffer, loads straight into registers.)
@@ -502,12 +626,13 @@ __device__ __forceinline__ void fwd_yz_body(const YzArgs& a, const int bx, const
   };
   {
     cplx v[R2y];
-    if (g < G && g < R1y) load_in(v, 0, g);
+    ytile += grp * (NY * ZC);
+    if (g < G && g < R1y) load_in(v, grp, g);
     for (int i = tid; i < NY; i += NT) tw_y[i] = a.tw_y[i];
     if (NY != NZ)
       for (int i = tid; i < NZ; i += NT) tw_z[i] = a.tw_z[i];
     __syncthreads();
-    for (int c = 0; c < NZH / ZC; ++c) {
+    for (int c = grp; c < NZH / ZC; c += NG) {
       if (g < G) {
         for (int k1 = g; k1 < R1y; k1 += G) {
           if (k1 != g) load_in(v, c, k1);          // the thread's first line of a chunk is already in registers
@@ -517,8 +642,9 @@ __device__ __forceinline__ void fwd_yz_body(const YzArgs& a, const int bx, const
           for (int q2 = 0; q2 < R2y; ++q2) o[q2 * ZC] = (q2 == 0) ? v[0] : mul_tw<-1>(v[q2], tw_y, k1 * q2);
         }
       }
-      __syncthreads();
-      if (g < G && g < R1y && c + 1 < NZH / ZC) load_in(v, c + 1, g);   // next chunk's loads fly during pass 2
+      ygroup_sync<NG, GT>(grp);
+      KS_PH(8);
+      if (g < G && g < R1y && c + NG < NZH / ZC) load_in(v, c + NG, g);   // next chunk's loads fly during pass 2
       if constexpr (YHALF) {
         // two line groups per DFT-R1y line: even outputs from one, odd outputs from the other (see k_inv_yz)
         constexpr int H = R1y / 2;
@@ -562,19 +688,52 @@ __device__ __forceinline__ void fwd_yz_body(const YzArgs& a, const int bx, const
           }
         }
       }
-      __syncthreads();
+      ygroup_sync<NG, GT>(grp);
+      KS_PH(9);
     }
+    if constexpr (NG > 1) __syncthreads();      // every group's stick columns are in place before the z transform
+    KS_PH(10);
   }
   }
   // H4 (z): type-B forward FFT on each stick
   const cplx* psi = a.psi + (size_t)b * a.npw;
   cplx* hpsi = a.hpsi + (size_t)b * a.npw;
   if constexpr (ZS == 1) {
+    // The plane waves of one x-plane are ONE contiguous run of psi (its sticks follow each other in the canonical order):
+    // the run streams into the now idle y tile by cp.async while the first z pass runs, so the last pass finds psi in
+    // shared memory instead of paying a dependent global load per output (clock64: 9.5k of 28.9k clocks per 128 x 128 plane
+    // went to this pass).  Planes whose run does not fit the y tile read psi from global memory as before.
+    const int pw0 = __ldg(a.stick + s0).x;
+    int npl;
+    {
+      const int4 sl = __ldg(a.stick + s0 + S - 1);
+      npl = sl.x + sl.z - pw0;
+    }
+#ifdef KSPW_FWD_PSI_GLOBAL
+    const bool staged = false;
+#else
+    const bool staged = npl <= NY * ZC * NG;
+#endif
+    if (staged) {
+      for (int i = tid; i < npl; i += NT) cp16m(ytile0 + i, psi + pw0 + i);
+      cp_commit_m();
+    }
     for (StickWalk w(tid, NT, S); w.j < R1z; w.next()) lineB_stage1<NZ, -1, facz<NZ>>(stile + w.s * SZ, 1, w.j, tw_z);
+    if (staged) cp_wait_n(0);
     __syncthreads();
+    KS_PH(11);
     // last pass + H5: DFT-R1z, then hpsi = |k+G|^2 psi + (.)/N written straight to the stick's run of hpsi
+    const cplx* psrc = staged ? (ytile0 - pw0) : psi;          // psrc[j] = psi[j] for the plane's run
     for (StickWalk w(tid, NT, S); w.j < R2z; w.next()) {
       const int4 si = __ldg(a.stick + s0 + w.s);
+      // |k+G|^2 of the line's outputs first: the loads fly during the codelet
+      double kk[R1z];
+#pragma unroll
+      for (int q1 = 0; q1 < R1z; ++q1) {
+        int idx = q1 * R2z + w.j - si.y;
+        if (idx < 0) idx += NZ;
+        kk[q1] = (idx < si.z) ? __ldg(a.g2 + si.x + idx) : 0.0;
+      }
       cplx v[R1z];
       const cplx* t = stile + w.s * SZ + w.j;
 #pragma unroll
@@ -586,12 +745,12 @@ __device__ __forceinline__ void fwd_yz_body(const YzArgs& a, const int bx, const
         if (idx < 0) idx += NZ;
         if (idx < si.z) {
           const int j = si.x + idx;
-          const cplx p = psi[j];
-          const double k = __ldg(a.g2 + j);
-          hpsi[j] = cmake(fma(k, p.x, v[q1].x * a.invN), fma(k, p.y, v[q1].y * a.invN));
+          const cplx p = psrc[j];
+          hpsi[j] = cmake(fma(kk[q1], p.x, v[q1].x * a.invN), fma(kk[q1], p.y, v[q1].y * a.invN));
         }
       }
     }
+    KS_PH(12);
   } else {
     // first z pass on this CTA's lines k1 = h*K1H + k1l (local offset k1l, twiddle index from the global k1)
     for (StickWalk w(tid, NT, S); w.j < K1H; w.next()) {
@@ -634,11 +793,11 @@ __device__ __forceinline__ void fwd_yz_body(const YzArgs& a, const int bx, const
 }
 
 template <int NY, int NZ>
-__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 0) k_fwd_yz(const __grid_constant__ YzArgs a) {
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::NT <= 256 ? 2 : 1) k_fwd_yz(const __grid_constant__ YzArgs a) {
   fwd_yz_body<NY, NZ>(a, blockIdx.x, blockIdx.y);
 }
 template <int NY, int NZ>
-__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::ZS > 1 ? 2 : 0) k_fwd_yz_k(const YzArgs* __restrict__ arr) {
+__global__ void __launch_bounds__(yzcfg<NY, NZ>::NT, yzcfg<NY, NZ>::NT <= 256 ? 2 : 1) k_fwd_yz_k(const YzArgs* __restrict__ arr) {
   __shared__ YzArgs a;
   if (threadIdx.x == 0) a = arr[blockIdx.z];
   __syncthreads();
@@ -945,6 +1104,39 @@ static size_t yz_smem(const HpsiPlan& P, int zc) {
   const size_t SZ = (size_t)((P.n3 / P.zs_yz) | 1);
   return sizeof(cplx) * ((size_t)P.n2 + (P.n2 == P.n3 ? 0 : P.n3) + (size_t)P.smax * SZ + (size_t)P.n2 * zc);
 }
+
+// Tensor map of the live-plane workspace seen as a 2-D array of doubles [batch_cap * L1 * n2 rows][2 * n3], box = one y tile
+// ([n2 rows][2 * zc doubles], dense in shared memory: no swizzle, no interleave).  cuTensorMapEncodeTiled is a driver entry
+// point: looked up through the runtime so that libkspw.so does not link libcuda.
+typedef CUresult (*ks_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                       const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                       CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+int ks_hpsi_make_tmap(HpsiPlan& P, std::string& err) {
+  P.tmap_ok = false;
+  bool want = false;
+#define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) want = yzcfg<A_, B_>::TMA;
+  KS_YZ_PAIRS(C_)
+#undef C_
+  if (!want || !P.d_planes) return KS_OK;
+  static ks_encode_tiled_fn enc = nullptr;
+  if (!enc) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) return KS_OK;   // no TMA path
+    enc = (ks_encode_tiled_fn)fn;
+  }
+  const cuuint64_t dims[2] = {(cuuint64_t)2 * P.n3, (cuuint64_t)P.batch_cap * P.L1 * P.n2};
+  const cuuint64_t strides[1] = {(cuuint64_t)2 * P.n3 * sizeof(double)};
+  const cuuint32_t box[2] = {(cuuint32_t)(2 * P.zc_yz), (cuuint32_t)P.n2};
+  const cuuint32_t estr[2] = {1, 1};
+  static_assert(sizeof(CUtensorMap) == sizeof(P.tmap_planes), "tensor map storage");
+  const CUresult r = enc((CUtensorMap*)P.tmap_planes, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, P.d_planes, dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { err = "cuTensorMapEncodeTiled failed for the live-plane workspace"; return KS_ECUDA; }
+  P.tmap_ok = true;
+  return KS_OK;
+}
 template <int NX> static constexpr size_t x_smem() {
   return sizeof(cplx) * ((size_t)NX + (size_t)NX * xcfg<NX>::ZC) + sizeof(unsigned) * (fac<NX>::R2 + 1) * ((fac<NX>::R1 + 3) & ~3);
 }
@@ -984,11 +1176,12 @@ int ks_hpsi_configure(HpsiPlan& P, std::string& err) {
   if (P.n2 == A_ && P.n3 == B_) {                                               \
     P.zc_yz = yzcfg<A_, B_>::ZC;                                                \
     P.zs_yz = yzcfg<A_, B_>::ZS;                                                \
-    P.smem_yz = yz_smem(P, P.zc_yz);                                            \
+    P.smem_yz = yz_smem(P, P.zc_yz * yzcfg<A_, B_>::NG);                        \
     if (P.smem_yz > KS_SMEM_MAX) { err = "yz kernels: stick tile does not fit in 227 KB of shared memory"; return KS_ENOMEM; } \
     /* the attribute belongs to the kernel, not to the context: opt in to the hardware maximum once, so contexts  \
        with different spheres (stick tiles) on the same plane size never lower each other's limit */               \
     e = opt_in(k_inv_yz<A_, B_>, KS_SMEM_MAX);                                  \
+    if (e == cudaSuccess) e = opt_in(k_inv_yz_tma<A_, B_>, KS_SMEM_MAX);        \
     if (e == cudaSuccess) e = opt_in(k_fwd_yz<A_, B_>, KS_SMEM_MAX);            \
     if (e == cudaSuccess) e = opt_in(k_inv_yz_k<A_, B_>, KS_SMEM_MAX_K);        \
     if (e == cudaSuccess) e = opt_in(k_fwd_yz_k<A_, B_>, KS_SMEM_MAX_K);        \
@@ -1028,7 +1221,12 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
   x.nb = nb; x.bg = ks_x_band_group(ceil_div(x.ncol, P.zc_x), nb);
   const dim3 gyz(P.L1 * P.zs_yz, nb), gx(ceil_div(x.ncol, P.zc_x), ceil_div(nb, x.bg));
   if (stage < 0 || stage == 0) {
-#define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_inv_yz<A_, B_><<<gyz, yzcfg<A_, B_>::NT, P.smem_yz, st>>>(a);
+#define C_(A_, B_)                                                                                          \
+    if (P.n2 == A_ && P.n3 == B_) {                                                                         \
+      if (yzcfg<A_, B_>::TMA && P.tmap_ok)                                                                  \
+        k_inv_yz_tma<A_, B_><<<gyz, yzcfg<A_, B_>::NT, P.smem_yz, st>>>(a, *(const CUtensorMap*)P.tmap_planes); \
+      else k_inv_yz<A_, B_><<<gyz, yzcfg<A_, B_>::NT, P.smem_yz, st>>>(a);                                 \
+    }
     KS_YZ_PAIRS(C_)
 #undef C_
   }

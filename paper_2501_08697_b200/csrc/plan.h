@@ -24,6 +24,8 @@ struct HpsiPlan {
   cplx* d_tw[3] = {nullptr, nullptr, nullptr};  // e^{+2 pi i t/n_i}
   cplx* d_planes = nullptr;    // workspace [batch][L1][n2][n3]
   int batch_cap = 0;           // bands the workspace holds
+  alignas(64) unsigned char tmap_planes[128] = {};   // CUtensorMap of d_planes (box = one y tile); rebuilt when d_planes moves
+  bool tmap_ok = false;
   double* d_rho_part = nullptr;  // density build: [rho_ng][n1][n2][n3] partial sums in position order (lazy)
   int rho_ng = 0;
 };
@@ -37,6 +39,9 @@ cudaError_t ks_fft_init_constants();
 // V(r) = Re sum_m vhat[m] e^{+2 pi i m.j/n} on the device by a plain O(N n) DFT per axis (create time
 // only), checked real, stored permuted.  vhat_host: [n1][n2][n3].  Returns KS_* and fills err.
 int ks_build_vperm(HpsiPlan& P, const cplx* vhat_host, cudaStream_t st, std::string& err);
+
+// (re)build the tensor map of the live-plane workspace for the kernels that store planes by TMA (after d_planes changed)
+int ks_hpsi_make_tmap(HpsiPlan& P, std::string& err);
 
 // fill zc_*/smem_* for the plan and opt the kernels into large dynamic shared memory
 int ks_hpsi_configure(HpsiPlan& P, std::string& err);
