@@ -57,7 +57,7 @@ int ks_create(ks_ctx** out, const double cell[9], const double k_frac[3], double
 void ks_destroy(ks_ctx* ctx);
 int ks_npw(const ks_ctx* ctx);
 int ks_set_stream(ks_ctx* ctx, void* cuda_stream /* cudaStream_t; NULL = default stream */);
-/* bands per launch of the three FFT kernels (0 = automatic: as many as 2 GB of live-plane workspace hold, at most 1024;
+/* bands per launch of the three FFT kernels (0 = automatic: as many as 9 GB of live-plane workspace hold, at most 1024;
  * the planes stream through HBM -- a batch small enough to stay in L2 measured slower) */
 int ks_set_fft_batch(ks_ctx* ctx, int nbatch);
 const char* ks_last_error(const ks_ctx* ctx);   /* ctx may be NULL: last ks_create failure */

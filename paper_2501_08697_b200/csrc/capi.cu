@@ -104,8 +104,11 @@ static int auto_batch(const HpsiPlan& P) {
   const char* env = getenv("KSPW_FFT_BATCH");
   if (env && atoi(env) > 0) return atoi(env);
   const double per = 16.0 * P.L1 * P.n2 * P.n3;
-  int b = (int)(2.0e9 / per);      // as many waves of CTAs per launch as 2 GB of planes allow (cfg 1: the whole 160-band
-  return std::max(2, std::min(b, 1024));   // block; measured 80 -> 160 bands: FFT path 51 -> 54 % of HBM); L2 cannot hold a useful batch
+  // as many bands per launch as 9 GB of live planes hold (cfg 1, cfg 4 and cfg 3: the whole block).  Measured, FFT path as a
+  // fraction of HBM: cfg 1 80 -> 160 bands 51 -> 54 %; cfg 3 26 / 52 / 104 / 260 bands 52.1 / 53.8 / 55.0 / 55.7 %: the planes
+  // stream through HBM and every launch ends with a partly filled wave, so fewer, larger launches win; L2 cannot hold a useful batch
+  int b = (int)(9.0e9 / per);
+  return std::max(2, std::min(b, 1024));
 }
 
 int ks_ensure_planes(ks_ctx* c, int nb, cudaStream_t sync_stream) {
@@ -153,7 +156,7 @@ static int create_impl(ks_ctx* c, const double* cell, const double* kf, double e
     }
   }
   // live planes, sticks, position maps (PW order is m1 slowest, so planes and sticks are contiguous runs)
-  std::vector<int> plane_s0, plane_y0;
+  std::vector<int> plane_s0, plane_y0, plane_pw0;
   std::vector<int4> stick;
   int nst = 0, smax = 0, cur_m1 = 0, cur_m2 = 0, cur_m3 = 0, s_in_plane = 0;
   for (int j = 0; j < P.npw; ++j) {
@@ -164,6 +167,7 @@ static int create_impl(ks_ctx* c, const double* cell, const double* kf, double e
       if (j && m1 != cur_m1 + 1) { err = "G sphere: live x-planes are not contiguous"; return KS_EINVAL; }
       plane_s0.push_back(nst);
       plane_y0.push_back(pmod(m2, P.n2));
+      plane_pw0.push_back(j);
       smax = std::max(smax, s_in_plane);
       s_in_plane = 0;
     }
@@ -177,6 +181,7 @@ static int create_impl(ks_ctx* c, const double* cell, const double* kf, double e
   }
   smax = std::max(smax, s_in_plane);
   plane_s0.push_back(nst);
+  plane_pw0.push_back(P.npw);
   P.L1 = (int)plane_y0.size();
   P.x0 = pmod(mil[0], P.n1);
   P.nsticks = nst;
@@ -185,6 +190,7 @@ static int create_impl(ks_ctx* c, const double* cell, const double* kf, double e
   int rc;
   if ((rc = upload(&P.d_plane_s0, plane_s0, err))) return rc;
   if ((rc = upload(&P.d_plane_y0, plane_y0, err))) return rc;
+  if ((rc = upload(&P.d_plane_pw0, plane_pw0, err))) return rc;
   if ((rc = upload(&P.d_stick, stick, err))) return rc;
   if ((rc = upload(&P.d_g2, g2, err))) return rc;
   for (int ax = 0; ax < 3; ++ax) {
@@ -249,7 +255,7 @@ extern "C" int ks_create(ks_ctx** out, const double cell[9], const double k_frac
 extern "C" void ks_destroy(ks_ctx* c) {
   if (!c) return;
   HpsiPlan& P = c->P;
-  cudaFree(P.d_plane_s0); cudaFree(P.d_plane_y0); cudaFree(P.d_stick);
+  cudaFree(P.d_plane_s0); cudaFree(P.d_plane_y0); cudaFree(P.d_plane_pw0); cudaFree(P.d_stick);
   cudaFree(P.d_g2); cudaFree(P.d_vperm); cudaFree(P.d_planes); cudaFree(P.d_rho_part);
   for (int i = 0; i < 3; ++i) cudaFree(P.d_tw[i]);
   cudaFree(c->d_beta); cudaFree(c->d_D); cudaFree(c->d_Q); cudaFree(c->d_proj_atom); cudaFree(c->d_off); cudaFree(c->d_doff);

@@ -182,6 +182,7 @@ struct YzArgs {
   cplx* planes;         // [nb][L1][NY][NZ]
   const int* plane_s0;  // [L1+1] first stick of each plane
   const int* plane_y0;  // [L1]   natural y index of the plane's first stick
+  const int* plane_pw0; // [L1+1] first plane wave of each plane: a plane's coefficients are ONE contiguous run of psi
   const int4* stick;    // [nsticks] {first PW, natural z index of the first PW, number of PWs, 0}
   const double* g2;
   const cplx* tw_y;
@@ -363,10 +364,13 @@ __device__ __forceinline__ void inv_yz_body(const YzArgs& a, const int bx, const
     constexpr bool JFAST = (ZS > 1);
     typename std::conditional<JFAST, JWalk<R2z>, StickWalk>::type w = make_walk<JFAST, R2z>(tid, NT, S);
 #define KS_W_OK(w_) (JFAST ? ((w_).s < S) : ((w_).j < R2z))
+    // (Staging the plane's run of psi in the idle y tile by cp.async, as the forward kernel does, was measured here too:
+    // 128 x 128 0.564 -> 0.570 ms, 96 x 96 0.266 -> 0.279 ms -- the opening phase is not bound by the scattered loads.)
+    const cplx* pbase = psi;
     cplx v[R1z];
     auto load_in = [&]() {
       const int4 si = __ldg(a.stick + s0 + w.s);
-      const cplx* src = psi + si.x;
+      const cplx* src = pbase + si.x;
 #pragma unroll
       for (int j1 = 0; j1 < R1z; ++j1) {
         int idx = j1 * R2z + w.j - si.y;
@@ -703,12 +707,7 @@ __device__ __forceinline__ void fwd_yz_body(const YzArgs& a, const int bx, const
     // the run streams into the now idle y tile by cp.async while the first z pass runs, so the last pass finds psi in
     // shared memory instead of paying a dependent global load per output (clock64: 9.5k of 28.9k clocks per 128 x 128 plane
     // went to this pass).  Planes whose run does not fit the y tile read psi from global memory as before.
-    const int pw0 = __ldg(a.stick + s0).x;
-    int npl;
-    {
-      const int4 sl = __ldg(a.stick + s0 + S - 1);
-      npl = sl.x + sl.z - pw0;
-    }
+    const int pw0 = a.plane_pw0[lx], npl = a.plane_pw0[lx + 1] - pw0;
 #ifdef KSPW_FWD_PSI_GLOBAL
     const bool staged = false;
 #else
@@ -1212,7 +1211,7 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
   if (nb > P.batch_cap) { err = "internal: FFT batch larger than workspace"; return KS_EINVAL; }
   YzArgs a;
   a.psi = psi; a.hpsi = hpsi; a.planes = P.d_planes;
-  a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.stick = P.d_stick;
+  a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.plane_pw0 = P.d_plane_pw0; a.stick = P.d_stick;
   a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
   a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.nb = nb; a.invN = 1.0 / (double)P.N;
   XArgs x;
@@ -1263,7 +1262,7 @@ void ks_kdesc_fill(void* host_desc, const KItem* items, int nk) {
     const HpsiPlan& P = *items[i].P;
     YzArgs& a = ya[i];
     a.psi = items[i].psi; a.hpsi = items[i].hpsi; a.planes = P.d_planes;
-    a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.stick = P.d_stick;
+    a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.plane_pw0 = P.d_plane_pw0; a.stick = P.d_stick;
     a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
     a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.nb = items[i].nb; a.invN = 1.0 / (double)P.N;
     XArgs& x = xa[i];
@@ -1346,7 +1345,7 @@ int ks_density_batch(HpsiPlan& P, const cplx* psi, const double* occ, int nb, in
   }
   YzArgs a;
   a.psi = psi; a.hpsi = nullptr; a.planes = P.d_planes;
-  a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.stick = P.d_stick;
+  a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.plane_pw0 = P.d_plane_pw0; a.stick = P.d_stick;
   a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
   a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.nb = nb; a.invN = 1.0 / (double)P.N;
   const dim3 gyz(P.L1 * P.zs_yz, nb);

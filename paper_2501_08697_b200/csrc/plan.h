@@ -17,6 +17,7 @@ struct HpsiPlan {
   // device arrays
   int* d_plane_s0 = nullptr;   // [L1+1] first stick of each plane
   int* d_plane_y0 = nullptr;   // [L1]   natural y index (m2min mod n2) of the plane's first stick
+  int* d_plane_pw0 = nullptr;  // [L1+1] first plane wave of each plane (the plane's coefficients are one contiguous run of psi)
   int4* d_stick = nullptr;     // [nsticks] {first PW, natural z index (m3min mod n3) of it, number of PWs, 0}:
                                //           a stick's coefficients are a contiguous run of psi, ascending in m3
   double* d_g2 = nullptr;      // [npw]  |k+G|^2

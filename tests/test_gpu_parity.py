@@ -179,7 +179,8 @@ def _boundary_bands(nb, batch, bg=8):
     return np.array(sorted(i for i in s if 0 <= i < nb))
 
 
-# FFT batch limits ks_create picks (2 GB of live planes): cfg 1 and cfg 2 whole block, cfg 3 125 bands, cfg 4 110 bands
+# bands per launch of the three FFT kernels: by default the whole block (up to 9 GB of live planes); 125 / 110 were round 1's
+# defaults for cfg 3 / cfg 4 and are kept as an explicit second run so that batch boundaries stay covered
 @pytest.mark.parametrize("c,k_index,batch", [(2, 0, 32), (2, 21, 32), (2, 63, 32), (1, 0, 160), (3, 0, 125), (4, 0, 110)])
 def test_hpsi_full_size(ks, oracle_mod, c, k_index, batch):
     """Full-size configs in the launch configuration bench.py times (whole block in one call); the oracle recomputes
@@ -188,6 +189,11 @@ def test_hpsi_full_size(ks, oracle_mod, c, k_index, batch):
     p = I.make_problem(c, k_index)
     ctx = ks.Context.from_problem(p)
     got = ctx.hpsi(_t(p.psi0)).cpu().numpy()
+    if batch < p.nbands:
+        ctx.set_fft_batch(batch)
+        got_b = ctx.hpsi(_t(p.psi0)).cpu().numpy()
+        # the FFT batches never change a bit of the local part; the projector products see the same block either way
+        assert np.array_equal(got, got_b)
     o = oracle_mod.Oracle.from_problem(p)
     sel = np.arange(p.nbands) if c == 2 else _boundary_bands(p.nbands, batch)
     ref = o.hpsi(p.psi0[sel])
