@@ -160,6 +160,17 @@ int ks_profile_end(ks_ctx* ctx, double* ms, long long* launches);
 /* C[M][N] (column-major, ldc) = A^H B;  A: DEVICE K x M column-major lda, B: K x N column-major ldb. */
 int ks_zgemm_hn(void* stream, int M, int N, int K, const ks_c128* A, long lda, const ks_c128* B,
                 long ldb, ks_c128* C, long ldc);
+/* The same product for callers that cannot call cudaMalloc (CUDA graph capture, serving loops): the split-K
+ * partial tiles live in a file-scope device array of 8 MiB (held by every GPU that loads the library until the
+ * process exits), so the call allocates nothing -- it launches two kernels on `stream`.  Limit: M * N <= 524 288
+ * complex128 elements (8 MiB / 16 B); beyond it the call returns KS_EINVAL with the limit in ks_last_error(NULL).
+ * Other errors: KS_EINVAL (M, N < 1, K < 0, NULL C, NULL A or B with K > 0, lda/ldb < K, ldc < M), KS_ECUDA.  Every call shares the one array:
+ * calls that overlap on the GPU (different streams) race; calls on one stream are ordered.  The array keeps the last
+ * call's contents, none of which a later call reads before writing.  The first call on a device looks up the array's
+ * device address and opts the kernels in to their shared memory (no allocation either); make it outside a capture.
+ * Same arithmetic as ks_zgemm_hn up to the split count (summation order over K).  ("BLAS".) */
+int ks_zgemm_hn_static(void* stream, int M, int N, int K, const ks_c128* A, long lda, const ks_c128* B,
+                       long ldb, ks_c128* C, long ldc);
 /* C[M][N] (column-major) = A B (accumulate=0) or C += A B (accumulate=1); A: M x K, B: K x N. */
 int ks_zgemm_nn(void* stream, int M, int N, int K, const ks_c128* A, long lda, const ks_c128* B,
                 long ldb, ks_c128* C, long ldc, int accumulate);

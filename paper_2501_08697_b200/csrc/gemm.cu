@@ -695,3 +695,105 @@ int ks_peak_run(double* dmma_tf, double* dfma_tf, std::string& err) {
   cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
   return KS_OK;
 }
+
+// ------------------------------------------------------------------------------------------------
+// ks_zgemm_hn_static: C = A^H B for callers that cannot call cudaMalloc (code under CUDA graph capture, serving loops,
+// harnesses that forbid allocation).  The same split-K kernels as ks_gemm_hn (k_gemm_hn<NJ> + k_splitk_reduce), with the
+// partial tiles in a file-scope device array instead of the growing GemmWs buffer.
+//
+//   * the array is KS_STATIC_SCRATCH_BYTES (8 MiB) on every GPU that loads the library, until the process exits;
+//   * nsplit * M * N complex partials must fit: M * N <= KS_STATIC_SCRATCH_ELEMS (524 288, e.g. 724 x 724), and the split
+//     count is capped at KS_STATIC_SCRATCH_ELEMS / (M * N) -- larger products are rejected with KS_EINVAL, never truncated;
+//   * nothing in the array has to start at zero: every element of part[0 : nsplit][N][M] that the reduction reads is
+//     written by exactly one CTA of the launch before it (every split owns a non-empty K range, or K = 0 and the one
+//     split writes zeros), so the previous call's contents are never observed;
+//   * every call shares the one array: two calls that overlap on the GPU (different streams, or two host threads on
+//     different streams) race on it.  Calls on one stream are ordered and safe.
+//
+// In host code `g_hn_scratch` is a host-side stand-in, not a device address; the address the kernels get comes from
+// cudaGetSymbolAddress, looked up once per device with that device current (static_setup), together with the kernels'
+// shared-memory opt-in.  The call itself launches two kernels and calls no cudaMalloc / cudaFree / allocating routine.
+// ------------------------------------------------------------------------------------------------
+#define KS_STATIC_SCRATCH_BYTES (8u << 20)
+#define KS_STATIC_SCRATCH_ELEMS (KS_STATIC_SCRATCH_BYTES / sizeof(cplx))
+static __device__ __align__(256) unsigned char g_hn_scratch[KS_STATIC_SCRATCH_BYTES];
+
+#define KS_STATIC_MAX_DEV 64
+static cplx* g_static_ptr[KS_STATIC_MAX_DEV];        // device address of g_hn_scratch on device d (nullptr: not set up yet)
+static std::atomic<bool> g_static_ready[KS_STATIC_MAX_DEV];
+
+template <int NJ>
+static cudaError_t static_opt_in() {
+  const size_t smem = sizeof(cplx) * GEMM_STAGES * (HN_MT + 32 * NJ) * LDK;
+  return cudaFuncSetAttribute(k_gemm_hn<NJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+}
+
+// once per device, with that device current
+static int static_setup(int dev, std::string& err) {
+  if (g_static_ready[dev].load(std::memory_order_acquire)) return KS_OK;
+  void* p = nullptr;
+  KS_CUDA_CHECK(cudaGetSymbolAddress(&p, g_hn_scratch), err);
+  KS_CUDA_CHECK(static_opt_in<1>(), err);
+  KS_CUDA_CHECK(static_opt_in<2>(), err);
+  KS_CUDA_CHECK(static_opt_in<3>(), err);
+  KS_CUDA_CHECK(static_opt_in<4>(), err);
+  KS_CUDA_CHECK(static_opt_in<5>(), err);
+  g_static_ptr[dev] = (cplx*)p;
+  g_static_ready[dev].store(true, std::memory_order_release);
+  return KS_OK;
+}
+
+template <int NJ>
+static int launch_hn_static(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
+                            long ldc, cplx* part, std::string& err) {
+  constexpr int HN_NT = 32 * NJ;
+  const size_t smem = sizeof(cplx) * GEMM_STAGES * (HN_MT + HN_NT) * LDK;
+  const int tm = ceil_div(M, HN_MT), tn = ceil_div(N, HN_NT);
+  // split K: fill one wave of CTA slots, at least 8 k-tiles per split, and never more partial tiles than the array holds
+  const int per_sm = std::max(1, (int)((227 * 1024) / (smem + 1024)));
+  const long slots = 148L * per_sm, tiles = (long)tm * tn;
+  const long cap_scratch = (long)(KS_STATIC_SCRATCH_ELEMS / ((size_t)M * N));      // >= 1: checked by the caller
+  const long cap_short = std::max(1, K / (8 * KT));
+  int nsplit = (int)std::max(1L, std::min(std::min(cap_short, cap_scratch), (slots + tiles - 1) / tiles));
+  int kchunk = ceil_div(std::max(K, 1), nsplit);
+  kchunk = ceil_div(kchunk, KT) * KT;
+  nsplit = std::max(1, ceil_div(std::max(K, 1), kchunk));      // only shrinks: still within the array
+  dim3 grid(tn, tm, nsplit);
+  k_gemm_hn<NJ><<<grid, GEMM_THREADS, smem, st>>>(M, N, K, A, lda, B, ldb, part, kchunk);
+  k_splitk_reduce<<<ceil_div((long)M * N, 256), 256, 0, st>>>(M, N, nsplit, part, C, ldc);
+  KS_CUDA_CHECK(cudaGetLastError(), err);
+  return KS_OK;
+}
+
+extern "C" int ks_zgemm_hn_static(void* stream, int M, int N, int K, const void* A, long lda, const void* B, long ldb, void* C,
+                                  long ldc) {
+  std::string& err = ks_global_error();
+  if (M < 1 || N < 1 || K < 0 || (K > 0 && (!A || !B)) || !C || lda < K || ldb < K || ldc < M) {
+    err = "ks_zgemm_hn_static: bad argument (M, N >= 1, K >= 0, lda, ldb >= K, ldc >= M, non-NULL device pointers unless K = 0)";
+    return KS_EINVAL;
+  }
+  if ((size_t)M * (size_t)N > KS_STATIC_SCRATCH_ELEMS) {
+    char b[256];
+    snprintf(b, sizeof b, "ks_zgemm_hn_static: M * N = %zu exceeds the static scratch array (%zu complex128 elements = %u MiB); "
+             "use ks_zgemm_hn, which allocates its workspace", (size_t)M * (size_t)N, (size_t)KS_STATIC_SCRATCH_ELEMS,
+             KS_STATIC_SCRATCH_BYTES >> 20);
+    err = b;
+    return KS_EINVAL;
+  }
+  int dev = 0;
+  KS_CUDA_CHECK(cudaGetDevice(&dev), err);
+  if (dev < 0 || dev >= KS_STATIC_MAX_DEV) { err = "ks_zgemm_hn_static: device index beyond 63"; return KS_EINVAL; }
+  const int rc = static_setup(dev, err);
+  if (rc != KS_OK) return rc;
+  cplx* part = g_static_ptr[dev];
+  cudaStream_t st = (cudaStream_t)stream;
+  const cplx *a = (const cplx*)A, *b = (const cplx*)B;
+  cplx* c = (cplx*)C;
+  switch (pick_nj(N, 32)) {
+    case 1: return launch_hn_static<1>(st, M, N, K, a, lda, b, ldb, c, ldc, part, err);
+    case 2: return launch_hn_static<2>(st, M, N, K, a, lda, b, ldb, c, ldc, part, err);
+    case 3: return launch_hn_static<3>(st, M, N, K, a, lda, b, ldb, c, ldc, part, err);
+    case 4: return launch_hn_static<4>(st, M, N, K, a, lda, b, ldb, c, ldc, part, err);
+    default: return launch_hn_static<5>(st, M, N, K, a, lda, b, ldb, c, ldc, part, err);
+  }
+}

@@ -46,6 +46,7 @@ _lib.ks_davidson_profile.argtypes = [_vp, _vp]
 _lib.ks_profile_begin.argtypes = [_vp]
 _lib.ks_profile_end.argtypes = [_vp, _vp, _vp]
 _lib.ks_zgemm_hn.argtypes = [_vp, _i, _i, _i, _vp, _l, _vp, _l, _vp, _l]
+_lib.ks_zgemm_hn_static.argtypes = [_vp, _i, _i, _i, _vp, _l, _vp, _l, _vp, _l]
 _lib.ks_zgemm_nn.argtypes = [_vp, _i, _i, _i, _vp, _l, _vp, _l, _vp, _l, _i]
 _lib.ks_eigh.argtypes = [_vp, _i, _vp, _l, _vp, _vp, _l, _vp]
 _lib.ks_dmma_peak.argtypes = [_vp, _vp]
@@ -54,7 +55,7 @@ _lib.ks_dmma_latency.argtypes = [_vp, _d]
 KS_OK, KS_NOTCONV = 0, 1
 EXPORTS = ("ks_pw_count", "ks_pw_list", "ks_create", "ks_destroy", "ks_npw", "ks_set_stream", "ks_set_fft_batch",
            "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_hpsi_batch", "ks_davidson_batch", "ks_density", "ks_density_host", "ks_chebyshev", "ks_cg", "ks_set_overlap", "ks_spsi", "ks_davidson", "ks_davidson_host",
-           "ks_davidson_profile", "ks_profile_begin", "ks_profile_end", "ks_zgemm_hn", "ks_zgemm_nn", "ks_eigh", "ks_dmma_peak", "ks_dmma_latency")
+           "ks_davidson_profile", "ks_profile_begin", "ks_profile_end", "ks_zgemm_hn", "ks_zgemm_hn_static", "ks_zgemm_nn", "ks_eigh", "ks_dmma_peak", "ks_dmma_latency")
 
 
 class KsError(RuntimeError):
@@ -336,6 +337,18 @@ def ks_zgemm_hn(A, B, stream=None):
     if rc:
         raise KsError(rc, _glob_err())
     return Cm
+
+
+def ks_zgemm_hn_static(A, B, out, stream=None):
+    """ks_zgemm_hn with the split-K partials in the library's static 8 MiB device array: the call allocates nothing, so the
+    caller passes the result buffer too.  A: [M][K], B: [N][K], out: [N][M] (complex128 CUDA, contiguous).  M * N <= 524 288."""
+    M, K = A.shape
+    N = B.shape[0]
+    assert out.shape == (N, M) and out.is_contiguous()
+    rc = _lib.ks_zgemm_hn_static(_stream_ptr(stream), M, N, K, _dev(A), K, _dev(B), K, _dev(out), M)
+    if rc:
+        raise KsError(rc, _glob_err())
+    return out
 
 
 def ks_zgemm_nn(A, B, Cm=None, accumulate=False, stream=None):
