@@ -126,7 +126,8 @@ __global__ void k_set_diag(int m, long ld, cplx* __restrict__ H, const double* _
   H[(long)j * ld + i] = cmake(i == j ? d[i] : 0.0, 0.0);
 }
 // after the new columns Hc[0:m1, m0:m1] were written: mirror them into the rows and symmetrise the corner
-__global__ void k_mirror(int m0, int m1, long ld, cplx* __restrict__ H) {
+// upper_only: the corner holds its upper triangle only (ks_gemm_hn with herm_r0): the lower one is its mirror image
+__global__ void k_mirror(int m0, int m1, long ld, cplx* __restrict__ H, int upper_only) {
   const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
   const int nn = m1 - m0;
   if (e >= (long)m1 * nn) return;
@@ -134,6 +135,13 @@ __global__ void k_mirror(int m0, int m1, long ld, cplx* __restrict__ H) {
   if (i < m0) {
     const cplx a = H[(long)j * ld + i];
     H[(long)i * ld + j] = cconj(a);
+  } else if (upper_only) {
+    if (i <= j) {
+      cplx a = H[(long)j * ld + i];          // row i, column j: the computed triangle
+      if (i == j) a.y = 0.0;
+      H[(long)j * ld + i] = a;
+      H[(long)i * ld + j] = cconj(a);
+    }
   } else if (i <= j) {
     const cplx a = H[(long)j * ld + i], b = H[(long)i * ld + j];
     const cplx s = cmake(0.5 * (a.x + b.x), (i == j) ? 0.0 : 0.5 * (a.y - b.y));
@@ -537,7 +545,9 @@ static int orth_pass(ks_ctx* c, cplx* src, int nu, cplx* dst, int m, int nproj_p
   k_drop_thresholds<<<ceil_div(nu, 128), 128, 0, st>>>(nu, projected ? w.lam0 : nullptr, w.lam, 1e-12, w.thr);
   k_col_scale<<<dim3(std::max(1, std::min(64, ceil_div(npw, 1024))), nu), 256, 0, st>>>(npw, src, w.lam);
   if (gen) RC(ks_spsi_impl(c, src, w.ST, nu));
-  RC(ks_gemm_hn(st, nu, nu, npw, src, npw, gen ? w.ST : src, npw, w.Us, nu, &c->gws, c->err));
+  // the Cholesky kernels read the upper triangle of the Gram matrix only: the tiles below its diagonal are not computed
+  static const bool herm_on = !(getenv("KSPW_HERM_SKIP") && atoi(getenv("KSPW_HERM_SKIP")) == 0);
+  RC(ks_gemm_hn(st, nu, nu, npw, src, npw, gen ? w.ST : src, npw, w.Us, nu, &c->gws, c->err, herm_on ? 0 : -1));
   ph.end(PH_ORTH);
   ph.begin();
   static std::atomic<bool> opted{false};
@@ -557,8 +567,11 @@ static int orth_pass(ks_ctx* c, cplx* src, int nu, cplx* dst, int m, int nproj_p
   k_trinv<<<ceil_div(nk, 4), 128, sizeof(cplx) * 4 * nk, st>>>(nu, w.Us, nu, w.idx, nk, w.S, nu);
   ph.end(PH_EIGH);
   ph.begin();
-  RC(ks_gemm_nn(st, npw, nk, nu, src, npw, w.S, nu, dst, npw, 0, c->err));
-  if (gen && sdst) RC(ks_gemm_nn(st, npw, nk, nu, w.ST, npw, w.S, nu, sdst, npw, 0, c->err));
+  // no column dropped: w.S = R^{-1} is upper triangular, column n ends at row n (with drops it ends at row kept[n] >= n,
+  // known on the device only: the full product then)
+  const int btri = (herm_on && nk == nu) ? 0 : -1;
+  RC(ks_gemm_nn(st, npw, nk, nu, src, npw, w.S, nu, dst, npw, 0, c->err, btri));
+  if (gen && sdst) RC(ks_gemm_nn(st, npw, nk, nu, w.ST, npw, w.S, nu, sdst, npw, 0, c->err, btri));
   ph.end(PH_ORTH);
   return KS_OK;
 }
@@ -717,8 +730,10 @@ int ks_davidson_impl(ks_ctx* c, cplx* psi, double* eig, int nb, double tol, int 
     // D2
     ph.begin();
     const int m1 = m + nk;
-    RC(ks_gemm_hn(st, m1, nk, npw, w.V, npw, Wnew, npw, w.Hc + (size_t)m * ldh, ldh, &c->gws, c->err));
-    k_mirror<<<ceil_div((long)m1 * nk, 256), 256, 0, st>>>(m, m1, ldh, w.Hc);
+    // the corner V_new^H (H V_new) is Hermitian: only the tiles that reach its upper triangle are computed, k_mirror fills the rest
+    static const bool herm_hc = !(getenv("KSPW_HERM_SKIP") && atoi(getenv("KSPW_HERM_SKIP")) == 0);
+    RC(ks_gemm_hn(st, m1, nk, npw, w.V, npw, Wnew, npw, w.Hc + (size_t)m * ldh, ldh, &c->gws, c->err, herm_hc ? m : -1));
+    k_mirror<<<ceil_div((long)m1 * nk, 256), 256, 0, st>>>(m, m1, ldh, w.Hc, herm_hc ? 1 : 0);
     ph.end(PH_PROJ);
     m = m1;
     // D3

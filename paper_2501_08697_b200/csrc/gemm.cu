@@ -41,15 +41,18 @@
 #define HN_MT 64
 
 // one CTA tile of C = A^H B over the K range [kbeg, kend): the partial tile goes to out (column-major M x N)
-template <int NJ>
+// WN = warps along N (WM = 8 / WN along M): WN = 4 is the wide tile above; WN = 1 gives an N-tile of 8*NJ columns (8 .. 40)
+// with 8-row warp tiles, for narrow products and for the ragged remainder of a wide one (N = 520 = 3 x 160 + 40: the 40
+// columns cost 40/480 of the main launch instead of a padded 64-wide tile, cfg 3: 3.31 -> 2.0 ms).
+template <int NJ, int WN = 4>
 __device__ __forceinline__ void gemm_hn_tile(int M, int N, const cplx* __restrict__ A, long lda, const cplx* __restrict__ B,
                                              long ldb, cplx* __restrict__ out, int m0, int n0, int kbeg, int kend) {
-  constexpr int HN_NT = 32 * NJ;
+  constexpr int WM = 8 / WN, MI = HN_MT / (8 * WM), HN_NT = 8 * NJ * WN;
   extern __shared__ cplx sm[];
   cplx* sA = sm;                                     // [stage][HN_MT][LDK]
   cplx* sB = sm + GEMM_STAGES * HN_MT * LDK;         // [stage][HN_NT][LDK]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int wm = warp & 1, wn = warp >> 1;
+  const int wm = warp % WM, wn = warp / WM;
   const int ntile = (kend - kbeg + KT - 1) / KT;
 
   auto load_stage = [&](int st, int kt) {
@@ -62,16 +65,17 @@ __device__ __forceinline__ void gemm_hn_tile(int M, int N, const cplx* __restric
       cp16(&sA[(st * HN_MT + col) * LDK + kk], ok ? &A[(long)(m0 + col) * lda + k0 + kk] : A, ok);
     }
 #pragma unroll
-    for (int r = 0; r < (HN_NT * KT) / GEMM_THREADS; ++r) {
+    for (int r = 0; r < (HN_NT * KT + GEMM_THREADS - 1) / GEMM_THREADS; ++r) {
       const int e = tid + r * GEMM_THREADS, col = e / KT, kk = e % KT;
+      if ((HN_NT * KT) % GEMM_THREADS != 0 && e >= HN_NT * KT) break;
       const bool ok = (n0 + col < N) && (k0 + kk < kend);
       cp16(&sB[(st * HN_NT + col) * LDK + kk], ok ? &B[(long)(n0 + col) * ldb + k0 + kk] : B, ok);
     }
   };
 
-  double cre[4][NJ][2], cim[4][NJ][2];
+  double cre[MI][NJ][2], cim[MI][NJ][2];
 #pragma unroll
-  for (int i = 0; i < 4; ++i)
+  for (int i = 0; i < MI; ++i)
 #pragma unroll
     for (int j = 0; j < NJ; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
 
@@ -97,7 +101,7 @@ __device__ __forceinline__ void gemm_hn_tile(int M, int N, const cplx* __restric
     if (more) load_stage((kt + GEMM_STAGES - 1) % GEMM_STAGES, kt + GEMM_STAGES - 1);
     cp_commit();
 #endif
-    const cplx* a = sA + ((kt % GEMM_STAGES) * HN_MT + wm * 32) * LDK;
+    const cplx* a = sA + ((kt % GEMM_STAGES) * HN_MT + wm * 8 * MI) * LDK;
     const cplx* b = sB + ((kt % GEMM_STAGES) * HN_NT + wn * 8 * NJ) * LDK;
 #pragma unroll
     for (int ks = 0; ks < KT; ks += 4) {
@@ -107,16 +111,16 @@ __device__ __forceinline__ void gemm_hn_tile(int M, int N, const cplx* __restric
         cp_commit();
       }
 #endif
-      cplx af[4], bf[NJ];
+      cplx af[MI], bf[NJ];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) af[i] = a[(i * 8 + fr) * LDK + ks + fk];
+      for (int i = 0; i < MI; ++i) af[i] = a[(i * 8 + fr) * LDK + ks + fk];
 #pragma unroll
       for (int j = 0; j < NJ; ++j) bf[j] = b[(j * 8 + fr) * LDK + ks + fk];
       // conj(a) b = (ar br + ai bi) + i (ar bi - ai br).  The two products of one accumulator are two DMMAs apart: enough,
       // the DMMA result latency is 27 clk against an issue interval of 16 (ks_dmma_latency); spreading them 8 NJ apart
       // measured no difference (cfg 3: 30.24 vs 30.29 ms)
 #pragma unroll
-      for (int i = 0; i < 4; ++i) {
+      for (int i = 0; i < MI; ++i) {
         const double nai = -af[i].y;
 #pragma unroll
         for (int j = 0; j < NJ; ++j) {
@@ -130,24 +134,26 @@ __device__ __forceinline__ void gemm_hn_tile(int M, int N, const cplx* __restric
   }
   cp_wait<0>();
 #pragma unroll
-  for (int i = 0; i < 4; ++i)
+  for (int i = 0; i < MI; ++i)
 #pragma unroll
     for (int j = 0; j < NJ; ++j)
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        const int m = m0 + wm * 32 + i * 8 + fr, n = n0 + wn * 8 * NJ + j * 8 + 2 * fk + h;
+        const int m = m0 + wm * 8 * MI + i * 8 + fr, n = n0 + wn * 8 * NJ + j * 8 + 2 * fk + h;
         if (m < M && n < N) out[(size_t)n * M + m] = cmake(cre[i][j][h], cim[i][j][h]);
       }
 }
 
-template <int NJ>
+template <int NJ, int WN = 4>
 __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_hn(int M, int N, int K, const cplx* __restrict__ A, long lda,
                                                           const cplx* __restrict__ B, long ldb, cplx* __restrict__ part,
-                                                          int kchunk) {
+                                                          int kchunk, int herm_r0) {
+  // Hermitian block (rows herm_r0..): tiles strictly below its diagonal are not computed
+  if (herm_r0 >= 0 && (int)(blockIdx.y * HN_MT) - herm_r0 > (int)(blockIdx.x * 8 * NJ * WN + 8 * NJ * WN - 1)) return;
   const int kbeg = blockIdx.z * kchunk;
   // partial tile -> part[z][n][m] (column-major M x N per split)
-  gemm_hn_tile<NJ>(M, N, A, lda, B, ldb, part + (size_t)blockIdx.z * M * N, blockIdx.y * HN_MT, blockIdx.x * 32 * NJ, kbeg,
-                   min(K, kbeg + kchunk));
+  gemm_hn_tile<NJ, WN>(M, N, A, lda, B, ldb, part + (size_t)blockIdx.z * M * N, blockIdx.y * HN_MT, blockIdx.x * 8 * NJ * WN, kbeg,
+                       min(K, kbeg + kchunk));
 }
 
 // Grouped form (ks_hpsi_batch): blockIdx.z = problem * nsplit + split; every problem has its own operands and sizes, the
@@ -164,9 +170,11 @@ __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_hn_g(const GemmProb* __re
   gemm_hn_tile<NJ>(p.M, p.N, p.A, p.lda, p.B, p.ldb, p.C + (size_t)z * p.M * p.N, m0, n0, kbeg, max(kend, kbeg));
 }
 
-__global__ void k_splitk_reduce(int M, int N, int nsplit, const cplx* __restrict__ part, cplx* __restrict__ C, long ldc) {
+__global__ void k_splitk_reduce(int M, int N, int nsplit, const cplx* __restrict__ part, cplx* __restrict__ C, long ldc,
+                                int herm_r0 = -1) {
   const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
   if (i >= (long)M * N) return;
+  if (herm_r0 >= 0 && (int)(i % M) - herm_r0 > (int)(i / M)) return;     // strictly below the diagonal of the Hermitian block
   double sr = 0, si = 0;
   for (int z = 0; z < nsplit; ++z) {   // fixed order: deterministic
     const cplx p = part[(size_t)z * M * N + i];
@@ -186,14 +194,14 @@ static int pick_nj(int N, int unit) {
   return best;
 }
 
-template <int NJ>
+template <int NJ, int WN = 4>
 static int launch_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
-                     long ldc, GemmWs* ws, std::string& err) {
-  constexpr int HN_NT = 32 * NJ;
+                     long ldc, GemmWs* ws, std::string& err, int herm_r0 = -1) {
+  constexpr int HN_NT = 8 * NJ * WN;
   static std::atomic<bool> opted{false};
   const size_t smem = sizeof(cplx) * GEMM_STAGES * (HN_MT + HN_NT) * LDK;
   if (!opted) {
-    KS_CUDA_CHECK(cudaFuncSetAttribute(k_gemm_hn<NJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err);
+    KS_CUDA_CHECK((cudaFuncSetAttribute(k_gemm_hn<NJ, WN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)), err);
     opted = true;
   }
   const int tm = ceil_div(M, HN_MT), tn = ceil_div(N, HN_NT);
@@ -201,7 +209,14 @@ static int launch_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long l
   // memory) about two tiles and (b) wastes less than 7 % of the last wave; each split keeps at least 8 k-tiles.
   // (Measured on cfg 1, 8 output tiles: 148 splits 0.84 ms, 37 splits = exactly two waves 0.78 ms.)
   const int per_sm = std::max(1, (int)((227 * 1024) / (smem + 1024)));
-  const long slots = 148L * per_sm, tiles = (long)tm * tn;
+  long tiles = (long)tm * tn;
+  if (herm_r0 >= 0) {       // tiles that do work
+    tiles = 0;
+    for (int y = 0; y < tm; ++y)
+      for (int x = 0; x < tn; ++x)
+        if (!(y * HN_MT - herm_r0 > x * HN_NT + HN_NT - 1)) ++tiles;
+  }
+  const long slots = 148L * per_sm;
   // CTAs of one launch take equal time, so they run as lockstep waves of `slots`: take the split count with the fullest
   // last wave among those that give at least two waves and keep >= 48 k-tiles per split (the pipeline prologue and the
   // partial-tile store stay < 1 %).  cfg 3 beta^H psi (81 tiles of 64 x 160): 7 splits = 3.83 waves (ncu: tensor pipe 68 %
@@ -233,8 +248,8 @@ static int launch_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long l
     ws->bytes = need;
   }
   dim3 grid(tn, tm, nsplit);
-  k_gemm_hn<NJ><<<grid, GEMM_THREADS, smem, st>>>(M, N, K, A, lda, B, ldb, ws->part, kchunk);
-  k_splitk_reduce<<<ceil_div((long)M * N, 256), 256, 0, st>>>(M, N, nsplit, ws->part, C, ldc);
+  k_gemm_hn<NJ, WN><<<grid, GEMM_THREADS, smem, st>>>(M, N, K, A, lda, B, ldb, ws->part, kchunk, herm_r0);
+  k_splitk_reduce<<<ceil_div((long)M * N, 256), 256, 0, st>>>(M, N, nsplit, ws->part, C, ldc, herm_r0);
   KS_CUDA_CHECK(cudaGetLastError(), err);
   return KS_OK;
 }
@@ -318,7 +333,7 @@ __global__ void __launch_bounds__(GEMV_T) k_gemv_nn(int M, int K, const cplx* __
 }
 
 int ks_gemm_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
-               long ldc, GemmWs* ws, std::string& err) {
+               long ldc, GemmWs* ws, std::string& err, int herm_r0) {
   if (M <= 0 || N <= 0) return KS_OK;
   if (K < 0 || !ws) { err = "ks_gemm_hn: bad argument"; return KS_EINVAL; }
   if (N <= 4 && K >= 1024) {
@@ -331,21 +346,44 @@ int ks_gemm_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, co
     KS_CUDA_CHECK(cudaGetLastError(), err);
     return KS_OK;
   }
-  // N beyond the widest tile and not a multiple of a wide one (N = 520 -> 17 tiles of 32 by the least-padding rule): whole
-  // 160-wide tiles first, the remainder in a second launch with its own least-padding tile
+  // Tile choice (KSPW_GEMM_NSPLIT=0: one launch with the least-padding wide tile, the round-1 rule):
+  //   N <= 40          one launch of 8*NJ-wide tiles (WN = 1): padding < 8 columns
+  //   N  > 160         whole 160-wide tiles, the rest (if any) by the same rules in a second launch
+  //   40 < N <= 160    32*NJ-wide tiles; a ragged tail of 1..24 columns beyond a multiple of 32 goes to a narrow launch
   static const bool nsplit_on = !(getenv("KSPW_GEMM_NSPLIT") && atoi(getenv("KSPW_GEMM_NSPLIT")) == 0);
-  if (nsplit_on && N > 160 && N % 160 != 0 && pick_nj(N, 32) < 4) {
-    const int main_n = N / 160 * 160;
-    const int rc = launch_hn<5>(st, M, main_n, K, A, lda, B, ldb, C, ldc, ws, err);
-    if (rc != KS_OK) return rc;
-    return ks_gemm_hn(st, M, N - main_n, K, A, lda, B + (long)main_n * ldb, ldb, C + (long)main_n * ldc, ldc, ws, err);
+  if (nsplit_on) {
+    if (N <= 40) {
+      switch ((N + 7) / 8) {
+        case 1: return launch_hn<1, 1>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+        case 2: return launch_hn<2, 1>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+        case 3: return launch_hn<3, 1>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+        case 4: return launch_hn<4, 1>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+        default: return launch_hn<5, 1>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+      }
+    }
+    int main_n = N;
+    if (N > 160) main_n = N / 160 * 160;
+    else if (N % 32 >= 1 && N % 32 <= 24) main_n = N / 32 * 32;
+    if (main_n < N) {
+      const int rc = ks_gemm_hn(st, M, main_n, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+      if (rc != KS_OK) return rc;
+      // the remainder's local column 0 is global column main_n: the diagonal of the Hermitian block moves down by main_n rows
+      return ks_gemm_hn(st, M, N - main_n, K, A, lda, B + (long)main_n * ldb, ldb, C + (long)main_n * ldc, ldc, ws, err,
+                        herm_r0 >= 0 ? herm_r0 + main_n : -1);
+    }
+    switch ((N + 31) / 32 > 5 ? 5 : (N + 31) / 32) {    // here N <= 160 or N % 160 == 0
+      case 2: return launch_hn<2>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+      case 3: return launch_hn<3>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+      case 4: return launch_hn<4>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+      default: return launch_hn<5>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+    }
   }
   switch (pick_nj(N, 32)) {
-    case 1: return launch_hn<1>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);
-    case 2: return launch_hn<2>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);
-    case 3: return launch_hn<3>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);
-    case 4: return launch_hn<4>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);
-    default: return launch_hn<5>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err);
+    case 1: return launch_hn<1>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+    case 2: return launch_hn<2>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+    case 3: return launch_hn<3>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+    case 4: return launch_hn<4>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
+    default: return launch_hn<5>(st, M, N, K, A, lda, B, ldb, C, ldc, ws, err, herm_r0);
   }
 }
 
@@ -356,15 +394,17 @@ int ks_gemm_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, co
 #define NN_MT 128
 #define LDM (NN_MT + 2)   // "m-contiguous" tile leading dimension: == 2 (mod 8)
 
-template <int NJ>
+// WN = warps along N (WM = 8 / WN along M): WN = 2 is the tile above; WN = 1 gives an N-tile of 8*NJ columns (8 .. 40) with
+// 16-row warp tiles, for narrow products and the ragged remainder of a wide one (see gemm_hn_tile).
+template <int NJ, int WN = 2>
 __device__ __forceinline__ void gemm_nn_tile(int M, int N, int K, const cplx* __restrict__ A, long lda, const cplx* __restrict__ B,
                                              long ldb, cplx* __restrict__ C, long ldc, int accumulate, int m0, int n0) {
-  constexpr int NN_NT = 16 * NJ;
+  constexpr int WM = 8 / WN, MI = NN_MT / (8 * WM), NN_NT = 8 * NJ * WN;
   extern __shared__ cplx sm[];
   cplx* sA = sm;                                   // [stage][KT][LDM]
   cplx* sB = sm + GEMM_STAGES * KT * LDM;          // [stage][NN_NT][LDK]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int wm = warp & 3, wn = warp >> 2;
+  const int wm = warp % WM, wn = warp / WM;
   const int ntile = (K + KT - 1) / KT;
 
   auto load_stage = [&](int st, int kt) {
@@ -376,16 +416,17 @@ __device__ __forceinline__ void gemm_nn_tile(int M, int N, int K, const cplx* __
       cp16(&sA[(st * KT + kk) * LDM + mm], ok ? &A[(long)(k0 + kk) * lda + m0 + mm] : A, ok);
     }
 #pragma unroll
-    for (int r = 0; r < (NN_NT * KT) / GEMM_THREADS; ++r) {
+    for (int r = 0; r < (NN_NT * KT + GEMM_THREADS - 1) / GEMM_THREADS; ++r) {
       const int e = tid + r * GEMM_THREADS, col = e / KT, kk = e % KT;
+      if ((NN_NT * KT) % GEMM_THREADS != 0 && e >= NN_NT * KT) break;
       const bool ok = (n0 + col < N) && (k0 + kk < K);
       cp16(&sB[(st * NN_NT + col) * LDK + kk], ok ? &B[(long)(n0 + col) * ldb + k0 + kk] : B, ok);
     }
   };
 
-  double cre[4][NJ][2], cim[4][NJ][2];
+  double cre[MI][NJ][2], cim[MI][NJ][2];
 #pragma unroll
-  for (int i = 0; i < 4; ++i)
+  for (int i = 0; i < MI; ++i)
 #pragma unroll
     for (int j = 0; j < NJ; ++j) cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0;
 
@@ -407,7 +448,7 @@ __device__ __forceinline__ void gemm_nn_tile(int M, int N, int K, const cplx* __
     if (more) load_stage((kt + GEMM_STAGES - 1) % GEMM_STAGES, kt + GEMM_STAGES - 1);
     cp_commit();
 #endif
-    const cplx* a = sA + (kt % GEMM_STAGES) * KT * LDM + wm * 32;
+    const cplx* a = sA + (kt % GEMM_STAGES) * KT * LDM + wm * 8 * MI;
     const cplx* b = sB + ((kt % GEMM_STAGES) * NN_NT + wn * 8 * NJ) * LDK;
 #pragma unroll
     for (int ks = 0; ks < KT; ks += 4) {
@@ -417,13 +458,13 @@ __device__ __forceinline__ void gemm_nn_tile(int M, int N, int K, const cplx* __
         cp_commit();
       }
 #endif
-      cplx af[4], bf[NJ];
+      cplx af[MI], bf[NJ];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) af[i] = a[(ks + fk) * LDM + i * 8 + fr];
+      for (int i = 0; i < MI; ++i) af[i] = a[(ks + fk) * LDM + i * 8 + fr];
 #pragma unroll
       for (int j = 0; j < NJ; ++j) bf[j] = b[(j * 8 + fr) * LDK + ks + fk];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) {
+      for (int i = 0; i < MI; ++i) {
         const double nai = -af[i].y;
 #pragma unroll
         for (int j = 0; j < NJ; ++j) {   // a b = (ar br - ai bi) + i (ar bi + ai br)
@@ -437,12 +478,12 @@ __device__ __forceinline__ void gemm_nn_tile(int M, int N, int K, const cplx* __
   }
   cp_wait<0>();
 #pragma unroll
-  for (int i = 0; i < 4; ++i)
+  for (int i = 0; i < MI; ++i)
 #pragma unroll
     for (int j = 0; j < NJ; ++j)
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        const int m = m0 + wm * 32 + i * 8 + fr, n = n0 + wn * 8 * NJ + j * 8 + 2 * fk + h;
+        const int m = m0 + wm * 8 * MI + i * 8 + fr, n = n0 + wn * 8 * NJ + j * 8 + 2 * fk + h;
         if (m < M && n < N) {
           cplx* p = &C[(long)n * ldc + m];
           cplx v = cmake(cre[i][j][h], cim[i][j][h]);
@@ -452,11 +493,14 @@ __device__ __forceinline__ void gemm_nn_tile(int M, int N, int K, const cplx* __
       }
 }
 
-template <int NJ>
+template <int NJ, int WN = 2>
 __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_nn(int M, int N, int K, const cplx* __restrict__ A, long lda,
                                                           const cplx* __restrict__ B, long ldb, cplx* __restrict__ C,
-                                                          long ldc, int accumulate) {
-  gemm_nn_tile<NJ>(M, N, K, A, lda, B, ldb, C, ldc, accumulate, blockIdx.x * NN_MT, blockIdx.y * 16 * NJ);
+                                                          long ldc, int accumulate, int btri_c0) {
+  // triangular B (B[k][n] = 0 for k > btri_c0 + n): this N-tile's products end at row btri_c0 + (its last column)
+  const int n0 = blockIdx.y * 8 * NJ * WN;
+  const int Keff = btri_c0 >= 0 ? min(K, btri_c0 + n0 + 8 * NJ * WN) : K;
+  gemm_nn_tile<NJ, WN>(M, N, Keff, A, lda, B, ldb, C, ldc, accumulate, blockIdx.x * NN_MT, n0);
 }
 template <int NJ>
 __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_nn_g(const GemmProb* __restrict__ probs, int accumulate) {
@@ -466,24 +510,24 @@ __global__ void __launch_bounds__(GEMM_THREADS) k_gemm_nn_g(const GemmProb* __re
   gemm_nn_tile<NJ>(p.M, p.N, p.K, p.A, p.lda, p.B, p.ldb, p.C, p.ldc, accumulate, m0, n0);
 }
 
-template <int NJ>
+template <int NJ, int WN = 2>
 static int launch_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
-                     long ldc, int accumulate, std::string& err) {
-  constexpr int NN_NT = 16 * NJ;
+                     long ldc, int accumulate, std::string& err, int btri_c0 = -1) {
+  constexpr int NN_NT = 8 * NJ * WN;
   static std::atomic<bool> opted{false};
   const size_t smem = sizeof(cplx) * GEMM_STAGES * (KT * LDM + NN_NT * LDK);
   if (!opted) {
-    KS_CUDA_CHECK(cudaFuncSetAttribute(k_gemm_nn<NJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), err);
+    KS_CUDA_CHECK((cudaFuncSetAttribute(k_gemm_nn<NJ, WN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)), err);
     opted = true;
   }
   dim3 grid(ceil_div(M, NN_MT), ceil_div(N, NN_NT));
-  k_gemm_nn<NJ><<<grid, GEMM_THREADS, smem, st>>>(M, N, K, A, lda, B, ldb, C, ldc, accumulate);
+  k_gemm_nn<NJ, WN><<<grid, GEMM_THREADS, smem, st>>>(M, N, K, A, lda, B, ldb, C, ldc, accumulate, btri_c0);
   KS_CUDA_CHECK(cudaGetLastError(), err);
   return KS_OK;
 }
 
 int ks_gemm_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb, cplx* C,
-               long ldc, int accumulate, std::string& err) {
+               long ldc, int accumulate, std::string& err, int btri_c0) {
   if (M <= 0 || N <= 0) return KS_OK;
   if (K < 0) { err = "ks_gemm_nn: bad argument"; return KS_EINVAL; }
   if (N <= 4 && M >= 1024 && K >= 1) {
@@ -497,21 +541,42 @@ int ks_gemm_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, co
     KS_CUDA_CHECK(cudaGetLastError(), err);
     return KS_OK;
   }
-  // N beyond the widest tile and not a multiple of it (N = 520 -> eleven 48-wide tiles by the least-padding rule): whole 80-wide
-  // tiles first (more DMMAs per fragment load, A re-read 7 instead of 11 times), the remainder in a second launch
+  // Tile choice (KSPW_GEMM_NSPLIT=0: one launch with the least-padding 16*NJ-wide tile, the round-1 rule):
+  //   N <= 40         one launch of 8*NJ-wide tiles (WN = 1)
+  //   N  > 80         whole 80-wide tiles (more DMMAs per fragment load, A re-read N/80 times), the rest in a second launch
+  //   40 < N <= 80    16*NJ-wide tiles; a ragged tail of 1..8 columns beyond a multiple of 16 goes to a narrow launch
   static const bool nsplit_on = !(getenv("KSPW_GEMM_NSPLIT") && atoi(getenv("KSPW_GEMM_NSPLIT")) == 0);
-  if (nsplit_on && N > 80 && N % 80 != 0 && pick_nj(N, 16) < 5) {
-    const int main_n = N / 80 * 80;
-    const int rc = launch_nn<5>(st, M, main_n, K, A, lda, B, ldb, C, ldc, accumulate, err);
-    if (rc != KS_OK) return rc;
-    return ks_gemm_nn(st, M, N - main_n, K, A, lda, B + (long)main_n * ldb, ldb, C + (long)main_n * ldc, ldc, accumulate, err);
+  if (nsplit_on) {
+    if (N <= 40) {
+      switch ((N + 7) / 8) {
+        case 1: return launch_nn<1, 1>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
+        case 2: return launch_nn<2, 1>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
+        case 3: return launch_nn<3, 1>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
+        case 4: return launch_nn<4, 1>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
+        default: return launch_nn<5, 1>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
+      }
+    }
+    int main_n = N;
+    if (N > 80) main_n = N / 80 * 80;
+    else if (N % 16 >= 1 && N % 16 <= 8) main_n = N / 16 * 16;
+    if (main_n < N) {
+      const int rc = ks_gemm_nn(st, M, main_n, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
+      if (rc != KS_OK) return rc;
+      return ks_gemm_nn(st, M, N - main_n, K, A, lda, B + (long)main_n * ldb, ldb, C + (long)main_n * ldc, ldc, accumulate, err,
+                        btri_c0 >= 0 ? btri_c0 + main_n : -1);
+    }
+    switch ((N + 15) / 16 > 5 ? 5 : (N + 15) / 16) {    // here N <= 80 or N % 80 == 0
+      case 3: return launch_nn<3>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
+      case 4: return launch_nn<4>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
+      default: return launch_nn<5>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
+    }
   }
   switch (pick_nj(N, 16)) {
-    case 1: return launch_nn<1>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
-    case 2: return launch_nn<2>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
-    case 3: return launch_nn<3>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
-    case 4: return launch_nn<4>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
-    default: return launch_nn<5>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err);
+    case 1: return launch_nn<1>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
+    case 2: return launch_nn<2>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
+    case 3: return launch_nn<3>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
+    case 4: return launch_nn<4>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
+    default: return launch_nn<5>(st, M, N, K, A, lda, B, ldb, C, ldc, accumulate, err, btri_c0);
   }
 }
 
@@ -759,7 +824,7 @@ static int launch_hn_static(cudaStream_t st, int M, int N, int K, const cplx* A,
   kchunk = ceil_div(kchunk, KT) * KT;
   nsplit = std::max(1, ceil_div(std::max(K, 1), kchunk));      // only shrinks: still within the array
   dim3 grid(tn, tm, nsplit);
-  k_gemm_hn<NJ><<<grid, GEMM_THREADS, smem, st>>>(M, N, K, A, lda, B, ldb, part, kchunk);
+  k_gemm_hn<NJ><<<grid, GEMM_THREADS, smem, st>>>(M, N, K, A, lda, B, ldb, part, kchunk, -1);
   k_splitk_reduce<<<ceil_div((long)M * N, 256), 256, 0, st>>>(M, N, nsplit, part, C, ldc);
   KS_CUDA_CHECK(cudaGetLastError(), err);
   return KS_OK;

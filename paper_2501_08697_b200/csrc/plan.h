@@ -71,10 +71,16 @@ struct GemmWs {          // split-K partial sums
   cplx* part = nullptr;
   size_t bytes = 0;
 };
+// herm_r0 >= 0: rows herm_r0 .. herm_r0 + N - 1 of C form a Hermitian N x N block (A's columns herm_r0.. and B's columns
+// span it: a Gram matrix T^H T with herm_r0 = 0, the corner V_new^H (H V_new) of the subspace matrix); only the tiles
+// that reach its upper triangle (row - herm_r0 <= column) are computed, the elements strictly below the diagonal are
+// NOT written (the caller mirrors or ignores them).
 int ks_gemm_hn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb,
-               cplx* C, long ldc, GemmWs* ws, std::string& err);
+               cplx* C, long ldc, GemmWs* ws, std::string& err, int herm_r0 = -1);
+// btri_c0 >= 0: B is upper triangular in the sense B[k][n] = 0 for k > btri_c0 + n (an inverse Cholesky factor, btri_c0 = 0):
+// every N-tile stops its K loop at its last non-zero row.
 int ks_gemm_nn(cudaStream_t st, int M, int N, int K, const cplx* A, long lda, const cplx* B, long ldb,
-               cplx* C, long ldc, int accumulate, std::string& err);
+               cplx* C, long ldc, int accumulate, std::string& err, int btri_c0 = -1);
 
 // grouped launches (ks_hpsi_batch): ng independent problems of similar size in one launch; dev_probs is a DEVICE array
 struct GemmProb {

@@ -31,7 +31,9 @@ def _rel(a, b):
 # ------------------------------------------------------------------ building blocks (T1)
 @pytest.mark.parametrize("M,N,K", [(8, 8, 515), (160, 37, 1503), (70, 130, 4099), (1, 1, 1), (64, 64, 16), (5, 3, 0),
                                    (512, 1, 37073), (23, 2, 4099), (64, 3, 1503), (7, 4, 8459),
-                                   (70, 200, 4099), (33, 520, 2050), (9, 163, 1503)])   # N > 160: whole 160-wide tiles + a remainder launch
+                                   (70, 200, 4099), (33, 520, 2050), (9, 163, 1503),    # N > 160: whole 160-wide tiles + a remainder launch
+                                   (1728, 40, 4099), (100, 13, 4099), (64, 24, 2050), (27, 100, 1503), (70, 182, 2050), (9, 41, 515),
+                                   (65, 8, 300), (130, 33, 1000)])                      # N <= 40: 8*NJ-wide tiles; ragged tails of 1..24 columns
 def test_zgemm_hn(ks, M, N, K):
     rng = np.random.default_rng(M * 1000 + N)
     A = rng.standard_normal((M, K)) + 1j * rng.standard_normal((M, K))
@@ -42,7 +44,9 @@ def test_zgemm_hn(ks, M, N, K):
 
 
 @pytest.mark.parametrize("M,N,K,acc", [(515, 8, 8, True), (1503, 23, 512, True), (4099, 70, 130, False), (1, 1, 1, False), (130, 65, 17, True),
-                                       (37073, 1, 512, True), (4099, 2, 64, False), (1503, 3, 1728, True), (8459, 4, 1, True)])
+                                       (37073, 1, 512, True), (4099, 2, 64, False), (1503, 3, 1728, True), (8459, 4, 1, True),
+                                       (4099, 40, 130, False), (1503, 13, 512, True), (2050, 520, 64, True), (515, 100, 33, False),
+                                       (130, 72, 40, True), (700, 5, 1040, False), (257, 41, 17, True)])   # narrow (8*NJ) tiles and ragged tails
 def test_zgemm_nn(ks, M, N, K, acc):
     rng = np.random.default_rng(M + N + K)
     A = rng.standard_normal((K, M)) + 1j * rng.standard_normal((K, M))
