@@ -449,11 +449,29 @@ __device__ __forceinline__ void jac_upd_tile(cplx* sm, cplx* Ap, cplx* Vp, long 
     const int gj = blk_index<32>(pb, j);
     X[(long)gj * ld + gi] = sT[i * JU_LD + j];
   }
+  // A stays Hermitian under U^H A U: the tile (b, ay) is the conjugate transpose of this one and no CTA computes it
+  // (jac_tile_decode deals out the tiles with ay <= b only)
+  if (isA && ay != b) {
+    for (int e = tid; e < 32 * 32; e += 256) {
+      const int j = e & 31, i = e >> 5;          // j fastest: consecutive rows of the mirrored tile
+      X[(long)blk_index<32>(pa, i) * ld + blk_index<32>(pb, j)] = cconj(sT[i * JU_LD + j]);
+    }
+  }
+}
+// tile t of a round -> (b, ay): first the npair (npair + 1) / 2 tiles of A on or above the block diagonal (ay <= b), then
+// the npair * nvt tiles of V (ay = npair + row block)
+__device__ __forceinline__ void jac_tile_decode(int t, int npair, int* b, int* ay) {
+  const int nA = npair * (npair + 1) / 2;
+  if (t >= nA) { t -= nA; *b = t % npair; *ay = npair + t / npair; return; }
+  int a = 0;
+  while (t >= npair - a) { t -= npair - a; ++a; }
+  *ay = a; *b = a + t;
 }
 
 __global__ void __launch_bounds__(256) k_jac_upd32(cplx* __restrict__ Ap, cplx* __restrict__ Vp, long ld, int npair,
                                                    const int2* __restrict__ pairs, const cplx* __restrict__ U) {
   extern __shared__ cplx sm[];
+  if (blockIdx.y < (unsigned)npair && blockIdx.y > blockIdx.x) return;     // below the block diagonal: written by tile (y, x)'s CTA
   jac_upd_tile(sm, Ap, Vp, ld, npair, pairs, U, blockIdx.x, blockIdx.y);
 }
 
@@ -469,7 +487,7 @@ __global__ void __launch_bounds__(256) k_jac_coop32(cplx* Ap, cplx* Vp, int np, 
   cg::grid_group grid = cg::this_grid();
   extern __shared__ cplx sm[];
   const int tid = threadIdx.x, npair = nblk / 2, nbk = JB / 2;
-  const int ntile = npair * (npair + np / 32);
+  const int ntile = npair * (npair + 1) / 2 + npair * (np / 32);
   int sweep = 0;
   for (; sweep < max_sweeps; ++sweep) {
     // off(A)_F^2 and ||A||_F^2 of the n x n part, fixed partition of the elements over the grid
@@ -517,7 +535,9 @@ __global__ void __launch_bounds__(256) k_jac_coop32(cplx* Ap, cplx* Vp, int np, 
       grid.sync();
       for (int t = blockIdx.x; t < ntile; t += gridDim.x) {
         __syncthreads();
-        jac_upd_tile(sm, Ap, Vp, np, npair, pr, U, t % npair, t / npair);
+        int tb, tay;
+        jac_tile_decode(t, npair, &tb, &tay);
+        jac_upd_tile(sm, Ap, Vp, np, npair, pr, U, tb, tay);
       }
       grid.sync();
     }
@@ -543,7 +563,8 @@ __global__ void __launch_bounds__(256) k_jac_round32(const cplx* __restrict__ Ao
   const int tid = threadIdx.x;
   if ((int)blockIdx.x >= npair) {
     // tile CTA: t -> (b, ay); A tiles read Aold and write Anew, V tiles update Vp in place
-    const int t = blockIdx.x - npair, b = t % npair, ay = t / npair;
+    int b, ay;
+    jac_tile_decode(blockIdx.x - npair, npair, &b, &ay);
     cplx *sT = sm, *sUa = sm + 32 * JU_LD, *sUb = sm + 64 * JU_LD;
     const bool isA = ay < npair;
     const int2 pb = pairs_cur[b];
@@ -592,6 +613,12 @@ __global__ void __launch_bounds__(256) k_jac_round32(const cplx* __restrict__ Ao
       const int gi = isA ? blk_index<32>(pa, i) : r0 + i;
       const int gj = blk_index<32>(pb, j);
       Xout[(long)gj * ld + gi] = sT[i * JU_LD + j];
+    }
+    if (isA && ay != b) {      // the mirror tile (b, ay) of the Hermitian matrix (no CTA computes it)
+      for (int e = tid; e < 32 * 32; e += 256) {
+        const int j = e & 31, i = e >> 5;
+        Xout[(long)blk_index<32>(pa, i) * ld + blk_index<32>(pb, j)] = cconj(sT[i * JU_LD + j]);
+      }
     }
     return;
   }
@@ -728,7 +755,7 @@ static int block_sweeps(cudaStream_t st, int n, const cplx* A, long lda, EighWs*
       if (!ws->red_sweeps) KS_CUDA_CHECK(cudaMalloc(&ws->red_sweeps, sizeof(double) * 2 * 40 + sizeof(int) * 2), err);
       KS_CUDA_CHECK(cudaMemsetAsync(ws->red_sweeps, 0, sizeof(double) * 2 * 40 + sizeof(int) * 2, st), err);
       int* d_sweeps = (int*)(ws->red_sweeps + 2 * 40);
-      const int ntile = npair * (npair + np / 32);
+      const int ntile = npair * (npair + 1) / 2 + npair * (np / 32);
       const int grid = std::min(coop_ctas.load(), std::max(ntile, npair));
       cplx *Ap_ = ws->Ap, *Vp_ = ws->Vp, *U_ = ws->U;
       const int2* pairs_ = ws->pairs;
@@ -767,7 +794,7 @@ static int block_sweeps(cudaStream_t st, int n, const cplx* A, long lda, EighWs*
       if (h[0] <= tol2 * h[1]) break;
       for (int r = 0; r < nr; ++r) {
         const int rn = (r + 1) % nr;
-        k_jac_round32<<<npair + npair * (npair + nvt), 256, smem_round, st>>>(
+        k_jac_round32<<<npair + npair * (npair + 1) / 2 + npair * nvt, 256, smem_round, st>>>(
             Acur, Aalt, ws->Vp, np, npair, nvt, ws->pairs + (size_t)r * npair, ws->where + (size_t)r * nblk, Ucur,
             ws->pairs + (size_t)rn * npair, Unext, inner, (rn > 0 && cross_rounds) ? 1 : 0);
         std::swap(Acur, Aalt);

@@ -822,13 +822,20 @@ struct XArgs {
   long ncol;            // NY*NZ
 };
 
-template <int NX> struct xcfg { static constexpr int ZC = 32, NT = 128, MINB = 4; };
-template <> struct xcfg<18> { static constexpr int ZC = 32, NT = 96, MINB = 4; };
-template <> struct xcfg<36> { static constexpr int ZC = 32, NT = 96, MINB = 4; };
-template <> struct xcfg<54> { static constexpr int ZC = 32, NT = 96, MINB = 4; };
+// STAGE: the next band's live rows stream into a staging buffer [L1][ZC] instead of the tile rows (see x_body)
+template <int NX> struct xcfg { static constexpr int ZC = 32, NT = 128, MINB = 4; static constexpr bool STAGE = false; };
+template <> struct xcfg<18> { static constexpr int ZC = 32, NT = 96, MINB = 4; static constexpr bool STAGE = false; };
+template <> struct xcfg<36> { static constexpr int ZC = 32, NT = 96, MINB = 4; static constexpr bool STAGE = false; };
+template <> struct xcfg<54> { static constexpr int ZC = 32, NT = 96, MINB = 4; static constexpr bool STAGE = false; };
 // 128: 16-column tiles and four 4-warp CTAs per SM beat 32-column tiles and two 8-warp CTAs (301 -> 283 us per 30-band launch);
 // the same halving for 96 (64-thread CTAs, eight per SM) is slightly slower (283 -> 289 us)
-template <> struct xcfg<128> { static constexpr int ZC = 16, NT = 128, MINB = 4; };
+#ifndef KSPW_X128_STAGE
+#define KSPW_X128_STAGE 0   // measured (cfg 3, 520 bands): refill of the tile rows after pass 3 4.41 ms, staging buffer 4.70 ms: off
+#endif
+#ifndef KSPW_X_VPRE
+#define KSPW_X_VPRE 0
+#endif
+template <> struct xcfg<128> { static constexpr int ZC = 16, NT = 128, MINB = 4; static constexpr bool STAGE = (KSPW_X128_STAGE != 0); };
 
 // The CTA walks over bg bands with the same columns.  Thread (pz, g) owns the codelet lines j2 = g, g+G, ...
 // in the first AND the last pass, i.e. the tile rows {j1*R2 + j2}: once the last pass of band b has read a
@@ -842,12 +849,18 @@ __device__ __forceinline__ void x_body(const XArgs& a, const int bx, const int b
   constexpr int ITEMS = (R2 + G - 1) / G;     // first/last-pass lines per thread
   constexpr int R1P = (R1 + 3) & ~3;          // row-offset table: R2+1 lines of R1P entries (line R2 is all dead)
   constexpr unsigned DEAD = 0xffffffffu;
+  // STG: the live rows of the NEXT band stream into a staging buffer [L1][ZC] right after pass 1 has taken the current
+  // band's rows out of it, so a band's global loads have all three passes of the band before it to land.  (Refilling the tile
+  // rows themselves is only possible after pass 3 has read them, i.e. a few store instructions before pass 1 of the next band
+  // wants them: ncu attributed 15 % of k_x<128>'s stall samples to that first shared-memory read, waiting on the cp.async.)
+  constexpr bool STG = xcfg<NX>::STAGE;
   static_assert(NT % ZC == 0, "thread count must be a multiple of the column chunk");
   static_assert(ITEMS <= 4, "cp_wait_n covers up to 4 groups in flight");
   extern __shared__ cplx sm[];
   cplx* tw = sm;
   cplx* tile = sm + NX;
-  unsigned* rofs = reinterpret_cast<unsigned*>(tile + NX * ZC);   // [R2+1][R1P]: element offset of row j1*R2+j2, or DEAD
+  unsigned* rofs = reinterpret_cast<unsigned*>(tile + NX * ZC);   // [R2+1][R1P]: element offset of row j1*R2+j2 (STG: its live-plane index), or DEAD
+  cplx* stage = reinterpret_cast<cplx*>(rofs + (R2 + 1) * R1P);    // STG only: [L1][ZC]  (the table is a multiple of 16 bytes)
   const int tid = threadIdx.x, pz = tid % ZC, g = tid / ZC;
   const unsigned ncol = (unsigned)a.ncol;      // one band's live planes (L1*ncol elements) fit 32-bit offsets
   const unsigned col = bx * ZC + pz;
@@ -864,7 +877,7 @@ __device__ __forceinline__ void x_body(const XArgs& a, const int bx, const int b
     if (j2 < R2 && j1 < R1) {
       int lx = j1 * R2 + j2 - a.x0;
       if (lx < 0) lx += NX;
-      if (lx < a.L1) o = (unsigned)lx * ncol;
+      if (lx < a.L1) o = STG ? (unsigned)lx : (unsigned)lx * ncol;
     }
     rofs[i] = o;
   }
@@ -886,30 +899,77 @@ __device__ __forceinline__ void x_body(const XArgs& a, const int bx, const int b
     line_offsets(o, j2);
 #pragma unroll
     for (int j1 = 0; j1 < R1; ++j1)
-      if (o[j1] != DEAD) cp16m(tcol + (j1 * R2 + j2) * ZC, src + o[j1]);
+      if (o[j1] != DEAD) {
+        if constexpr (STG) cp16m(stage + o[j1] * ZC + pz, src + o[j1] * ncol);
+        else cp16m(tcol + (j1 * R2 + j2) * ZC, src + o[j1]);
+      }
     cp_commit_m();
   };
 #pragma unroll
   for (int i = 0; i < ITEMS; ++i) prefetch_line(base, g + i * G);
 
   for (int b = b0; b < b1; ++b, base += bstride) {
+    const bool more = b + 1 < b1;
     // pass 1 (type-A stage 1): own prefetched rows -> registers -> DFT-R1 -> twiddle -> tile
 #pragma unroll
     for (int i = 0; i < ITEMS; ++i) {
       const int j2 = g + i * G;
-      cp_wait_n(ITEMS - 1 - i);
+      // STG: every line's turn leaves ITEMS - 1 younger groups in flight (the refills issued below included)
+      cp_wait_n(STG ? ITEMS - 1 : ITEMS - 1 - i);
       if (R2 % G == 0 || j2 < R2) {
         unsigned o[R1P];
         line_offsets(o, j2);
         cplx v[R1];
 #pragma unroll
-        for (int j1 = 0; j1 < R1; ++j1) v[j1] = (o[j1] != DEAD) ? tcol[(j1 * R2 + j2) * ZC] : cmake(0.0, 0.0);
+        for (int j1 = 0; j1 < R1; ++j1) {
+          if constexpr (STG) v[j1] = (o[j1] != DEAD) ? stage[o[j1] * ZC + pz] : cmake(0.0, 0.0);
+          else v[j1] = (o[j1] != DEAD) ? tcol[(j1 * R2 + j2) * ZC] : cmake(0.0, 0.0);
+        }
         dft<R1, +1>(v);
+        if constexpr (STG) {                 // v is consumed: the line's staging rows are free for the next band
+          if (more) {
+#pragma unroll
+            for (int j1 = 0; j1 < R1; ++j1)
+              if (o[j1] != DEAD) cp16m(stage + o[j1] * ZC + pz, base + bstride + o[j1] * ncol);
+          }
+        }
         cplx* out = tcol + j2 * ZC;
 #pragma unroll
         for (int k1 = 0; k1 < R1; ++k1) out[k1 * R2 * ZC] = (k1 == 0) ? v[0] : mul_tw<+1>(v[k1], tw, j2 * k1);
       }
+      if constexpr (STG) cp_commit_m();      // one group per line and band, empty or not: uniform accounting
     }
+#if KSPW_X_VPRE
+    // V(r) of the thread's first pass-2 line is requested BEFORE the barrier and each later line's one line ahead, so the
+    // (mostly L2) latency of these loads runs under the barrier wait and the previous line's codelets (ncu: 6 % of
+    // k_x<128>'s stall samples sat on the first use of vr)
+    double vr[R2];
+    if (g < R1) {
+      const double* vp = vbase + (size_t)g * R2 * a.ncol;
+#pragma unroll
+      for (int k2 = 0; k2 < R2; ++k2) vr[k2] = __ldg(vp + (unsigned)k2 * ncol);
+    }
+    __syncthreads();
+    // pass 2: type-A stage 2, V(r), type-B stage 1 on the same R2 elements, in registers
+    for (int k1 = g; k1 < R1; k1 += G) {
+      cplx v[R2];
+      cplx* t = tcol + k1 * R2 * ZC;
+#pragma unroll
+      for (int j2 = 0; j2 < R2; ++j2) v[j2] = t[j2 * ZC];
+      dft<R2, +1>(v);
+#pragma unroll
+      for (int k2 = 0; k2 < R2; ++k2) v[k2] = cmake(v[k2].x * vr[k2], v[k2].y * vr[k2]);
+      if (k1 + G < R1) {
+        const double* vp = vbase + (size_t)(k1 + G) * R2 * a.ncol;
+#pragma unroll
+        for (int k2 = 0; k2 < R2; ++k2) vr[k2] = __ldg(vp + (unsigned)k2 * ncol);
+      }
+      dft<R2, -1>(v);
+#pragma unroll
+      for (int q2 = 0; q2 < R2; ++q2) t[q2 * ZC] = (q2 == 0) ? v[0] : mul_tw<-1>(v[q2], tw, k1 * q2);
+    }
+    __syncthreads();
+#else
     __syncthreads();
     // pass 2: type-A stage 2, V(r), type-B stage 1 on the same R2 elements, in registers
     for (int k1 = g; k1 < R1; k1 += G) {
@@ -929,8 +989,8 @@ __device__ __forceinline__ void x_body(const XArgs& a, const int bx, const int b
       for (int q2 = 0; q2 < R2; ++q2) t[q2 * ZC] = (q2 == 0) ? v[0] : mul_tw<-1>(v[q2], tw, k1 * q2);
     }
     __syncthreads();
-    // pass 3 (type-B stage 2): tile -> DFT-R1 -> live planes (natural x = q1*R2 + q2); refill the line
-    const bool more = b + 1 < b1;
+#endif
+    // pass 3 (type-B stage 2): tile -> DFT-R1 -> live planes (natural x = q1*R2 + q2); refill the line (tile-row variant)
 #pragma unroll
     for (int i = 0; i < ITEMS; ++i) {
       const int q2 = g + i * G;
@@ -943,16 +1003,19 @@ __device__ __forceinline__ void x_body(const XArgs& a, const int bx, const int b
         for (int k1 = 0; k1 < R1; ++k1) v[k1] = t[k1 * R2 * ZC];
         dft<R1, -1>(v);
       }
-      if (more) {                                    // v is consumed: the line's rows are free
+      if constexpr (!STG) {
+        if (more) {                                    // v is consumed: the line's rows are free
 #pragma unroll
-        for (int j1 = 0; j1 < R1; ++j1)
-          if (o[j1] != DEAD) cp16m(tcol + (j1 * R2 + q2) * ZC, base + bstride + o[j1]);
-        cp_commit_m();
+          for (int j1 = 0; j1 < R1; ++j1)
+            if (o[j1] != DEAD) cp16m(tcol + (j1 * R2 + q2) * ZC, base + bstride + o[j1]);
+          cp_commit_m();
+        }
       }
 #pragma unroll
       for (int q1 = 0; q1 < R1; ++q1)
-        if (o[q1] != DEAD) base[o[q1]] = v[q1];
+        if (o[q1] != DEAD) base[STG ? o[q1] * ncol : o[q1]] = v[q1];
     }
+    // no barrier here: pass 1 of the next band writes the tile rows {k1*R2 + j2} that this same thread read in pass 3
   }
 }
 
@@ -1136,8 +1199,9 @@ int ks_hpsi_make_tmap(HpsiPlan& P, std::string& err) {
   P.tmap_ok = true;
   return KS_OK;
 }
-template <int NX> static constexpr size_t x_smem() {
-  return sizeof(cplx) * ((size_t)NX + (size_t)NX * xcfg<NX>::ZC) + sizeof(unsigned) * (fac<NX>::R2 + 1) * ((fac<NX>::R1 + 3) & ~3);
+template <int NX> static constexpr size_t x_smem(int L1) {      // L1 = NX: the most any context of this size can need
+  return sizeof(cplx) * ((size_t)NX + (size_t)NX * xcfg<NX>::ZC + (xcfg<NX>::STAGE ? (size_t)L1 * xcfg<NX>::ZC : 0)) +
+         sizeof(unsigned) * (fac<NX>::R2 + 1) * ((fac<NX>::R1 + 3) & ~3);
 }
 
 // the forward yz kernel runs as clusters of ZS CTAs along x when the plane's z' positions are split (yzcfg)
@@ -1188,7 +1252,8 @@ int ks_hpsi_configure(HpsiPlan& P, std::string& err) {
   KS_YZ_PAIRS(C_)
 #undef C_
   KS_CUDA_CHECK(e, err);
-#define C_(N_) if (P.n1 == N_) { P.zc_x = xcfg<N_>::ZC; P.smem_x = x_smem<N_>(); e = opt_in(k_x<N_>, P.smem_x); if (e == cudaSuccess) e = opt_in(k_x_k<N_>, P.smem_x); }
+  // (opt-in to the size's maximum, L1 = n1, for the same reason as above)
+#define C_(N_) if (P.n1 == N_) { P.zc_x = xcfg<N_>::ZC; P.smem_x = x_smem<N_>(P.L1); e = opt_in(k_x<N_>, x_smem<N_>(N_)); if (e == cudaSuccess) e = opt_in(k_x_k<N_>, x_smem<N_>(N_)); }
   KS_X_SIZES(C_)
 #undef C_
   KS_CUDA_CHECK(e, err);
@@ -1275,9 +1340,10 @@ int ks_hpsi_local_launch_k(const KItem* items, int nk, const void* dev_desc, cud
   if (nk <= 0) return KS_OK;
   const HpsiPlan& P0 = *items[0].P;
   int nbmax = 0, l1max = 0;
-  size_t smem_yz = 0;
+  size_t smem_yz = 0, smem_x = 0;
   for (int i = 0; i < nk; ++i) {
     const HpsiPlan& P = *items[i].P;
+    smem_x = std::max(smem_x, P.smem_x);
     if (P.n1 != P0.n1 || P.n2 != P0.n2 || P.n3 != P0.n3) { err = "ks_hpsi_batch: the k-points of a batch must share the FFT grid"; return KS_EINVAL; }
     if (items[i].nb > P.batch_cap) { err = "internal: FFT batch larger than workspace"; return KS_EINVAL; }
     nbmax = std::max(nbmax, items[i].nb); l1max = std::max(l1max, P.L1);
@@ -1296,7 +1362,7 @@ int ks_hpsi_local_launch_k(const KItem* items, int nk, const void* dev_desc, cud
 #undef C_
   }
   if (stage < 0 || stage == 1) {
-#define C_(N_) if (P0.n1 == N_) k_x_k<N_><<<gx, xcfg<N_>::NT, P0.smem_x, st>>>(xa);
+#define C_(N_) if (P0.n1 == N_) k_x_k<N_><<<gx, xcfg<N_>::NT, smem_x, st>>>(xa);
     KS_X_SIZES(C_)
 #undef C_
   }
