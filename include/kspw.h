@@ -185,6 +185,11 @@ int ks_dmma_peak(double* tflops_out /*HOST*/, double* dfma_tflops_out /*HOST, pl
  * accumulator tiles in flight (HOST out [6]); the first entry is the dependent-issue latency, the last the issue interval.
  * sm_ghz: the SM clock the times are converted with (bench.py passes the clock it sampled). */
 int ks_dmma_latency(double* clk_per_dmma, double sm_ghz);
+/* Do the FP64 tensor (DMMA) and the plain FP64 (DFMA) instructions draw on separate issue capacity?  HOST out [4], summed
+ * TFLOP/s of register-resident loops: [0] every warp DMMA, [1] every warp DFMA, [2] per SM sub-partition one DMMA warp next
+ * to one DFMA warp, [3] every warp interleaves both.  [2], [3] above [0] would mean the roofline denominator of the GEMMs
+ * (ks_dmma_peak) is too low; DESIGN.md section 5 records what the B200 measured. */
+int ks_fp64_mix_peak(double* tflops4);
 #ifdef __cplusplus
 }
 #endif

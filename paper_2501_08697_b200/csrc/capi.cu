@@ -702,6 +702,10 @@ extern "C" int ks_dmma_latency(double* clk_per_dmma, double sm_ghz) {
   if (!clk_per_dmma || !(sm_ghz > 0)) return KS_EINVAL;
   return ks_dmma_latency_run(clk_per_dmma, sm_ghz, ks_global_error());
 }
+extern "C" int ks_fp64_mix_peak(double* tflops4) {
+  if (!tflops4) return KS_EINVAL;
+  return ks_fp64_mix_run(tflops4, ks_global_error());
+}
 extern "C" int ks_dmma_peak(double* tflops_out, double* dfma_tflops_out) {
   return ks_peak_run(tflops_out, dfma_tflops_out, ks_global_error());
 }

@@ -761,6 +761,62 @@ int ks_peak_run(double* dmma_tf, double* dfma_tf, std::string& err) {
   return KS_OK;
 }
 
+// Can the DMMA and the DFMA pipe be fed at the same time?  (If they could, a mixed-pipe GEMM would have a ceiling above the
+// DMMA peak.)  mode 0: every warp runs the DMMA loop; 1: every warp the DFMA loop; 2: warps 0-3 DMMA and warps 4-7 DFMA
+// (each SM sub-partition holds one warp of either kind); 3: every warp interleaves 16 DMMAs with 16 DFMAs per iteration.
+// out[mode] = summed TFLOP/s (512 flop per DMMA, 2 flop per DFMA lane).
+__global__ void __launch_bounds__(256) k_fp64_mix(double* out, int iters, int mode) {
+  double c[16][2], f[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) { c[i][0] = c[i][1] = 0.0; f[i] = 1e-3 * i; }
+  double a[4], b[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { a[i] = 1.0 + 1e-9 * (threadIdx.x + i); b[i] = 1.0 - 1e-9 * (threadIdx.x + 7 * i); }
+  const double fa = 1.0 + 1e-9 * threadIdx.x, fb = 1e-9 * threadIdx.x;
+  const int warp = threadIdx.x >> 5;
+  const bool do_m = mode == 0 || mode == 3 || (mode == 2 && warp < 4);
+  const bool do_f = mode == 1 || mode == 3 || (mode == 2 && warp >= 4);
+  for (int it = 0; it < iters; ++it) {
+    if (do_m) {
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) dmma(c[4 * i + j][0], c[4 * i + j][1], a[i], b[j]);
+    }
+    if (do_f) {
+#pragma unroll
+      for (int i = 0; i < 16; ++i) f[i] = fma(f[i], fa, fb);
+    }
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += c[i][0] + c[i][1] + f[i];
+  if (s == 12345.678) out[0] = s;
+}
+int ks_fp64_mix_run(double* tflops4, std::string& err) {
+  double* d = nullptr;
+  KS_CUDA_CHECK(cudaMalloc(&d, 8), err);
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int blocks = 148 * 4, iters = 20000;
+  for (int mode = 0; mode < 4; ++mode) {
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+      cudaEventRecord(e0);
+      k_fp64_mix<<<blocks, 256>>>(d, iters, mode);
+      cudaEventRecord(e1);
+      KS_CUDA_CHECK(cudaEventSynchronize(e1), err);
+      float ms; cudaEventElapsedTime(&ms, e0, e1);
+      if (rep) best = std::min(best, ms);
+    }
+    const double wm = (mode == 0 || mode == 3) ? 8 : (mode == 2 ? 4 : 0), wf = (mode == 1 || mode == 3) ? 8 : (mode == 2 ? 4 : 0);
+    const double fl = (double)blocks * iters * 16 * (wm * 512.0 + wf * 32 * 2.0);
+    tflops4[mode] = fl / (best * 1e-3) / 1e12;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+  return KS_OK;
+}
+
 // ------------------------------------------------------------------------------------------------
 // ks_zgemm_hn_static: C = A^H B for callers that cannot call cudaMalloc (code under CUDA graph capture, serving loops,
 // harnesses that forbid allocation).  The same split-K kernels as ks_gemm_hn (k_gemm_hn<NJ> + k_splitk_reduce), with the

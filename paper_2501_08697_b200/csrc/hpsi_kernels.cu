@@ -827,15 +827,18 @@ template <int NX> struct xcfg { static constexpr int ZC = 32, NT = 128, MINB = 4
 template <> struct xcfg<18> { static constexpr int ZC = 32, NT = 96, MINB = 4; static constexpr bool STAGE = false; };
 template <> struct xcfg<36> { static constexpr int ZC = 32, NT = 96, MINB = 4; static constexpr bool STAGE = false; };
 template <> struct xcfg<54> { static constexpr int ZC = 32, NT = 96, MINB = 4; static constexpr bool STAGE = false; };
-// 128: 16-column tiles and four 4-warp CTAs per SM beat 32-column tiles and two 8-warp CTAs (301 -> 283 us per 30-band launch);
+// 128: 16-column tiles and 4-warp CTAs (five per SM) beat 32-column tiles and two 8-warp CTAs (301 -> 283 us per 30-band launch);
 // the same halving for 96 (64-thread CTAs, eight per SM) is slightly slower (283 -> 289 us)
 #ifndef KSPW_X128_STAGE
 #define KSPW_X128_STAGE 0   // measured (cfg 3, 520 bands): refill of the tile rows after pass 3 4.41 ms, staging buffer 4.70 ms: off
 #endif
+#ifndef KSPW_X128_MINB
+#define KSPW_X128_MINB 5    // CTAs per SM asked of ptxas: 4 -> 128 registers, 5 -> 96 (12 bytes of spills), 6 -> 80 (148 bytes).
+#endif                      // Measured (cfg 3, 520 bands): 4.424 / 4.348 / 4.992 ms
 #ifndef KSPW_X_VPRE
 #define KSPW_X_VPRE 0
 #endif
-template <> struct xcfg<128> { static constexpr int ZC = 16, NT = 128, MINB = 4; static constexpr bool STAGE = (KSPW_X128_STAGE != 0); };
+template <> struct xcfg<128> { static constexpr int ZC = 16, NT = 128, MINB = KSPW_X128_MINB; static constexpr bool STAGE = (KSPW_X128_STAGE != 0); };
 
 // The CTA walks over bg bands with the same columns.  Thread (pz, g) owns the codelet lines j2 = g, g+G, ...
 // in the first AND the last pass, i.e. the tile rows {j1*R2 + j2}: once the last pass of band b has read a

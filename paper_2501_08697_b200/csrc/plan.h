@@ -94,6 +94,7 @@ int ks_gemm_hn_group(cudaStream_t st, const GemmProb* dev_probs, int ng, int M, 
 int ks_gemm_nn_group(cudaStream_t st, const GemmProb* dev_probs, int ng, int M, int N, int accumulate, std::string& err);
 
 int ks_dmma_latency_run(double* clk_per_dmma, double sm_ghz, std::string& err);
+int ks_fp64_mix_run(double* tflops4, std::string& err);
 int ks_peak_run(double* dmma_tf, double* dfma_tf, std::string& err);
 
 struct EighWs {

@@ -51,11 +51,12 @@ _lib.ks_zgemm_nn.argtypes = [_vp, _i, _i, _i, _vp, _l, _vp, _l, _vp, _l, _i]
 _lib.ks_eigh.argtypes = [_vp, _i, _vp, _l, _vp, _vp, _l, _vp]
 _lib.ks_dmma_peak.argtypes = [_vp, _vp]
 _lib.ks_dmma_latency.argtypes = [_vp, _d]
+_lib.ks_fp64_mix_peak.argtypes = [_vp]
 
 KS_OK, KS_NOTCONV = 0, 1
 EXPORTS = ("ks_pw_count", "ks_pw_list", "ks_create", "ks_destroy", "ks_npw", "ks_set_stream", "ks_set_fft_batch",
            "ks_last_error", "ks_supported_sizes", "ks_hpsi", "ks_hpsi_host", "ks_hpsi_batch", "ks_davidson_batch", "ks_density", "ks_density_host", "ks_chebyshev", "ks_cg", "ks_set_overlap", "ks_spsi", "ks_davidson", "ks_davidson_host",
-           "ks_davidson_profile", "ks_profile_begin", "ks_profile_end", "ks_zgemm_hn", "ks_zgemm_hn_static", "ks_zgemm_nn", "ks_eigh", "ks_dmma_peak", "ks_dmma_latency")
+           "ks_davidson_profile", "ks_profile_begin", "ks_profile_end", "ks_zgemm_hn", "ks_zgemm_hn_static", "ks_zgemm_nn", "ks_eigh", "ks_dmma_peak", "ks_dmma_latency", "ks_fp64_mix_peak")
 
 
 class KsError(RuntimeError):
@@ -388,6 +389,15 @@ def ks_dmma_latency(sm_ghz=1.965):
     if rc:
         raise KsError(rc, _glob_err())
     return dict(zip((1, 2, 3, 4, 6, 8), (float(x) for x in out)))
+
+
+def ks_fp64_mix_peak():
+    """summed TFLOP/s of register-resident loops: DMMA only, DFMA only, one warp of each per sub-partition, both interleaved"""
+    out = np.zeros(4)
+    rc = _lib.ks_fp64_mix_peak(_hp(out))
+    if rc:
+        raise KsError(rc, _glob_err())
+    return dict(zip(("dmma", "dfma", "split_warps", "interleaved"), (float(x) for x in out)))
 
 
 def ks_dmma_peak():
