@@ -486,9 +486,19 @@ __device__ __forceinline__ void gemm_nn_tile(int M, int N, int K, const cplx* __
         const int m = m0 + wm * 8 * MI + i * 8 + fr, n = n0 + wn * 8 * NJ + j * 8 + 2 * fk + h;
         if (m < M && n < N) {
           cplx* p = &C[(long)n * ldc + m];
+#ifndef KSPW_GEMM_NN_RMW
+          // C += tile as two reductions without a return value (SASS RED.ADD.F64): every element has exactly one writer in
+          // the launch, so the sum is the same IEEE addition as load-add-store, bit for bit and deterministic -- but the
+          // thread does not wait ~1 us for each of its 40 old values in turn (stores to C may alias the next load, so the
+          // compiler keeps load-add-store pairs in order: ncu showed the DMMA pipe idle for ~9 % of a CTA's life at cfg 3,
+          // more where K is short)
+          if (accumulate) { atomicAdd(&p->x, cre[i][j][h]); atomicAdd(&p->y, cim[i][j][h]); }
+          else *p = cmake(cre[i][j][h], cim[i][j][h]);
+#else
           cplx v = cmake(cre[i][j][h], cim[i][j][h]);
           if (accumulate) { const cplx o = *p; v.x += o.x; v.y += o.y; }
           *p = v;
+#endif
         }
       }
 }
