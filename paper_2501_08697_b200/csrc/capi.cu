@@ -507,6 +507,9 @@ extern "C" int ks_hpsi_host(ks_ctx* c, const ks_c128* psi_host, ks_c128* hpsi_ho
   // chunk = a multiple of 32 bands (the GEMM tile unit: no padded columns inside a chunk), about eight chunks per block.
   // Measured (band-applications/s through host buffers): cfg 1, 160 bands: 32 -> 39.2k, 64 -> 37.9k, 40 -> 33.7k;
   // cfg 3, 520 bands: 64 -> 6.78k, 96 -> 6.58k, 128 -> 6.56k, 160 -> 6.62k, 65 (the old nbands/8 rule) -> 5.41k.
+  // Round 2: graded chunks (small head and tail, 1.5x growth up to 224 bands in between, so that only a short first H2D and
+  // last D2H stay exposed) measured SLOWER than uniform ones -- cfg 3 7.25k vs 7.49k, cfg 1 41.5k vs 42.1k, cfg 4 14.37k vs
+  // 14.47k: a long chunk's H2D does not hide behind the shorter chunks before it.
   static const int env_per = getenv("KSPW_HOST_CHUNK_BANDS") ? atoi(getenv("KSPW_HOST_CHUNK_BANDS")) : 0;
   const int per = env_per > 0 ? env_per : std::max(32, nbands / 8 / 32 * 32);
   KS_CUDA_CHECK(cudaEventRecord(c->ev_start, c->stream), c->err);          // order after earlier work on the stream
