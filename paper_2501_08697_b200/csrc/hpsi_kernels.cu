@@ -189,6 +189,7 @@ struct YzArgs {
   const cplx* tw_z;
   int npw, L1, smax;
   int nb;               // bands of this k-point (k-batched launches: CTAs beyond it leave at once)
+  int pf_dist;          // L2 prefetch distance in CTAs (0 = off), see inv_yz_body / fwd_yz_body
   double invN;
 };
 
@@ -404,6 +405,30 @@ __device__ __forceinline__ void inv_yz_body(const YzArgs& a, const int bx, const
   for (StickWalk w(tid, NT, S); w.j < K1H; w.next()) lineA_stage2<NZ, +1, facz<NZ>>(stile + w.s * SZ, 1, w.j);
   __syncthreads();
   KS_PH(1);
+#ifndef KSPW_NO_PSI_PREFETCH
+  // A CTA opens with a chain of dependent global loads that ends in the scattered reads of its plane's run of psi -- cold
+  // DRAM reads queued behind the plane stores of the CTAs before it (clock64: 7.1 k of a 128 x 128 plane's 25.3 k clocks pass
+  // before the first z pass is over, ~2 k of them arithmetic), with nothing else resident on the SM.  So every CTA asks L2
+  // for the psi run of the CTA `pf_dist` places ahead in launch order (about one wave: it starts when this one ends,
+  // on whichever SM) -- one prefetch per 128-byte line, one instruction per thread.
+  {
+    // (z'-split planes: the ZS CTAs of a plane read the same run; the first of them asks for the plane pf_dist CTAs ahead.
+    //  Measured: 128 x 128 k_inv_yz 2.86 -> 2.71 ms per 520 bands at one wave (148), no gain at two; 96 x 288 1.00 -> 0.97 ms;
+    //  96 x 96, two CTAs per SM: no change.)
+    if (a.pf_dist > 0 && h == 0) {
+      const long j = (long)b * gridDim.x + bx + a.pf_dist;
+      const int lx2 = (int)(j % gridDim.x) / ZS;
+      const long b2 = j / gridDim.x;
+      if (b2 < a.nb) {
+        const int p0 = a.plane_pw0[lx2], np2 = a.plane_pw0[lx2 + 1] - p0;
+        const char* q = reinterpret_cast<const char*>(a.psi + (size_t)b2 * a.npw + p0);
+        const char* q0 = reinterpret_cast<const char*>(reinterpret_cast<size_t>(q) & ~(size_t)127);
+        const long bytes = (q + (size_t)np2 * sizeof(cplx)) - q0;
+        for (long o = (long)tid * 128; o < bytes; o += (long)NT * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(q0 + o));
+      }
+    }
+  }
+#endif
   // H2 (y): for each chunk of z' positions, type-A inverse FFT along y; output straight to HBM
   cplx* plane = a.planes + ((size_t)b * a.L1 + lx) * ((size_t)NY * NZ) + h * NZH;
   const int grp = tid / GT, gt = tid % GT;
@@ -699,6 +724,23 @@ __device__ __forceinline__ void fwd_yz_body(const YzArgs& a, const int bx, const
     KS_PH(10);
   }
   }
+#ifndef KSPW_NO_PLANE_PREFETCH
+  // the same idea as in k_inv_yz: a CTA opens by waiting for the first chunk of its plane (cold DRAM reads, nothing else
+  // resident on the SM), so every CTA asks L2 for the first chunk of every y group of the plane `pf_dist` CTAs ahead
+  if constexpr (ZS == 1 && !yzcfg<NY, NZ>::DBF) {
+    if (a.pf_dist > 0) {
+      const long j = (long)b * gridDim.x + bx + a.pf_dist;
+      const int lx2 = (int)(j % gridDim.x);
+      const long b2 = j / gridDim.x;
+      if (b2 < a.nb) {
+        constexpr int LPR = (NG * ZC * (int)sizeof(cplx) + 127) / 128;      // 128-byte lines per plane row
+        const char* q = reinterpret_cast<const char*>(a.planes + ((size_t)b2 * a.L1 + lx2) * ((size_t)NY * NZ));
+        for (int i = tid; i < NY * LPR; i += NT)
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(q + (size_t)(i / LPR) * NZ * sizeof(cplx) + (size_t)(i % LPR) * 128));
+      }
+    }
+  }
+#endif
   // H4 (z): type-B forward FFT on each stick
   const cplx* psi = a.psi + (size_t)b * a.npw;
   cplx* hpsi = a.hpsi + (size_t)b * a.npw;
@@ -911,6 +953,9 @@ __device__ __forceinline__ void x_body(const XArgs& a, const int bx, const int b
 #pragma unroll
   for (int i = 0; i < ITEMS; ++i) prefetch_line(base, g + i * G);
 
+  // (An L2 prefetch of the first band of the CTA one wave ahead -- what k_inv_yz / k_fwd_yz do for their opening loads -- was
+  // measured here too: 128: 4.344 -> 4.414 ms, 96: 0.573 -> 0.601 ms, and 4.382 / 0.598 ms with the distance set to 0: the extra
+  // live registers cost more than the cold first band.)
   for (int b = b0; b < b1; ++b, base += bstride) {
     const bool more = b + 1 < b1;
     // pass 1 (type-A stage 1): own prefetched rows -> registers -> DFT-R1 -> twiddle -> tile
@@ -1273,6 +1318,16 @@ static int ks_x_band_group(int nchunk, int nb) {
   return std::min(bg, nb);
 }
 
+// L2 prefetch distance of k_inv_yz: the number of CTAs in flight (one wave), KSPW_PF_DIST=<n> overrides (0 = off)
+static int ks_pf_dist(const HpsiPlan& P) {
+  static int nsm = 0;
+  if (!nsm) { int dev = 0; cudaGetDevice(&dev); if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) nsm = 148; }
+  static const int env_pf = getenv("KSPW_PF_DIST") ? atoi(getenv("KSPW_PF_DIST")) : -1;
+  // CTAs per SM: one where the stick tile fills the SM, two otherwise (launch bounds of the yz kernels)
+  const int per_sm = P.smem_yz > KS_SMEM_MAX / 2 ? 1 : 2;
+  return env_pf >= 0 ? env_pf : nsm * per_sm;
+}
+
 int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb, cudaStream_t st,
                          std::string& err, int stage) {
   if (nb <= 0) return KS_OK;
@@ -1282,6 +1337,7 @@ int ks_hpsi_local_launch(const HpsiPlan& P, const cplx* psi, cplx* hpsi, int nb,
   a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.plane_pw0 = P.d_plane_pw0; a.stick = P.d_stick;
   a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
   a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.nb = nb; a.invN = 1.0 / (double)P.N;
+  a.pf_dist = ks_pf_dist(P);
   XArgs x;
   x.planes = P.d_planes; x.vperm = P.d_vperm; x.tw_x = P.d_tw[0];
   x.L1 = P.L1; x.x0 = P.x0; x.ncol = (long)P.n2 * P.n3;
@@ -1333,6 +1389,7 @@ void ks_kdesc_fill(void* host_desc, const KItem* items, int nk) {
     a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.plane_pw0 = P.d_plane_pw0; a.stick = P.d_stick;
     a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
     a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.nb = items[i].nb; a.invN = 1.0 / (double)P.N;
+    a.pf_dist = 0;      // k-batched grids: the launch order runs over k-points with different spheres: no prefetch
     XArgs& x = xa[i];
     x.planes = P.d_planes; x.vperm = P.d_vperm; x.tw_x = P.d_tw[0];
     x.L1 = P.L1; x.x0 = P.x0; x.ncol = ncol; x.nb = items[i].nb; x.bg = std::min(bg, std::max(1, items[i].nb));
@@ -1417,6 +1474,7 @@ int ks_density_batch(HpsiPlan& P, const cplx* psi, const double* occ, int nb, in
   a.plane_s0 = P.d_plane_s0; a.plane_y0 = P.d_plane_y0; a.plane_pw0 = P.d_plane_pw0; a.stick = P.d_stick;
   a.g2 = P.d_g2; a.tw_y = P.d_tw[1]; a.tw_z = P.d_tw[2];
   a.npw = P.npw; a.L1 = P.L1; a.smax = P.smax; a.nb = nb; a.invN = 1.0 / (double)P.N;
+  a.pf_dist = ks_pf_dist(P);
   const dim3 gyz(P.L1 * P.zs_yz, nb);
 #define C_(A_, B_) if (P.n2 == A_ && P.n3 == B_) k_inv_yz<A_, B_><<<gyz, yzcfg<A_, B_>::NT, P.smem_yz, st>>>(a);
   KS_YZ_PAIRS(C_)
