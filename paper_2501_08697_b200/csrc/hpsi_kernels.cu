@@ -595,6 +595,17 @@ __device__ __forceinline__ void fwd_yz_body(const YzArgs& a, const int bx, const
   const int grp = tid / GT, gt = tid % GT;
   const int pz = gt % ZC, g = gt / ZC;
   KS_PH_INIT();
+#ifndef KSPW_NO_PSI_PREFETCH
+  // z'-split planes: the last pass reads psi (for |k+G|^2 psi) straight from global memory, one dependent load per output,
+  // long after k_inv_yz brought it in; the ZS CTAs of the plane ask L2 for the plane's run now, a y transform ahead of its use
+  if constexpr (ZS > 1) {
+    const int p0 = a.plane_pw0[lx], np2 = a.plane_pw0[lx + 1] - p0;
+    const char* q = reinterpret_cast<const char*>(a.psi + (size_t)b * a.npw + p0);
+    const char* q0 = reinterpret_cast<const char*>(reinterpret_cast<size_t>(q) & ~(size_t)127);
+    const long bytes = (q + (size_t)np2 * sizeof(cplx)) - q0;
+    for (long o = ((long)h * NT + tid) * 128; o < bytes; o += (long)ZS * NT * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(q0 + o));
+  }
+#endif
   // H4 (y), type B, forward.  The y tile is split into two half-width buffers: while chunk c (ZF = ZC/2 columns) is
   // transformed in place in one of them, chunk c+1 streams into the other by cp.async, so the plane loads are
   // in flight during both codelet passes.  (Odd ZC: single buffer, loads straight into registers.)
