@@ -598,7 +598,10 @@ __device__ __forceinline__ void fwd_yz_body(const YzArgs& a, const int bx, const
 #ifndef KSPW_NO_PSI_PREFETCH
   // z'-split planes: the last pass reads psi (for |k+G|^2 psi) straight from global memory, one dependent load per output,
   // long after k_inv_yz brought it in; the ZS CTAs of the plane ask L2 for the plane's run now, a y transform ahead of its use
-  if constexpr (ZS > 1) {
+#ifndef KSPW_FWD_PF_ALL
+#define KSPW_FWD_PF_ALL 0     // unsplit planes stage the run by cp.async after the y transform; the same request ahead of it
+#endif                        // measured slower: 128 x 128 2.839 -> 2.938 ms, 96 x 96 0.321 -> 0.324 ms
+  if constexpr (ZS > 1 || KSPW_FWD_PF_ALL) {
     const int p0 = a.plane_pw0[lx], np2 = a.plane_pw0[lx + 1] - p0;
     const char* q = reinterpret_cast<const char*>(a.psi + (size_t)b * a.npw + p0);
     const char* q0 = reinterpret_cast<const char*>(reinterpret_cast<size_t>(q) & ~(size_t)127);
