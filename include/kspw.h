@@ -68,7 +68,9 @@ int ks_supported_sizes(int* sizes, int cap);
 /* hpsi = H psi for a block of bands (steps H1-H8 of DESIGN.md §1).
  * psi, hpsi: DEVICE [nbands][npw], caller-owned, must not alias.  Asynchronous on the stream. */
 int ks_hpsi(ks_ctx* ctx, const ks_c128* psi, ks_c128* hpsi, int nbands);
-/* same through HOST buffers (copies H2D / D2H inside, synchronises before returning) */
+/* same through HOST buffers (copies H2D / D2H inside, synchronises before returning).  The block is processed in chunks of
+ * bands so that the copies overlap the kernels (the first chunk half as long as the others); the projector sums of a chunk are
+ * split over K differently from those of the whole block, so the result equals ks_hpsi's to rounding, not bit for bit. */
 int ks_hpsi_host(ks_ctx* ctx, const ks_c128* psi_host, ks_c128* hpsi_host, int nbands);
 
 /* ---- many k-points at once (the batched multi-k entry point) ------------------------------
